@@ -1,0 +1,199 @@
+"""ctypes binding of oracle/qmc_oracle.c (TEST INFRASTRUCTURE; numpy in, numpy out).
+
+Argument marshalling only: every number comes out of the C file.  See the header of
+qmc_oracle.c for the passages of PAPER.md each function follows.
+"""
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "qmc_oracle.c")
+_LIB = os.path.join(_HERE, "libqmc_oracle.so")
+_lib = None
+
+_dp = ctypes.POINTER(ctypes.c_double)
+_fp = ctypes.POINTER(ctypes.c_float)
+_ip = ctypes.POINTER(ctypes.c_int)
+_bp = ctypes.POINTER(ctypes.c_ubyte)
+
+
+def build(force=False):
+    """Compile qmc_oracle.c with gcc -O2 (no fast-math, no intrinsics) into oracle/."""
+    if (not force and os.path.exists(_LIB)
+            and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC)):
+        return _LIB
+    cmd = ["gcc", "-O2", "-std=c99", "-fopenmp", "-shared", "-fPIC", "-o", _LIB, _SRC, "-lm"]
+    subprocess.run(cmd, check=True)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        lib = ctypes.CDLL(_LIB)
+        lib.orc_spline_vgl.restype = ctypes.c_int
+        lib.orc_spline_vgl.argtypes = [ctypes.c_int] * 4 + [_dp, _fp, ctypes.c_int, _dp, _dp, _dp, _dp]
+        lib.orc_lu_inverse.restype = ctypes.c_int
+        lib.orc_lu_inverse.argtypes = [ctypes.c_int, _dp, _dp, _dp, _ip]
+        lib.orc_binv_from_A.restype = ctypes.c_int
+        lib.orc_binv_from_A.argtypes = [ctypes.c_int, _dp, _dp, _dp, _ip]
+        lib.orc_det_ratio.restype = ctypes.c_double
+        lib.orc_det_ratio.argtypes = [ctypes.c_int, _dp, ctypes.c_int, _dp]
+        lib.orc_sm_update.restype = ctypes.c_int
+        lib.orc_sm_update.argtypes = [ctypes.c_int, _dp, ctypes.c_int, _dp, ctypes.c_double]
+        lib.orc_slater_matrix.restype = ctypes.c_int
+        lib.orc_slater_matrix.argtypes = [ctypes.c_int] * 4 + [_dp, _fp, ctypes.c_int, ctypes.c_int, _dp, _dp]
+        lib.orc_sweep.restype = ctypes.c_int
+        lib.orc_sweep.argtypes = ([ctypes.c_int] * 4 + [_dp, _fp, ctypes.c_int, ctypes.c_int,
+                                  _dp, _dp, _dp, _dp, _ip, _dp, _dp, ctypes.c_int, ctypes.c_int,
+                                  _dp, _bp, _bp, _fp, _dp, ctypes.c_int, ctypes.c_int])
+        lib.orc_max_threads.restype = ctypes.c_int
+        lib.orc_max_threads.argtypes = []
+        _lib = lib
+    return _lib
+
+
+def _d(a):
+    return None if a is None else a.ctypes.data_as(_dp)
+
+
+def _c64(a, shape=None):
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    if shape is not None:
+        assert a.shape == tuple(shape), (a.shape, shape)
+    return a
+
+
+def _coefs(coefs):
+    assert coefs.dtype == np.float32 and coefs.ndim == 4 and coefs.flags.c_contiguous
+    return coefs
+
+
+def _check(rc, what):
+    if rc != 0:
+        raise RuntimeError(f"oracle {what} failed with code {rc}")
+
+
+def max_threads():
+    return int(_load().orc_max_threads())
+
+
+def spline_vgl(coefs, lattice, pos, want_gl=True):
+    """coefs float32 [nx][ny][nz][norb]; pos [npos][3] -> v [npos][norb], g [npos][3][norb], l."""
+    lib = _load()
+    coefs = _coefs(coefs)
+    nx, ny, nz, norb = coefs.shape
+    lat = _c64(lattice).reshape(9)
+    pos = _c64(pos).reshape(-1, 3)
+    npos = pos.shape[0]
+    v = np.empty((npos, norb))
+    g = np.empty((npos, 3, norb)) if want_gl else None
+    l = np.empty((npos, norb)) if want_gl else None
+    rc = lib.orc_spline_vgl(nx, ny, nz, norb, _d(lat), coefs.ctypes.data_as(_fp), npos,
+                            _d(pos), _d(v), _d(g), _d(l))
+    _check(rc, "spline_vgl")
+    return (v, g, l) if want_gl else v
+
+
+def lu_inverse(A):
+    """A [n][n] -> (Ainv, log|det A|, sign)."""
+    lib = _load()
+    A = _c64(A)
+    n = A.shape[0]
+    Ainv = np.empty((n, n))
+    ld = ctypes.c_double(0.0)
+    sg = ctypes.c_int(0)
+    rc = lib.orc_lu_inverse(n, _d(A), _d(Ainv), ctypes.byref(ld), ctypes.byref(sg))
+    _check(rc, "lu_inverse")
+    return Ainv, ld.value, sg.value
+
+
+def binv_from_A(A):
+    """A [n][n] -> (B = (A^-1)^T, log|det A|, sign)."""
+    lib = _load()
+    A = _c64(A)
+    n = A.shape[0]
+    B = np.empty((n, n))
+    ld = ctypes.c_double(0.0)
+    sg = ctypes.c_int(0)
+    rc = lib.orc_binv_from_A(n, _d(A), _d(B), ctypes.byref(ld), ctypes.byref(sg))
+    _check(rc, "binv_from_A")
+    return B, ld.value, sg.value
+
+
+def det_ratio(B, k, phi):
+    lib = _load()
+    B = _c64(B)
+    phi = _c64(phi)
+    return float(lib.orc_det_ratio(B.shape[0], _d(B), int(k), _d(phi)))
+
+
+def sm_update(B, k, phi, R):
+    """Returns the updated copy of B."""
+    lib = _load()
+    B = _c64(B).copy()
+    phi = _c64(phi)
+    _check(lib.orc_sm_update(B.shape[0], _d(B), int(k), _d(phi), float(R)), "sm_update")
+    return B
+
+
+def slater_matrix(coefs, lattice, pos):
+    """pos [nw][nel][3] -> A [nw][nel][nel], A[w][i][j] = phi_j(r_wi)."""
+    lib = _load()
+    coefs = _coefs(coefs)
+    nx, ny, nz, norb = coefs.shape
+    lat = _c64(lattice).reshape(9)
+    pos = _c64(pos)
+    nw, nel, _ = pos.shape
+    A = np.empty((nw, nel, nel))
+    rc = lib.orc_slater_matrix(nx, ny, nz, norb, _d(lat), coefs.ctypes.data_as(_fp), nw, nel,
+                               _d(pos), _d(A))
+    _check(rc, "slater_matrix")
+    return A
+
+
+def sweep(coefs, lattice, pos, B, logdet, sign, delta, unif, A=None, iel_count=None,
+          forced=None, phi_in=None, want_phi=False, mode=0, nthreads=1):
+    """Run nsweeps particle-by-particle sweeps.  Inputs are copied; returns a dict with
+    pos, B, A, logdet, sign, ratios [nsweeps][nel][nw], accept (uint8, same shape), phi."""
+    lib = _load()
+    coefs = _coefs(coefs)
+    nx, ny, nz, norb = coefs.shape
+    lat = _c64(lattice).reshape(9)
+    pos = _c64(pos).copy()
+    nw, nel, _ = pos.shape
+    B = _c64(B, (nw, nel, nel)).copy()
+    A = None if A is None else _c64(A, (nw, nel, nel)).copy()
+    logdet = _c64(logdet, (nw,)).copy()
+    sign = np.ascontiguousarray(sign, dtype=np.int32).copy()
+    delta = _c64(delta)
+    nsweeps = delta.shape[0]
+    assert delta.shape == (nsweeps, nel, nw, 3)
+    unif = _c64(unif, (nsweeps, nel, nw))
+    if iel_count is None:
+        iel_count = nel
+    ratios = np.zeros((nsweeps, nel, nw))
+    accept = np.zeros((nsweeps, nel, nw), dtype=np.uint8)
+    f_ptr = None
+    if forced is not None:
+        forced = np.ascontiguousarray(forced, dtype=np.uint8)
+        assert forced.shape == (nsweeps, nel, nw)
+        f_ptr = forced.ctypes.data_as(_bp)
+    p_ptr = None
+    if phi_in is not None:
+        assert phi_in.dtype == np.float32 and phi_in.flags.c_contiguous
+        assert phi_in.shape == (nsweeps, nel, nw, nel)
+        p_ptr = phi_in.ctypes.data_as(_fp)
+    phi_out = np.zeros((nsweeps, nel, nw, nel)) if want_phi else None
+    rc = lib.orc_sweep(nx, ny, nz, norb, _d(lat), coefs.ctypes.data_as(_fp), nw, nel,
+                       _d(pos), _d(B), _d(A), _d(logdet), sign.ctypes.data_as(_ip),
+                       _d(delta), _d(unif), nsweeps, int(iel_count), _d(ratios),
+                       accept.ctypes.data_as(_bp), f_ptr, p_ptr, _d(phi_out), int(mode),
+                       int(nthreads))
+    _check(rc, "sweep")
+    return dict(pos=pos, B=B, A=A, logdet=logdet, sign=sign, ratios=ratios, accept=accept,
+                phi=phi_out)

@@ -1,0 +1,400 @@
+"""Pins of the fp64 CPU oracle (oracle/qmc_oracle.c) against facts the paper's formulation
+and the mathematics fix -- none of them re-types the oracle's own formulas:
+
+  P-a  partition of unity (constant table)
+  P-b  linear / P-c quadratic and bilinear reproduction (index offset of eq. 33;
+       gradient and Laplacian scaling, incl. the cross terms on a skewed cell)
+  P-d  plane-wave table: closed form at the grid nodes, across the periodic wrap
+  P-e  periodicity, P-f C2 continuity across cell faces
+  P-s  scipy.interpolate.BSpline tensor product (de Boor recursion, a library routine)
+  P-g  central finite differences of the oracle's own value
+  P-h  ratio vs Leibniz-expansion and numpy determinants (N <= 16)          L299, L325
+  P-i  Sherman-Morrison vs numpy.linalg.inv of the row-replaced matrix      L299
+  P-j  sweep: sum of log|R| over accepted moves telescopes to the LU log-det difference
+  P-k  sweep: B_final^T A_final = I with A recomputed from the final positions
+  P-m  accept control flow (u = 0, u -> 1, zero displacement)               L195-199, eq. 12
+"""
+import itertools
+import math
+
+import numpy as np
+import pytest
+from scipy.interpolate import BSpline
+
+import oracle
+from paper_1802_06922_b200 import inputs
+
+SKEW = np.array([[3.1, 0.2, -0.1], [0.4, 2.7, 0.3], [-0.2, 0.5, 3.4]])
+ORTHO = np.diag([2.4, 3.0, 3.5])
+
+
+def rand_table(rng, grid, norb):
+    return rng.uniform(-1, 1, size=(*grid, norb)).astype(np.float32)
+
+
+def grid_coords(lat, grid, pos):
+    """Reduced grid coordinates s in [0, N_d) and J[j][d] = d s_d / d r_j, via numpy only."""
+    li = np.linalg.inv(lat)
+    u = pos @ li
+    u = u - np.floor(u)
+    s = u * np.asarray(grid, dtype=np.float64)
+    J = li * np.asarray(grid, dtype=np.float64)[None, :]
+    return s, J
+
+
+# ----------------------------------------------------------------------------- P-a
+@pytest.mark.parametrize("lat", [ORTHO, SKEW])
+def test_partition_of_unity(lat):
+    rng = np.random.default_rng(1)
+    grid, norb = (7, 5, 6), 3
+    coefs = np.empty((*grid, norb), dtype=np.float32)
+    coefs[..., 0], coefs[..., 1], coefs[..., 2] = 0.75, -2.5, 1.0
+    pos = rng.uniform(-2, 2, size=(50, 3)) @ lat
+    v, g, l = oracle.spline_vgl(coefs, lat, pos)
+    assert np.allclose(v, np.array([0.75, -2.5, 1.0])[None, :], atol=1e-14)
+    assert np.max(np.abs(g)) < 1e-13
+    assert np.max(np.abs(l)) < 1e-12
+
+
+# ----------------------------------------------------------------------------- P-b, P-c
+@pytest.mark.parametrize("lat", [ORTHO, SKEW])
+def test_polynomial_reproduction(lat):
+    """c = alpha + beta*ix -> phi = alpha + beta*(s_x + 1): control point m is supported on
+    [m-3, m+1) (eq. 33's convention), so the spline of c_i = i is s + 1.  c = ix^2 ->
+    (s_x+1)^2 + 1/3.  c = ix*iy -> (s_x+1)(s_y+1)."""
+    rng = np.random.default_rng(2)
+    grid = (16, 14, 12)
+    ix = np.arange(grid[0], dtype=np.float64)[:, None, None]
+    iy = np.arange(grid[1], dtype=np.float64)[None, :, None]
+    one = np.ones(grid)
+    alpha, beta = 0.5, 0.25
+    coefs = np.stack([alpha + beta * ix * one, ix * ix * one, ix * iy * one,
+                      (iy * iy * one)], axis=-1).astype(np.float32)
+    # stay away from the periodic wrap: s_d in [0, N_d - 4)
+    sfrac = rng.uniform(0, 1, size=(60, 3)) * (np.array(grid) - 4.0)
+    pos = (sfrac / np.array(grid)) @ lat
+    s, J = grid_coords(lat, grid, pos)
+    v, g, l = oracle.spline_vgl(coefs, lat, pos)
+    sx, sy = s[:, 0], s[:, 1]
+    assert np.allclose(v[:, 0], alpha + beta * (sx + 1), atol=1e-12)
+    assert np.allclose(v[:, 1], (sx + 1) ** 2 + 1.0 / 3.0, atol=1e-11)
+    assert np.allclose(v[:, 2], (sx + 1) * (sy + 1), atol=1e-11)
+    # gradients: d/dr_j = sum_d J[j][d] d/ds_d
+    for j in range(3):
+        assert np.allclose(g[:, j, 0], beta * J[j, 0], atol=1e-12)
+        assert np.allclose(g[:, j, 1], 2 * (sx + 1) * J[j, 0], atol=1e-10)
+        assert np.allclose(g[:, j, 2], (sy + 1) * J[j, 0] + (sx + 1) * J[j, 1], atol=1e-10)
+    assert np.max(np.abs(l[:, 0])) < 1e-11
+    assert np.allclose(l[:, 1], 2.0 * np.dot(J[:, 0], J[:, 0]), atol=1e-9)
+    assert np.allclose(l[:, 2], 2.0 * np.dot(J[:, 0], J[:, 1]), atol=1e-9)   # cross term
+    assert np.allclose(l[:, 3], 2.0 * np.dot(J[:, 1], J[:, 1]), atol=1e-9)
+
+
+def test_orthorhombic_gradient_scale():
+    """On an orthorhombic cell d/dx = (Nx/Lx) d/ds_x exactly."""
+    grid, L = (10, 10, 10), np.array([2.0, 4.0, 5.0])
+    iz = np.arange(10, dtype=np.float64)[None, None, :] * np.ones(grid)
+    coefs = iz[..., None].astype(np.float32)
+    pos = np.array([[0.3, 0.7, 1.1], [1.2, 3.3, 2.2]])
+    v, g, l = oracle.spline_vgl(coefs, np.diag(L), pos)
+    assert np.allclose(g[:, 2, 0], 10 / 5.0, atol=1e-13)
+    assert np.allclose(g[:, :2, 0], 0.0, atol=1e-13)
+    assert np.allclose(v[:, 0], pos[:, 2] / 5.0 * 10 + 1.0, atol=1e-13)
+
+
+# ----------------------------------------------------------------------------- P-d
+def test_planewave_nodes_closed_form():
+    """c = cos(kappa.i + theta), kappa_d = 2 pi n_d / N_d.  At the grid nodes (t = 0) the cubic
+    B-spline weights are (1,4,1,0)/6, whence phi = prod_d (2+cos kappa_d)/3 * cos(psi),
+    psi = kappa.(i+1) + theta;  d/ds_x -> -sin(kappa_x) * (...) sin(psi);
+    d2/ds_x2 -> 2(cos kappa_x - 1) (...) cos(psi).  Includes nodes that wrap in x and z."""
+    grid = (16, 12, 20)
+    nvec, theta = np.array([3, -2, 5]), 0.7
+    kap = 2 * np.pi * nvec / np.array(grid)
+    I = np.stack(np.meshgrid(*[np.arange(n) for n in grid], indexing="ij"), axis=-1)
+    coefs = np.cos(I @ kap + theta)[..., None].astype(np.float32)
+    cd = coefs[..., 0].astype(np.float64)          # the exact fp32 bits the oracle sees
+    lat = ORTHO
+    nodes = np.array([[2, 3, 4], [15, 5, 19], [14, 11, 18], [13, 0, 17], [0, 0, 0]])
+    pos = (nodes / np.array(grid)) @ lat
+    v, g, l = oracle.spline_vgl(coefs, lat, pos)
+    s, J = grid_coords(lat, grid, pos)
+    al = (2 + np.cos(kap)) / 3
+    for p, nd in enumerate(nodes):
+        psi = kap @ (nd + 1) + theta
+        phi = al.prod() * np.cos(psi)
+        # fp32 rounding of the table bounds the mismatch: |dc| <= 6e-8
+        assert abs(v[p, 0] - phi) < 2e-7
+        d1 = np.array([-np.sin(kap[d]) * al.prod() / al[d] * np.sin(psi) for d in range(3)])
+        d2 = np.array([2 * (np.cos(kap[d]) - 1) * al.prod() / al[d] * np.cos(psi) for d in range(3)])
+        assert np.allclose(g[p, :, 0], J @ d1, atol=2e-6)
+        assert abs(l[p, 0] - np.sum(np.diag(J) ** 2 * d2)) < 2e-5
+        # and exactly (to rounding) from the fp32 table itself with the node weights
+        w = np.array([1, 4, 1]) / 6.0
+        acc = 0.0
+        for a, b, c in itertools.product(range(3), repeat=3):
+            acc += w[a] * w[b] * w[c] * cd[(nd[0] + a) % 16, (nd[1] + b) % 12, (nd[2] + c) % 20]
+        assert abs(v[p, 0] - acc) < 1e-14
+
+
+# ----------------------------------------------------------------------------- P-e, P-f
+def test_periodicity_and_continuity():
+    rng = np.random.default_rng(3)
+    grid, norb = (6, 7, 5), 4
+    coefs = rand_table(rng, grid, norb)
+    lat = SKEW
+    pos = rng.uniform(0, 1, size=(20, 3)) @ lat
+    v0, g0, l0 = oracle.spline_vgl(coefs, lat, pos)
+    shift = np.array([[1, 0, 0], [0, -2, 1], [3, 1, -1]]) @ lat
+    for sh in shift:
+        v1, g1, l1 = oracle.spline_vgl(coefs, lat, pos + sh)
+        assert np.max(np.abs(v1 - v0)) < 1e-12
+        assert np.max(np.abs(g1 - g0)) < 1e-10
+        assert np.max(np.abs(l1 - l0)) < 1e-8
+    # C2 continuity across every cell face, incl. the periodic one (value, grad, lap)
+    eps = 1e-9
+    for d in range(3):
+        for face in range(grid[d] + 1):
+            u = rng.uniform(0.05, 0.95, size=3)
+            u[d] = face / grid[d]
+            um, up = u.copy(), u.copy()
+            um[d] -= eps / grid[d]
+            up[d] += eps / grid[d]
+            vm, gm, lm = oracle.spline_vgl(coefs, lat, (um @ lat)[None])
+            vp, gp, lp = oracle.spline_vgl(coefs, lat, (up @ lat)[None])
+            assert np.max(np.abs(vm - vp)) < 1e-7
+            assert np.max(np.abs(gm - gp)) < 1e-6
+            assert np.max(np.abs(lm - lp)) < 1e-4     # third derivative jumps: O(eps) gap
+
+
+# ----------------------------------------------------------------------------- P-s
+def _scipy_basis(n, s, nu):
+    """All basis values (nu-th derivative) of the uniform cubic B-spline with control point m
+    supported on [m-3, m+1): knots t_j = j - 3.  Returns [npts][n+3] for extended control
+    points m = 0..n+2 (m >= n wraps to m - n)."""
+    ncoef = n + 3
+    t = np.arange(-3, ncoef + 1, dtype=np.float64)
+    return BSpline(t, np.eye(ncoef), 3)(s, nu=nu)
+
+
+@pytest.mark.parametrize("lat", [ORTHO, SKEW])
+def test_against_scipy_bspline(lat):
+    rng = np.random.default_rng(4)
+    grid, norb = (6, 5, 7), 5
+    coefs = rand_table(rng, grid, norb)
+    pos = rng.uniform(-1, 2, size=(80, 3)) @ lat          # also outside the home cell
+    s, J = grid_coords(lat, grid, pos)
+    ext = coefs.astype(np.float64)
+    ext = np.concatenate([ext, ext[:3]], axis=0)
+    ext = np.concatenate([ext, ext[:, :3]], axis=1)
+    ext = np.concatenate([ext, ext[:, :, :3]], axis=2)
+    Bs = [[_scipy_basis(grid[d], s[:, d], nu) for nu in range(3)] for d in range(3)]
+
+    def contract(nx_, ny_, nz_):
+        return np.einsum("pi,pj,pk,ijkn->pn", Bs[0][nx_], Bs[1][ny_], Bs[2][nz_], ext)
+
+    v_ref = contract(0, 0, 0)
+    d1 = np.stack([contract(1, 0, 0), contract(0, 1, 0), contract(0, 0, 1)], axis=1)   # [p][d][n]
+    H = np.empty((len(pos), 3, 3, norb))
+    orders = {(0, 0): (2, 0, 0), (1, 1): (0, 2, 0), (2, 2): (0, 0, 2),
+              (0, 1): (1, 1, 0), (0, 2): (1, 0, 1), (1, 2): (0, 1, 1)}
+    for (d, e), o in orders.items():
+        H[:, d, e] = H[:, e, d] = contract(*o)
+    g_ref = np.einsum("jd,pdn->pjn", J, d1)
+    l_ref = np.einsum("jd,je,pden->pn", J, J, H)
+    v, g, l = oracle.spline_vgl(coefs, lat, pos)
+    assert np.max(np.abs(v - v_ref)) < 1e-13
+    assert np.max(np.abs(g - g_ref)) < 1e-12
+    assert np.max(np.abs(l - l_ref)) < 1e-11
+
+
+# ----------------------------------------------------------------------------- P-g
+def test_finite_differences():
+    x = inputs.make_inputs(inputs.custom_config("fd", (12, 10, 14), 6, SKEW * 2.0, nw=4))
+    coefs, lat = x.coefs_numpy(), x.lattice
+    pos = x.pos.reshape(-1, 3)[:12]
+    v, g, l = oracle.spline_vgl(coefs, lat, pos)
+    h = 1e-4 * 0.4
+    lap_fd = np.zeros_like(l)
+    for j in range(3):
+        e = np.zeros(3)
+        e[j] = h
+        vp = oracle.spline_vgl(coefs, lat, pos + e, want_gl=False)
+        vm = oracle.spline_vgl(coefs, lat, pos - e, want_gl=False)
+        gfd = (vp - vm) / (2 * h)
+        assert np.max(np.abs(gfd - g[:, j, :])) < 1e-7 * max(1.0, np.max(np.abs(g)))
+        lap_fd += (vp - 2 * v + vm) / (h * h)
+    assert np.max(np.abs(lap_fd - l)) < 1e-5 * max(1.0, np.max(np.abs(l)))
+
+
+# ----------------------------------------------------------------------------- P-h, P-i, LU
+def _leibniz_det(A):
+    n = A.shape[0]
+    tot = 0.0
+    for perm in itertools.permutations(range(n)):
+        sgn = 1
+        for i in range(n):
+            for j in range(i + 1, n):
+                if perm[i] > perm[j]:
+                    sgn = -sgn
+        tot += sgn * math.prod(A[i, perm[i]] for i in range(n))
+    return tot
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 5, 6])
+def test_ratio_vs_leibniz(n):
+    rng = np.random.default_rng(10 + n)
+    A = rng.normal(size=(n, n))
+    B, ld, sg = oracle.binv_from_A(A)
+    d0 = _leibniz_det(A)
+    assert abs(sg * math.exp(ld) - d0) < 1e-12 * max(1, abs(d0))
+    for k in range(n):
+        phi = rng.normal(size=n)
+        A2 = A.copy()
+        A2[k] = phi
+        assert abs(oracle.det_ratio(B, k, phi) - _leibniz_det(A2) / d0) < 1e-10 * max(1, abs(_leibniz_det(A2) / d0))
+
+
+@pytest.mark.parametrize("n", [4, 11, 16])
+def test_ratio_and_sm_vs_numpy(n):
+    rng = np.random.default_rng(20 + n)
+    A = rng.normal(size=(n, n))
+    B, ld, sg = oracle.binv_from_A(A)
+    sgn_np, ld_np = np.linalg.slogdet(A)
+    assert sg == int(sgn_np) and abs(ld - ld_np) < 1e-11
+    assert np.max(np.abs(B.T - np.linalg.inv(A))) < 1e-10
+    Ai, ld2, sg2 = oracle.lu_inverse(A)
+    assert np.max(np.abs(Ai @ A - np.eye(n))) < 1e-11
+    for k in [0, n // 2, n - 1]:
+        phi = rng.normal(size=n)
+        A2 = A.copy()
+        A2[k] = phi
+        R = oracle.det_ratio(B, k, phi)
+        assert abs(R - np.linalg.det(A2) / np.linalg.det(A)) < 1e-9 * max(1, abs(R))
+        B2 = oracle.sm_update(B, k, phi, R)
+        assert np.max(np.abs(B2.T - np.linalg.inv(A2))) < 1e-8 * max(1.0, np.max(np.abs(B2)))
+        # chain: keep moving from the updated state
+        A, B = A2, B2
+
+
+def test_sm_64_vs_direct_inverse():
+    rng = np.random.default_rng(31)
+    n = 64
+    A = rng.normal(size=(n, n))
+    B, _, _ = oracle.binv_from_A(A)
+    for k in range(n):
+        phi = rng.normal(size=n)
+        R = oracle.det_ratio(B, k, phi)
+        B = oracle.sm_update(B, k, phi, R)
+        A[k] = phi
+    assert np.max(np.abs(B.T - np.linalg.inv(A))) < 1e-9 * np.max(np.abs(B))
+
+
+def test_lu_flags_singular():
+    A = np.array([[1.0, 2.0, 3.0], [2.0, 4.0, 6.0], [0.0, 1.0, 1.0]])
+    with pytest.raises(RuntimeError):
+        oracle.lu_inverse(A)
+
+
+def test_lu_needs_pivoting():
+    A = np.array([[0.0, 1.0], [1.0, 0.0]])
+    Ai, ld, sg = oracle.lu_inverse(A)
+    assert sg == -1 and abs(ld) < 1e-15 and np.allclose(Ai, A)
+
+
+# ----------------------------------------------------------------------------- sweeps
+@pytest.fixture(scope="module")
+def sweep_case():
+    cfg = inputs.custom_config("sweep", (12, 10, 14), 24, SKEW * 2.0, nw=3, nsweeps=2, sigma=0.25)
+    x = inputs.make_inputs(cfg)
+    coefs = x.coefs_numpy()
+    A = oracle.slater_matrix(coefs, x.lattice, x.pos)
+    B = np.empty_like(A)
+    ld = np.empty(cfg.nw)
+    sg = np.empty(cfg.nw, dtype=np.int32)
+    for w in range(cfg.nw):
+        B[w], ld[w], sg[w] = oracle.binv_from_A(A[w])
+    return x, coefs, A, B, ld, sg
+
+
+def test_slater_matrix_layout(sweep_case):
+    """A[w][i][j] = phi_j(r_wi) (L325): row = electron, column = orbital."""
+    x, coefs, A, *_ = sweep_case
+    v = oracle.spline_vgl(coefs, x.lattice, x.pos[1, 5][None], want_gl=False)
+    assert np.array_equal(A[1, 5], v[0])
+
+
+def test_sweep_telescoping_and_inverse(sweep_case):
+    x, coefs, A, B, ld, sg = sweep_case
+    out = oracle.sweep(coefs, x.lattice, x.pos, B, ld, sg, x.delta, x.unif, A=A)
+    acc = out["accept"].astype(bool)
+    assert 0 < acc.sum() < acc.size
+    A_fin = oracle.slater_matrix(coefs, x.lattice, out["pos"])
+    assert np.max(np.abs(A_fin - out["A"])) < 1e-13
+    for w in range(x.cfg.nw):
+        s_np, l_np = np.linalg.slogdet(A_fin[w])
+        s0, l0 = np.linalg.slogdet(A[w])
+        tele = np.sum(np.log(np.abs(out["ratios"][..., w][acc[..., w]])))
+        assert abs(tele - (l_np - l0)) < 1e-8
+        assert abs(out["logdet"][w] - l_np) < 1e-8
+        assert out["sign"][w] == int(s_np)
+        res = out["B"][w].T @ A_fin[w] - np.eye(x.cfg.norb)
+        assert np.max(np.sum(np.abs(res), axis=1)) < 1e-8
+    # decisions follow eq. 12: accept iff R^2 > u
+    assert np.array_equal(acc, out["ratios"] ** 2 > x.unif)
+    # accepted electrons moved by exactly delta, rejected ones stayed
+    moved = np.zeros_like(x.pos)
+    for s in range(x.cfg.nsweeps):
+        moved += np.where(acc[s].T[..., None], np.transpose(x.delta[s], (1, 0, 2)), 0.0)
+    assert np.max(np.abs(out["pos"] - (x.pos + moved))) < 1e-14
+
+
+def test_sweep_sm_equals_definitional(sweep_case):
+    """Mode 0 (Sherman-Morrison) reaches the result of mode 1 (LU recompute after every
+    accepted move) to rounding."""
+    x, coefs, A, B, ld, sg = sweep_case
+    o0 = oracle.sweep(coefs, x.lattice, x.pos, B, ld, sg, x.delta, x.unif, A=A, mode=0)
+    o1 = oracle.sweep(coefs, x.lattice, x.pos, B, ld, sg, x.delta, x.unif, A=A, mode=1)
+    assert np.array_equal(o0["accept"], o1["accept"])
+    assert np.max(np.abs(o0["ratios"] - o1["ratios"])) < 1e-9
+    assert np.max(np.abs(o0["B"] - o1["B"])) < 1e-9 * max(1.0, np.max(np.abs(o1["B"])))
+
+
+def test_sweep_forced_and_replay(sweep_case):
+    x, coefs, A, B, ld, sg = sweep_case
+    free = oracle.sweep(coefs, x.lattice, x.pos, B, ld, sg, x.delta, x.unif, A=A, want_phi=True)
+    forced = oracle.sweep(coefs, x.lattice, x.pos, B, ld, sg, x.delta, 1.0 - x.unif, A=A,
+                          forced=free["accept"])
+    assert np.array_equal(forced["accept"], free["accept"])
+    assert np.array_equal(forced["B"], free["B"]) and np.array_equal(forced["pos"], free["pos"])
+    # replay of recorded orbital vectors (here rounded to fp32 -> small, nonzero change)
+    phi32 = free["phi"].astype(np.float32)
+    rep = oracle.sweep(coefs, x.lattice, x.pos, B, ld, sg, x.delta, x.unif, forced=free["accept"],
+                       phi_in=phi32)
+    assert 0 < np.max(np.abs(rep["B"] - free["B"])) < 1e-4 * np.max(np.abs(free["B"]))
+    # partial sweep: only the first 5 electrons are moved
+    part = oracle.sweep(coefs, x.lattice, x.pos, B, ld, sg, x.delta[:1], x.unif[:1], iel_count=5)
+    assert np.array_equal(part["accept"][0, :5], free["accept"][0, :5])
+    assert not part["accept"][0, 5:].any()
+    assert np.array_equal(part["pos"][:, 5:], x.pos[:, 5:])
+
+
+def test_accept_control_flow(sweep_case):
+    x, coefs, A, B, ld, sg = sweep_case
+    zeros = np.zeros_like(x.unif)
+    out = oracle.sweep(coefs, x.lattice, x.pos, B, ld, sg, x.delta, zeros)
+    assert out["accept"].all()                       # R != 0 w.p. 1  ->  R^2 > 0
+    tot = np.transpose(x.delta.sum(axis=0), (1, 0, 2))
+    assert np.max(np.abs(out["pos"] - (x.pos + tot))) < 1e-13
+    ones = np.full_like(x.unif, 1.0 - 2.0 ** -53)
+    out1 = oracle.sweep(coefs, x.lattice, x.pos, B, ld, sg, x.delta, ones)
+    assert np.array_equal(out1["accept"].astype(bool), np.abs(out1["ratios"]) >= 1.0)
+    # zero displacement: the new row equals the old one -> R = 1, B unchanged
+    nod = oracle.sweep(coefs, x.lattice, x.pos, B, ld, sg, np.zeros_like(x.delta), zeros)
+    assert np.max(np.abs(nod["ratios"] - 1.0)) < 1e-10
+    assert np.max(np.abs(nod["B"] - B)) < 1e-9 * np.max(np.abs(B))
+    assert np.array_equal(nod["pos"], x.pos)
+    # multi-threaded run gives the same bits (walkers are independent, L181)
+    out_mt = oracle.sweep(coefs, x.lattice, x.pos, B, ld, sg, x.delta, x.unif, nthreads=3)
+    out_st = oracle.sweep(coefs, x.lattice, x.pos, B, ld, sg, x.delta, x.unif, nthreads=1)
+    assert np.array_equal(out_mt["B"], out_st["B"]) and np.array_equal(out_mt["ratios"], out_st["ratios"])
