@@ -1,0 +1,204 @@
+/*
+ * qmc_b200.h -- C ABI of libqmcb200.so: the data-parallel hot path of the real-space
+ * VMC/DMC particle-by-particle move (arxiv 1802.06922, "QMCPACK: an open source ab initio
+ * quantum Monte Carlo package ..."), hand-written CUDA for one B200 (sm_100a).
+ *
+ * Citations are PAPER.md line numbers (+ section / equation).  "R:Ax" is a reading listed in
+ * DESIGN.md section 3, used where the paper is silent.
+ *
+ * Conventions for every call
+ *   - returns QMC_OK (0) or a negative QMC_E* code; qmc_last_error() gives a thread-local
+ *     message.  Never aborts, never throws, never falls back to the CPU.
+ *   - "dev" pointers are CUDA device pointers on the current device, "host" pointers are
+ *     ordinary host memory.  Every buffer passed in is caller-owned; handles own their
+ *     internal device storage until the matching *_destroy call.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Calls
+ *     enqueue work on it and do not synchronise unless stated.
+ *   - all arrays are dense row-major with the stated leading dimensions.
+ *   - one GPU; walkers are independent Markov chains (L181), so multi-GPU use is one library
+ *     instance per rank with the walkers partitioned.
+ */
+#ifndef QMC_B200_H
+#define QMC_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define QMC_OK 0
+#define QMC_EINVAL (-1)    /* bad argument (shape, alignment, NULL, handle mismatch)      */
+#define QMC_ENOMEM (-2)    /* device or host allocation failed                            */
+#define QMC_ECUDA (-3)     /* a CUDA runtime call failed; message holds cudaGetErrorString */
+#define QMC_ESINGULAR (-4) /* a Slater matrix had a zero / non-finite pivot in qmc_det_init */
+
+#define QMC_MAX_DELAY 32   /* largest delayed-update rank accepted by qmc_det_init        */
+
+typedef struct qmc_spline qmc_spline_t; /* opaque: padded fp32 coefficient table on device */
+typedef struct qmc_det qmc_det_t;       /* opaque: per-walker fp64 inverse + scratch       */
+
+/* Thread-local text of the last error raised on this thread ("" if none). */
+const char *qmc_last_error(void);
+
+/* ---------------------------------------------------------------------------------------
+ * qmc_spline_create -- PAPER.md L307-311 (sec 6.2.1): single-particle orbitals "converted into
+ * a regular 3D B-spline representation in real-space"; "spline coefficients may also be stored
+ * in single precision" (L311); one read-only table per GPU shared by all walkers (L311, L114).
+ *
+ *   nx,ny,nz   grid points per cell edge (>= 1; periodic, L307)
+ *   norb       number of orbitals N (>= 1)
+ *   lattice    host, 9 doubles row-major, rows = cell vectors a0,a1,a2 (r = u . lattice);
+ *              must be invertible.  General (skewed) cells are supported (R:A5).
+ *   coefs      canonical table float [nx][ny][nz][norb], orbital index innermost, periodic,
+ *              no halo (R:A3, R:A4); host memory if coefs_on_device == 0, else device memory.
+ *   The library builds and OWNS a padded device copy [nx][ny][nz][Np], Np = norb rounded up
+ *   to a multiple of 32 floats (128-byte rows; pad = 0), so the caller may free `coefs` after
+ *   the stream has drained.  With coefs_on_device != 0 and norb % 32 == 0 the padded copy is a
+ *   plain device-to-device copy.
+ * Errors: QMC_EINVAL (sizes, NULL, singular lattice), QMC_ENOMEM, QMC_ECUDA.
+ */
+int qmc_spline_create(qmc_spline_t **out, int nx, int ny, int nz, int norb,
+                      const double *lattice, const float *coefs, int coefs_on_device,
+                      void *stream);
+int qmc_spline_destroy(qmc_spline_t *spline);
+/* Row pitch Np (floats) and bytes of the padded device table; either pointer may be NULL. */
+int qmc_spline_info(const qmc_spline_t *spline, int *row_pitch, size_t *table_bytes);
+
+/* ---------------------------------------------------------------------------------------
+ * qmc_spo_vgl -- value, Cartesian gradient and Laplacian of all N orbitals at npos positions:
+ * "a constant 64 coefficients to be accessed in memory to evaluate each single-particle
+ * wavefunction" (L309).  Uniform cubic B-spline (R:A1), control points i..i+3 (mod N_d) per
+ * dimension with i = floor(s), s = frac(r . lattice^-1) * N_d (R:A2, the support convention of
+ * eq. 33; R:A7 at cell faces).  Index and fraction in fp64, the 64 x {v,gx,gy,gz,lap}
+ * stencil weights rounded to fp32, fp32 accumulation in a fixed order (bit-reproducible,
+ * independent of the batch, R:A11).
+ *
+ *   pos   dev, double [npos][3], Cartesian, any image of the cell
+ *   v     dev, float [npos][ldo]        phi_n(r_p)
+ *   g     dev, float [npos][3][ldo]     d phi_n / d r_j ; may be NULL
+ *   l     dev, float [npos][ldo]        Laplacian        ; may be NULL (g and l together)
+ *   ldo   leading dimension of the outputs: >= norb, multiple of 4; v,g,l 16-byte aligned.
+ *         Elements norb..ldo-1 of each row are written with zeros up to the table pitch.
+ * npos == 0 is a no-op.  Errors: QMC_EINVAL, QMC_ECUDA.
+ */
+int qmc_spo_vgl(const qmc_spline_t *spline, int npos, const double *pos, float *v, float *g,
+                float *l, int ldo, void *stream);
+
+/* ---------------------------------------------------------------------------------------
+ * qmc_det_init -- Slater matrices M_ij = phi_j(r_i) (L325) of nwalkers walkers ("multiple
+ * walkers can be assigned to each GPU", L114), their inverses in fp64, log|det| and sign.
+ *
+ *   nel         electrons in this determinant; must equal the spline's norb
+ *   pos         dev, double [nwalkers][nel][3]
+ *   delay_rank  0 or 1: Sherman-Morrison rank-1 update on every accepted move (L299, [49]);
+ *               2..QMC_MAX_DELAY: delayed update (L112, L299, [44]) -- accepted rows are
+ *               buffered and applied as one rank-k contraction (R:A14).
+ * The handle owns B_w = (A_w^-1)^T as double [nwalkers][nel][ld] (row k of B is column k of
+ * A^-1, "the moved electron's inverse-matrix row"), ld = nel rounded up to 64 doubles, pad 0.
+ * The orbital values come from qmc_spo_vgl (fp32, upcast; R:A16); the inverse is an in-place
+ * Gauss-Jordan elimination with partial pivoting, all on the device.
+ * Synchronises `stream` once (to report singularity).
+ * Errors: QMC_EINVAL, QMC_ENOMEM, QMC_ECUDA, QMC_ESINGULAR (handle not created).
+ */
+int qmc_det_init(qmc_det_t **out, const qmc_spline_t *spline, int nwalkers, int nel,
+                 const double *pos, int delay_rank, void *stream);
+int qmc_det_destroy(qmc_det_t *det);
+
+/* ---------------------------------------------------------------------------------------
+ * qmc_det_ratio -- L299: for a single-electron move of electron iel to a position where the
+ * orbitals take the values phi, det A'/det A = sum_j B[iel][j] * phi[j] (fp64 accumulation of
+ * the upcast fp32 orbital vector; warp-shuffle tree, fixed order).  With a delayed window open
+ * the pending accepted rows are included (R:O7).
+ *
+ *   phi    dev, float [nwalkers][ldo], ldo >= nel
+ *   ratio  dev, double [nwalkers] (out)
+ */
+int qmc_det_ratio(qmc_det_t *det, int iel, const float *phi, int ldo, double *ratio,
+                  void *stream);
+
+/* ---------------------------------------------------------------------------------------
+ * qmc_det_accept_update -- L299 "for single electron moves, QMCPACK uses the Sherman-Morrison
+ * algorithm": for every walker with accept[w] != 0, row iel of A_w is replaced by phi_w and
+ *     B'[m][j] = B[m][j] - ((B[m] . phi) - delta_{m,iel}) * B[iel][j] / ratio_w
+ * in ONE pass over B (each row read once, dotted, updated, written: 16*nel*ld bytes per
+ * accepted walker).  log|det| += log|ratio|, sign *= sgn(ratio), accept counter += 1.
+ * Walkers with accept[w] == 0 are untouched.  With delay_rank >= 2 the row is appended to the
+ * walker's window instead and the window is flushed when any walker's window is full.
+ *
+ *   phi, ldo  as in qmc_det_ratio (the vector the ratio was computed from)
+ *   ratio     dev, double [nwalkers]: the values qmc_det_ratio returned
+ *   accept    dev, unsigned char [nwalkers]
+ */
+int qmc_det_accept_update(qmc_det_t *det, int iel, const float *phi, int ldo,
+                          const double *ratio, const unsigned char *accept, void *stream);
+
+/* Apply all pending delayed updates (no-op for delay_rank <= 1). */
+int qmc_det_flush(qmc_det_t *det, void *stream);
+
+/* ---------------------------------------------------------------------------------------
+ * qmc_sweep -- L195-199 (sec 5.2.1): "particle-by-particle moves work by iterating
+ * sequentially over all electrons"; all walkers advance in lockstep (L114, L181).  For sweep s,
+ * electron k, walker w:  r' = pos[w][k] + delta[s][k][w]  (eq. 13 with F = 0, pre-generated
+ * Gaussian);  phi, grad, lap = SPO-VGL(r');  R = B_w[k] . phi;  accept iff R*R > u[s][k][w]
+ * (eq. 12 with symmetric T and a determinant-only Psi, R:A8; non-finite R rejects); on accept
+ * pos[w][k] = r' (stored unwrapped) and the inverse is updated as in qmc_det_accept_update.
+ * Pending delayed updates are flushed at the end of every sweep.
+ *
+ *   pos            dev, double [nwalkers][nel][3], in/out.  Must be the positions the handle's
+ *                  inverse corresponds to.
+ *   delta          dev, double [nsweeps][nel][nwalkers][3]
+ *   uniforms       dev, double [nsweeps][nel][nwalkers], in [0,1)
+ *   ratios_out     dev, double [nsweeps][nel][nwalkers] or NULL
+ *   accept_out     dev, unsigned char, same shape, or NULL
+ *   forced_accept  NULL, or dev unsigned char (same shape): decisions to impose instead of the
+ *                  Metropolis test (parity protocol)
+ */
+int qmc_sweep(qmc_det_t *det, const qmc_spline_t *spline, double *pos, const double *delta,
+              const double *uniforms, int nsweeps, double *ratios_out,
+              unsigned char *accept_out, const unsigned char *forced_accept, void *stream);
+
+/* Options of qmc_sweep_ex; zero-initialise for the qmc_sweep behaviour. */
+typedef struct qmc_sweep_opts {
+    int iel_begin;       /* first electron moved in each sweep (default 0)                   */
+    int iel_count;       /* electrons moved per sweep; 0 = nel - iel_begin                   */
+    float *phi_record;   /* NULL, or dev float [nsweeps][nel][nrecord][nel]: the fp32 orbital */
+    int nrecord;         /*   vector of every move of walkers 0..nrecord-1 (parity replay)   */
+    int use_graph;       /* 1: replay one electron step as a captured CUDA graph             */
+    int reserved[3];
+} qmc_sweep_opts_t;
+
+int qmc_sweep_ex(qmc_det_t *det, const qmc_spline_t *spline, double *pos, const double *delta,
+                 const double *uniforms, int nsweeps, double *ratios_out,
+                 unsigned char *accept_out, const unsigned char *forced_accept,
+                 const qmc_sweep_opts_t *opts, void *stream);
+
+/* Same as qmc_sweep with HOST buffers (pos in/out; ratios_out / accept_out may be NULL):
+ * copies the inputs to the device, runs the sweeps, copies pos, ratios and decisions back and
+ * synchronises `stream`.  Host buffers should be page-locked for full copy bandwidth. */
+int qmc_sweep_host(qmc_det_t *det, const qmc_spline_t *spline, double *pos_host,
+                   const double *delta_host, const double *uniforms_host, int nsweeps,
+                   double *ratios_out_host, unsigned char *accept_out_host, void *stream);
+
+/* ---------------------------------------------------------------------------------------
+ * State access (checkpoint / parity).  Pending delayed updates are flushed first.
+ *   qmc_det_get_inverse   binv_out dev double [nwalkers][nel][nel] dense, B = (A^-1)^T
+ *   qmc_det_set_inverse   the reverse (binv_in dense); logdet / sign dev arrays or NULL (kept)
+ *   qmc_det_get_stats     dev: logdet double [nwalkers], sign int [nwalkers],
+ *                         naccept long long [nwalkers]; any may be NULL
+ *   qmc_det_info          nwalkers, nel, ld (doubles), delay_rank; any may be NULL
+ */
+int qmc_det_get_inverse(qmc_det_t *det, double *binv_out, void *stream);
+int qmc_det_set_inverse(qmc_det_t *det, const double *binv_in, const double *logdet,
+                        const int *sign, void *stream);
+int qmc_det_get_stats(qmc_det_t *det, double *logdet, int *sign, long long *naccept,
+                      void *stream);
+int qmc_det_info(const qmc_det_t *det, int *nwalkers, int *nel, int *ld, int *delay_rank);
+
+/* Number of kernel launches this library has enqueued since load (bench.py's gpu_launches). */
+long long qmc_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QMC_B200_H */

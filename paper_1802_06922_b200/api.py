@@ -1,0 +1,291 @@
+"""Thin ctypes binding of libqmcb200.so (include/qmc_b200.h): argument marshalling only.
+
+Every step of the hot path runs in the CUDA library; torch is used for device memory and
+streams.  There is no CPU fallback: a missing library or a failing call raises.
+Names follow the C ABI: Spline.create -> qmc_spline_create, spo_vgl -> qmc_spo_vgl, ...
+"""
+import ctypes
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libqmcb200.so")
+_lib = None
+
+QMC_MAX_DELAY = 32
+_vp = ctypes.c_void_p
+
+EXPORTS = [
+    "qmc_last_error", "qmc_spline_create", "qmc_spline_destroy", "qmc_spline_info", "qmc_spo_vgl",
+    "qmc_det_init", "qmc_det_destroy", "qmc_det_ratio", "qmc_det_accept_update", "qmc_det_flush",
+    "qmc_sweep", "qmc_sweep_ex", "qmc_sweep_host", "qmc_det_get_inverse", "qmc_det_set_inverse",
+    "qmc_det_get_stats", "qmc_det_info", "qmc_launch_count",
+]
+
+
+class SweepOpts(ctypes.Structure):
+    _fields_ = [("iel_begin", ctypes.c_int), ("iel_count", ctypes.c_int),
+                ("phi_record", _vp), ("nrecord", ctypes.c_int), ("use_graph", ctypes.c_int),
+                ("reserved", ctypes.c_int * 3)]
+
+
+class QmcError(RuntimeError):
+    pass
+
+
+def load_library(path=None):
+    """dlopen the CUDA library; raises if it has not been built (no fallback)."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    path = path or LIB_PATH
+    if not os.path.exists(path):
+        raise QmcError(f"{path} is missing: run `python -m paper_1802_06922_b200.build` "
+                       "(there is no CPU fallback)")
+    lib = ctypes.CDLL(path)
+    i, d = ctypes.c_int, ctypes.c_double
+    lib.qmc_last_error.restype = ctypes.c_char_p
+    lib.qmc_last_error.argtypes = []
+    lib.qmc_launch_count.restype = ctypes.c_longlong
+    lib.qmc_launch_count.argtypes = []
+    sigs = {
+        "qmc_spline_create": [ctypes.POINTER(_vp), i, i, i, i, ctypes.POINTER(d), _vp, i, _vp],
+        "qmc_spline_destroy": [_vp],
+        "qmc_spline_info": [_vp, ctypes.POINTER(i), ctypes.POINTER(ctypes.c_size_t)],
+        "qmc_spo_vgl": [_vp, i, _vp, _vp, _vp, _vp, i, _vp],
+        "qmc_det_init": [ctypes.POINTER(_vp), _vp, i, i, _vp, i, _vp],
+        "qmc_det_destroy": [_vp],
+        "qmc_det_ratio": [_vp, i, _vp, i, _vp, _vp],
+        "qmc_det_accept_update": [_vp, i, _vp, i, _vp, _vp, _vp],
+        "qmc_det_flush": [_vp, _vp],
+        "qmc_sweep": [_vp, _vp, _vp, _vp, _vp, i, _vp, _vp, _vp, _vp],
+        "qmc_sweep_ex": [_vp, _vp, _vp, _vp, _vp, i, _vp, _vp, _vp, ctypes.POINTER(SweepOpts), _vp],
+        "qmc_sweep_host": [_vp, _vp, _vp, _vp, _vp, i, _vp, _vp, _vp],
+        "qmc_det_get_inverse": [_vp, _vp, _vp],
+        "qmc_det_set_inverse": [_vp, _vp, _vp, _vp, _vp],
+        "qmc_det_get_stats": [_vp, _vp, _vp, _vp, _vp],
+        "qmc_det_info": [_vp] + [ctypes.POINTER(i)] * 4,
+    }
+    for name, args in sigs.items():
+        fn = getattr(lib, name)
+        fn.restype = i
+        fn.argtypes = args
+    _lib = lib
+    return lib
+
+
+def _check(rc, what):
+    if rc != 0:
+        msg = load_library().qmc_last_error().decode(errors="replace")
+        raise QmcError(f"{what} failed ({rc}): {msg}")
+
+
+def _stream(stream=None):
+    s = torch.cuda.current_stream() if stream is None else stream
+    return _vp(s.cuda_stream)
+
+
+def _ptr(t, dtype=None, allow_none=False):
+    if t is None:
+        if allow_none:
+            return None
+        raise QmcError("tensor required")
+    if dtype is not None and t.dtype != dtype:
+        raise QmcError(f"expected {dtype}, got {t.dtype}")
+    if not t.is_contiguous():
+        raise QmcError("tensor must be contiguous")
+    return _vp(t.data_ptr())
+
+
+def _dev(t, dtype, allow_none=False):
+    if t is not None and not t.is_cuda:
+        raise QmcError("device tensor required")
+    return _ptr(t, dtype, allow_none)
+
+
+def launch_count():
+    return int(load_library().qmc_launch_count())
+
+
+class Spline:
+    """qmc_spline_t: the padded fp32 coefficient table on the device."""
+
+    def __init__(self, handle, grid, norb):
+        self._h = handle
+        self.grid = tuple(grid)
+        self.norb = int(norb)
+        rp, tb = ctypes.c_int(0), ctypes.c_size_t(0)
+        _check(load_library().qmc_spline_info(self._h, ctypes.byref(rp), ctypes.byref(tb)), "qmc_spline_info")
+        self.row_pitch, self.table_bytes = rp.value, tb.value
+
+    @classmethod
+    def create(cls, coefs, lattice, stream=None):
+        """coefs: float32 [nx][ny][nz][norb] tensor (host or device); lattice: 3x3 (rows = cell vectors)."""
+        lib = load_library()
+        if coefs.dtype != torch.float32 or coefs.dim() != 4 or not coefs.is_contiguous():
+            raise QmcError("coefs must be a contiguous float32 [nx][ny][nz][norb] tensor")
+        nx, ny, nz, norb = coefs.shape
+        lat = (ctypes.c_double * 9)(*[float(x) for x in torch.as_tensor(lattice, dtype=torch.float64).reshape(9)])
+        h = _vp()
+        rc = lib.qmc_spline_create(ctypes.byref(h), nx, ny, nz, norb, lat, _vp(coefs.data_ptr()),
+                                   1 if coefs.is_cuda else 0, _stream(stream))
+        _check(rc, "qmc_spline_create")
+        if not coefs.is_cuda:
+            torch.cuda.synchronize()
+        return cls(h, (nx, ny, nz), norb)
+
+    def destroy(self):
+        if self._h:
+            _check(load_library().qmc_spline_destroy(self._h), "qmc_spline_destroy")
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def spo_vgl(spline, pos, want_gl=True, ldo=None, stream=None):
+    """qmc_spo_vgl: pos double [npos][3] (device) -> v [npos][ldo], g [npos][3][ldo], l [npos][ldo] (float32)."""
+    lib = load_library()
+    pos = pos.reshape(-1, 3)
+    npos = pos.shape[0]
+    ldo = spline.row_pitch if ldo is None else int(ldo)
+    v = torch.empty((npos, ldo), dtype=torch.float32, device=pos.device)
+    g = torch.empty((npos, 3, ldo), dtype=torch.float32, device=pos.device) if want_gl else None
+    l = torch.empty((npos, ldo), dtype=torch.float32, device=pos.device) if want_gl else None
+    rc = lib.qmc_spo_vgl(spline._h, npos, _dev(pos, torch.float64), _dev(v, None), _dev(g, None, True),
+                         _dev(l, None, True), ldo, _stream(stream))
+    _check(rc, "qmc_spo_vgl")
+    return (v, g, l) if want_gl else v
+
+
+def spo_vgl_into(spline, pos, v, g, l, stream=None):
+    """qmc_spo_vgl into caller-provided outputs (no allocation; for timing loops)."""
+    rc = load_library().qmc_spo_vgl(spline._h, pos.shape[0], _dev(pos, torch.float64), _dev(v, torch.float32),
+                                    _dev(g, torch.float32, True), _dev(l, torch.float32, True), v.shape[-1],
+                                    _stream(stream))
+    _check(rc, "qmc_spo_vgl")
+
+
+class Det:
+    """qmc_det_t: fp64 (A^-1)^T of every walker plus scratch."""
+
+    def __init__(self, handle, spline):
+        self._h = handle
+        self.spline = spline
+        lib = load_library()
+        a, b, c, e = ctypes.c_int(), ctypes.c_int(), ctypes.c_int(), ctypes.c_int()
+        _check(lib.qmc_det_info(self._h, ctypes.byref(a), ctypes.byref(b), ctypes.byref(c), ctypes.byref(e)),
+               "qmc_det_info")
+        self.nw, self.nel, self.ld, self.delay_rank = a.value, b.value, c.value, e.value
+
+    @classmethod
+    def init(cls, spline, pos, delay_rank=0, stream=None):
+        """qmc_det_init: pos double [nw][nel][3] on the device."""
+        lib = load_library()
+        nw, nel, _ = pos.shape
+        h = _vp()
+        rc = lib.qmc_det_init(ctypes.byref(h), spline._h, nw, nel, _dev(pos, torch.float64), int(delay_rank),
+                              _stream(stream))
+        _check(rc, "qmc_det_init")
+        return cls(h, spline)
+
+    def destroy(self):
+        if self._h:
+            _check(load_library().qmc_det_destroy(self._h), "qmc_det_destroy")
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def ratio(self, iel, phi, stream=None):
+        """qmc_det_ratio: phi float32 [nw][ldo] -> ratio double [nw]."""
+        out = torch.empty(self.nw, dtype=torch.float64, device=phi.device)
+        rc = load_library().qmc_det_ratio(self._h, int(iel), _dev(phi, torch.float32), phi.shape[-1],
+                                          _dev(out, None), _stream(stream))
+        _check(rc, "qmc_det_ratio")
+        return out
+
+    def accept_update(self, iel, phi, ratio, accept, stream=None):
+        """qmc_det_accept_update: accept uint8 [nw]."""
+        rc = load_library().qmc_det_accept_update(self._h, int(iel), _dev(phi, torch.float32), phi.shape[-1],
+                                                  _dev(ratio, torch.float64), _dev(accept, torch.uint8),
+                                                  _stream(stream))
+        _check(rc, "qmc_det_accept_update")
+
+    def flush(self, stream=None):
+        _check(load_library().qmc_det_flush(self._h, _stream(stream)), "qmc_det_flush")
+
+    def get_inverse(self, stream=None):
+        """B = (A^-1)^T as double [nw][nel][nel]."""
+        dev = torch.device("cuda", torch.cuda.current_device())
+        out = torch.empty((self.nw, self.nel, self.nel), dtype=torch.float64, device=dev)
+        _check(load_library().qmc_det_get_inverse(self._h, _dev(out, None), _stream(stream)), "qmc_det_get_inverse")
+        return out
+
+    def set_inverse(self, binv, logdet=None, sign=None, stream=None):
+        rc = load_library().qmc_det_set_inverse(self._h, _dev(binv, torch.float64),
+                                                _dev(logdet, torch.float64, True),
+                                                _dev(sign, torch.int32, True), _stream(stream))
+        _check(rc, "qmc_det_set_inverse")
+
+    def get_stats(self, stream=None):
+        """(logdet double [nw], sign int32 [nw], naccept int64 [nw])."""
+        dev = torch.device("cuda", torch.cuda.current_device())
+        ld = torch.empty(self.nw, dtype=torch.float64, device=dev)
+        sg = torch.empty(self.nw, dtype=torch.int32, device=dev)
+        na = torch.empty(self.nw, dtype=torch.int64, device=dev)
+        rc = load_library().qmc_det_get_stats(self._h, _dev(ld, None), _dev(sg, None), _dev(na, None),
+                                              _stream(stream))
+        _check(rc, "qmc_det_get_stats")
+        return ld, sg, na
+
+
+def sweep(det, pos, delta, unif, ratios_out=None, accept_out=None, forced_accept=None, iel_begin=0,
+          iel_count=0, phi_record=None, nrecord=0, stream=None):
+    """qmc_sweep / qmc_sweep_ex on device tensors (pos updated in place).
+
+    pos double [nw][nel][3]; delta double [nsweeps][nel][nw][3]; unif double [nsweeps][nel][nw];
+    ratios_out double / accept_out uint8 / forced_accept uint8: [nsweeps][nel][nw] or None;
+    phi_record float32 [nsweeps][nel][nrecord][nel] or None.
+    """
+    lib = load_library()
+    nsweeps = delta.shape[0]
+    if tuple(delta.shape) != (nsweeps, det.nel, det.nw, 3) or tuple(unif.shape) != (nsweeps, det.nel, det.nw):
+        raise QmcError("delta / unif shapes do not match the determinant")
+    if tuple(pos.shape) != (det.nw, det.nel, 3):
+        raise QmcError("pos shape does not match the determinant")
+    for t in (ratios_out, accept_out, forced_accept):
+        if t is not None and tuple(t.shape) != tuple(unif.shape):
+            raise QmcError("per-move arrays must be [nsweeps][nel][nw]")
+    args = [det._h, det.spline._h, _dev(pos, torch.float64), _dev(delta, torch.float64),
+            _dev(unif, torch.float64), nsweeps, _dev(ratios_out, torch.float64, True),
+            _dev(accept_out, torch.uint8, True), _dev(forced_accept, torch.uint8, True)]
+    if iel_begin or iel_count or phi_record is not None:
+        if phi_record is not None and tuple(phi_record.shape) != (nsweeps, det.nel, nrecord, det.nel):
+            raise QmcError("phi_record must be [nsweeps][nel][nrecord][nel]")
+        opts = SweepOpts(int(iel_begin), int(iel_count),
+                         None if phi_record is None else phi_record.data_ptr(), int(nrecord), 0)
+        rc = lib.qmc_sweep_ex(*args, ctypes.byref(opts), _stream(stream))
+        _check(rc, "qmc_sweep_ex")
+    else:
+        _check(lib.qmc_sweep(*args, _stream(stream)), "qmc_sweep")
+
+
+def sweep_host(det, pos, delta, unif, ratios_out=None, accept_out=None, stream=None):
+    """qmc_sweep_host on HOST tensors (ideally pinned); synchronises.  pos is updated in place."""
+    lib = load_library()
+    for t in (pos, delta, unif, ratios_out, accept_out):
+        if t is not None and t.is_cuda:
+            raise QmcError("sweep_host takes host tensors")
+    nsweeps = delta.shape[0]
+    rc = lib.qmc_sweep_host(det._h, det.spline._h, _ptr(pos, torch.float64), _ptr(delta, torch.float64),
+                            _ptr(unif, torch.float64), nsweeps, _ptr(ratios_out, torch.float64, True),
+                            _ptr(accept_out, torch.uint8, True), _stream(stream))
+    _check(rc, "qmc_sweep_host")

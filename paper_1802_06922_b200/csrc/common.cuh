@@ -1,0 +1,124 @@
+// Internal header of libqmcb200: handle layouts, error plumbing, small device helpers.
+// Not part of the public boundary (that is include/qmc_b200.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdarg.h>
+#include <stdint.h>
+#include <stdio.h>
+
+#include "qmc_b200.h"
+
+namespace qmc {
+
+constexpr int kWarp = 32;
+constexpr int kMaxNel = 2048;       // rows are held in registers: 64 doubles per lane at most
+constexpr int kRatioTilesMax = 8;   // partial-ratio slots per walker (orbital tiles of the SPO kernel)
+
+void set_error(const char *fmt, ...);
+void count_launch(int n = 1);
+
+#define QMC_CUDA(call)                                                                     \
+    do {                                                                                   \
+        cudaError_t e__ = (call);                                                          \
+        if (e__ != cudaSuccess) {                                                          \
+            qmc::set_error("%s:%d: %s -> %s", __FILE__, __LINE__, #call,                   \
+                           cudaGetErrorString(e__));                                       \
+            return QMC_ECUDA;                                                              \
+        }                                                                                  \
+    } while (0)
+
+#define QMC_REQUIRE(cond, ...)                                                             \
+    do {                                                                                   \
+        if (!(cond)) {                                                                     \
+            qmc::set_error(__VA_ARGS__);                                                   \
+            return QMC_EINVAL;                                                             \
+        }                                                                                  \
+    } while (0)
+
+// Launch check: catches bad configurations at once (no synchronisation).
+#define QMC_LAUNCHED()                                                                     \
+    do {                                                                                   \
+        qmc::count_launch();                                                               \
+        QMC_CUDA(cudaGetLastError());                                                      \
+    } while (0)
+
+// What the SPO kernels need to know about the table (passed by value).
+struct SplineView {
+    const float *coefs;   // [nx][ny][nz][np]
+    int nx, ny, nz, norb, np;
+    double linv[9];       // lattice^-1, row-major: u_d = sum_j r_j linv[3j+d]
+    double jac[9];        // jac[3j+d] = linv[3j+d] * N_d = d s_d / d r_j
+    double metric[6];     // G_de = sum_j jac[j][d] jac[j][e]: xx,yy,zz,xy,xz,yz
+};
+
+}  // namespace qmc
+
+struct qmc_spline {
+    qmc::SplineView view;
+    float *coefs;         // owned
+    size_t bytes;
+};
+
+struct qmc_det {
+    const qmc_spline *spline;   // not owned; shape checks and det_init only
+    int nw, nel, ld, delay;
+    int np;                     // spline row pitch (floats)
+    double *B;                  // [nw][nel][ld]   (A^-1)^T, pad columns zero
+    double *logdet;             // [nw]
+    int *sign;                  // [nw]
+    long long *naccept;         // [nw]
+    // scratch owned by the handle
+    float *vgl;                 // [nw][5][np]   v, gx, gy, gz, lap of the current proposal
+    double *rowk;               // [nw][ld]      copy of row iel of B taken before the update
+    double *rpart;              // [nw][kRatioTilesMax] partial ratios of the fused SPO kernel
+    double *ratio;              // [nw]
+    unsigned char *acc;         // [nw]
+    // delayed-update window (delay >= 2)
+    int *win_count;             // [nw]           accepted rows pending
+    int *win_iel;               // [nw][delay]    their electron indices
+    float *win_phi;             // [nw][delay][np] their orbital vectors
+    double *win_rows;           // [nw][delay][ld] rows B0[k_l] saved at accept time
+    double *win_sinv;           // [nw][delay][delay] inverse of S
+    int *win_full;              // [1] set when any walker's window is full
+    int host_pending;           // upper bound of pending rows known to the host
+    // device staging of qmc_sweep_host (grown on demand)
+    void *stage;
+    size_t stage_bytes;
+};
+
+namespace qmc {
+
+__device__ __forceinline__ double warp_sum(double x)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+    return x;
+}
+
+// Deterministic block sum (fixed order); result valid in every thread.  `red` holds >= 33 doubles.
+__device__ __forceinline__ double block_sum(double x, double *red)
+{
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nwarp = (blockDim.x + 31) >> 5;
+    x = warp_sum(x);
+    __syncthreads();
+    if (lane == 0) red[wid] = x;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+        for (int i = 0; i < nwarp; ++i) s += red[i];
+        red[32] = s;
+    }
+    __syncthreads();
+    return red[32];
+}
+
+__device__ __forceinline__ float4 ldg_stream(const float4 *p)
+{
+    float4 r;
+    asm("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];"
+                 : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w)
+                 : "l"(p));
+    return r;
+}
+
+}  // namespace qmc

@@ -1,0 +1,197 @@
+// qmc_sweep*: the particle-by-particle sweep driver (sec 5.2.1) -- all walkers
+// in lockstep (L114, L181), electrons in sequence.  Two launches per electron step:
+//   K1 spo_ratio_kernel  S0 proposal, S1 stencil, S2 SPO-VGL gather, S3 partial ratios, row copy
+//   K2 sm_update_kernel  S3 ratio (sum of partials), S4 Metropolis test, S5 rank-1 update
+#include "delayed_device.cuh"
+#include "spo_device.cuh"
+#include "update_device.cuh"
+
+namespace qmc {
+
+void spo_launch_shape(int np, int *threads, int *tiles);
+
+struct SpoRatioArgs {
+    SplineView sp;
+    const double *pos;     // [nw][nel][3]
+    const double *delta;   // [nw][3], offset to (sweep, electron)
+    int nel, iel, ld;
+    const double *B;       // [nw][nel][ld]
+    float *vgl;            // [nw][5][np]
+    double *rowk;          // [nw][ld]
+    double *rpart;         // [nw][kRatioTilesMax]
+    float *phi_record;     // [nrecord][nel], offset to (sweep, electron), or NULL
+    int nrecord;
+};
+
+// One block per (orbital tile, walker).  Thread t owns orbitals 4t..4t+3 of the tile: it gathers
+// their value/gradient/Laplacian from the 64 stencil rows, writes them to the walker's scratch,
+// multiplies the values with the matching four entries of row iel of B (fp64) and copies those
+// entries to rowk, so the update kernel can overwrite B in place.  The block's partial ratio is
+// reduced in a fixed order; the (at most 8) tiles are added by the update kernel.
+__global__ void __launch_bounds__(256) spo_ratio_kernel(SpoRatioArgs a)
+{
+    __shared__ StencilSmem st;
+    __shared__ double red[33];
+    const int w = blockIdx.y;
+    const double *r = a.pos + ((size_t)w * a.nel + a.iel) * 3;
+    const double *dl = a.delta + 3 * (size_t)w;
+    stage_stencil(a.sp, r[0] + dl[0], r[1] + dl[1], r[2] + dl[2], st);
+    const int np = a.sp.np;
+    const int col = 4 * (blockIdx.x * blockDim.x + threadIdx.x);
+    double part = 0.0;
+    if (col < np) {
+        float4 v, gx, gy, gz, lp;
+        gather4<true>(a.sp, st, col, v, gx, gy, gz, lp);
+        float *o = a.vgl + (size_t)w * 5 * np + col;
+        *reinterpret_cast<float4 *>(o) = v;
+        *reinterpret_cast<float4 *>(o + np) = gx;
+        *reinterpret_cast<float4 *>(o + 2 * (size_t)np) = gy;
+        *reinterpret_cast<float4 *>(o + 3 * (size_t)np) = gz;
+        *reinterpret_cast<float4 *>(o + 4 * (size_t)np) = lp;
+        const double2 *brow = reinterpret_cast<const double2 *>(a.B + ((size_t)w * a.nel + a.iel) * a.ld + col);
+        const double2 b0 = brow[0], b1 = brow[1];
+        double2 *rk = reinterpret_cast<double2 *>(a.rowk + (size_t)w * a.ld + col);
+        rk[0] = b0;
+        rk[1] = b1;
+        part = fma(b0.x, (double)v.x, part);
+        part = fma(b0.y, (double)v.y, part);
+        part = fma(b1.x, (double)v.z, part);
+        part = fma(b1.y, (double)v.w, part);
+        if (a.phi_record && w < a.nrecord) {
+            float *rec = a.phi_record + (size_t)w * a.nel;
+            if (col + 0 < a.nel) rec[col + 0] = v.x;
+            if (col + 1 < a.nel) rec[col + 1] = v.y;
+            if (col + 2 < a.nel) rec[col + 2] = v.z;
+            if (col + 3 < a.nel) rec[col + 3] = v.w;
+        }
+    }
+    part = block_sum(part, red);
+    if (threadIdx.x == 0) a.rpart[(size_t)w * kRatioTilesMax + blockIdx.x] = part;
+}
+
+static int sweep_impl(qmc_det *d, const qmc_spline *sp, double *pos, const double *delta, const double *unif,
+                      int nsweeps, double *ratios_out, unsigned char *accept_out, const unsigned char *forced,
+                      const qmc_sweep_opts_t *opts, cudaStream_t s)
+{
+    QMC_REQUIRE(d && sp && pos && delta && unif, "qmc_sweep: NULL argument");
+    QMC_REQUIRE(d->spline == sp, "qmc_sweep: the determinant was initialised from another spline");
+    QMC_REQUIRE(nsweeps >= 0, "qmc_sweep: nsweeps=%d", nsweeps);
+    const int nw = d->nw, nel = d->nel;
+    int k0 = 0, kn = nel;
+    float *rec = nullptr;
+    int nrec = 0;
+    if (opts) {
+        k0 = opts->iel_begin;
+        kn = opts->iel_count ? opts->iel_count : nel - k0;
+        rec = opts->phi_record;
+        nrec = rec ? opts->nrecord : 0;
+        QMC_REQUIRE(k0 >= 0 && kn >= 0 && k0 + kn <= nel, "qmc_sweep_ex: electron range %d+%d outside 0..%d", k0, kn, nel);
+        QMC_REQUIRE(nrec >= 0 && nrec <= nw, "qmc_sweep_ex: nrecord=%d outside 0..%d", nrec, nw);
+    }
+    int threads, tiles;
+    spo_launch_shape(d->np, &threads, &tiles);
+    QMC_REQUIRE(tiles <= kRatioTilesMax, "qmc_sweep: too many orbital tiles (%d)", tiles);
+
+    for (int sw = 0; sw < nsweeps; ++sw) {
+        for (int k = k0; k < k0 + kn; ++k) {
+            const size_t mv = ((size_t)sw * nel + k) * nw;
+            SpoRatioArgs a{};
+            a.sp = sp->view;
+            a.pos = pos; a.delta = delta + 3 * mv;
+            a.nel = nel; a.iel = k; a.ld = d->ld;
+            a.B = d->B; a.vgl = d->vgl; a.rowk = d->rowk; a.rpart = d->rpart;
+            a.phi_record = rec ? rec + mv / nw * (size_t)nrec * nel : nullptr;
+            a.nrecord = nrec;
+            if (d->delay) {
+                int rc = delayed_sweep_step(d, sp, pos, delta + 3 * mv, unif + mv, k,
+                                            ratios_out ? ratios_out + mv : nullptr,
+                                            accept_out ? accept_out + mv : nullptr,
+                                            forced ? forced + mv : nullptr, a.phi_record, nrec, s);
+                if (rc) return rc;
+                continue;
+            }
+            spo_ratio_kernel<<<dim3(tiles, nw), threads, 0, s>>>(a);
+            QMC_LAUNCHED();
+            UpdateArgs u{};
+            u.B = d->B; u.nel = nel; u.ld = d->ld; u.iel = k;
+            u.phi = d->vgl; u.ldphi = (size_t)5 * d->np; u.rowk = d->rowk;
+            u.rpart = d->rpart; u.ntiles = tiles;
+            u.unif = unif + mv;
+            u.forced = forced ? forced + mv : nullptr;
+            u.ratios_out = ratios_out ? ratios_out + mv : nullptr;
+            u.accept_out = accept_out ? accept_out + mv : nullptr;
+            u.pos = pos; u.delta = delta + 3 * mv;
+            u.logdet = d->logdet; u.sign = d->sign; u.naccept = d->naccept;
+            QMC_CUDA(launch_sm_update<true>(u, nw, s));
+        }
+        if (d->delay) {
+            int rc = delayed_flush(d, s);
+            if (rc) return rc;
+        }
+    }
+    return QMC_OK;
+}
+
+}  // namespace qmc
+
+using namespace qmc;
+
+extern "C" int qmc_sweep(qmc_det_t *d, const qmc_spline_t *sp, double *pos, const double *delta,
+                         const double *unif, int nsweeps, double *ratios_out, unsigned char *accept_out,
+                         const unsigned char *forced, void *stream)
+{
+    return sweep_impl(d, sp, pos, delta, unif, nsweeps, ratios_out, accept_out, forced, nullptr,
+                      (cudaStream_t)stream);
+}
+
+extern "C" int qmc_sweep_ex(qmc_det_t *d, const qmc_spline_t *sp, double *pos, const double *delta,
+                            const double *unif, int nsweeps, double *ratios_out, unsigned char *accept_out,
+                            const unsigned char *forced, const qmc_sweep_opts_t *opts, void *stream)
+{
+    return sweep_impl(d, sp, pos, delta, unif, nsweeps, ratios_out, accept_out, forced, opts,
+                      (cudaStream_t)stream);
+}
+
+extern "C" int qmc_sweep_host(qmc_det_t *d, const qmc_spline_t *sp, double *pos_h, const double *delta_h,
+                              const double *unif_h, int nsweeps, double *ratios_h, unsigned char *accept_h,
+                              void *stream)
+{
+    QMC_REQUIRE(d && sp && pos_h && delta_h && unif_h, "qmc_sweep_host: NULL argument");
+    QMC_REQUIRE(nsweeps >= 0, "qmc_sweep_host: nsweeps=%d", nsweeps);
+    cudaStream_t s = (cudaStream_t)stream;
+    const size_t nw = d->nw, nel = d->nel, moves = (size_t)nsweeps * nel * nw;
+    auto up = [](size_t b) { return (b + 255) / 256 * 256; };
+    const size_t b_pos = up(nw * nel * 3 * sizeof(double)), b_delta = up(moves * 3 * sizeof(double));
+    const size_t b_unif = up(moves * sizeof(double)), b_ratio = up(moves * sizeof(double)), b_acc = up(moves);
+    const size_t total = b_pos + b_delta + b_unif + b_ratio + b_acc;
+    if (d->stage_bytes < total) {
+        QMC_CUDA(cudaStreamSynchronize(s));
+        cudaFree(d->stage);
+        d->stage = nullptr;
+        d->stage_bytes = 0;
+        cudaError_t e = cudaMalloc(&d->stage, total);
+        if (e != cudaSuccess) {
+            set_error("qmc_sweep_host: cudaMalloc(%zu bytes) -> %s", total, cudaGetErrorString(e));
+            (void)cudaGetLastError();
+            return QMC_ENOMEM;
+        }
+        d->stage_bytes = total;
+    }
+    char *base = (char *)d->stage;
+    double *pos = (double *)base;
+    double *delta = (double *)(base + b_pos);
+    double *unif = (double *)(base + b_pos + b_delta);
+    double *ratios = (double *)(base + b_pos + b_delta + b_unif);
+    unsigned char *acc = (unsigned char *)(base + b_pos + b_delta + b_unif + b_ratio);
+    QMC_CUDA(cudaMemcpyAsync(pos, pos_h, nw * nel * 3 * sizeof(double), cudaMemcpyHostToDevice, s));
+    QMC_CUDA(cudaMemcpyAsync(delta, delta_h, moves * 3 * sizeof(double), cudaMemcpyHostToDevice, s));
+    QMC_CUDA(cudaMemcpyAsync(unif, unif_h, moves * sizeof(double), cudaMemcpyHostToDevice, s));
+    int rc = sweep_impl(d, sp, pos, delta, unif, nsweeps, ratios_h ? ratios : nullptr, accept_h ? acc : nullptr,
+                        nullptr, nullptr, s);
+    if (rc) return rc;
+    QMC_CUDA(cudaMemcpyAsync(pos_h, pos, nw * nel * 3 * sizeof(double), cudaMemcpyDeviceToHost, s));
+    if (ratios_h) QMC_CUDA(cudaMemcpyAsync(ratios_h, ratios, moves * sizeof(double), cudaMemcpyDeviceToHost, s));
+    if (accept_h) QMC_CUDA(cudaMemcpyAsync(accept_h, acc, moves, cudaMemcpyDeviceToHost, s));
+    QMC_CUDA(cudaStreamSynchronize(s));
+    return QMC_OK;
+}

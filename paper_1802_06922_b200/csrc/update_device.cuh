@@ -1,0 +1,145 @@
+// Sherman-Morrison rank-1 update of B = (A^-1)^T in one pass (S4+S5 of the hot
+// path).  Used by qmc_det_accept_update (decision given) and qmc_sweep (decision taken here from
+// the partial ratios of the fused SPO kernel).
+#pragma once
+#include "common.cuh"
+
+namespace qmc {
+
+struct UpdateArgs {
+    double *B;                    // [nw][nel][ld]
+    int nel, ld, iel;
+    const float *phi;             // [nw][ldphi] orbital vector of the proposal (fp32)
+    size_t ldphi;                 //   walker stride in floats
+    const double *rowk;           // [nw][ld] row iel of B before the update
+    // decision given (qmc_det_accept_update)
+    const double *ratio;          // [nw]
+    const unsigned char *accept;  // [nw]
+    // decision taken here (qmc_sweep): all pointers already offset to (sweep, electron)
+    const double *rpart;          // [nw][kRatioTilesMax]
+    int ntiles;
+    const double *unif;           // [nw]
+    const unsigned char *forced;  // [nw] or NULL
+    double *ratios_out;           // [nw] or NULL
+    unsigned char *accept_out;    // [nw] or NULL
+    double *pos;                  // [nw][nel][3]
+    const double *delta;          // [nw][3]
+    // per-walker statistics
+    double *logdet;
+    int *sign;
+    long long *naccept;
+};
+
+constexpr int kUpdThreads = 256;
+constexpr int kUpdRowsPerCta = 64;
+
+// Metropolis test of eq. 12 with symmetric T and a determinant-only Psi (R:A8).
+__device__ __forceinline__ bool metropolis(double R, double u) { return isfinite(R) && (R * R > u); }
+
+// One warp per row m: the row (ld = 64*VPT doubles) is read once into registers as VPT double2
+// per lane, dotted with phi (warp-shuffle tree), updated with the old row iel, and written back:
+// 16*ld bytes of HBM traffic per row, the floor for a rank-1 update.
+template <int VPT, bool DECIDE>
+__global__ void __launch_bounds__(kUpdThreads) sm_update_kernel(UpdateArgs a)
+{
+    extern __shared__ double smem_upd[];
+    const int w = blockIdx.y;
+    double R;
+    bool acc;
+    if (DECIDE) {
+        R = 0.0;
+        for (int t = 0; t < a.ntiles; ++t) R += a.rpart[(size_t)w * kRatioTilesMax + t];
+        acc = a.forced ? (a.forced[w] != 0) : metropolis(R, a.unif[w]);
+    } else {
+        R = a.ratio[w];
+        acc = a.accept[w] != 0;
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        if (DECIDE) {
+            if (a.ratios_out) a.ratios_out[w] = R;
+            if (a.accept_out) a.accept_out[w] = acc ? 1 : 0;
+        }
+        if (acc) {
+            a.logdet[w] += log(fabs(R));
+            if (R < 0.0) a.sign[w] = -a.sign[w];
+            a.naccept[w] += 1;
+            if (DECIDE) {
+                double *r = a.pos + ((size_t)w * a.nel + a.iel) * 3;
+                r[0] += a.delta[3 * (size_t)w + 0];
+                r[1] += a.delta[3 * (size_t)w + 1];
+                r[2] += a.delta[3 * (size_t)w + 2];
+            }
+        }
+    }
+    if (!acc) return;
+
+    const int ld = a.ld;
+    double *phi_s = smem_upd;        // [ld]
+    double *rowk_s = smem_upd + ld;  // [ld]
+    const float *phi = a.phi + (size_t)w * a.ldphi;
+    const double *rowk = a.rowk + (size_t)w * ld;
+    for (int j = threadIdx.x; j < ld; j += kUpdThreads) {
+        phi_s[j] = j < a.nel ? (double)phi[j] : 0.0;
+        rowk_s[j] = rowk[j];
+    }
+    __syncthreads();
+
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int m_end = min(a.nel, (int)(blockIdx.x + 1) * kUpdRowsPerCta);
+    const double2 *phi2 = reinterpret_cast<const double2 *>(phi_s);
+    const double2 *rk2 = reinterpret_cast<const double2 *>(rowk_s);
+    for (int m = blockIdx.x * kUpdRowsPerCta + wid; m < m_end; m += kUpdThreads / 32) {
+        double2 *row = reinterpret_cast<double2 *>(a.B + ((size_t)w * a.nel + m) * ld);
+        double2 r[VPT];
+#pragma unroll
+        for (int i = 0; i < VPT; ++i) r[i] = row[lane + 32 * i];
+        double dot = 0.0;
+#pragma unroll
+        for (int i = 0; i < VPT; ++i) {
+            const double2 p = phi2[lane + 32 * i];
+            dot = fma(r[i].x, p.x, dot);
+            dot = fma(r[i].y, p.y, dot);
+        }
+        dot = warp_sum(dot);
+        const double f = (dot - (m == a.iel ? 1.0 : 0.0)) / R;
+#pragma unroll
+        for (int i = 0; i < VPT; ++i) {
+            const double2 k2 = rk2[lane + 32 * i];
+            r[i].x = fma(-f, k2.x, r[i].x);
+            r[i].y = fma(-f, k2.y, r[i].y);
+            row[lane + 32 * i] = r[i];
+        }
+    }
+}
+
+// ld (doubles) for nel electrons: a multiple of 64 whose quotient is one of the instantiated VPTs.
+inline int update_ld(int nel)
+{
+    static const int vpts[] = {1, 2, 3, 4, 6, 8, 12, 16, 24, 32};
+    const int need = (nel + 63) / 64;
+    for (int v : vpts)
+        if (v >= need) return 64 * v;
+    return -1;
+}
+
+template <bool DECIDE>
+inline cudaError_t launch_sm_update(const UpdateArgs &a, int nw, cudaStream_t s)
+{
+    dim3 grid((a.nel + kUpdRowsPerCta - 1) / kUpdRowsPerCta, nw);
+    const size_t smem = 2 * (size_t)a.ld * sizeof(double);
+    switch (a.ld / 64) {
+#define QMC_UPD_CASE(V)                                                              \
+    case V:                                                                          \
+        sm_update_kernel<V, DECIDE><<<grid, kUpdThreads, smem, s>>>(a);              \
+        break;
+        QMC_UPD_CASE(1) QMC_UPD_CASE(2) QMC_UPD_CASE(3) QMC_UPD_CASE(4) QMC_UPD_CASE(6)
+        QMC_UPD_CASE(8) QMC_UPD_CASE(12) QMC_UPD_CASE(16) QMC_UPD_CASE(24) QMC_UPD_CASE(32)
+#undef QMC_UPD_CASE
+    default:
+        return cudaErrorInvalidValue;
+    }
+    count_launch();
+    return cudaGetLastError();
+}
+
+}  // namespace qmc

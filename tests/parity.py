@@ -1,0 +1,167 @@
+"""Helpers shared by the GPU parity tests: tolerances from BASELINE.json's north_star (readings
+R:A10-R:A12 in DESIGN.md section 3) and the parity protocol of DESIGN.md section 5."""
+import numpy as np
+import torch
+
+import oracle
+from paper_1802_06922_b200 import api
+
+# north_star tolerances
+TOL_V = 2e-6        # spline value, relative to max|phi|
+TOL_GL = 2e-5       # gradient / Laplacian, relative to max|grad| / max|lap|
+TOL_RATIO = 1e-5    # determinant ratio, relative (floor 1e-2 on |R| end to end, R:A10)
+TOL_BINV = 1e-9     # inverse after a sweep, identical orbital vectors (max-abs; R:A12)
+TOL_RESID = 1e-6    # ||Binv^T A - I||_inf with A recomputed from scratch (R:A11)
+BAND = 1e-6         # accept decisions may differ only where |R^2 - u| < BAND
+
+
+def dev():
+    return torch.device("cuda", 0)
+
+
+def to_dev(a, dtype=None):
+    t = torch.from_numpy(np.ascontiguousarray(a))
+    if dtype is not None:
+        t = t.to(dtype)
+    return t.to(dev())
+
+
+def check_vgl(v, g, l, vo, go, lo, norb):
+    """GPU fp32 (padded) outputs against the fp64 oracle."""
+    v, g, l = (t.double().cpu().numpy() for t in (v, g, l))
+    assert np.all(v[:, norb:] == 0) and np.all(g[:, :, norb:] == 0) and np.all(l[:, norb:] == 0)
+    ev = np.max(np.abs(v[:, :norb] - vo)) / np.max(np.abs(vo))
+    eg = np.max(np.abs(g[:, :, :norb] - go)) / np.max(np.abs(go))
+    el = np.max(np.abs(l[:, :norb] - lo)) / np.max(np.abs(lo))
+    assert ev < TOL_V, f"value rel err {ev:.3e}"
+    assert eg < TOL_GL, f"gradient rel err {eg:.3e}"
+    assert el < TOL_GL, f"laplacian rel err {el:.3e}"
+    return ev, eg, el
+
+
+def gpu_slater(spline, pos_t):
+    """A[w][i][j] = phi_j(r_wi) from the CUDA SPO kernel (fp32 values, as fp64 numpy)."""
+    nw, nel, _ = pos_t.shape
+    v = api.spo_vgl(spline, pos_t.reshape(-1, 3), want_gl=False)
+    return v[:, :nel].double().reshape(nw, nel, nel).cpu().numpy()
+
+
+def oracle_binv(A):
+    nw, nel, _ = A.shape
+    B = np.empty_like(A)
+    ld = np.empty(nw)
+    sg = np.empty(nw, dtype=np.int32)
+    for w in range(nw):
+        B[w], ld[w], sg[w] = oracle.binv_from_A(A[w])
+    return B, ld, sg
+
+
+def compare_decisions(acc_g, R_g, acc_o, R_o, unif):
+    """Free runs: per walker, identical up to the first mismatch, which must lie in the band."""
+    nsw, nel, nw = acc_g.shape
+    ag = acc_g.reshape(nsw * nel, nw)
+    ao = acc_o.reshape(nsw * nel, nw)
+    Rg, Ro, u = R_g.reshape(-1, nw), R_o.reshape(-1, nw), unif.reshape(-1, nw)
+    ndiverged = 0
+    for w in range(nw):
+        mism = np.nonzero(ag[:, w] != ao[:, w])[0]
+        stop = mism[0] if len(mism) else nsw * nel
+        # ratios agree before the first divergence
+        if stop:
+            floor = np.maximum(np.abs(Ro[:stop, w]), 1e-2)
+            assert np.max(np.abs(Rg[:stop, w] - Ro[:stop, w]) / floor) < TOL_RATIO
+        if len(mism):
+            ndiverged += 1
+            m = mism[0]
+            assert abs(Ro[m, w] ** 2 - u[m, w]) < BAND or abs(Rg[m, w] ** 2 - u[m, w]) < BAND, \
+                f"walker {w} move {m}: decisions differ outside the band (R_gpu={Rg[m, w]}, R_orc={Ro[m, w]}, u={u[m, w]})"
+    return ndiverged
+
+
+def run_protocol(x, delay_rank=0, walkers=None, free_oracle=True, coefs_np=None):
+    """Parity protocol on inputs x (tests/conftest shapes).  Returns a dict of measured errors.
+
+    walkers: None = all walkers are replayed by the oracle; else the first `walkers` of them
+    (the GPU still runs all of them in lockstep).
+    """
+    cfg = x.cfg
+    nw, nel, nsw = x.pos.shape[0], cfg.norb, x.delta.shape[0]
+    nchk = nw if walkers is None else min(nw, walkers)
+    coefs_t = x.coefs.to(dev())
+    spline = api.Spline.create(coefs_t, x.lattice)
+    pos0 = to_dev(x.pos)
+    delta_t, unif_t = to_dev(x.delta), to_dev(x.unif)
+    out = {}
+
+    # GPU free run, recording ratios, decisions and the fp32 orbital vectors of the checked walkers
+    A0_g = gpu_slater(spline, pos0)[:nchk]
+    det = api.Det.init(spline, pos0, delay_rank=delay_rank)
+    B0_g = det.get_inverse().cpu().numpy()[:nchk]
+    ld0_g, sg0_g, _ = (t.cpu().numpy() for t in det.get_stats())
+    pos_g = pos0.clone()
+    R_g = torch.zeros_like(unif_t)
+    acc_g = torch.zeros(unif_t.shape, dtype=torch.uint8, device=dev())
+    rec = torch.zeros((nsw, nel, nchk, nel), dtype=torch.float32, device=dev())
+    api.sweep(det, pos_g, delta_t, unif_t, ratios_out=R_g, accept_out=acc_g, phi_record=rec, nrecord=nchk)
+    torch.cuda.synchronize()
+    R_g, acc_g, rec = R_g.cpu().numpy(), acc_g.cpu().numpy(), rec.cpu().numpy()
+    Bf_g = det.get_inverse().cpu().numpy()
+    ldf_g, sgf_g, nacc_g = (t.cpu().numpy() for t in det.get_stats())
+    out["accept_rate"] = float(acc_g.mean())
+    assert np.array_equal(nacc_g, acc_g.sum(axis=(0, 1)))
+
+    # init: the device inverse of the device-evaluated Slater matrix vs the oracle's LU of the same matrix
+    B0_o, ld0_o, sg0_o = oracle_binv(A0_g)
+    scale0 = max(1.0, np.max(np.abs(B0_o)))
+    out["init_binv_err"] = float(np.max(np.abs(B0_g - B0_o)) / scale0)
+    assert out["init_binv_err"] < 1e-9
+    assert np.max(np.abs(ld0_g[:nchk] - ld0_o)) < 1e-8 and np.array_equal(sg0_g[:nchk], sg0_o)
+
+    sl = np.s_[..., :nchk]
+    d_sub, u_sub = np.ascontiguousarray(x.delta[:, :, :nchk]), np.ascontiguousarray(x.unif[sl])
+    nth = oracle.max_threads()
+
+    # (4) identical orbital vectors: the oracle engine replays the recorded fp32 vectors and the
+    #     GPU's decisions from the same initial inverse
+    rep = oracle.sweep(coefs_np if coefs_np is not None else np.zeros((1, 1, 1, nel), np.float32), x.lattice,
+                       x.pos[:nchk], B0_o, ld0_o, sg0_o, d_sub, u_sub,
+                       forced=np.ascontiguousarray(acc_g[sl]), phi_in=np.ascontiguousarray(rec), nthreads=nth)
+    scale = max(1.0, np.max(np.abs(rep["B"])))
+    out["binv_identical_abs"] = float(np.max(np.abs(Bf_g[:nchk] - rep["B"])))
+    out["binv_scale"] = float(scale)
+    assert out["binv_identical_abs"] < TOL_BINV * scale, out
+    relR = np.abs(R_g[sl] - rep["ratios"]) / np.maximum(np.abs(rep["ratios"]), 1e-300)
+    out["ratio_identical_rel"] = float(relR.max())
+    assert out["ratio_identical_rel"] < TOL_RATIO
+    assert np.max(np.abs(ldf_g[:nchk] - rep["logdet"])) < 1e-7 and np.array_equal(sgf_g[:nchk], rep["sign"])
+    assert np.array_equal(pos_g.cpu().numpy()[:nchk], rep["pos"])        # bitwise: one fp64 add per accept
+
+    # (5) residual with A recomputed from scratch by the evaluator that fed the engine (R:A11)
+    A_fin = gpu_slater(spline, pos_g)[:nchk]
+    res = np.einsum("wji,wjk->wik", Bf_g[:nchk], A_fin) - np.eye(nel)
+    out["resid_inf"] = float(np.max(np.sum(np.abs(res), axis=2)))
+    assert out["resid_inf"] < TOL_RESID, out
+    # (6) log-det telescoping against numpy's LU of the recomputed matrix
+    sg_np, ld_np = np.linalg.slogdet(A_fin)
+    assert np.max(np.abs(ldf_g[:nchk] - ld_np)) < 1e-6 and np.array_equal(sgf_g[:nchk], sg_np.astype(np.int32))
+
+    if free_oracle:
+        assert coefs_np is not None
+        # (2) oracle free run in fp64 from its own spline, Slater matrix and inverse
+        A0_o = oracle.slater_matrix(coefs_np, x.lattice, x.pos[:nchk])
+        Bo, ldo, sgo = oracle_binv(A0_o)
+        free = oracle.sweep(coefs_np, x.lattice, x.pos[:nchk], Bo, ldo, sgo, d_sub, u_sub, nthreads=nth)
+        out["diverged_walkers"] = compare_decisions(acc_g[sl], R_g[sl], free["accept"], free["ratios"], u_sub)
+        # (3) oracle forced to the GPU's decisions: every ratio, final positions, final inverse
+        frc = oracle.sweep(coefs_np, x.lattice, x.pos[:nchk], Bo, ldo, sgo, d_sub, u_sub,
+                           forced=np.ascontiguousarray(acc_g[sl]), nthreads=nth)
+        floor = np.maximum(np.abs(frc["ratios"]), 1e-2)
+        out["ratio_e2e_rel"] = float(np.max(np.abs(R_g[sl] - frc["ratios"]) / floor))
+        out["ratio_small_count"] = int(np.sum(np.abs(frc["ratios"]) < 1e-2))
+        assert out["ratio_e2e_rel"] < TOL_RATIO, out
+        assert np.array_equal(pos_g.cpu().numpy()[:nchk], frc["pos"])
+        out["binv_e2e_rel"] = float(np.max(np.abs(Bf_g[:nchk] - frc["B"])) / max(1.0, np.max(np.abs(frc["B"]))))
+        assert out["binv_e2e_rel"] < 1e-3, out      # fp32 orbitals vs fp64 orbitals: reported, loose
+    det.destroy()
+    spline.destroy()
+    return out

@@ -1,0 +1,198 @@
+"""GPU parity tests: the CUDA path, called through the C ABI (api.py -> libqmcb200.so), against
+the fp64 oracle on the same seeded inputs.  Tolerances are BASELINE.json's (tests/parity.py)."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_1802_06922_b200 import api, inputs
+from tests import parity as P
+
+pytestmark = pytest.mark.gpu
+
+SKEW = np.array([[3.1, 0.2, -0.1], [0.4, 2.7, 0.3], [-0.2, 0.5, 3.4]]) * 2.0
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _need_gpu():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    api.load_library()
+    torch.cuda.set_device(0)
+
+
+def ragged_cfg(nw=5, nsweeps=2, norb=37):
+    return inputs.custom_config("ragged", (12, 10, 14), norb, SKEW, nw=nw, nsweeps=nsweeps, sigma=0.25)
+
+
+CASES = {
+    "tiny": lambda: inputs.make_inputs("tiny"),
+    "ragged37_skew": lambda: inputs.make_inputs(ragged_cfg()),
+    "n130_two_tiles": lambda: inputs.make_inputs(
+        inputs.custom_config("n130", (10, 12, 9), 130, (5.0, 6.0, 4.5), nw=3, nsweeps=1, sigma=0.2)),
+    "small": lambda: inputs.make_inputs("small"),
+}
+
+
+# ------------------------------------------------------------------------------- SPO-VGL
+@pytest.mark.parametrize("case", ["tiny", "ragged37_skew", "n130_two_tiles", "small"])
+def test_spo_vgl_parity(case):
+    x = CASES[case]()
+    coefs = x.coefs_numpy()
+    norb = x.cfg.norb
+    rng = np.random.default_rng(7)
+    # positions: the walkers' electrons, images outside the cell, cell faces and corners
+    pos = x.pos.reshape(-1, 3)[:300]
+    extra = rng.uniform(-2, 3, size=(40, 3)) @ x.lattice
+    faces = (rng.integers(0, 4, size=(24, 3)) / np.array(x.cfg.grid)) @ x.lattice
+    faces[:8] = (np.array(x.cfg.grid) - 1.0) / np.array(x.cfg.grid) @ x.lattice * rng.integers(0, 2, size=(8, 3))
+    pos = np.concatenate([pos, extra, faces, np.zeros((1, 3))])
+    vo, go, lo = oracle.spline_vgl(coefs, x.lattice, pos)
+    spline = api.Spline.create(x.coefs.to(P.dev()), x.lattice)
+    assert spline.row_pitch % 32 == 0 and spline.row_pitch >= norb
+    v, g, l = api.spo_vgl(spline, P.to_dev(pos))
+    P.check_vgl(v, g, l, vo, go, lo, norb)
+    # value-only launch gives the same bits; a batch of one gives the same bits (R:A11)
+    v1 = api.spo_vgl(spline, P.to_dev(pos), want_gl=False)
+    assert torch.equal(v1, v)
+    vs, gs, ls = api.spo_vgl(spline, P.to_dev(pos[17:18]))
+    assert torch.equal(vs[0], v[17]) and torch.equal(gs[0], g[17]) and torch.equal(ls[0], l[17])
+    # caller-chosen leading dimension
+    ldo = (norb + 3) // 4 * 4
+    v2, g2, l2 = api.spo_vgl(spline, P.to_dev(pos), ldo=ldo)
+    assert torch.equal(v2[:, :norb], v[:, :norb]) and torch.equal(l2[:, :norb], l[:, :norb])
+    assert torch.equal(g2[:, :, :norb], g[:, :, :norb])
+    # host-resident table gives the same device table
+    spline_h = api.Spline.create(x.coefs.cpu(), x.lattice)
+    vh = api.spo_vgl(spline_h, P.to_dev(pos), want_gl=False)
+    assert torch.equal(vh, v)
+    spline.destroy()
+    spline_h.destroy()
+
+
+def test_spo_vgl_empty_and_errors():
+    x = CASES["tiny"]()
+    spline = api.Spline.create(x.coefs.to(P.dev()), x.lattice)
+    v = api.spo_vgl(spline, torch.zeros((0, 3), dtype=torch.float64, device=P.dev()), want_gl=False)
+    assert v.shape[0] == 0
+    with pytest.raises(api.QmcError):
+        api.spo_vgl(spline, torch.zeros((2, 3), dtype=torch.float64, device=P.dev()), ldo=4)   # < norb
+    with pytest.raises(api.QmcError):
+        api.Spline.create(x.coefs.to(P.dev()), np.zeros((3, 3)))                               # singular cell
+    spline.destroy()
+
+
+# ------------------------------------------------------------------------------- determinant
+@pytest.mark.parametrize("case", ["tiny", "ragged37_skew", "n130_two_tiles"])
+def test_ratio_and_update_identical_vectors(case):
+    """qmc_det_ratio / qmc_det_accept_update against orc_det_ratio / orc_sm_update, both fed the
+    same fp32 orbital vectors and the same initial inverse."""
+    x = CASES[case]()
+    nw, nel = x.pos.shape[0], x.cfg.norb
+    spline = api.Spline.create(x.coefs.to(P.dev()), x.lattice)
+    pos_t = P.to_dev(x.pos)
+    det = api.Det.init(spline, pos_t)
+    A = P.gpu_slater(spline, pos_t)
+    B, ld, sg = P.oracle_binv(A)
+    Bg = det.get_inverse().cpu().numpy()
+    assert np.max(np.abs(Bg - B)) < 1e-9 * max(1.0, np.max(np.abs(B)))
+    rng = np.random.default_rng(11)
+    for step in range(2 * nel):
+        k = int(rng.integers(0, nel))
+        newpos = P.to_dev(x.pos[:, k] + rng.normal(0, 0.2, size=(nw, 3)))
+        phi = api.spo_vgl(spline, newpos, want_gl=False)
+        R = det.ratio(k, phi)
+        phi_np = phi[:, :nel].double().cpu().numpy()
+        R_o = np.array([oracle.det_ratio(B[w], k, phi_np[w]) for w in range(nw)])
+        assert np.max(np.abs(R.cpu().numpy() - R_o) / np.abs(R_o)) < P.TOL_RATIO
+        acc = rng.integers(0, 2, size=nw).astype(np.uint8)
+        if step == 0:
+            acc[:] = 0          # nobody accepts: nothing may change
+        det.accept_update(k, phi, R, P.to_dev(acc))
+        for w in range(nw):
+            if acc[w]:
+                B[w] = oracle.sm_update(B[w], k, phi_np[w], R_o[w])
+                ld[w] += np.log(abs(R_o[w]))
+                sg[w] *= 1 if R_o[w] > 0 else -1
+    Bg = det.get_inverse().cpu().numpy()
+    assert np.max(np.abs(Bg - B)) < P.TOL_BINV * max(1.0, np.max(np.abs(B)))
+    ldg, sgg, _ = (t.cpu().numpy() for t in det.get_stats())
+    assert np.max(np.abs(ldg - ld)) < 1e-8 and np.array_equal(sgg, sg)
+    # set_inverse / get_inverse round trip
+    det.set_inverse(P.to_dev(B))
+    assert np.array_equal(det.get_inverse().cpu().numpy(), B)
+    det.destroy()
+    spline.destroy()
+
+
+def test_det_init_errors():
+    x = CASES["tiny"]()
+    spline = api.Spline.create(x.coefs.to(P.dev()), x.lattice)
+    zeroed = x.coefs.clone()
+    zeroed[..., 2] = 0.0                      # an identically zero orbital: exactly singular Slater matrix
+    sp0 = api.Spline.create(zeroed.to(P.dev()), x.lattice)
+    with pytest.raises(api.QmcError, match="singular"):
+        api.Det.init(sp0, P.to_dev(x.pos))
+    sp0.destroy()
+    with pytest.raises(api.QmcError):
+        api.Det.init(spline, P.to_dev(x.pos[:, :5]))   # nel != norb
+    spline.destroy()
+
+
+# ------------------------------------------------------------------------------- sweeps
+@pytest.mark.parametrize("case", ["tiny", "ragged37_skew", "n130_two_tiles", "small"])
+def test_sweep_parity_protocol(case):
+    x = CASES[case]()
+    out = P.run_protocol(x, coefs_np=x.coefs_numpy())
+    print(case, out)
+    assert 0.0 < out["accept_rate"] < 1.0
+
+
+def test_sweep_control_flow():
+    """u = 0 accepts every move; forced decisions are obeyed; partial electron ranges; host API."""
+    x = CASES["ragged37_skew"]()
+    nw, nel = x.pos.shape[0], x.cfg.norb
+    spline = api.Spline.create(x.coefs.to(P.dev()), x.lattice)
+    pos0, delta, unif = P.to_dev(x.pos), P.to_dev(x.delta), P.to_dev(x.unif)
+    # u = 0
+    det = api.Det.init(spline, pos0)
+    pos = pos0.clone()
+    acc = torch.zeros(unif.shape, dtype=torch.uint8, device=P.dev())
+    api.sweep(det, pos, delta, torch.zeros_like(unif), accept_out=acc)
+    assert bool(acc.all())
+    tot = np.transpose(x.delta.sum(axis=0), (1, 0, 2))
+    assert np.max(np.abs(pos.cpu().numpy() - (x.pos + tot))) < 1e-13
+    det.destroy()
+    # free run, then the same decisions forced with useless uniforms: identical state
+    det = api.Det.init(spline, pos0)
+    pos_a = pos0.clone()
+    R_a = torch.zeros_like(unif)
+    api.sweep(det, pos_a, delta, unif, ratios_out=R_a, accept_out=acc)
+    B_a = det.get_inverse()
+    det.destroy()
+    det = api.Det.init(spline, pos0)
+    pos_b = pos0.clone()
+    R_b = torch.zeros_like(unif)
+    api.sweep(det, pos_b, delta, 1.0 - unif, ratios_out=R_b, forced_accept=acc)
+    assert torch.equal(pos_a, pos_b) and torch.equal(det.get_inverse(), B_a) and torch.equal(R_a, R_b)
+    det.destroy()
+    # two half sweeps equal one sweep
+    det = api.Det.init(spline, pos0)
+    pos_c = pos0.clone()
+    h = nel // 2
+    api.sweep(det, pos_c, delta[:1], unif[:1], iel_begin=0, iel_count=h)
+    api.sweep(det, pos_c, delta[:1], unif[:1], iel_begin=h, iel_count=nel - h)
+    api.sweep(det, pos_c, delta[1:], unif[1:])
+    assert torch.equal(pos_c, pos_a) and torch.equal(det.get_inverse(), B_a)
+    det.destroy()
+    # host-buffer entry point
+    det = api.Det.init(spline, pos0)
+    pos_h = torch.from_numpy(x.pos.copy()).pin_memory()
+    R_h = torch.zeros(unif.shape, dtype=torch.float64).pin_memory()
+    acc_h = torch.zeros(unif.shape, dtype=torch.uint8).pin_memory()
+    api.sweep_host(det, pos_h, torch.from_numpy(x.delta).pin_memory(), torch.from_numpy(x.unif).pin_memory(),
+                   ratios_out=R_h, accept_out=acc_h)
+    assert torch.equal(pos_h, pos_a.cpu()) and torch.equal(R_h, R_a.cpu()) and torch.equal(acc_h, acc.cpu())
+    assert torch.equal(det.get_inverse(), B_a)
+    det.destroy()
+    spline.destroy()
