@@ -1,0 +1,334 @@
+#!/usr/bin/env python
+"""bench.py -- electron moves/s of the particle-by-particle sweep (SPO-VGL + ratio + inverse update).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config large] [--delay 0] [--impl ours|reference]
+
+One STEP is one full sweep of the configuration: every electron of every walker is proposed once
+(qmc_sweep with nsweeps = 1): S0 proposal, S1 stencil, S2 SPO-VGL gather, S3 ratio, S4 Metropolis
+test, S5 inverse update.  Default workload: BASELINE.json's "large supercell"
+(128^3 grid, N = 1024, 512 walkers, 8.6 GB fp32 table, 4.3 GB of fp64 inverses).  Inputs are
+seeded and synthetic (paper_1802_06922_b200/inputs.py).  Prints ONE JSON line on rank 0.
+
+Multi-GPU (torchrun, one rank per GPU): walkers are independent Markov chains, so
+each rank runs its own 512 walkers against its own replica of the table; there is no data-path
+collective ("scaling": "weak").  Time = max over ranks.
+
+--impl reference times the fp64 CPU oracle (oracle/qmc_oracle.c), as it stands, on the host cores,
+on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+import numpy as np
+import torch
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1802_06922_b200 import inputs  # noqa: E402
+
+METRIC = "electron moves/s at N=1024 (spline VGL+ratio+SM update); HBM GB/s vs peak"
+UNIT = "moves/s"
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons with NVML every 100 ms while the timed region runs."""
+
+    def __init__(self, index):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def _run(self):
+        nv = self.nv
+        names = {
+            getattr(nv, "nvmlClocksThrottleReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(nv, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0x4): "sw_power_cap",
+            getattr(nv, "nvmlClocksThrottleReasonHwPowerBrakeSlowdown", 0x80): "hw_power_brake",
+        }
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            self._stop.wait(0.1)
+
+    def start(self):
+        if self.nv is not None:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+
+    def stop(self):
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join()
+        med = statistics.median(self.samples) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons)}
+
+
+def cpu_sample(x, coefs_np, target_s=15.0):
+    """The oracle, as it stands, on a bounded sample of the workload: `cores` walkers (one per
+    thread) x the first M electron moves of a sweep.  Returns (moves/s, cores, sample text, seconds)."""
+    import oracle
+    cores = len(os.sched_getaffinity(0))
+    nthreads = max(1, min(cores, oracle.max_threads(), 32, x.pos.shape[0]))
+    nwc, nel = nthreads, x.cfg.norb
+    pos = np.ascontiguousarray(x.pos[:nwc])
+    B, ld, sg = oracle.init_walkers(coefs_np, x.lattice, pos, nthreads=nthreads)       # untimed set-up
+    delta = np.ascontiguousarray(x.delta[:1, :, :nwc])
+    unif = np.ascontiguousarray(x.unif[:1, :, :nwc])
+    probe = min(8, nel)
+    t0 = time.perf_counter()
+    oracle.sweep(coefs_np, x.lattice, pos, B, ld, sg, delta, unif, iel_count=probe, nthreads=nthreads)
+    t_probe = time.perf_counter() - t0
+    m = int(min(nel, max(probe, target_s / max(t_probe / probe, 1e-6))))
+    t0 = time.perf_counter()
+    out = oracle.sweep(coefs_np, x.lattice, pos, B, ld, sg, delta, unif, iel_count=m, nthreads=nthreads)
+    dt = time.perf_counter() - t0
+    acc = float(out["accept"][0, :m].mean())
+    text = (f"{nwc} walkers x first {m} electron moves of one sweep of config '{x.cfg.name}' "
+            f"(accept {acc:.2f}), {nthreads} OpenMP threads, {dt:.1f} s")
+    return nwc * m / dt, nthreads, text, dt
+
+
+def run_reference(args, rank, world):
+    """--impl reference: the CPU oracle arm (rank 0 only)."""
+    if rank != 0:
+        return
+    cfg = inputs.CONFIGS[args.config]
+    dev = "cuda" if torch.cuda.is_available() else "cpu"
+    x = inputs.make_inputs(cfg, device=dev, nw=min(cfg.nw, 64), nsweeps=1)
+    coefs_np = x.coefs_numpy()
+    x.coefs = None
+    if dev == "cuda":
+        torch.cuda.empty_cache()
+    vals, secs = [], []
+    per_step = max(5.0, min(30.0, 120.0 / max(1, args.steps + args.warmup)))
+    info = None
+    for i in range(args.warmup + args.steps):
+        v, cores, text, dt = cpu_sample(x, coefs_np, target_s=per_step)
+        if i >= args.warmup:
+            vals.append(v)
+            secs.append(dt)
+            info = (cores, text)
+    value = float(np.mean(vals))
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "impl": "reference", "n_gpus": 0,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean(secs)),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic (seeded; paper_1802_06922_b200/inputs.py)",
+        "config": {"workload": args.config, "grid": list(cfg.grid), "N": cfg.norb,
+                   "sample": info[1]},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": info[0], "kind": "oracle", "sample": info[1]},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="large", choices=list(inputs.CONFIGS))
+    ap.add_argument("--delay", type=int, default=0, help="0 = Sherman-Morrison rank-1; k >= 2 = delayed rank-k")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--walkers", type=int, default=0, help="override walkers per GPU (debug)")
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+    args.warmup = max(args.warmup, 3)
+
+    from paper_1802_06922_b200 import api
+    api.load_library()                       # no fallback: raises if the CUDA library is missing
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (use --impl reference for the CPU oracle)"
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    cfg = inputs.CONFIGS[args.config]
+    nw = args.walkers or cfg.nw
+    nel = cfg.norb
+    nsteps_total = args.warmup + args.steps
+    # every rank draws the inputs of all ranks and keeps its own walkers (weak scaling)
+    x = inputs.make_inputs(cfg, device=dev, nw=nw * world, nsweeps=nsteps_total)
+    sl = slice(rank * nw, (rank + 1) * nw)
+    pos_np = np.ascontiguousarray(x.pos[sl])
+    delta_np = np.ascontiguousarray(x.delta[:, :, sl])
+    unif_np = np.ascontiguousarray(x.unif[:, :, sl])
+
+    spline = api.Spline.create(x.coefs, x.lattice)
+    torch.cuda.synchronize()
+    coefs_np = None
+    want_cpu = rank == 0 and world == 1 and not args.no_cpu_baseline
+    if want_cpu:
+        coefs_np = x.coefs_numpy()
+    x.coefs = None
+    torch.cuda.empty_cache()
+
+    pos = torch.from_numpy(pos_np).to(dev)
+    delta = torch.from_numpy(delta_np).to(dev)
+    unif = torch.from_numpy(unif_np).to(dev)
+    accept = torch.zeros(unif.shape, dtype=torch.uint8, device=dev)
+    ratios = torch.zeros(unif.shape, dtype=torch.float64, device=dev)
+    t0 = time.perf_counter()
+    det = api.Det.init(spline, pos, delay_rank=args.delay)
+    torch.cuda.synchronize()
+    t_init = time.perf_counter() - t0
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    def step(i):
+        api.sweep(det, pos, delta[i:i + 1], unif[i:i + 1], ratios_out=ratios[i:i + 1], accept_out=accept[i:i + 1])
+
+    # ---- device-resident timing: inputs in HBM, CUDA events on the launching stream
+    for i in range(args.warmup):
+        step(i)
+    barrier()
+    det.profile(True)
+    launches0 = api.launch_count()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for i in range(args.warmup, nsteps_total):
+        step(i)
+    e1.record()
+    barrier()
+    clocks = sampler.stop()
+    launches = api.launch_count() - launches0
+    ms = e0.elapsed_time(e1)
+    prof = det.profile_read()
+    det.profile(False)
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    moves = args.steps * nel * nw * world
+    value = moves / (ms * 1e-3)
+    acc_timed = accept[args.warmup:].to(torch.float64)
+    n_acc = float(acc_timed.sum().item())
+    acc_rate = n_acc / acc_timed.numel()
+
+    # ---- roofline of the dominant kernel (rank-local, from the per-launch CUDA events)
+    peak, peak_src = measured_peaks()
+    ld = det.ld
+    dom = max(prof, key=lambda k: prof[k][0])
+    kms, kn = prof[dom]
+    spo_ms, spo_n = prof["spo_ratio"]
+    spo_bytes_per_launch = nw * (64 * spline.row_pitch * 4 + 5 * spline.row_pitch * 4 + 2 * 8 * ld)
+    upd_bytes_per_accept = 16 * nel * ld + 12 * nel
+    if dom == "sm_update":
+        bytes_per_launch = (n_acc / max(kn, 1)) * upd_bytes_per_accept
+    elif dom == "spo_ratio":
+        bytes_per_launch = spo_bytes_per_launch
+    else:
+        bytes_per_launch = float("nan")
+    achieved = bytes_per_launch / (kms / max(kn, 1) * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                "launches": kn, "avg_us": 1e3 * kms / max(kn, 1),
+                "bytes_per_launch": bytes_per_launch, "share_of_step": kms / ms}
+    kernels = {k: {"ms": v[0], "launches": v[1]} for k, v in prof.items() if v[1]}
+    if spo_n:
+        kernels["spo_ratio"]["GB/s"] = spo_bytes_per_launch / (spo_ms / spo_n * 1e-3) / 1e9
+        kernels["spo_ratio"]["frac"] = kernels["spo_ratio"]["GB/s"] / peak
+
+    # ---- end to end through the C ABI with HOST buffers (pinned): H2D of pos/delta/unif and D2H
+    #      of pos/ratios/decisions inside the timed region, every step
+    pos_h = pos.cpu().pin_memory()
+    delta_h = torch.from_numpy(delta_np).pin_memory()
+    unif_h = torch.from_numpy(unif_np).pin_memory()
+    ratios_h = torch.zeros(unif_h.shape, dtype=torch.float64).pin_memory()
+    accept_h = torch.zeros(unif_h.shape, dtype=torch.uint8).pin_memory()
+
+    def step_host(i):
+        api.sweep_host(det, pos_h, delta_h[i:i + 1], unif_h[i:i + 1], ratios_out=ratios_h[i:i + 1],
+                       accept_out=accept_h[i:i + 1])
+
+    step_host(0)
+    barrier()
+    e0.record()
+    for i in range(args.warmup, nsteps_total):
+        step_host(i)
+    e1.record()
+    barrier()
+    ms_e2e = e0.elapsed_time(e1)
+    if world > 1:
+        t = torch.tensor([ms_e2e], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_e2e = float(t.item())
+    h2d = pos_h.numel() * 8 + delta_h[0].numel() * 8 + unif_h[0].numel() * 8
+    d2h = pos_h.numel() * 8 + ratios_h[0].numel() * 8 + accept_h[0].numel()
+    e2e = {"value": moves / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d * world,
+           "d2h_bytes_per_step": d2h * world}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic (seeded; paper_1802_06922_b200/inputs.py)",
+        "config": {"workload": args.config, "grid": list(cfg.grid), "N": nel, "walkers_per_gpu": nw,
+                   "update": "sherman-morrison rank-1" if det.delay_rank == 0 else f"delayed rank-{det.delay_rank}",
+                   "step": "one full sweep (N electron moves x walkers)",
+                   "l2": "working set (8.6 GB table + 4.3 GB inverses) exceeds L2; no flush needed",
+                   "spo_dtype": "f32", "accept_rate": acc_rate, "init_s": t_init},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
+        "kernels": kernels, "spline_evals_per_s": value * nel,
+    }
+
+    if want_cpu:
+        xs = inputs.QmcInputs(cfg, x.lattice, None, pos_np, delta_np, unif_np)
+        v, cores, text, _ = cpu_sample(xs, coefs_np)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": text}
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    det.destroy()
+    spline.destroy()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

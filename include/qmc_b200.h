@@ -195,6 +195,20 @@ int qmc_det_get_stats(qmc_det_t *det, double *logdet, int *sign, long long *nacc
                       void *stream);
 int qmc_det_info(const qmc_det_t *det, int *nwalkers, int *nel, int *ld, int *delay_rank);
 
+/* ---------------------------------------------------------------------------------------
+ * Per-kernel timing of qmc_sweep* (bench.py's roofline): with profiling enabled every kernel
+ * launch of a sweep is bracketed by CUDA events on the launching stream.
+ *   qmc_det_profile(det, 1)   enable and reset;  (det, 0) disable
+ *   qmc_det_profile_read      synchronises the recorded events and returns, per kernel kind,
+ *                             the summed device time in ms and the number of launches; host
+ *                             arrays of QMC_PROF_KINDS entries.  Kinds: 0 fused SPO-VGL+ratio,
+ *                             1 rank-1 update, 2 delayed ratio, 3 delayed accept, 4 delayed flush.
+ *                             Resets the recorder.
+ */
+#define QMC_PROF_KINDS 5
+int qmc_det_profile(qmc_det_t *det, int enable);
+int qmc_det_profile_read(qmc_det_t *det, double *ms_host, long long *launches_host);
+
 /* Number of kernel launches this library has enqueued since load (bench.py's gpu_launches). */
 long long qmc_launch_count(void);
 

@@ -51,6 +51,9 @@ def _load():
         lib.orc_sweep.argtypes = ([ctypes.c_int] * 4 + [_dp, _fp, ctypes.c_int, ctypes.c_int,
                                   _dp, _dp, _dp, _dp, _ip, _dp, _dp, ctypes.c_int, ctypes.c_int,
                                   _dp, _bp, _bp, _fp, _dp, ctypes.c_int, ctypes.c_int])
+        lib.orc_init_walkers.restype = ctypes.c_int
+        lib.orc_init_walkers.argtypes = ([ctypes.c_int] * 4 + [_dp, _fp, ctypes.c_int, ctypes.c_int,
+                                         _dp, _dp, _dp, _dp, _ip, ctypes.c_int])
         lib.orc_max_threads.restype = ctypes.c_int
         lib.orc_max_threads.argtypes = []
         _lib = lib
@@ -154,6 +157,24 @@ def slater_matrix(coefs, lattice, pos):
                                _d(pos), _d(A))
     _check(rc, "slater_matrix")
     return A
+
+
+def init_walkers(coefs, lattice, pos, nthreads=1, want_A=False):
+    """pos [nw][nel][3] -> (B [nw][nel][nel], logdet [nw], sign [nw]) (+ A if want_A)."""
+    lib = _load()
+    coefs = _coefs(coefs)
+    nx, ny, nz, norb = coefs.shape
+    lat = _c64(lattice).reshape(9)
+    pos = _c64(pos)
+    nw, nel, _ = pos.shape
+    A = np.empty((nw, nel, nel)) if want_A else None
+    B = np.empty((nw, nel, nel))
+    ld = np.empty(nw)
+    sg = np.empty(nw, dtype=np.int32)
+    rc = lib.orc_init_walkers(nx, ny, nz, norb, _d(lat), coefs.ctypes.data_as(_fp), nw, nel, _d(pos),
+                              _d(A), _d(B), _d(ld), sg.ctypes.data_as(_ip), int(nthreads))
+    _check(rc, "init_walkers")
+    return (B, ld, sg, A) if want_A else (B, ld, sg)
 
 
 def sweep(coefs, lattice, pos, B, logdet, sign, delta, unif, A=None, iel_count=None,

@@ -400,6 +400,35 @@ int orc_slater_matrix(int nx, int ny, int nz, int norb, const double lattice[9],
     return orc_spline_vgl(nx, ny, nz, norb, lattice, coefs, nw * nel, pos, A, NULL, NULL);
 }
 
+/* Slater matrix, B = (A^-1)^T, log|det| and sign of every walker (walkers are independent,
+ * L181: OpenMP over walkers).  A may be NULL.  Returns 0 or the first error code met. */
+int orc_init_walkers(int nx, int ny, int nz, int norb, const double lattice[9], const float *coefs,
+                     int nw, int nel, const double *pos, double *A, double *B, double *logdet,
+                     int *sign, int nthreads)
+{
+    if (nel != norb) return -1;
+    int rc_all = 0;
+    size_t nn = (size_t)nel * nel;
+#ifdef _OPENMP
+    if (nthreads < 1) nthreads = 1;
+#pragma omp parallel for schedule(dynamic) num_threads(nthreads)
+#endif
+    for (int w = 0; w < nw; ++w) {
+        double *Aw = A ? A + (size_t)w * nn : (double *)malloc(nn * sizeof(double));
+        int rc = Aw ? 0 : -2;
+        if (!rc) rc = orc_spline_vgl(nx, ny, nz, norb, lattice, coefs, nel, pos + (size_t)w * nel * 3, Aw, NULL, NULL);
+        if (!rc) rc = orc_binv_from_A(nel, Aw, B + (size_t)w * nn, logdet + w, sign + w);
+        if (!A) free(Aw);
+        if (rc) {
+#ifdef _OPENMP
+#pragma omp critical
+#endif
+            if (!rc_all) rc_all = rc;
+        }
+    }
+    return rc_all;
+}
+
 int orc_max_threads(void)
 {
 #ifdef _OPENMP

@@ -20,8 +20,9 @@ EXPORTS = [
     "qmc_last_error", "qmc_spline_create", "qmc_spline_destroy", "qmc_spline_info", "qmc_spo_vgl",
     "qmc_det_init", "qmc_det_destroy", "qmc_det_ratio", "qmc_det_accept_update", "qmc_det_flush",
     "qmc_sweep", "qmc_sweep_ex", "qmc_sweep_host", "qmc_det_get_inverse", "qmc_det_set_inverse",
-    "qmc_det_get_stats", "qmc_det_info", "qmc_launch_count",
+    "qmc_det_get_stats", "qmc_det_info", "qmc_launch_count", "qmc_det_profile", "qmc_det_profile_read",
 ]
+PROF_KINDS = ["spo_ratio", "sm_update", "delayed_ratio", "delayed_accept", "delayed_flush"]
 
 
 class SweepOpts(ctypes.Structure):
@@ -66,6 +67,8 @@ def load_library(path=None):
         "qmc_det_set_inverse": [_vp, _vp, _vp, _vp, _vp],
         "qmc_det_get_stats": [_vp, _vp, _vp, _vp, _vp],
         "qmc_det_info": [_vp] + [ctypes.POINTER(i)] * 4,
+        "qmc_det_profile": [_vp, i],
+        "qmc_det_profile_read": [_vp, ctypes.POINTER(d), ctypes.POINTER(ctypes.c_longlong)],
     }
     for name, args in sigs.items():
         fn = getattr(lib, name)
@@ -234,6 +237,18 @@ class Det:
                                                 _dev(logdet, torch.float64, True),
                                                 _dev(sign, torch.int32, True), _stream(stream))
         _check(rc, "qmc_det_set_inverse")
+
+    def profile(self, enable=True):
+        """qmc_det_profile: bracket every sweep kernel with CUDA events (and reset the recorder)."""
+        _check(load_library().qmc_det_profile(self._h, 1 if enable else 0), "qmc_det_profile")
+
+    def profile_read(self):
+        """qmc_det_profile_read -> {kind: (total ms, launches)}; synchronises the recorded events."""
+        n = len(PROF_KINDS)
+        ms = (ctypes.c_double * n)()
+        cnt = (ctypes.c_longlong * n)()
+        _check(load_library().qmc_det_profile_read(self._h, ms, cnt), "qmc_det_profile_read")
+        return {k: (ms[j], cnt[j]) for j, k in enumerate(PROF_KINDS)}
 
     def get_stats(self, stream=None):
         """(logdet double [nw], sign int32 [nw], naccept int64 [nw])."""

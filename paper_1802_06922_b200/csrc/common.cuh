@@ -6,6 +6,8 @@
 #include <stdint.h>
 #include <stdio.h>
 
+#include <vector>
+
 #include "qmc_b200.h"
 
 namespace qmc {
@@ -84,7 +86,20 @@ struct qmc_det {
     // device staging of qmc_sweep_host (grown on demand)
     void *stage;
     size_t stage_bytes;
+    // per-kernel timing (qmc_det_profile): CUDA events around every launch of a sweep
+    int prof_on;
+    std::vector<cudaEvent_t> *prof_events;   // pool, pairs (start, stop)
+    std::vector<int> *prof_kinds;            // kind of pair i
+    size_t prof_used;                        // events handed out since the last reset
 };
+
+namespace qmc {
+enum ProfKind { kProfSpoRatio = 0, kProfUpdate = 1, kProfDelayedRatio = 2, kProfDelayedAccept = 3,
+                kProfDelayedFlush = 4, kProfKinds = 5 };
+// Record a start / stop event pair around a launch when profiling is enabled (no-ops otherwise).
+void prof_start(qmc_det *d, int kind, cudaStream_t s);
+void prof_stop(qmc_det *d, cudaStream_t s);
+}
 
 namespace qmc {
 

@@ -198,9 +198,35 @@ static int dev_alloc(T **p, size_t count, const char *what)
     return QMC_OK;
 }
 
+void prof_start(qmc_det *d, int kind, cudaStream_t s)
+{
+    if (!d->prof_on) return;
+    if (!d->prof_events) { d->prof_events = new std::vector<cudaEvent_t>(); d->prof_kinds = new std::vector<int>(); }
+    while (d->prof_events->size() < d->prof_used + 2) {
+        cudaEvent_t e;
+        if (cudaEventCreate(&e) != cudaSuccess) { d->prof_on = 0; return; }
+        d->prof_events->push_back(e);
+    }
+    d->prof_kinds->resize(d->prof_used / 2 + 1);
+    (*d->prof_kinds)[d->prof_used / 2] = kind;
+    cudaEventRecord((*d->prof_events)[d->prof_used], s);
+}
+
+void prof_stop(qmc_det *d, cudaStream_t s)
+{
+    if (!d->prof_on) return;
+    cudaEventRecord((*d->prof_events)[d->prof_used + 1], s);
+    d->prof_used += 2;
+}
+
 static void det_free(qmc_det *d)
 {
     if (!d) return;
+    if (d->prof_events) {
+        for (cudaEvent_t e : *d->prof_events) cudaEventDestroy(e);
+        delete d->prof_events;
+        delete d->prof_kinds;
+    }
     cudaFree(d->B); cudaFree(d->logdet); cudaFree(d->sign); cudaFree(d->naccept);
     cudaFree(d->vgl); cudaFree(d->rowk); cudaFree(d->rpart); cudaFree(d->ratio); cudaFree(d->acc);
     cudaFree(d->win_count); cudaFree(d->win_iel); cudaFree(d->win_phi); cudaFree(d->win_rows);
@@ -331,6 +357,30 @@ extern "C" int qmc_det_destroy(qmc_det_t *d)
     det_free(d);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) { set_error("qmc_det_destroy: %s", cudaGetErrorString(e)); return QMC_ECUDA; }
+    return QMC_OK;
+}
+
+extern "C" int qmc_det_profile(qmc_det_t *d, int enable)
+{
+    QMC_REQUIRE(d, "qmc_det_profile: NULL handle");
+    d->prof_on = enable ? 1 : 0;
+    d->prof_used = 0;
+    return QMC_OK;
+}
+
+extern "C" int qmc_det_profile_read(qmc_det_t *d, double *ms, long long *launches)
+{
+    QMC_REQUIRE(d && ms && launches, "qmc_det_profile_read: NULL argument");
+    for (int k = 0; k < kProfKinds; ++k) { ms[k] = 0.0; launches[k] = 0; }
+    for (size_t i = 0; i + 1 < d->prof_used; i += 2) {
+        QMC_CUDA(cudaEventSynchronize((*d->prof_events)[i + 1]));
+        float t = 0.f;
+        QMC_CUDA(cudaEventElapsedTime(&t, (*d->prof_events)[i], (*d->prof_events)[i + 1]));
+        const int k = (*d->prof_kinds)[i / 2];
+        ms[k] += (double)t;
+        launches[k] += 1;
+    }
+    d->prof_used = 0;
     return QMC_OK;
 }
 

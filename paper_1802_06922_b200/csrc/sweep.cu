@@ -110,7 +110,9 @@ static int sweep_impl(qmc_det *d, const qmc_spline *sp, double *pos, const doubl
                 if (rc) return rc;
                 continue;
             }
+            prof_start(d, kProfSpoRatio, s);
             spo_ratio_kernel<<<dim3(tiles, nw), threads, 0, s>>>(a);
+            prof_stop(d, s);
             QMC_LAUNCHED();
             UpdateArgs u{};
             u.B = d->B; u.nel = nel; u.ld = d->ld; u.iel = k;
@@ -122,7 +124,10 @@ static int sweep_impl(qmc_det *d, const qmc_spline *sp, double *pos, const doubl
             u.accept_out = accept_out ? accept_out + mv : nullptr;
             u.pos = pos; u.delta = delta + 3 * mv;
             u.logdet = d->logdet; u.sign = d->sign; u.naccept = d->naccept;
-            QMC_CUDA(launch_sm_update<true>(u, nw, s));
+            prof_start(d, kProfUpdate, s);
+            cudaError_t ue = launch_sm_update<true>(u, nw, s);
+            prof_stop(d, s);
+            QMC_CUDA(ue);
         }
         if (d->delay) {
             int rc = delayed_flush(d, s);

@@ -84,7 +84,8 @@ def custom_config(name, grid, norb, lattice, nw, nsweeps=1, sigma=None, coef_kin
         lens = lat if lat.ndim == 1 else np.linalg.norm(lat.reshape(3, 3), axis=1)
         sigma = 0.8 * float(np.min(lens / np.asarray(grid)))
     if kmax is None:
-        kmax = tuple(max(1, min(g // 6, 8)) for g in grid)
+        # pool of (2k+1)^3 plane waves must exceed norb, or the Slater matrix is singular (R:A17)
+        kmax = tuple(max(1, min(g // 3, 8)) for g in grid)
     lat_t = tuple(map(float, lat)) if lat.ndim == 1 else tuple(map(tuple, lat.reshape(3, 3).tolist()))
     return QmcConfig(name, index, tuple(grid), int(norb), lat_t, int(nw), int(nsweeps),
                      float(sigma), coef_kind, tuple(kmax))

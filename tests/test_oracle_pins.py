@@ -398,3 +398,11 @@ def test_accept_control_flow(sweep_case):
     out_mt = oracle.sweep(coefs, x.lattice, x.pos, B, ld, sg, x.delta, x.unif, nthreads=3)
     out_st = oracle.sweep(coefs, x.lattice, x.pos, B, ld, sg, x.delta, x.unif, nthreads=1)
     assert np.array_equal(out_mt["B"], out_st["B"]) and np.array_equal(out_mt["ratios"], out_st["ratios"])
+
+
+def test_init_walkers_matches_numpy(sweep_case):
+    x, coefs, A, B, ld, sg = sweep_case
+    B2, ld2, sg2, A2 = oracle.init_walkers(coefs, x.lattice, x.pos, nthreads=2, want_A=True)
+    assert np.array_equal(A2, A) and np.array_equal(B2, B) and np.array_equal(ld2, ld) and np.array_equal(sg2, sg)
+    for w in range(x.cfg.nw):
+        assert np.max(np.abs(B2[w].T - np.linalg.inv(A[w]))) < 1e-9 * np.max(np.abs(B2[w]))
