@@ -329,6 +329,8 @@ int orc_sm_update(int n, double *B, int k, const double *phi, double R)
  *   phi_out NULL, or double [nsweeps][nel][nw][nel]: the vectors used
  *   mode    0 = Sherman-Morrison update on accept (orc_sm_update);
  *           1 = definitional: recompute B by LU from A after every accept
+ *   bnorm_out  NULL, or [nsweeps][nel][nw]: sum_j |B[k][j]| of the row used by each ratio (a
+ *           diagnostic: it bounds how an error in phi propagates into R)
  *   nthreads  OpenMP threads over walkers (<=1: serial)
  *
  * Accept iff R*R > u; a non-finite R is rejected (R:A8).  On accept:
@@ -339,7 +341,7 @@ int orc_sweep(int nx, int ny, int nz, int norb, const double lattice[9], const f
               int nw, int nel, double *pos, double *B, double *A, double *logdet, int *sign,
               const double *delta, const double *unif, int nsweeps, int iel_count,
               double *ratios_out, unsigned char *accept_out, const unsigned char *forced,
-              const float *phi_in, double *phi_out, int mode, int nthreads)
+              const float *phi_in, double *phi_out, int mode, int nthreads, double *bnorm_out)
 {
     if (nel != norb || nw < 0 || nsweeps < 0 || iel_count < 0 || iel_count > nel) return -1;
     if (mode == 1 && !A) return -1;
@@ -372,6 +374,11 @@ int orc_sweep(int nx, int ny, int nz, int norb, const double lattice[9], const f
                 if (forced) acc = forced[mv] != 0;
                 else acc = isfinite(R) && (R * R > unif[mv]);
                 if (ratios_out) ratios_out[mv] = R;
+                if (bnorm_out) {
+                    double bn = 0.0;
+                    for (int j = 0; j < nel; ++j) bn += fabs(Bw[(size_t)k * nel + j]);
+                    bnorm_out[mv] = bn;
+                }
                 if (accept_out) accept_out[mv] = (unsigned char)acc;
                 if (!acc) continue;
                 rk[0] = rnew[0]; rk[1] = rnew[1]; rk[2] = rnew[2];

@@ -406,3 +406,14 @@ def test_init_walkers_matches_numpy(sweep_case):
     assert np.array_equal(A2, A) and np.array_equal(B2, B) and np.array_equal(ld2, ld) and np.array_equal(sg2, sg)
     for w in range(x.cfg.nw):
         assert np.max(np.abs(B2[w].T - np.linalg.inv(A[w]))) < 1e-9 * np.max(np.abs(B2[w]))
+
+
+def test_bnorm_diagnostic(sweep_case):
+    """bnorm_out is the 1-norm of the row the ratio used: for the first move of walker w that is
+    row 0 of the initial inverse."""
+    x, coefs, A, B, ld, sg = sweep_case
+    out = oracle.sweep(coefs, x.lattice, x.pos, B, ld, sg, x.delta, x.unif, want_bnorm=True)
+    for w in range(x.cfg.nw):
+        assert abs(out["bnorm"][0, 0, w] - np.sum(np.abs(B[w, 0]))) < 1e-12
+    # |R - R'| <= bnorm * max|phi - phi'| for any perturbed orbital vector
+    assert np.all(out["bnorm"] > 0)
