@@ -82,7 +82,8 @@ struct qmc_det {
     double *win_rows;           // [nw][delay][ld] rows B0[k_l] saved at accept time
     double *win_sinv;           // [nw][delay][delay] inverse of S
     int *win_full;              // [1] set when any walker's window is full
-    int host_pending;           // upper bound of pending rows known to the host
+    int host_pending;           // electron steps appended to the open window (host bookkeeping)
+    unsigned char *win_host_iel;   // host [nel]: electrons touched in the open window
     // device staging of qmc_sweep_host (grown on demand)
     void *stage;
     size_t stage_bytes;

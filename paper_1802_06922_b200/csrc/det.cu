@@ -1,6 +1,7 @@
 // qmc_det_*: per-walker fp64 inverse of the Slater matrix, determinant ratio and
 // Sherman-Morrison update (L299).  See include/qmc_b200.h for the contract.
 #include <math.h>
+#include <stdlib.h>
 
 #include <new>
 #include <vector>
@@ -231,6 +232,7 @@ static void det_free(qmc_det *d)
     cudaFree(d->vgl); cudaFree(d->rowk); cudaFree(d->rpart); cudaFree(d->ratio); cudaFree(d->acc);
     cudaFree(d->win_count); cudaFree(d->win_iel); cudaFree(d->win_phi); cudaFree(d->win_rows);
     cudaFree(d->win_sinv); cudaFree(d->win_full); cudaFree(d->stage);
+    free(d->win_host_iel);
     delete d;
 }
 
@@ -305,6 +307,14 @@ extern "C" int qmc_det_init(qmc_det_t **out, const qmc_spline_t *sp, int nw, int
         return rc;
     }
     if (K) {
+        const int kmax = delayed_max_rank(ld);
+        if (K > kmax) {
+            set_error("qmc_det_init: delay_rank=%d does not fit shared memory for nel=%d (max %d)", K, nel, kmax);
+            det_free(d);
+            return QMC_EINVAL;
+        }
+        d->win_host_iel = (unsigned char *)calloc((size_t)nel, 1);
+        if (!d->win_host_iel) { set_error("qmc_det_init: host allocation failed"); det_free(d); return QMC_ENOMEM; }
         if ((rc = dev_alloc(&d->win_count, nw, "win_count")) || (rc = dev_alloc(&d->win_iel, (size_t)nw * K, "win_iel")) ||
             (rc = dev_alloc(&d->win_phi, (size_t)nw * K * np, "win_phi")) ||
             (rc = dev_alloc(&d->win_rows, (size_t)nw * K * ld, "win_rows")) ||
@@ -429,7 +439,7 @@ extern "C" int qmc_det_flush(qmc_det_t *d, void *stream)
 {
     QMC_REQUIRE(d, "qmc_det_flush: NULL handle");
     if (!d->delay) return QMC_OK;
-    return delayed_flush(d, (cudaStream_t)stream);
+    return delayed_flush_reset_host(d, (cudaStream_t)stream);
 }
 
 extern "C" int qmc_det_get_inverse(qmc_det_t *d, double *out, void *stream)

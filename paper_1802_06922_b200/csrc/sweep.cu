@@ -28,6 +28,7 @@ struct SpoRatioArgs {
 // multiplies the values with the matching four entries of row iel of B (fp64) and copies those
 // entries to rowk, so the update kernel can overwrite B in place.  The block's partial ratio is
 // reduced in a fixed order; the (at most 8) tiles are added by the update kernel.
+template <bool WITH_RATIO>
 __global__ void __launch_bounds__(256) spo_ratio_kernel(SpoRatioArgs a)
 {
     __shared__ StencilSmem st;
@@ -48,15 +49,17 @@ __global__ void __launch_bounds__(256) spo_ratio_kernel(SpoRatioArgs a)
         *reinterpret_cast<float4 *>(o + 2 * (size_t)np) = gy;
         *reinterpret_cast<float4 *>(o + 3 * (size_t)np) = gz;
         *reinterpret_cast<float4 *>(o + 4 * (size_t)np) = lp;
-        const double2 *brow = reinterpret_cast<const double2 *>(a.B + ((size_t)w * a.nel + a.iel) * a.ld + col);
-        const double2 b0 = brow[0], b1 = brow[1];
-        double2 *rk = reinterpret_cast<double2 *>(a.rowk + (size_t)w * a.ld + col);
-        rk[0] = b0;
-        rk[1] = b1;
-        part = fma(b0.x, (double)v.x, part);
-        part = fma(b0.y, (double)v.y, part);
-        part = fma(b1.x, (double)v.z, part);
-        part = fma(b1.y, (double)v.w, part);
+        if (WITH_RATIO) {
+            const double2 *brow = reinterpret_cast<const double2 *>(a.B + ((size_t)w * a.nel + a.iel) * a.ld + col);
+            const double2 b0 = brow[0], b1 = brow[1];
+            double2 *rk = reinterpret_cast<double2 *>(a.rowk + (size_t)w * a.ld + col);
+            rk[0] = b0;
+            rk[1] = b1;
+            part = fma(b0.x, (double)v.x, part);
+            part = fma(b0.y, (double)v.y, part);
+            part = fma(b1.x, (double)v.z, part);
+            part = fma(b1.y, (double)v.w, part);
+        }
         if (a.phi_record && w < a.nrecord) {
             float *rec = a.phi_record + (size_t)w * a.nel;
             if (col + 0 < a.nel) rec[col + 0] = v.x;
@@ -65,8 +68,28 @@ __global__ void __launch_bounds__(256) spo_ratio_kernel(SpoRatioArgs a)
             if (col + 3 < a.nel) rec[col + 3] = v.w;
         }
     }
-    part = block_sum(part, red);
-    if (threadIdx.x == 0) a.rpart[(size_t)w * kRatioTilesMax + blockIdx.x] = part;
+    if (WITH_RATIO) {
+        part = block_sum(part, red);
+        if (threadIdx.x == 0) a.rpart[(size_t)w * kRatioTilesMax + blockIdx.x] = part;
+    }
+}
+
+int spo_proposal_vgl(qmc_det *d, const qmc_spline *sp, const double *pos, const double *delta, int iel,
+                     float *phi_record, int nrecord, cudaStream_t s)
+{
+    int threads, tiles;
+    spo_launch_shape(d->np, &threads, &tiles);
+    SpoRatioArgs a{};
+    a.sp = sp->view;
+    a.pos = pos; a.delta = delta;
+    a.nel = d->nel; a.iel = iel; a.ld = d->ld;
+    a.B = d->B; a.vgl = d->vgl; a.rowk = d->rowk; a.rpart = d->rpart;
+    a.phi_record = phi_record; a.nrecord = nrecord;
+    prof_start(d, kProfSpoRatio, s);
+    spo_ratio_kernel<false><<<dim3(tiles, d->nw), threads, 0, s>>>(a);
+    prof_stop(d, s);
+    QMC_LAUNCHED();
+    return QMC_OK;
 }
 
 static int sweep_impl(qmc_det *d, const qmc_spline *sp, double *pos, const double *delta, const double *unif,
@@ -111,7 +134,7 @@ static int sweep_impl(qmc_det *d, const qmc_spline *sp, double *pos, const doubl
                 continue;
             }
             prof_start(d, kProfSpoRatio, s);
-            spo_ratio_kernel<<<dim3(tiles, nw), threads, 0, s>>>(a);
+            spo_ratio_kernel<true><<<dim3(tiles, nw), threads, 0, s>>>(a);
             prof_stop(d, s);
             QMC_LAUNCHED();
             UpdateArgs u{};
@@ -130,7 +153,7 @@ static int sweep_impl(qmc_det *d, const qmc_spline *sp, double *pos, const doubl
             QMC_CUDA(ue);
         }
         if (d->delay) {
-            int rc = delayed_flush(d, s);
+            int rc = delayed_flush_reset_host(d, s);
             if (rc) return rc;
         }
     }

@@ -218,3 +218,79 @@ def test_full_size_sampled(name, nchk, npos):
     spline.destroy()
     out = P.run_protocol(x, walkers=nchk, free_oracle=(name == "mid"), coefs_np=coefs_np)
     print(name, out)
+
+
+# ------------------------------------------------------------------------------- delayed rank-k
+@pytest.mark.parametrize("case,K", [("tiny", 2), ("tiny", 5), ("ragged37_skew", 4), ("ragged37_skew", 16),
+                                    ("n130_two_tiles", 7), ("small", 16), ("small", 32)])
+def test_delayed_sweep_parity_protocol(case, K):
+    """The delayed update has no oracle of its own: it must reach the Sherman-Morrison / LU result
+    (DESIGN.md R:O7), so the same protocol and tolerances apply.  Windows of K steps do not divide
+    the sweep length in most cases (ragged last window), and rejected moves leave windows partly
+    filled."""
+    x = CASES[case]()
+    out = P.run_protocol(x, delay_rank=K, coefs_np=x.coefs_numpy())
+    print(case, K, out)
+
+
+def test_delayed_equals_rank1_on_gpu():
+    x = CASES["n130_two_tiles"]()
+    spline = api.Spline.create(x.coefs.to(P.dev()), x.lattice)
+    pos0, delta, unif = P.to_dev(x.pos), P.to_dev(x.delta), P.to_dev(x.unif)
+    res = {}
+    for K in (0, 3, 16):
+        det = api.Det.init(spline, pos0, delay_rank=K)
+        assert det.delay_rank == (K if K > 1 else 0)
+        pos = pos0.clone()
+        R = torch.zeros_like(unif)
+        acc = torch.zeros(unif.shape, dtype=torch.uint8, device=P.dev())
+        api.sweep(det, pos, delta, unif, ratios_out=R, accept_out=acc)
+        res[K] = (pos, R, acc, det.get_inverse(), det.get_stats())
+        det.destroy()
+    for K in (3, 16):
+        assert torch.equal(res[K][2], res[0][2]) and torch.equal(res[K][0], res[0][0])
+        assert float((res[K][1] - res[0][1]).abs().max() / res[0][1].abs().max()) < 1e-11
+        scale = float(res[0][3].abs().max())
+        assert float((res[K][3] - res[0][3]).abs().max()) < 1e-10 * scale
+        assert float((res[K][4][0] - res[0][4][0]).abs().max()) < 1e-9
+        assert torch.equal(res[K][4][1], res[0][4][1]) and torch.equal(res[K][4][2], res[0][4][2])
+    spline.destroy()
+
+
+def test_delayed_standalone_api():
+    """qmc_det_ratio / qmc_det_accept_update / qmc_det_flush with delay_rank = 4: electrons in any
+    order, repeated electrons (forces an early flush), all-reject steps, explicit flush."""
+    x = CASES["ragged37_skew"]()
+    nw, nel = x.pos.shape[0], x.cfg.norb
+    spline = api.Spline.create(x.coefs.to(P.dev()), x.lattice)
+    pos_t = P.to_dev(x.pos)
+    det = api.Det.init(spline, pos_t, delay_rank=4)
+    B, ld, sg = P.oracle_binv(P.gpu_slater(spline, pos_t))
+    rng = np.random.default_rng(5)
+    order = list(rng.integers(0, nel, size=40)) + [3, 3, 3, 7, 3]
+    for step, k in enumerate(order):
+        k = int(k)
+        phi = api.spo_vgl(spline, P.to_dev(x.pos[:, k] + rng.normal(0, 0.2, size=(nw, 3))), want_gl=False)
+        R = det.ratio(k, phi)
+        phi_np = phi[:, :nel].double().cpu().numpy()
+        R_o = np.array([oracle.det_ratio(B[w], k, phi_np[w]) for w in range(nw)])
+        assert np.max(np.abs(R.cpu().numpy() - R_o) / np.abs(R_o)) < P.TOL_RATIO, step
+        acc = rng.integers(0, 2, size=nw).astype(np.uint8)
+        if step % 7 == 0:
+            acc[:] = 0
+        det.accept_update(k, phi, R, P.to_dev(acc))
+        for w in range(nw):
+            if acc[w]:
+                B[w] = oracle.sm_update(B[w], k, phi_np[w], R_o[w])
+                ld[w] += np.log(abs(R_o[w]))
+                sg[w] *= 1 if R_o[w] > 0 else -1
+        if step == 20:
+            det.flush()
+    Bg = det.get_inverse().cpu().numpy()          # flushes the open window
+    assert np.max(np.abs(Bg - B)) < P.TOL_BINV * max(1.0, np.max(np.abs(B)))
+    ldg, sgg, _ = (t.cpu().numpy() for t in det.get_stats())
+    assert np.max(np.abs(ldg - ld)) < 1e-8 and np.array_equal(sgg, sg)
+    det.destroy()
+    with pytest.raises(api.QmcError):
+        api.Det.init(spline, pos_t, delay_rank=33)
+    spline.destroy()
