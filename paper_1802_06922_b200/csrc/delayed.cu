@@ -175,226 +175,7 @@ __global__ void __launch_bounds__(kStepThreads) delayed_step_kernel(DelayedStepA
     }
 }
 
-// ---------------------------------------------------------------------------------------------
-// flush
-
-// Reduce NV (power of two <= 32) per-lane partials across the warp with NV-1 + log2(32/NV)
-// shuffle-adds; afterwards lane L holds the total of value L / (32 / NV).  Fixed order.
-template <int NV>
-__device__ __forceinline__ double warp_multi_reduce(double (&v)[NV])
-{
-    const int lane = threadIdx.x & 31;
-    int n = NV;
-#pragma unroll
-    for (int off = 16; off >= 1; off >>= 1) {
-        if (n > 1) {
-            n >>= 1;
-            const bool upper = (lane & off) != 0;
-#pragma unroll
-            for (int i = 0; i < NV / 2; ++i) {
-                if (i < n) {
-                    const double send = upper ? v[i] : v[i + n];
-                    const double keep = upper ? v[i + n] : v[i];
-                    v[i] = keep + __shfl_xor_sync(0xffffffffu, send, off);
-                }
-            }
-        } else {
-            v[0] += __shfl_xor_sync(0xffffffffu, v[0], off);
-        }
-    }
-    return v[0];
-}
-
-struct FlushArgs {
-    double *B;                    // [nw][nel][ld]
-    int nel, ld, np, K;
-    const int *win_count;
-    const int *win_iel;
-    const float *win_phi;
-    const double *win_rows;
-    const double *win_sinv;
-};
-
-constexpr int kFlushThreads = 256;
-constexpr int kFlushRowsPerCta = 64;
-
-// Single pass over B.  The window's orbital vectors (fp32) and saved rows (fp64) live in shared
-// memory for the whole CTA; a warp keeps RPW rows of B in registers, forms their p dots with the
-// vectors (multi-value butterfly reduction), multiplies by S^-1, and subtracts the p saved rows.
-template <int VPT, int KPAD, int RPW>
-__global__ void __launch_bounds__(kFlushThreads, 1) delayed_flush_kernel(FlushArgs a)
-{
-    extern __shared__ __align__(16) unsigned char smem_flush[];
-    const int w = blockIdx.y;
-    const int p = a.win_count[w];
-    if (p == 0) return;
-    const int ld = a.ld, K = a.K, np = a.np;
-    double *rows_s = reinterpret_cast<double *>(smem_flush);                    // [K][ld]
-    float *v_s = reinterpret_cast<float *>(rows_s + (size_t)K * ld);            // [K][ld]
-    double *sinv_s = reinterpret_cast<double *>(v_s + (size_t)K * ld);          // [KPAD][KPAD]
-    int *kl_s = reinterpret_cast<int *>(sinv_s + KPAD * KPAD);                  // [KPAD]
-    const double *rows_g = a.win_rows + (size_t)w * K * ld;
-    const float *v_g = a.win_phi + (size_t)w * K * np;
-    for (int e = threadIdx.x; e < p * (ld / 2); e += kFlushThreads) {
-        const int l = e / (ld / 2), c = e % (ld / 2);
-        reinterpret_cast<double2 *>(rows_s + (size_t)l * ld)[c] =
-            reinterpret_cast<const double2 *>(rows_g + (size_t)l * ld)[c];
-        float2 f = make_float2(0.f, 0.f);
-        if (2 * c < np) f = reinterpret_cast<const float2 *>(v_g + (size_t)l * np)[c];
-        reinterpret_cast<float2 *>(v_s + (size_t)l * ld)[c] = f;
-    }
-    for (int e = threadIdx.x; e < KPAD * KPAD; e += kFlushThreads) {
-        const int i = e / KPAD, j = e % KPAD;
-        sinv_s[e] = (i < p && j < p) ? a.win_sinv[(size_t)w * K * K + i * K + j] : 0.0;
-    }
-    if (threadIdx.x < KPAD) kl_s[threadIdx.x] = threadIdx.x < p ? a.win_iel[(size_t)w * K + threadIdx.x] : -1;
-    __syncthreads();
-
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    constexpr int NV = KPAD * RPW;                 // partials per lane, <= 32
-    constexpr int LPV = 32 / NV;                   // lanes per value after the reduction
-    const int my_val = lane / LPV;                 // value index this lane ends up holding
-    const int my_row = my_val / KPAD, my_l = my_val % KPAD;
-    const int m_begin = blockIdx.x * kFlushRowsPerCta, m_end = min(a.nel, m_begin + kFlushRowsPerCta);
-    for (int m0 = m_begin + wid * RPW; m0 < m_end; m0 += (kFlushThreads / 32) * RPW) {
-        double2 r[RPW][VPT];
-#pragma unroll
-        for (int q = 0; q < RPW; ++q) {
-            const int m = min(m0 + q, a.nel - 1);
-            const double2 *row = reinterpret_cast<const double2 *>(a.B + ((size_t)w * a.nel + m) * ld);
-#pragma unroll
-            for (int i = 0; i < VPT; ++i) r[q][i] = row[lane + 32 * i];
-        }
-        double part[NV];
-#pragma unroll
-        for (int i = 0; i < NV; ++i) part[i] = 0.0;
-#pragma unroll
-        for (int l = 0; l < KPAD; ++l) {
-            if (l < p) {
-                const float2 *vl = reinterpret_cast<const float2 *>(v_s + (size_t)l * ld);
-#pragma unroll
-                for (int i = 0; i < VPT; ++i) {
-                    const float2 f = vl[lane + 32 * i];
-                    const double fx = f.x, fy = f.y;
-#pragma unroll
-                    for (int q = 0; q < RPW; ++q)
-                        part[q * KPAD + l] = fma(r[q][i].x, fx, fma(r[q][i].y, fy, part[q * KPAD + l]));
-                }
-            }
-        }
-        // lane holds q_{my_l}(row my_row)
-        double qv = warp_multi_reduce<NV>(part);
-        if (my_l < p && kl_s[my_l] == m0 + my_row) qv -= 1.0;
-        // t_l = sum_l' S^-1[l][l'] q_l'   (lane computes the t of its own (row, l))
-        double t = 0.0;
-#pragma unroll
-        for (int l2 = 0; l2 < KPAD; ++l2) {
-            const double ql = __shfl_sync(0xffffffffu, qv, (my_row * KPAD + l2) * LPV);
-            t = fma(sinv_s[my_l * KPAD + l2], ql, t);
-        }
-#pragma unroll
-        for (int l = 0; l < KPAD; ++l) {
-            if (l < p) {
-                double tl[RPW];
-#pragma unroll
-                for (int q = 0; q < RPW; ++q) tl[q] = __shfl_sync(0xffffffffu, t, (q * KPAD + l) * LPV);
-                const double2 *rl = reinterpret_cast<const double2 *>(rows_s + (size_t)l * ld);
-#pragma unroll
-                for (int i = 0; i < VPT; ++i) {
-                    const double2 k2 = rl[lane + 32 * i];
-#pragma unroll
-                    for (int q = 0; q < RPW; ++q) {
-                        r[q][i].x = fma(-tl[q], k2.x, r[q][i].x);
-                        r[q][i].y = fma(-tl[q], k2.y, r[q][i].y);
-                    }
-                }
-            }
-        }
-#pragma unroll
-        for (int q = 0; q < RPW; ++q) {
-            if (m0 + q < m_end) {
-                double2 *row = reinterpret_cast<double2 *>(a.B + ((size_t)w * a.nel + m0 + q) * ld);
-#pragma unroll
-                for (int i = 0; i < VPT; ++i) row[lane + 32 * i] = r[q][i];
-            }
-        }
-    }
-}
-
-__global__ void reset_window_kernel(int nw, int *win_count)
-{
-    const int w = blockIdx.x * blockDim.x + threadIdx.x;
-    if (w < nw) win_count[w] = 0;
-}
-
-static size_t flush_smem_bytes(int K, int kpad, int ld)
-{
-    return (size_t)K * ld * (sizeof(double) + sizeof(float)) + (size_t)kpad * kpad * sizeof(double) +
-           (size_t)kpad * sizeof(int);
-}
-
-static int kpad_of(int K) { int k = 2; while (k < K) k <<= 1; return k; }
-
-// Largest delay rank whose window fits the flush kernel's shared memory for this ld.
-int delayed_max_rank(int ld)
-{
-    int best = 0;
-    for (int K = 2; K <= QMC_MAX_DELAY; ++K)
-        if (flush_smem_bytes(K, kpad_of(K), ld) <= 227 * 1024) best = K;
-    return best;
-}
-
-template <int VPT, int KPAD, int RPW>
-static cudaError_t launch_flush_t(const FlushArgs &a, int nw, size_t smem, cudaStream_t s)
-{
-    auto kern = delayed_flush_kernel<VPT, KPAD, RPW>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    dim3 grid((a.nel + kFlushRowsPerCta - 1) / kFlushRowsPerCta, nw);
-    kern<<<grid, kFlushThreads, smem, s>>>(a);
-    return cudaGetLastError();
-}
-
-template <int VPT>
-static cudaError_t launch_flush_v(const FlushArgs &a, int nw, cudaStream_t s)
-{
-    const int kpad = kpad_of(a.K);
-    const size_t smem = flush_smem_bytes(a.K, kpad, a.ld);
-    constexpr bool two = VPT <= 16;
-    switch (kpad) {
-    case 2: return launch_flush_t<VPT, 2, two ? 2 : 1>(a, nw, smem, s);
-    case 4: return launch_flush_t<VPT, 4, two ? 2 : 1>(a, nw, smem, s);
-    case 8: return launch_flush_t<VPT, 8, two ? 2 : 1>(a, nw, smem, s);
-    case 16: return launch_flush_t<VPT, 16, two ? 2 : 1>(a, nw, smem, s);
-    case 32: return launch_flush_t<VPT, 32, 1>(a, nw, smem, s);
-    }
-    return cudaErrorInvalidValue;
-}
-
-int delayed_flush(qmc_det *d, cudaStream_t s)
-{
-    if (!d->delay || d->host_pending == 0) return QMC_OK;
-    FlushArgs a{};
-    a.B = d->B; a.nel = d->nel; a.ld = d->ld; a.np = d->np; a.K = d->delay;
-    a.win_count = d->win_count; a.win_iel = d->win_iel; a.win_phi = d->win_phi;
-    a.win_rows = d->win_rows; a.win_sinv = d->win_sinv;
-    cudaError_t e;
-    prof_start(d, kProfDelayedFlush, s);
-    switch (d->ld / 64) {
-#define QMC_FL_CASE(V) case V: e = launch_flush_v<V>(a, d->nw, s); break;
-        QMC_FL_CASE(1) QMC_FL_CASE(2) QMC_FL_CASE(3) QMC_FL_CASE(4) QMC_FL_CASE(6)
-        QMC_FL_CASE(8) QMC_FL_CASE(12) QMC_FL_CASE(16) QMC_FL_CASE(24) QMC_FL_CASE(32)
-#undef QMC_FL_CASE
-    default: e = cudaErrorInvalidValue;
-    }
-    prof_stop(d, s);
-    count_launch();
-    QMC_CUDA(e);
-    reset_window_kernel<<<(d->nw + 127) / 128, 128, 0, s>>>(d->nw, d->win_count);
-    QMC_LAUNCHED();
-    d->host_pending = 0;
-    return QMC_OK;
-}
+// The flush (two DMMA contractions in one pass over B) lives in flush.cu.
 
 static cudaError_t launch_step(const DelayedStepArgs &a, int nw, cudaStream_t s)
 {
