@@ -31,10 +31,18 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-from paper_1802_06922_b200 import inputs  # noqa: E402
+from paper_1802_06922_b200 import inputs, sharding  # noqa: E402
 
 METRIC = "electron moves/s at N=1024 (spline VGL+ratio+SM update); HBM GB/s vs peak"
 UNIT = "moves/s"
+# delayed rank measured by default per config (BASELINE.json: large = rank-16; xlarge asks for rank-32,
+# the flush kernel's shared-memory window holds rank 8 at N = 2048: DESIGN.md section 6)
+DEFAULT_DELAY = {"tiny": 0, "small": 16, "mid": 16, "large": 16, "xlarge": 8}
+# fp64 tensor-core peak measured with a DMMA.8x8x4 issue loop on this pool's B200 (profiles/r01_fp64_peak.md)
+FP64_DMMA_PEAK = 37.0
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures
+# (profiles/*.md), large config
+NCU_TRAFFIC = {"sm_update": 6.725e9, "spo_ratio": 140.7e6}
 
 
 def measured_peaks():
@@ -160,7 +168,9 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="large", choices=list(inputs.CONFIGS))
-    ap.add_argument("--delay", type=int, default=0, help="0 = Sherman-Morrison rank-1; k >= 2 = delayed rank-k")
+    ap.add_argument("--delay", type=int, default=-1,
+                    help="inverse update: 0 = Sherman-Morrison rank-1; k >= 2 = delayed rank-k; default: the "
+                         "config's delayed rank as the headline AND rank-1 as a variant in the same line")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--walkers", type=int, default=0, help="override walkers per GPU (debug)")
@@ -189,10 +199,8 @@ def main():
     nsteps_total = args.warmup + args.steps
     # every rank draws the inputs of all ranks and keeps its own walkers (weak scaling)
     x = inputs.make_inputs(cfg, device=dev, nw=nw * world, nsweeps=nsteps_total)
-    sl = slice(rank * nw, (rank + 1) * nw)
-    pos_np = np.ascontiguousarray(x.pos[sl])
-    delta_np = np.ascontiguousarray(x.delta[:, :, sl])
-    unif_np = np.ascontiguousarray(x.unif[:, :, sl])
+    pos_np, delta_np, unif_np = sharding.shard_inputs(x.pos, x.delta, x.unif, rank, world)
+    assert pos_np.shape[0] == nw
 
     spline = api.Spline.create(x.coefs, x.lattice)
     torch.cuda.synchronize()
@@ -203,15 +211,11 @@ def main():
     x.coefs = None
     torch.cuda.empty_cache()
 
-    pos = torch.from_numpy(pos_np).to(dev)
     delta = torch.from_numpy(delta_np).to(dev)
     unif = torch.from_numpy(unif_np).to(dev)
-    accept = torch.zeros(unif.shape, dtype=torch.uint8, device=dev)
-    ratios = torch.zeros(unif.shape, dtype=torch.float64, device=dev)
-    t0 = time.perf_counter()
-    det = api.Det.init(spline, pos, delay_rank=args.delay)
-    torch.cuda.synchronize()
-    t_init = time.perf_counter() - t0
+    delta_h = torch.from_numpy(delta_np).pin_memory()
+    unif_h = torch.from_numpy(unif_np).pin_memory()
+    peak, peak_src = measured_peaks()
 
     def barrier():
         torch.cuda.synchronize()
@@ -219,104 +223,128 @@ def main():
             dist.barrier()
             torch.cuda.synchronize()
 
-    def step(i):
-        api.sweep(det, pos, delta[i:i + 1], unif[i:i + 1], ratios_out=ratios[i:i + 1], accept_out=accept[i:i + 1])
+    def max_over_ranks(ms):
+        return sharding.max_over_ranks(ms, device=dev)
 
-    # ---- device-resident timing: inputs in HBM, CUDA events on the launching stream
-    for i in range(args.warmup):
-        step(i)
-    barrier()
-    det.profile(True)
-    launches0 = api.launch_count()
-    sampler = ClockSampler(local_rank)
-    sampler.start()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    for i in range(args.warmup, nsteps_total):
-        step(i)
-    e1.record()
-    barrier()
-    clocks = sampler.stop()
-    launches = api.launch_count() - launches0
-    ms = e0.elapsed_time(e1)
-    prof = det.profile_read()
-    det.profile(False)
-    if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    moves = args.steps * nel * nw * world
-    value = moves / (ms * 1e-3)
-    acc_timed = accept[args.warmup:].to(torch.float64)
-    n_acc = float(acc_timed.sum().item())
-    acc_rate = n_acc / acc_timed.numel()
+    def run_arm(delay):
+        """W warm-up sweeps + K timed sweeps with the inverse update `delay` (0 = rank-1), device
+        resident; then the same K sweeps end to end from pinned host buffers."""
+        pos = torch.from_numpy(pos_np).to(dev)
+        accept = torch.zeros(unif.shape, dtype=torch.uint8, device=dev)
+        ratios = torch.zeros(unif.shape, dtype=torch.float64, device=dev)
+        t0 = time.perf_counter()
+        det = api.Det.init(spline, pos, delay_rank=delay)
+        torch.cuda.synchronize()
+        t_init = time.perf_counter() - t0
 
-    # ---- roofline of the dominant kernel (rank-local, from the per-launch CUDA events)
-    peak, peak_src = measured_peaks()
-    ld = det.ld
-    dom = max(prof, key=lambda k: prof[k][0])
-    kms, kn = prof[dom]
-    spo_ms, spo_n = prof["spo_ratio"]
-    spo_bytes_per_launch = nw * (64 * spline.row_pitch * 4 + 5 * spline.row_pitch * 4 + 2 * 8 * ld)
-    upd_bytes_per_accept = 16 * nel * ld + 12 * nel
-    if dom == "sm_update":
-        bytes_per_launch = (n_acc / max(kn, 1)) * upd_bytes_per_accept
-    elif dom == "spo_ratio":
-        bytes_per_launch = spo_bytes_per_launch
-    else:
-        bytes_per_launch = float("nan")
-    achieved = bytes_per_launch / (kms / max(kn, 1) * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
-                "launches": kn, "avg_us": 1e3 * kms / max(kn, 1),
-                "bytes_per_launch": bytes_per_launch, "share_of_step": kms / ms}
-    kernels = {k: {"ms": v[0], "launches": v[1]} for k, v in prof.items() if v[1]}
-    if spo_n:
-        kernels["spo_ratio"]["GB/s"] = spo_bytes_per_launch / (spo_ms / spo_n * 1e-3) / 1e9
-        kernels["spo_ratio"]["frac"] = kernels["spo_ratio"]["GB/s"] / peak
+        def step(i):
+            api.sweep(det, pos, delta[i:i + 1], unif[i:i + 1], ratios_out=ratios[i:i + 1], accept_out=accept[i:i + 1])
 
-    # ---- end to end through the C ABI with HOST buffers (pinned): H2D of pos/delta/unif and D2H
-    #      of pos/ratios/decisions inside the timed region, every step
-    pos_h = pos.cpu().pin_memory()
-    delta_h = torch.from_numpy(delta_np).pin_memory()
-    unif_h = torch.from_numpy(unif_np).pin_memory()
-    ratios_h = torch.zeros(unif_h.shape, dtype=torch.float64).pin_memory()
-    accept_h = torch.zeros(unif_h.shape, dtype=torch.uint8).pin_memory()
+        # ---- device-resident timing: inputs in HBM, CUDA events on the launching stream
+        for i in range(args.warmup):
+            step(i)
+        barrier()
+        det.profile(True)
+        launches0 = api.launch_count()
+        sampler = ClockSampler(local_rank)
+        sampler.start()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for i in range(args.warmup, nsteps_total):
+            step(i)
+        e1.record()
+        barrier()
+        clocks = sampler.stop()
+        launches = api.launch_count() - launches0
+        ms = e0.elapsed_time(e1)
+        prof = det.profile_read()
+        det.profile(False)
+        ms = max_over_ranks(ms)
+        moves = args.steps * nel * nw * world
+        value = moves / (ms * 1e-3)
+        acc_timed = accept[args.warmup:].to(torch.float64)
+        n_acc = float(acc_timed.sum().item())
+        acc_rate = n_acc / acc_timed.numel()
 
-    def step_host(i):
-        api.sweep_host(det, pos_h, delta_h[i:i + 1], unif_h[i:i + 1], ratios_out=ratios_h[i:i + 1],
-                       accept_out=accept_h[i:i + 1])
+        # ---- roofline of the dominant kernel (rank-local, from the per-launch CUDA events)
+        ld, npitch, K = det.ld, spline.row_pitch, det.delay_rank
+        per_launch = {   # algorithmic bytes per launch (DESIGN.md section 6)
+            "spo_ratio": nw * (64 * npitch * 4 + 5 * npitch * 4 + (0 if K else 2 * 8 * ld)),
+            "sm_update": (n_acc / max(prof["sm_update"][1], 1)) * (16 * nel * ld + 12 * nel),
+            "delayed_flush": nw * 16 * nel * ld + (n_acc / max(prof["delayed_flush"][1], 1)) * (8 * ld + 4 * npitch),
+        }
+        kernels = {}
+        for k, (kms, kn) in prof.items():
+            if not kn:
+                continue
+            kernels[k] = {"ms": kms, "launches": kn, "avg_us": 1e3 * kms / kn, "share_of_step": kms / ms}
+            if k in per_launch:
+                gbs = per_launch[k] / (kms / kn * 1e-3) / 1e9
+                kernels[k].update({"bytes_per_launch": per_launch[k], "GB/s": gbs, "frac_of_hbm_peak": gbs / peak})
+        if "delayed_flush" in kernels:   # two fp64 contractions on the tensor cores: 4 KPAD N ld flop / walker
+            kpad = (K + 7) // 8 * 8
+            fl = 4.0 * kpad * nel * ld * nw
+            kernels["delayed_flush"].update({"flops_per_launch": fl, "fp64_TFLOP/s": fl / (kernels["delayed_flush"]["avg_us"] * 1e-6) / 1e12,
+                                             "fp64_dmma_peak_TFLOP/s": FP64_DMMA_PEAK})
+        dom = max(kernels, key=lambda k: kernels[k]["ms"])
+        kd = kernels[dom]
+        roofline = {"bound": "hbm", "kernel": dom, "achieved": kd.get("GB/s"), "peak": peak, "unit": "GB/s",
+                    "frac": kd.get("frac_of_hbm_peak"), "traffic": NCU_TRAFFIC.get(dom), "peak_source": peak_src,
+                    "launches": kd["launches"], "avg_us": kd["avg_us"], "bytes_per_launch": kd.get("bytes_per_launch"),
+                    "share_of_step": kd["share_of_step"]}
 
-    step_host(0)
-    barrier()
-    e0.record()
-    for i in range(args.warmup, nsteps_total):
-        step_host(i)
-    e1.record()
-    barrier()
-    ms_e2e = e0.elapsed_time(e1)
-    if world > 1:
-        t = torch.tensor([ms_e2e], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_e2e = float(t.item())
-    h2d = pos_h.numel() * 8 + delta_h[0].numel() * 8 + unif_h[0].numel() * 8
-    d2h = pos_h.numel() * 8 + ratios_h[0].numel() * 8 + accept_h[0].numel()
-    e2e = {"value": moves / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d * world,
-           "d2h_bytes_per_step": d2h * world}
+        # ---- end to end through the C ABI with HOST buffers (pinned): H2D of pos/delta/unif and D2H
+        #      of pos/ratios/decisions inside the timed region, every step
+        pos_h = pos.cpu().pin_memory()
+        ratios_h = torch.zeros(unif_h.shape, dtype=torch.float64).pin_memory()
+        accept_h = torch.zeros(unif_h.shape, dtype=torch.uint8).pin_memory()
 
+        def step_host(i):
+            api.sweep_host(det, pos_h, delta_h[i:i + 1], unif_h[i:i + 1], ratios_out=ratios_h[i:i + 1],
+                           accept_out=accept_h[i:i + 1])
+
+        step_host(0)
+        barrier()
+        e0.record()
+        for i in range(args.warmup, nsteps_total):
+            step_host(i)
+        e1.record()
+        barrier()
+        ms_e2e = max_over_ranks(e0.elapsed_time(e1))
+        h2d = pos_h.numel() * 8 + delta_h[0].numel() * 8 + unif_h[0].numel() * 8
+        d2h = pos_h.numel() * 8 + ratios_h[0].numel() * 8 + accept_h[0].numel()
+        e2e = {"value": moves / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d * world,
+               "d2h_bytes_per_step": d2h * world}
+        update = "sherman-morrison rank-1" if K == 0 else f"delayed rank-{K} (same result as rank-1)"
+        det.destroy()
+        return {"value": value, "ms_per_step": ms / args.steps, "update": update, "accept_rate": acc_rate,
+                "init_s": t_init, "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
+                "kernels": kernels, "spline_evals_per_s": value * nel}
+
+    ws_table, ws_binv = cfg.table_bytes() / 1e9, nw * nel * nel * 8 / 1e9
+    l2_note = (f"working set ({ws_table:.2f} GB table + {ws_binv:.2f} GB inverses) "
+               + ("exceeds the 126 MB L2; no flush needed" if ws_table + ws_binv > 0.5 else
+                  "fits L2: numbers are L2-resident, not HBM rooflines"))
+    delays = [args.delay] if args.delay >= 0 else [DEFAULT_DELAY.get(args.config, 0), 0]
+    arms = [run_arm(dl) for dl in dict.fromkeys(delays)]
+    main_arm = arms[0]
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+        "metric": METRIC, "value": main_arm["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": main_arm["ms_per_step"], "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic (seeded; paper_1802_06922_b200/inputs.py)",
         "config": {"workload": args.config, "grid": list(cfg.grid), "N": nel, "walkers_per_gpu": nw,
-                   "update": "sherman-morrison rank-1" if det.delay_rank == 0 else f"delayed rank-{det.delay_rank}",
+                   "update": main_arm["update"],
                    "step": "one full sweep (N electron moves x walkers)",
-                   "l2": "working set (8.6 GB table + 4.3 GB inverses) exceeds L2; no flush needed",
-                   "spo_dtype": "f32", "accept_rate": acc_rate, "init_s": t_init},
-        "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
-        "kernels": kernels, "spline_evals_per_s": value * nel,
+                   "l2": l2_note,
+                   "spo_dtype": "f32", "accept_rate": main_arm["accept_rate"], "init_s": main_arm["init_s"]},
+        "clocks": main_arm["clocks"], "e2e": main_arm["e2e"], "gpu_launches": main_arm["gpu_launches"],
+        "roofline": main_arm["roofline"], "kernels": main_arm["kernels"],
+        "spline_evals_per_s": main_arm["spline_evals_per_s"],
     }
+    if len(arms) > 1:
+        line["variants"] = {a["update"]: {k: a[k] for k in ("value", "ms_per_step", "accept_rate", "clocks", "e2e",
+                                                            "gpu_launches", "roofline", "kernels")} for a in arms[1:]}
 
     if want_cpu:
         xs = inputs.QmcInputs(cfg, x.lattice, None, pos_np, delta_np, unif_np)
@@ -324,7 +352,6 @@ def main():
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": text}
     if rank == 0:
         print(json.dumps(line), flush=True)
-    det.destroy()
     spline.destroy()
     if world > 1:
         dist.destroy_process_group()

@@ -64,7 +64,6 @@ __device__ __forceinline__ void group_sync(int id, int nthreads)
 {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
-
 struct FlushArgs {
     double *B;                    // [nw][nel][ld]
     int nel, ld, np, K;
@@ -80,7 +79,7 @@ struct FlushArgs {
 //   rows_s  double [KPAD][LD + 2]   B-fragment of step 2: lane (g,t) reads row 8nt+2t+h, column n0+g
 //   v_s     float  [KPAD][LD + 8]   B-fragment of step 1: lane (g,t) reads row 8nt+g, columns n0+2t,+1
 //   sinv_s  double [KPAD][KPAD + 4]
-//   part_s  double [NG][NWC][8][KPAD + 4]   partial Q of each column warp
+//   part_s  double [2][NG][NWC][8][KPAD + 4]   partial Q of each column warp, by block parity
 //   kl_s    int [KPAD],  mbar
 template <int KPAD, int LD, int NWC, int NG>
 struct FlushSmem {
@@ -89,14 +88,17 @@ struct FlushSmem {
     static constexpr size_t v_off = rows_off + (size_t)KPAD * RS * sizeof(double);
     static constexpr size_t sinv_off = v_off + (size_t)KPAD * VS * sizeof(float);
     static constexpr size_t part_off = sinv_off + (size_t)KPAD * SS * sizeof(double);
-    static constexpr size_t kl_off = part_off + (size_t)NG * NWC * 8 * PS * sizeof(double);
+    static constexpr size_t part_bytes = (size_t)NG * NWC * 8 * PS * sizeof(double);
+    // two partial buffers (by block parity) save a barrier per block; one when shared memory is short
+    static constexpr int PB = (part_off + 2 * part_bytes + KPAD * sizeof(int) + 16 <= 227 * 1024) ? 2 : 1;
+    static constexpr size_t kl_off = part_off + PB * part_bytes;
     static constexpr size_t mbar_off = kl_off + (size_t)KPAD * sizeof(int);
     static constexpr size_t bytes = mbar_off + 16;
 };
 
 constexpr size_t kSmemMax = 227 * 1024;
 
-template <int KPAD, int NWC, int TW, int NG>
+template <int KPAD, int NWC, int TW, int NG, bool PF>
 __global__ void __launch_bounds__(32 * NWC * NG, 1) flush_dmma_kernel(FlushArgs a)
 {
     constexpr int LD = NWC * TW * 8;
@@ -149,17 +151,29 @@ __global__ void __launch_bounds__(32 * NWC * NG, 1) flush_dmma_kernel(FlushArgs 
         }
     }
 
-    // ---- stream row blocks: group `grp` takes blocks grp, grp + NG, ... of this CTA's rows
+    // ---- stream row blocks: group `grp` takes blocks grp, grp + NG, ... of this CTA's rows.
+    // With PF the next block's rows are requested before the current block is contracted, so the
+    // HBM stream (loads of block i+1, stores of block i-1) runs under the DMMA work of block i.
     const int m_begin = blockIdx.x * a.rows_per_cta;
     const int m_end = min(nel, m_begin + a.rows_per_cta);
     const int col0 = 8 * TW * wc;
+    double *const walker_B = a.B + (size_t)w * nel * LD + col0 + 2 * t;
     bool staged = false;
-    for (int m0 = m_begin + 8 * grp; m0 < m_end; m0 += 8 * NG) {
-        const int m = m0 + g;
-        double *rowp = a.B + ((size_t)w * nel + min(m, nel - 1)) * LD + col0 + 2 * t;
-        double2 r[TW];
+    int m0 = m_begin + 8 * grp;
+    double2 r[TW], rn[PF ? TW : 1];
+    if (m0 < m_end) {
+        const double *src = walker_B + (size_t)min(m0 + g, nel - 1) * LD;
 #pragma unroll
-        for (int i = 0; i < TW; ++i) r[i] = *reinterpret_cast<const double2 *>(rowp + 8 * i);
+        for (int i = 0; i < TW; ++i) r[i] = *reinterpret_cast<const double2 *>(src + 8 * i);
+    }
+    for (int it = 0; m0 < m_end; m0 += 8 * NG, ++it) {
+        const int m = m0 + g;
+        const int m0n = m0 + 8 * NG;
+        if (PF && m0n < m_end) {
+            const double *src = walker_B + (size_t)min(m0n + g, nel - 1) * LD;
+#pragma unroll
+            for (int i = 0; i < TW; ++i) rn[PF ? i : 0] = *reinterpret_cast<const double2 *>(src + 8 * i);
+        }
         if (!staged) {
             mbar_wait(mbar, 0);
             staged = true;
@@ -179,7 +193,9 @@ __global__ void __launch_bounds__(32 * NWC * NG, 1) flush_dmma_kernel(FlushArgs 
                 }
             }
         }
-        double *ps = part_s + ((size_t)(grp * NWC + wc) * 8 + g) * PS;
+        // partials are double-buffered by block parity: one barrier per block is enough
+        double *pbuf = part_s + (size_t)((L::PB == 2 ? (it & 1) : 0) * NG + grp) * NWC * 8 * PS;
+        double *ps = pbuf + ((size_t)wc * 8 + g) * PS;
 #pragma unroll
         for (int nt = 0; nt < NT; ++nt)
             if (8 * nt < p) *reinterpret_cast<double2 *>(ps + 8 * nt + 2 * t) = make_double2(cq[nt][0], cq[nt][1]);
@@ -190,14 +206,14 @@ __global__ void __launch_bounds__(32 * NWC * NG, 1) flush_dmma_kernel(FlushArgs 
         for (int kq = 0; kq < KPAD / 4; ++kq) {
             double s = 0.0;
             if (4 * kq < p8) {
-                const double *pp = part_s + ((size_t)grp * NWC * 8 + g) * PS + 4 * kq + t;
+                const double *pp = pbuf + (size_t)g * PS + 4 * kq + t;
 #pragma unroll
                 for (int c = 0; c < NWC; ++c) s += pp[(size_t)c * 8 * PS];
                 if (kl_s[4 * kq + t] == m) s -= 1.0;
             }
             qa[kq] = s;
         }
-        group_sync(1 + grp, 32 * NWC);          // part_s may be overwritten by the next block
+        if (L::PB == 1) group_sync(1 + grp, 32 * NWC);
         // T = Q S^-T (C fragments), negated
         double tq[NT][2];
 #pragma unroll
@@ -223,8 +239,17 @@ __global__ void __launch_bounds__(32 * NWC * NG, 1) flush_dmma_kernel(FlushArgs 
             }
         }
         if (m < nel) {
+            double *dst = walker_B + (size_t)m * LD;
 #pragma unroll
-            for (int i = 0; i < TW; ++i) *reinterpret_cast<double2 *>(rowp + 8 * i) = r[i];
+            for (int i = 0; i < TW; ++i) *reinterpret_cast<double2 *>(dst + 8 * i) = r[i];
+        }
+        if (PF) {
+#pragma unroll
+            for (int i = 0; i < TW; ++i) r[i] = rn[PF ? i : 0];
+        } else if (m0n < m_end) {
+            const double *src = walker_B + (size_t)min(m0n + g, nel - 1) * LD;
+#pragma unroll
+            for (int i = 0; i < TW; ++i) r[i] = *reinterpret_cast<const double2 *>(src + 8 * i);
         }
     }
     if (!staged) mbar_wait(mbar, 0);            // never leave with bulk copies in flight
@@ -236,26 +261,24 @@ __global__ void reset_window_kernel(int nw, int *win_count)
     if (w < nw) win_count[w] = 0;
 }
 
-static int kpad_of(int K) { return (K + 7) / 8 * 8; }
-
-// (NWC, TW, NG) for ld = 64 v
+// Launch shape for ld = 64 v: NWC column warps x TW 8-column tiles per warp, NG row groups per
+// CTA, PF = prefetch the next row block (needs 2 x 4 TW data registers per thread).
 struct FlushShape { int nwc, tw, ng; };
+#define QMC_FLUSH_SHAPES(X) \
+    X(1, 1, 8, 4, true) X(2, 2, 8, 4, true) X(3, 3, 8, 4, true) X(4, 4, 8, 4, true) X(6, 6, 8, 2, true) \
+    X(8, 8, 8, 2, true) X(12, 6, 16, 2, false) X(16, 8, 16, 2, false) X(24, 12, 16, 1, false) X(32, 16, 16, 1, false)
+
 static FlushShape flush_shape(int v)
 {
     switch (v) {
-    case 1: return {1, 8, 4};
-    case 2: return {2, 8, 4};
-    case 3: return {3, 8, 4};
-    case 4: return {4, 8, 4};
-    case 6: return {6, 8, 2};
-    case 8: return {8, 8, 2};
-    case 12: return {6, 16, 2};
-    case 16: return {8, 16, 2};
-    case 24: return {12, 16, 1};
-    case 32: return {16, 16, 1};
+#define X(V, NWC, TW, NG, PF) case V: return {NWC, TW, NG};
+        QMC_FLUSH_SHAPES(X)
+#undef X
     }
     return {0, 0, 0};
 }
+
+static int kpad_of(int K) { return (K + 7) / 8 * 8; }
 
 static size_t flush_smem_bytes(int kpad, int ld)
 {
@@ -273,14 +296,14 @@ int delayed_max_rank(int ld)
     return best;
 }
 
-template <int KPAD, int NWC, int TW, int NG>
+template <int KPAD, int NWC, int TW, int NG, bool PF>
 static cudaError_t launch_flush_t(const FlushArgs &a, int nw, cudaStream_t s)
 {
     using L = FlushSmem<KPAD, NWC * TW * 8, NWC, NG>;
     if constexpr (L::bytes > kSmemMax) {
         return cudaErrorInvalidValue;
     } else {
-        auto kern = flush_dmma_kernel<KPAD, NWC, TW, NG>;
+        auto kern = flush_dmma_kernel<KPAD, NWC, TW, NG, PF>;
         static bool configured = false;
         if (!configured) {
             cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L::bytes);
@@ -293,14 +316,14 @@ static cudaError_t launch_flush_t(const FlushArgs &a, int nw, cudaStream_t s)
     }
 }
 
-template <int NWC, int TW, int NG>
+template <int NWC, int TW, int NG, bool PF>
 static cudaError_t launch_flush_k(const FlushArgs &a, int nw, cudaStream_t s)
 {
     switch (kpad_of(a.K)) {
-    case 8: return launch_flush_t<8, NWC, TW, NG>(a, nw, s);
-    case 16: return launch_flush_t<16, NWC, TW, NG>(a, nw, s);
-    case 24: return launch_flush_t<24, NWC, TW, NG>(a, nw, s);
-    case 32: return launch_flush_t<32, NWC, TW, NG>(a, nw, s);
+    case 8: return launch_flush_t<8, NWC, TW, NG, PF>(a, nw, s);
+    case 16: return launch_flush_t<16, NWC, TW, NG, PF>(a, nw, s);
+    case 24: return launch_flush_t<24, NWC, TW, NG, PF>(a, nw, s);
+    case 32: return launch_flush_t<32, NWC, TW, NG, PF>(a, nw, s);
     }
     return cudaErrorInvalidValue;
 }
@@ -319,16 +342,9 @@ int delayed_flush(qmc_det *d, cudaStream_t s)
     cudaError_t e;
     prof_start(d, kProfDelayedFlush, s);
     switch (d->ld / 64) {
-    case 1: e = launch_flush_k<1, 8, 4>(a, d->nw, s); break;
-    case 2: e = launch_flush_k<2, 8, 4>(a, d->nw, s); break;
-    case 3: e = launch_flush_k<3, 8, 4>(a, d->nw, s); break;
-    case 4: e = launch_flush_k<4, 8, 4>(a, d->nw, s); break;
-    case 6: e = launch_flush_k<6, 8, 2>(a, d->nw, s); break;
-    case 8: e = launch_flush_k<8, 8, 2>(a, d->nw, s); break;
-    case 12: e = launch_flush_k<6, 16, 2>(a, d->nw, s); break;
-    case 16: e = launch_flush_k<8, 16, 2>(a, d->nw, s); break;
-    case 24: e = launch_flush_k<12, 16, 1>(a, d->nw, s); break;
-    case 32: e = launch_flush_k<16, 16, 1>(a, d->nw, s); break;
+#define X(V, NWC, TW, NG, PF) case V: e = launch_flush_k<NWC, TW, NG, PF>(a, d->nw, s); break;
+        QMC_FLUSH_SHAPES(X)
+#undef X
     default: e = cudaErrorInvalidValue;
     }
     prof_stop(d, s);
