@@ -42,7 +42,7 @@ DEFAULT_DELAY = {"tiny": 0, "small": 16, "mid": 16, "large": 16, "xlarge": 8}
 FP64_DMMA_PEAK = 37.0
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures
 # (profiles/*.md), large config
-NCU_TRAFFIC = {"sm_update": 6.725e9, "spo_ratio": 140.7e6}
+NCU_TRAFFIC = {"sm_update": 6.725e9}
 
 
 def measured_peaks():
@@ -269,7 +269,8 @@ def main():
         # ---- roofline of the dominant kernel (rank-local, from the per-launch CUDA events)
         ld, npitch, K = det.ld, spline.row_pitch, det.delay_rank
         per_launch = {   # algorithmic bytes per launch
-            "spo_ratio": nw * (64 * npitch * 4 + 5 * npitch * 4 + (0 if K else 2 * 8 * ld)),
+            "spo_vgl": (args.steps * nel * nw / max(prof["spo_vgl"][1], 1)) * (64 + 5) * npitch * 4,
+            "ratio_rowcopy": nw * (2 * 8 * ld + 4 * nel),
             "sm_update": (n_acc / max(prof["sm_update"][1], 1)) * (16 * nel * ld + 12 * nel),
             "delayed_flush": nw * 16 * nel * ld + (n_acc / max(prof["delayed_flush"][1], 1)) * (8 * ld + 4 * npitch),
         }

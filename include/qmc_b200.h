@@ -201,11 +201,12 @@ int qmc_det_info(const qmc_det_t *det, int *nwalkers, int *nel, int *ld, int *de
  *   qmc_det_profile(det, 1)   enable and reset;  (det, 0) disable
  *   qmc_det_profile_read      synchronises the recorded events and returns, per kernel kind,
  *                             the summed device time in ms and the number of launches; host
- *                             arrays of QMC_PROF_KINDS entries.  Kinds: 0 fused SPO-VGL+ratio,
- *                             1 rank-1 update, 2 delayed ratio, 3 delayed accept, 4 delayed flush.
+ *                             arrays of QMC_PROF_KINDS entries.  Kinds: 0 SPO-VGL of a batch of
+ *                             electron steps, 1 rank-1 update, 2 delayed ratio/decide/append,
+ *                             3 delayed accept (standalone), 4 delayed flush, 5 ratio + row copy.
  *                             Resets the recorder.
  */
-#define QMC_PROF_KINDS 5
+#define QMC_PROF_KINDS 6
 int qmc_det_profile(qmc_det_t *det, int enable);
 int qmc_det_profile_read(qmc_det_t *det, double *ms_host, long long *launches_host);
 

@@ -22,7 +22,7 @@ EXPORTS = [
     "qmc_sweep", "qmc_sweep_ex", "qmc_sweep_host", "qmc_det_get_inverse", "qmc_det_set_inverse",
     "qmc_det_get_stats", "qmc_det_info", "qmc_launch_count", "qmc_det_profile", "qmc_det_profile_read",
 ]
-PROF_KINDS = ["spo_ratio", "sm_update", "delayed_ratio", "delayed_accept", "delayed_flush"]
+PROF_KINDS = ["spo_vgl", "sm_update", "delayed_ratio", "delayed_accept", "delayed_flush", "ratio_rowcopy"]
 
 
 class SweepOpts(ctypes.Structure):

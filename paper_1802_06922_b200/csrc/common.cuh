@@ -14,7 +14,8 @@ namespace qmc {
 
 constexpr int kWarp = 32;
 constexpr int kMaxNel = 2048;       // rows are held in registers: 64 doubles per lane at most
-constexpr int kRatioTilesMax = 8;   // partial-ratio slots per walker (orbital tiles of the SPO kernel)
+constexpr int kRatioTilesMax = 8;   // partial-ratio slots per walker
+constexpr int kSpoBatch = 16;       // electron steps per SPO-VGL launch in rank-1 mode (delayed: the window)
 
 void set_error(const char *fmt, ...);
 void count_launch(int n = 1);
@@ -70,7 +71,8 @@ struct qmc_det {
     int *sign;                  // [nw]
     long long *naccept;         // [nw]
     // scratch owned by the handle
-    float *vgl;                 // [nw][5][np]   v, gx, gy, gz, lap of the current proposal
+    int spo_batch;              // electron steps whose SPO-VGL is evaluated per launch (qmc_sweep)
+    float *vgl;                 // [spo_batch][nw][5][np]   v, gx, gy, gz, lap of the proposals of a batch
     double *rowk;               // [nw][ld]      copy of row iel of B taken before the update
     double *rpart;              // [nw][kRatioTilesMax] partial ratios of the fused SPO kernel
     double *ratio;              // [nw]
@@ -96,7 +98,8 @@ struct qmc_det {
 
 namespace qmc {
 enum ProfKind { kProfSpoRatio = 0, kProfUpdate = 1, kProfDelayedRatio = 2, kProfDelayedAccept = 3,
-                kProfDelayedFlush = 4, kProfKinds = 5 };
+                kProfDelayedFlush = 4, kProfRatio = 5, kProfKinds = 6 };
+static_assert(kProfKinds == QMC_PROF_KINDS, "qmc_b200.h and common.cuh disagree on the profiling kinds");
 // Record a start / stop event pair around a launch when profiling is enabled (no-ops otherwise).
 void prof_start(qmc_det *d, int kind, cudaStream_t s);
 void prof_stop(qmc_det *d, cudaStream_t s);

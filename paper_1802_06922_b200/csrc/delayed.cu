@@ -18,8 +18,6 @@
 
 namespace qmc {
 
-void spo_launch_shape(int np, int *threads, int *tiles);
-
 constexpr int kStepThreads = 256;
 
 struct DelayedStepArgs {
@@ -244,19 +242,17 @@ int delayed_flush_reset_host(qmc_det *d, cudaStream_t s)
     return QMC_OK;
 }
 
-int delayed_sweep_step(qmc_det *d, const qmc_spline *sp, double *pos, const double *delta, const double *unif,
-                       int iel, double *ratios_out, unsigned char *accept_out, const unsigned char *forced,
-                       float *phi_record, int nrecord, cudaStream_t s)
+int delayed_sweep_step(qmc_det *d, double *pos, const double *delta, const double *unif, int iel,
+                       const float *phi, double *ratios_out, unsigned char *accept_out,
+                       const unsigned char *forced, cudaStream_t s)
 {
     if (d->host_pending >= d->delay || (d->host_pending && d->win_host_iel[iel])) {
         int rc = delayed_flush_reset_host(d, s);
         if (rc) return rc;
     }
-    // K1: SPO-VGL at the proposed positions (into the walker scratch), K2: ratio / decide / append
-    int rc = spo_proposal_vgl(d, sp, pos, delta, iel, phi_record, nrecord, s);
-    if (rc) return rc;
+    // ratio against the window / decide / append
     DelayedStepArgs a{};
-    fill_common(a, d, iel, d->vgl, (size_t)5 * d->np);
+    fill_common(a, d, iel, phi, (size_t)5 * d->np);
     a.mode = 0;
     a.unif = unif; a.forced = forced; a.ratios_out = ratios_out; a.accept_out = accept_out;
     a.pos = pos; a.delta = delta;

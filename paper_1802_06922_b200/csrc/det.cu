@@ -11,8 +11,6 @@
 
 namespace qmc {
 
-void spo_launch_shape(int np, int *threads, int *tiles);
-
 // ---------------------------------------------------------------------------------------------
 // det_init kernels
 
@@ -296,11 +294,12 @@ extern "C" int qmc_det_init(qmc_det_t **out, const qmc_spline_t *sp, int nw, int
     d->spline = sp;
     d->nw = nw; d->nel = nel; d->ld = update_ld(nel); d->np = sp->view.np;
     d->delay = delay_rank <= 1 ? 0 : delay_rank;
+    d->spo_batch = d->delay ? d->delay : kSpoBatch;
     const int ld = d->ld, np = d->np, K = d->delay;
     int rc;
     if ((rc = dev_alloc(&d->B, (size_t)nw * nel * ld, "B")) || (rc = dev_alloc(&d->logdet, nw, "logdet")) ||
         (rc = dev_alloc(&d->sign, nw, "sign")) || (rc = dev_alloc(&d->naccept, nw, "naccept")) ||
-        (rc = dev_alloc(&d->vgl, (size_t)nw * 5 * np, "vgl")) || (rc = dev_alloc(&d->rowk, (size_t)nw * ld, "rowk")) ||
+        (rc = dev_alloc(&d->vgl, (size_t)d->spo_batch * nw * 5 * np, "vgl")) || (rc = dev_alloc(&d->rowk, (size_t)nw * ld, "rowk")) ||
         (rc = dev_alloc(&d->rpart, (size_t)nw * kRatioTilesMax, "rpart")) || (rc = dev_alloc(&d->ratio, nw, "ratio")) ||
         (rc = dev_alloc(&d->acc, nw, "acc"))) {
         det_free(d);
@@ -326,7 +325,7 @@ extern "C" int qmc_det_init(qmc_det_t **out, const qmc_spline_t *sp, int nw, int
     cudaError_t e = cudaMemsetAsync(d->B, 0, (size_t)nw * nel * ld * sizeof(double), s);
     if (e == cudaSuccess) e = cudaMemsetAsync(d->rowk, 0, (size_t)nw * ld * sizeof(double), s);
     if (e == cudaSuccess) e = cudaMemsetAsync(d->rpart, 0, (size_t)nw * kRatioTilesMax * sizeof(double), s);
-    if (e == cudaSuccess) e = cudaMemsetAsync(d->vgl, 0, (size_t)nw * 5 * np * sizeof(float), s);
+    if (e == cudaSuccess) e = cudaMemsetAsync(d->vgl, 0, (size_t)d->spo_batch * nw * 5 * np * sizeof(float), s);
     if (e == cudaSuccess && K) e = cudaMemsetAsync(d->win_count, 0, (size_t)nw * sizeof(int), s);
     if (e == cudaSuccess && K) e = cudaMemsetAsync(d->win_full, 0, sizeof(int), s);
     if (e == cudaSuccess && K) e = cudaMemsetAsync(d->win_rows, 0, (size_t)nw * K * ld * sizeof(double), s);

@@ -1,7 +1,9 @@
 // qmc_sweep*: the particle-by-particle sweep driver (sec 5.2.1) -- all walkers
-// in lockstep (L114, L181), electrons in sequence.  Two launches per electron step:
-//   K1 spo_ratio_kernel  S0 proposal, S1 stencil, S2 SPO-VGL gather, S3 partial ratios, row copy
-//   K2 sm_update_kernel  S3 ratio (sum of partials), S4 Metropolis test, S5 rank-1 update
+// in lockstep (L114, L181), electrons in sequence.  Launches:
+//   K1 spo_batch_kernel      S0 proposal, S1 stencil, S2 SPO-VGL gather -- once per batch of steps
+//   K2 ratio_rowcopy_kernel  S3 ratio, copy of row k                    -- per electron step
+//   K3 sm_update_kernel      S4 Metropolis test, S5 rank-1 update       -- per electron step
+// (delayed mode: K2/K3 are delayed_step_kernel per step and flush_dmma_kernel per window)
 #include "delayed_device.cuh"
 #include "spo_device.cuh"
 #include "update_device.cuh"
@@ -10,83 +12,87 @@ namespace qmc {
 
 void spo_launch_shape(int np, int *threads, int *tiles);
 
-struct SpoRatioArgs {
+// SPO-VGL of a BATCH of electron steps in one launch.  The proposal of electron k does not depend
+// on the outcome of the moves before it (r' = pos[w][k] + delta, and pos[w][k] only changes at step
+// k itself), so the gathers of `nb` consecutive steps are issued together: nb * nw positions keep
+// every SM streaming (a single step's 512 positions is a 25 us launch that never leaves the ramp).
+struct SpoBatchArgs {
     SplineView sp;
     const double *pos;     // [nw][nel][3]
-    const double *delta;   // [nw][3], offset to (sweep, electron)
-    int nel, iel, ld;
-    const double *B;       // [nw][nel][ld]
-    float *vgl;            // [nw][5][np]
-    double *rowk;          // [nw][ld]
-    double *rpart;         // [nw][kRatioTilesMax]
-    float *phi_record;     // [nrecord][nel], offset to (sweep, electron), or NULL
+    const double *delta;   // [nb][nw][3], offset to (sweep, first electron of the batch)
+    int nel, iel0, nw;
+    float *vgl;            // [nb][nw][5][np]
+    float *phi_record;     // [nb][nrecord][nel], offset to (sweep, first electron), or NULL
     int nrecord;
 };
 
-// One block per (orbital tile, walker).  Thread t owns orbitals 4t..4t+3 of the tile: it gathers
-// their value/gradient/Laplacian from the 64 stencil rows, writes them to the walker's scratch,
-// multiplies the values with the matching four entries of row iel of B (fp64) and copies those
-// entries to rowk, so the update kernel can overwrite B in place.  The block's partial ratio is
-// reduced in a fixed order; the (at most 8) tiles are added by the update kernel.
-template <bool WITH_RATIO>
-__global__ void __launch_bounds__(256) spo_ratio_kernel(SpoRatioArgs a)
+// One block per (orbital tile, walker, step of the batch).  Thread t owns orbitals 4t..4t+3 of the
+// tile: it gathers their value/gradient/Laplacian from the 64 stencil rows (S0-S2).
+__global__ void __launch_bounds__(256) spo_batch_kernel(SpoBatchArgs a)
 {
     __shared__ StencilSmem st;
-    __shared__ double red[33];
-    const int w = blockIdx.y;
-    const double *r = a.pos + ((size_t)w * a.nel + a.iel) * 3;
-    const double *dl = a.delta + 3 * (size_t)w;
+    const int w = blockIdx.y, j = blockIdx.z;
+    const double *r = a.pos + ((size_t)w * a.nel + a.iel0 + j) * 3;
+    const double *dl = a.delta + 3 * ((size_t)j * a.nw + w);
     stage_stencil(a.sp, r[0] + dl[0], r[1] + dl[1], r[2] + dl[2], st);
     const int np = a.sp.np;
     const int col = 4 * (blockIdx.x * blockDim.x + threadIdx.x);
-    double part = 0.0;
-    if (col < np) {
-        float4 v, gx, gy, gz, lp;
-        gather4<true>(a.sp, st, col, v, gx, gy, gz, lp);
-        float *o = a.vgl + (size_t)w * 5 * np + col;
-        *reinterpret_cast<float4 *>(o) = v;
-        *reinterpret_cast<float4 *>(o + np) = gx;
-        *reinterpret_cast<float4 *>(o + 2 * (size_t)np) = gy;
-        *reinterpret_cast<float4 *>(o + 3 * (size_t)np) = gz;
-        *reinterpret_cast<float4 *>(o + 4 * (size_t)np) = lp;
-        if (WITH_RATIO) {
-            const double2 *brow = reinterpret_cast<const double2 *>(a.B + ((size_t)w * a.nel + a.iel) * a.ld + col);
-            const double2 b0 = brow[0], b1 = brow[1];
-            double2 *rk = reinterpret_cast<double2 *>(a.rowk + (size_t)w * a.ld + col);
-            rk[0] = b0;
-            rk[1] = b1;
-            part = fma(b0.x, (double)v.x, part);
-            part = fma(b0.y, (double)v.y, part);
-            part = fma(b1.x, (double)v.z, part);
-            part = fma(b1.y, (double)v.w, part);
-        }
-        if (a.phi_record && w < a.nrecord) {
-            float *rec = a.phi_record + (size_t)w * a.nel;
-            if (col + 0 < a.nel) rec[col + 0] = v.x;
-            if (col + 1 < a.nel) rec[col + 1] = v.y;
-            if (col + 2 < a.nel) rec[col + 2] = v.z;
-            if (col + 3 < a.nel) rec[col + 3] = v.w;
-        }
-    }
-    if (WITH_RATIO) {
-        part = block_sum(part, red);
-        if (threadIdx.x == 0) a.rpart[(size_t)w * kRatioTilesMax + blockIdx.x] = part;
+    if (col >= np) return;
+    float4 v, gx, gy, gz, lp;
+    gather4<true>(a.sp, st, col, v, gx, gy, gz, lp);
+    float *o = a.vgl + ((size_t)j * a.nw + w) * 5 * np + col;
+    *reinterpret_cast<float4 *>(o) = v;
+    *reinterpret_cast<float4 *>(o + np) = gx;
+    *reinterpret_cast<float4 *>(o + 2 * (size_t)np) = gy;
+    *reinterpret_cast<float4 *>(o + 3 * (size_t)np) = gz;
+    *reinterpret_cast<float4 *>(o + 4 * (size_t)np) = lp;
+    if (a.phi_record && w < a.nrecord) {
+        float *rec = a.phi_record + ((size_t)j * a.nrecord + w) * a.nel;
+        if (col + 0 < a.nel) rec[col + 0] = v.x;
+        if (col + 1 < a.nel) rec[col + 1] = v.y;
+        if (col + 2 < a.nel) rec[col + 2] = v.z;
+        if (col + 3 < a.nel) rec[col + 3] = v.w;
     }
 }
 
-int spo_proposal_vgl(qmc_det *d, const qmc_spline *sp, const double *pos, const double *delta, int iel,
-                     float *phi_record, int nrecord, cudaStream_t s)
+// S3 for the rank-1 path: R_w = B_w[iel] . phi_w (fp64, fixed order) and a copy of row iel, so that
+// the update kernel can overwrite B in place.  One block per walker.
+__global__ void __launch_bounds__(256)
+ratio_rowcopy_kernel(const double *__restrict__ B, int nel, int ld, int iel, const float *__restrict__ phi,
+                     size_t ldphi, double *__restrict__ rowk, double *__restrict__ rpart)
+{
+    __shared__ double red[33];
+    const int w = blockIdx.x;
+    const double2 *row = reinterpret_cast<const double2 *>(B + ((size_t)w * nel + iel) * ld);
+    const float2 *ph = reinterpret_cast<const float2 *>(phi + (size_t)w * ldphi);
+    double2 *dst = reinterpret_cast<double2 *>(rowk + (size_t)w * ld);
+    double acc = 0.0;
+    for (int j = threadIdx.x; j < ld / 2; j += 256) {
+        const double2 b = row[j];
+        dst[j] = b;
+        if (2 * j < nel) {          // phi is padded with zeros up to the table pitch >= nel
+            const float2 f = ph[j];
+            acc = fma(b.x, (double)f.x, acc);
+            acc = fma(b.y, (double)f.y, acc);
+        }
+    }
+    acc = block_sum(acc, red);
+    if (threadIdx.x == 0) rpart[(size_t)w * kRatioTilesMax] = acc;
+}
+
+int spo_batch_vgl(qmc_det *d, const qmc_spline *sp, const double *pos, const double *delta, int iel0, int nb,
+                  float *phi_record, int nrecord, cudaStream_t s)
 {
     int threads, tiles;
     spo_launch_shape(d->np, &threads, &tiles);
-    SpoRatioArgs a{};
+    SpoBatchArgs a{};
     a.sp = sp->view;
     a.pos = pos; a.delta = delta;
-    a.nel = d->nel; a.iel = iel; a.ld = d->ld;
-    a.B = d->B; a.vgl = d->vgl; a.rowk = d->rowk; a.rpart = d->rpart;
+    a.nel = d->nel; a.iel0 = iel0; a.nw = d->nw;
+    a.vgl = d->vgl;
     a.phi_record = phi_record; a.nrecord = nrecord;
     prof_start(d, kProfSpoRatio, s);
-    spo_ratio_kernel<false><<<dim3(tiles, d->nw), threads, 0, s>>>(a);
+    spo_batch_kernel<<<dim3(tiles, d->nw, nb), threads, 0, s>>>(a);
     prof_stop(d, s);
     QMC_LAUNCHED();
     return QMC_OK;
@@ -111,36 +117,36 @@ static int sweep_impl(qmc_det *d, const qmc_spline *sp, double *pos, const doubl
         QMC_REQUIRE(k0 >= 0 && kn >= 0 && k0 + kn <= nel, "qmc_sweep_ex: electron range %d+%d outside 0..%d", k0, kn, nel);
         QMC_REQUIRE(nrec >= 0 && nrec <= nw, "qmc_sweep_ex: nrecord=%d outside 0..%d", nrec, nw);
     }
-    int threads, tiles;
-    spo_launch_shape(d->np, &threads, &tiles);
-    QMC_REQUIRE(tiles <= kRatioTilesMax, "qmc_sweep: too many orbital tiles (%d)", tiles);
-
+    const int batch = d->spo_batch;
+    const size_t slot_stride = (size_t)nw * 5 * d->np;
     for (int sw = 0; sw < nsweeps; ++sw) {
         for (int k = k0; k < k0 + kn; ++k) {
             const size_t mv = ((size_t)sw * nel + k) * nw;
-            SpoRatioArgs a{};
-            a.sp = sp->view;
-            a.pos = pos; a.delta = delta + 3 * mv;
-            a.nel = nel; a.iel = k; a.ld = d->ld;
-            a.B = d->B; a.vgl = d->vgl; a.rowk = d->rowk; a.rpart = d->rpart;
-            a.phi_record = rec ? rec + mv / nw * (size_t)nrec * nel : nullptr;
-            a.nrecord = nrec;
-            if (d->delay) {
-                int rc = delayed_sweep_step(d, sp, pos, delta + 3 * mv, unif + mv, k,
+            const int slot = (k - k0) % batch;
+            if (slot == 0) {          // K1: SPO-VGL of the next `nb` electron steps, all walkers
+                const int nb = min(batch, k0 + kn - k);
+                int rc = spo_batch_vgl(d, sp, pos, delta + 3 * mv, k, nb,
+                                       rec ? rec + mv / nw * (size_t)nrec * nel : nullptr, nrec, s);
+                if (rc) return rc;
+            }
+            const float *phi = d->vgl + slot * slot_stride;
+            if (d->delay) {           // K2: ratio against the window, decision, append (flushes every K steps)
+                int rc = delayed_sweep_step(d, pos, delta + 3 * mv, unif + mv, k, phi,
                                             ratios_out ? ratios_out + mv : nullptr,
                                             accept_out ? accept_out + mv : nullptr,
-                                            forced ? forced + mv : nullptr, a.phi_record, nrec, s);
+                                            forced ? forced + mv : nullptr, s);
                 if (rc) return rc;
                 continue;
             }
-            prof_start(d, kProfSpoRatio, s);
-            spo_ratio_kernel<true><<<dim3(tiles, nw), threads, 0, s>>>(a);
+            // K2: ratio + row copy, K3: decision + rank-1 update
+            prof_start(d, kProfRatio, s);
+            ratio_rowcopy_kernel<<<nw, 256, 0, s>>>(d->B, nel, d->ld, k, phi, (size_t)5 * d->np, d->rowk, d->rpart);
             prof_stop(d, s);
             QMC_LAUNCHED();
             UpdateArgs u{};
             u.B = d->B; u.nel = nel; u.ld = d->ld; u.iel = k;
-            u.phi = d->vgl; u.ldphi = (size_t)5 * d->np; u.rowk = d->rowk;
-            u.rpart = d->rpart; u.ntiles = tiles;
+            u.phi = phi; u.ldphi = (size_t)5 * d->np; u.rowk = d->rowk;
+            u.rpart = d->rpart; u.ntiles = 1;
             u.unif = unif + mv;
             u.forced = forced ? forced + mv : nullptr;
             u.ratios_out = ratios_out ? ratios_out + mv : nullptr;
