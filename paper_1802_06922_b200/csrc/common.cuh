@@ -80,8 +80,12 @@ struct qmc_det {
     // delayed-update window (delay >= 2)
     int *win_count;             // [nw]           accepted rows pending
     int *win_iel;               // [nw][delay]    their electron indices
-    float *win_phi;             // [nw][delay][np] their orbital vectors
-    double *win_rows;           // [nw][delay][ld] rows B0[k_l] saved at accept time
+    int *win_slot;              // [nw][delay]    slot of row / vector l in win_rows / win_vec
+    float *win_phi;             // [nw][delay][np] orbital vectors appended by qmc_det_accept_update
+    double *win_rows;           // [nw][delay][ld] rows B0[k_l] (qmc_det_accept_update), turned into R' = S^-T Rows for the flush
+    int win_rows_raw;           // win_rows still holds the raw rows (the flush converts them first)
+    const float *win_vec;       // where the flush finds the vectors: win_phi, or the SPO-VGL scratch (qmc_sweep)
+    size_t win_vec_wstride, win_vec_sstride;   // its walker and slot strides (floats)
     double *win_sinv;           // [nw][delay][delay] inverse of S
     int *win_full;              // [1] set when any walker's window is full
     int host_pending;           // electron steps appended to the open window (host bookkeeping)

@@ -10,8 +10,9 @@
 //   flush:  q_l(m) = v_l . B0[m] - [k_l == m],  t(m) = S^-1 q(m),
 //           B[m] = B0[m] - sum_l t_l(m) * B0[k_l]      -- one pass over B: 16 N ld bytes / walker.
 //
-// A window is K consecutive electron steps of the lockstep sweep (R:A14), so the host schedules
-// the flushes and no device -> host traffic is needed.
+// This file is the STEP-BY-STEP form behind qmc_det_ratio / qmc_det_accept_update in delayed mode
+// (one launch per call, 2p+1 dots against the window).  qmc_sweep uses the one-launch-per-window
+// form in window.cu.  The host schedules the flushes, so no device -> host traffic is needed.
 #include "delayed_device.cuh"
 #include "spo_device.cuh"
 #include "update_device.cuh"
@@ -31,16 +32,10 @@ struct DelayedStepArgs {
     float *win_phi;               // [nw][K][np]
     double *win_rows;             // [nw][K][ld]
     double *win_sinv;             // [nw][K][K]
-    // mode: decide here (sweep) or ratio only / accept only (standalone API)
-    int mode;                     // 0 = sweep step (ratio + decide + append), 1 = ratio only, 2 = append only
-    double *ratio_io;             // [nw]  mode 1: out; mode 2: in
+    int *win_slot;                // [nw][K]  slot l of win_rows / win_phi holds accepted move l
+    int mode;                     // 1 = ratio only, 2 = append only (the caller's decision)
+    double *ratio_io;             // [nw]  mode 1: out
     const unsigned char *accept_in;   // [nw] mode 2
-    const double *unif;           // [nw]  mode 0
-    const unsigned char *forced;  // [nw] or NULL, mode 0
-    double *ratios_out;           // [nw] or NULL, mode 0
-    unsigned char *accept_out;    // [nw] or NULL, mode 0
-    double *pos;                  // [nw][nel][3], mode 0
-    const double *delta;          // [nw][3], mode 0
     double *logdet;
     int *sign;
     long long *naccept;
@@ -48,8 +43,8 @@ struct DelayedStepArgs {
 
 // One block per walker.  Each thread owns column quads j = 4*tid (+ 4*blockDim per pass): it
 // accumulates the 2p+1 partial dots d, x_m, c_l over its columns; the block reduces them in a
-// fixed order; warp 0 finishes the ratio, takes the Metropolis decision and, on accept, grows the
-// window (row copy, orbital vector copy, bordered S^-1).
+// fixed order; warp 0 finishes the ratio and, on accept, the block grows the window (row copy,
+// orbital vector copy, bordered S^-1).
 template <int KMAX>
 __global__ void __launch_bounds__(kStepThreads) delayed_step_kernel(DelayedStepArgs a)
 {
@@ -124,15 +119,8 @@ __global__ void __launch_bounds__(kStepThreads) delayed_step_kernel(DelayedStepA
         double R = s_tot[0];
         for (int m = 0; m < p; ++m) R -= s_tot[1 + m] * s_y[m];
         bool acc_w = false;
-        if (a.mode == 2) {
-            acc_w = a.accept_in[w] != 0;      // the caller's decision; R equals the ratio it was given
-        } else if (a.mode == 0) {
-            acc_w = a.forced ? (a.forced[w] != 0) : metropolis(R, a.unif[w]);
-            if (a.ratios_out) a.ratios_out[w] = R;
-            if (a.accept_out) a.accept_out[w] = acc_w ? 1 : 0;
-        } else {
-            a.ratio_io[w] = R;
-        }
+        if (a.mode == 2) acc_w = a.accept_in[w] != 0;      // the caller's decision; R equals the ratio it was given
+        else a.ratio_io[w] = R;
         s_tot[0] = R;
         s_flag = acc_w;
     }
@@ -143,13 +131,8 @@ __global__ void __launch_bounds__(kStepThreads) delayed_step_kernel(DelayedStepA
         a.logdet[w] += log(fabs(R));
         if (R < 0.0) a.sign[w] = -a.sign[w];
         a.naccept[w] += 1;
-        if (a.mode == 0) {
-            double *r = a.pos + ((size_t)w * a.nel + a.iel) * 3;
-            r[0] += a.delta[3 * (size_t)w + 0];
-            r[1] += a.delta[3 * (size_t)w + 1];
-            r[2] += a.delta[3 * (size_t)w + 2];
-        }
         a.win_iel[(size_t)w * K + p] = a.iel;
+        a.win_slot[(size_t)w * K + p] = p;
         a.win_count[w] = p + 1;
     }
     // append the orbital vector and the row B0[k]
@@ -188,7 +171,7 @@ static void fill_common(DelayedStepArgs &a, qmc_det *d, int iel, const float *ph
 {
     a.B = d->B; a.nel = d->nel; a.ld = d->ld; a.np = d->np; a.iel = iel; a.K = d->delay;
     a.phi = phi; a.ldphi = ldphi;
-    a.win_count = d->win_count; a.win_iel = d->win_iel; a.win_phi = d->win_phi;
+    a.win_count = d->win_count; a.win_iel = d->win_iel; a.win_slot = d->win_slot; a.win_phi = d->win_phi;
     a.win_rows = d->win_rows; a.win_sinv = d->win_sinv;
     a.logdet = d->logdet; a.sign = d->sign; a.naccept = d->naccept;
 }
@@ -231,6 +214,10 @@ int delayed_accept(qmc_det *d, int iel, const float *phi, int ldo, const double 
     QMC_CUDA(e);
     d->host_pending += 1;
     d->win_host_iel[iel] = 1;
+    d->win_rows_raw = 1;
+    d->win_vec = d->win_phi;
+    d->win_vec_wstride = (size_t)d->delay * d->np;
+    d->win_vec_sstride = (size_t)d->np;
     return QMC_OK;
 }
 
@@ -239,29 +226,6 @@ int delayed_flush_reset_host(qmc_det *d, cudaStream_t s)
     int rc = delayed_flush(d, s);
     if (rc) return rc;
     if (d->win_host_iel) memset(d->win_host_iel, 0, (size_t)d->nel);
-    return QMC_OK;
-}
-
-int delayed_sweep_step(qmc_det *d, double *pos, const double *delta, const double *unif, int iel,
-                       const float *phi, double *ratios_out, unsigned char *accept_out,
-                       const unsigned char *forced, cudaStream_t s)
-{
-    if (d->host_pending >= d->delay || (d->host_pending && d->win_host_iel[iel])) {
-        int rc = delayed_flush_reset_host(d, s);
-        if (rc) return rc;
-    }
-    // ratio against the window / decide / append
-    DelayedStepArgs a{};
-    fill_common(a, d, iel, phi, (size_t)5 * d->np);
-    a.mode = 0;
-    a.unif = unif; a.forced = forced; a.ratios_out = ratios_out; a.accept_out = accept_out;
-    a.pos = pos; a.delta = delta;
-    prof_start(d, kProfDelayedRatio, s);
-    cudaError_t e = launch_step(a, d->nw, s);
-    prof_stop(d, s);
-    QMC_CUDA(e);
-    d->host_pending += 1;
-    d->win_host_iel[iel] = 1;
     return QMC_OK;
 }
 

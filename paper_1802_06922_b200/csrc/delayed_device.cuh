@@ -10,10 +10,9 @@ int delayed_accept(qmc_det *d, int iel, const float *phi, int ldo, const double 
 int delayed_flush(qmc_det *d, cudaStream_t s);
 int delayed_flush_reset_host(qmc_det *d, cudaStream_t s);   // flush + forget the host-side window bookkeeping
 int delayed_max_rank(int ld);                                // largest K whose window fits shared memory
-// One electron step of qmc_sweep in delayed mode (all pointers offset to the step); phi is the
-// step's slot of the batched SPO-VGL scratch, [nw][5][np].
-int delayed_sweep_step(qmc_det *d, double *pos, const double *delta, const double *unif, int iel,
-                       const float *phi, double *ratios_out, unsigned char *accept_out,
-                       const unsigned char *forced, cudaStream_t s);
+// One window of qmc_sweep in delayed mode: electrons iel0 .. iel0+nb-1 (nb <= delay rank), whose
+// SPO-VGL is in d->vgl; ratios, decisions, moves and the flush.  Pointers are offset to the first step.
+int delayed_sweep_window(qmc_det *d, double *pos, const double *delta, const double *unif, int iel0, int nb,
+                         double *ratios_out, unsigned char *accept_out, const unsigned char *forced, cudaStream_t s);
 
 }  // namespace qmc

@@ -228,7 +228,7 @@ static void det_free(qmc_det *d)
     }
     cudaFree(d->B); cudaFree(d->logdet); cudaFree(d->sign); cudaFree(d->naccept);
     cudaFree(d->vgl); cudaFree(d->rowk); cudaFree(d->rpart); cudaFree(d->ratio); cudaFree(d->acc);
-    cudaFree(d->win_count); cudaFree(d->win_iel); cudaFree(d->win_phi); cudaFree(d->win_rows);
+    cudaFree(d->win_count); cudaFree(d->win_iel); cudaFree(d->win_slot); cudaFree(d->win_phi); cudaFree(d->win_rows);
     cudaFree(d->win_sinv); cudaFree(d->win_full); cudaFree(d->stage);
     free(d->win_host_iel);
     delete d;
@@ -315,12 +315,16 @@ extern "C" int qmc_det_init(qmc_det_t **out, const qmc_spline_t *sp, int nw, int
         d->win_host_iel = (unsigned char *)calloc((size_t)nel, 1);
         if (!d->win_host_iel) { set_error("qmc_det_init: host allocation failed"); det_free(d); return QMC_ENOMEM; }
         if ((rc = dev_alloc(&d->win_count, nw, "win_count")) || (rc = dev_alloc(&d->win_iel, (size_t)nw * K, "win_iel")) ||
+            (rc = dev_alloc(&d->win_slot, (size_t)nw * K, "win_slot")) ||
             (rc = dev_alloc(&d->win_phi, (size_t)nw * K * np, "win_phi")) ||
             (rc = dev_alloc(&d->win_rows, (size_t)nw * K * ld, "win_rows")) ||
             (rc = dev_alloc(&d->win_sinv, (size_t)nw * K * K, "win_sinv")) || (rc = dev_alloc(&d->win_full, 1, "win_full"))) {
             det_free(d);
             return rc;
         }
+        d->win_vec = d->win_phi;
+        d->win_vec_wstride = (size_t)K * np;
+        d->win_vec_sstride = (size_t)np;
     }
     cudaError_t e = cudaMemsetAsync(d->B, 0, (size_t)nw * nel * ld * sizeof(double), s);
     if (e == cudaSuccess) e = cudaMemsetAsync(d->rowk, 0, (size_t)nw * ld * sizeof(double), s);

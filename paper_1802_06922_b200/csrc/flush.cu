@@ -3,30 +3,25 @@
 // multiplication [44]", L299; formulas: DESIGN.md section 3, R:O7):
 //
 //     Q[m][l] = B0[m] . v_l - [k_l == m]          (N x N)(N x p)     step 1
-//     T       = Q S^-T                             (N x p)(p x p)
-//     B[m]    = B0[m] - sum_l T[m][l] * B0[k_l]    (N x p)(p x N)     step 2
+//     B[m]    = B0[m] - sum_l Q[m][l] * R'[l]      (N x p)(p x N)     step 2,  R' = S^-T Rows
 //
 // in ONE pass over B (16 N ld bytes per walker): a warp keeps an 8-row x (8 TW)-column block of B
 // in registers.  With the contraction index of step 1 permuted so that one lane's `double2` of a
 // row serves two consecutive k-steps, the registers a lane loads (row g, columns 2t, 2t+1 of every
 // 8-column tile) are at once the A fragments of step 1 and the C fragments of step 2 of
-// mma.sync.m8n8k4.f64 (SASS: DMMA.8x8x4), and T's C fragments are step 2's A fragments when its
-// contraction index is permuted the same way: no shuffles, no transposes.
+// mma.sync.m8n8k4.f64 (SASS: DMMA.8x8x4); Q, summed over the column slices, is read back from
+// shared memory directly in A-fragment layout for step 2: no shuffles, no transposes.
 //
-// The walker's window (p saved rows in fp64, p orbital vectors in fp32, S^-1) is staged once per
-// CTA into shared memory with TMA bulk copies (cp.async.bulk + mbarrier) and shared by NG warp
-// groups that stream different row blocks out of phase, so one group's DMMA work overlaps the
-// other group's HBM loads and stores.
+// The walker's window (p rows of R' in fp64, p orbital vectors in fp32) is staged once per CTA into
+// shared memory with TMA bulk copies (cp.async.bulk + mbarrier).  For large N the columns of a row
+// block are split over a thread-block CLUSTER (each CTA stages only its column slice of the window,
+// so two or three CTAs fit an SM and one CTA's HBM stream runs under another's DMMA work); the
+// partial Q of the slices are exchanged through distributed shared memory once per row block.
+#include <stdlib.h>
 #include "delayed_device.cuh"
+#include "dmma.cuh"
 
 namespace qmc {
-
-__device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double b)
-{
-    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
-                 : "+d"(c0), "+d"(c1)
-                 : "d"(a), "d"(b));
-}
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -64,100 +59,98 @@ __device__ __forceinline__ void group_sync(int id, int nthreads)
 {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
+// thread-block cluster helpers (CS > 1: the CTAs of a cluster own column slices of the same rows)
+__device__ __forceinline__ uint32_t cluster_ctarank()
+{
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ void cluster_arrive()
+{
+    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void cluster_wait()
+{
+    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// read a double from the shared memory of CTA `rank` of this cluster (distributed shared memory)
+__device__ __forceinline__ double ld_dsmem(const double *local, uint32_t rank)
+{
+    uint32_t raddr;
+    double v;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(raddr) : "r"(smem_u32(local)), "r"(rank));
+    asm volatile("ld.shared::cluster.f64 %0, [%1];" : "=d"(v) : "r"(raddr) : "memory");
+    return v;
+}
+
 struct FlushArgs {
     double *B;                    // [nw][nel][ld]
     int nel, ld, np, K;
     int rows_per_cta;             // multiple of 8 * NG
     const int *win_count;
     const int *win_iel;
-    const float *win_phi;
-    const double *win_rows;
-    const double *win_sinv;
+    const int *win_slot;          // [nw][K] slot of accepted move l in win_rows / vec
+    const float *vec;             // orbital vector of (walker w, slot s) at vec + w * vec_wstride + s * vec_sstride
+    size_t vec_wstride, vec_sstride;
+    const double *win_rows;       // [nw][K][ld] R'[l] = (S^-T Rows)[l], accepted order
 };
 
-// Shared-memory geometry (strides chosen so every fragment load is bank-conflict free):
-//   rows_s  double [KPAD][LD + 2]   B-fragment of step 2: lane (g,t) reads row 8nt+2t+h, column n0+g
-//   v_s     float  [KPAD][LD + 8]   B-fragment of step 1: lane (g,t) reads row 8nt+g, columns n0+2t,+1
-//   sinv_s  double [KPAD][KPAD + 4]
-//   part_s  double [2][NG][NWC][8][KPAD + 4]   partial Q of each column warp, by block parity
+// Shared-memory geometry of one CTA, which owns LDC = ld / CS columns (strides chosen so every
+// fragment load is bank-conflict free):
+//   rows_s  double [KPAD][LDC + 4]  B-fragment of step 2: lane (g,t) reads row 4kq+t, column n0+g
+//   v_s     float  [KPAD][LDC + 8]  B-fragment of step 1: lane (g,t) reads row 8nt+g, columns n0+2t,+1
+//   part_s  double [PB][NG][NWC][8][KPAD + 4]   partial Q of each column warp (CS == 1: by block parity)
+//   cpart_s double [2][8][KPAD + 4]             CS > 1: this CTA's partial Q, read by its cluster peers
 //   kl_s    int [KPAD],  mbar
-template <int KPAD, int LD, int NWC, int NG>
+template <int KPAD, int LDC, int NWC, int NG, int CS>
 struct FlushSmem {
-    static constexpr int RS = LD + 2, VS = LD + 8, SS = KPAD + 4, PS = KPAD + 4;
+    static constexpr int RS = LDC + 4, VS = LDC + 8, PS = KPAD + 4;
     static constexpr size_t rows_off = 0;
     static constexpr size_t v_off = rows_off + (size_t)KPAD * RS * sizeof(double);
-    static constexpr size_t sinv_off = v_off + (size_t)KPAD * VS * sizeof(float);
-    static constexpr size_t part_off = sinv_off + (size_t)KPAD * SS * sizeof(double);
+    static constexpr size_t part_off = v_off + (size_t)KPAD * VS * sizeof(float);
     static constexpr size_t part_bytes = (size_t)NG * NWC * 8 * PS * sizeof(double);
-    // two partial buffers (by block parity) save a barrier per block; one when shared memory is short
-    static constexpr int PB = (part_off + 2 * part_bytes + KPAD * sizeof(int) + 16 <= 227 * 1024) ? 2 : 1;
-    static constexpr size_t kl_off = part_off + PB * part_bytes;
+    static constexpr size_t cpart_bytes = CS > 1 ? (size_t)2 * 8 * PS * sizeof(double) : 0;
+    // CS == 1: two partial buffers (by block parity) save a barrier per block; one when shared
+    // memory is short.  CS > 1: the cluster barrier of every block already orders their reuse.
+    static constexpr int PB =
+        (CS == 1 && part_off + 2 * part_bytes + KPAD * sizeof(int) + 16 <= 227 * 1024) ? 2 : 1;
+    static constexpr size_t cpart_off = part_off + PB * part_bytes;
+    static constexpr size_t kl_off = cpart_off + cpart_bytes;
     static constexpr size_t mbar_off = kl_off + (size_t)KPAD * sizeof(int);
     static constexpr size_t bytes = mbar_off + 16;
 };
 
 constexpr size_t kSmemMax = 227 * 1024;
 
-template <int KPAD, int NWC, int TW, int NG, bool PF>
-__global__ void __launch_bounds__(32 * NWC * NG, 1) flush_dmma_kernel(FlushArgs a)
+// Row-block loop of the flush for a window of NTA active 8-wide tiles (8 NTA - 7 <= p <= 8 NTA): a
+// compile-time count keeps the DMMA sequences free of branches, so the shared-memory operand loads
+// and the fp32 -> fp64 conversions are scheduled ahead of the tensor-core instructions.
+template <int KPAD, int NWC, int TW, int NG, bool PF, int CS, int NTA>
+__device__ __forceinline__ void flush_stream(const FlushArgs &a, int w, const double *rows_s, const float *v_s,
+                                             double *part_s, double *cpart_s, const int *kl_s, uint64_t *mbar,
+                                             int crank, int colbase)
 {
-    constexpr int LD = NWC * TW * 8;
-    constexpr int NT = KPAD / 8;
-    using L = FlushSmem<KPAD, LD, NWC, NG>;
-    constexpr int RS = L::RS, VS = L::VS, SS = L::SS, PS = L::PS;
+    constexpr int LDC = NWC * TW * 8;
+    constexpr int LD = LDC * CS;
+    using L = FlushSmem<KPAD, LDC, NWC, NG, CS>;
+    constexpr int RS = L::RS, VS = L::VS, PS = L::PS;
     constexpr int NTHREADS = 32 * NWC * NG;
-    extern __shared__ __align__(128) unsigned char smem_flush[];
-    double *rows_s = reinterpret_cast<double *>(smem_flush + L::rows_off);
-    float *v_s = reinterpret_cast<float *>(smem_flush + L::v_off);
-    double *sinv_s = reinterpret_cast<double *>(smem_flush + L::sinv_off);
-    double *part_s = reinterpret_cast<double *>(smem_flush + L::part_off);
-    int *kl_s = reinterpret_cast<int *>(smem_flush + L::kl_off);
-    uint64_t *mbar = reinterpret_cast<uint64_t *>(smem_flush + L::mbar_off);
-
-    const int w = blockIdx.y;
-    const int p = a.win_count[w];
-    if (p == 0) return;
-    const int p8 = (p + 7) & ~7;
+    constexpr int KQA = 2 * NTA;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int g = lane >> 2, t = lane & 3;
     const int grp = warp / NWC, wc = warp % NWC;
-    const int K = a.K, np = a.np, nel = a.nel;
+    const int nel = a.nel;
 
-    // ---- stage the window: zero what the bulk copies do not write, then TMA the rows in
-    if (tid == 0) mbar_init(mbar, 1);
-    for (int e = tid; e < p * (LD - np); e += NTHREADS) {          // pad columns of the vectors
-        const int l = e / (LD - np), c = np + e % (LD - np);
-        v_s[l * VS + c] = 0.f;
-    }
-    for (int e = tid; e < (p8 - p) * LD; e += NTHREADS) {          // rows p..p8-1 of the last tile
-        const int l = p + e / LD, c = e % LD;
-        v_s[l * VS + c] = 0.f;
-        rows_s[l * RS + c] = 0.0;
-    }
-    for (int e = tid; e < KPAD * KPAD; e += NTHREADS) {
-        const int i = e / KPAD, j = e % KPAD;
-        sinv_s[i * SS + j] = (i < p && j < p) ? a.win_sinv[(size_t)w * K * K + i * K + j] : 0.0;
-    }
-    if (tid < KPAD) kl_s[tid] = tid < p ? a.win_iel[(size_t)w * K + tid] : -1;
-    __syncthreads();
-    if (warp == 0) {
-        if (lane == 0) mbar_arrive_expect_tx(mbar, (uint32_t)p * (uint32_t)(LD * sizeof(double) + np * sizeof(float)));
-        __syncwarp();
-        const double *rows_g = a.win_rows + (size_t)w * K * LD;
-        const float *v_g = a.win_phi + (size_t)w * K * np;
-        for (int l = lane; l < p; l += 32) {
-            bulk_g2s(rows_s + l * RS, rows_g + (size_t)l * LD, LD * sizeof(double), mbar);
-            bulk_g2s(v_s + l * VS, v_g + (size_t)l * np, np * sizeof(float), mbar);
-        }
-    }
-
-    // ---- stream row blocks: group `grp` takes blocks grp, grp + NG, ... of this CTA's rows.
-    // With PF the next block's rows are requested before the current block is contracted, so the
-    // HBM stream (loads of block i+1, stores of block i-1) runs under the DMMA work of block i.
-    const int m_begin = blockIdx.x * a.rows_per_cta;
+    // group `grp` takes blocks grp, grp + NG, ... of this CTA's rows.  With PF the next block's rows
+    // are requested before the current block is contracted, so the HBM stream (loads of block i+1,
+    // stores of block i-1) runs under the DMMA work of block i.
+    const int m_begin = (blockIdx.x / CS) * a.rows_per_cta;
     const int m_end = min(nel, m_begin + a.rows_per_cta);
-    const int col0 = 8 * TW * wc;
-    double *const walker_B = a.B + (size_t)w * nel * LD + col0 + 2 * t;
+    const int col0 = 8 * TW * wc;                                  // within the CTA's slice
+    double *const walker_B = a.B + (size_t)w * nel * LD + colbase + col0 + 2 * t;
+    const float *const vfrag = v_s + g * VS + col0 + 2 * t;        // step-1 B fragments of this lane
+    const double *const rfrag = rows_s + t * RS + col0 + g;        // step-2 B fragments of this lane
     bool staged = false;
     int m0 = m_begin + 8 * grp;
     double2 r[TW], rn[PF ? TW : 1];
@@ -179,64 +172,68 @@ __global__ void __launch_bounds__(32 * NWC * NG, 1) flush_dmma_kernel(FlushArgs 
             staged = true;
         }
         // step 1: partial Q over this warp's columns
-        double cq[NT][2];
+        double cq[NTA][2];
 #pragma unroll
-        for (int nt = 0; nt < NT; ++nt) cq[nt][0] = cq[nt][1] = 0.0;
+        for (int nt = 0; nt < NTA; ++nt) cq[nt][0] = cq[nt][1] = 0.0;
 #pragma unroll
         for (int i = 0; i < TW; ++i) {
 #pragma unroll
-            for (int nt = 0; nt < NT; ++nt) {
-                if (8 * nt < p) {
-                    const float2 f = *reinterpret_cast<const float2 *>(v_s + (8 * nt + g) * VS + col0 + 8 * i + 2 * t);
-                    dmma884(cq[nt][0], cq[nt][1], r[i].x, (double)f.x);
-                    dmma884(cq[nt][0], cq[nt][1], r[i].y, (double)f.y);
-                }
+            for (int nt = 0; nt < NTA; ++nt) {
+                const float2 f = *reinterpret_cast<const float2 *>(vfrag + 8 * nt * VS + 8 * i);
+                dmma884(cq[nt][0], cq[nt][1], r[i].x, (double)f.x);
+                dmma884(cq[nt][0], cq[nt][1], r[i].y, (double)f.y);
             }
         }
-        // partials are double-buffered by block parity: one barrier per block is enough
+        // CS == 1: partials are double-buffered by block parity, one barrier per block is enough
         double *pbuf = part_s + (size_t)((L::PB == 2 ? (it & 1) : 0) * NG + grp) * NWC * 8 * PS;
         double *ps = pbuf + ((size_t)wc * 8 + g) * PS;
 #pragma unroll
-        for (int nt = 0; nt < NT; ++nt)
-            if (8 * nt < p) *reinterpret_cast<double2 *>(ps + 8 * nt + 2 * t) = make_double2(cq[nt][0], cq[nt][1]);
-        group_sync(1 + grp, 32 * NWC);
-        // Q as A fragments: lane (g,t), k-step k' holds Q[m0+g][4k'+t], summed over the column warps
-        double qa[KPAD / 4];
+        for (int nt = 0; nt < NTA; ++nt)
+            *reinterpret_cast<double2 *>(ps + 8 * nt + 2 * t) = make_double2(cq[nt][0], cq[nt][1]);
+        // Q as A fragments: lane (g,t), k-step kq holds Q[m0+g][4kq+t], summed over the column slices
+        double qa[KQA];
+        if constexpr (CS == 1) {
+            group_sync(1 + grp, 32 * NWC);
 #pragma unroll
-        for (int kq = 0; kq < KPAD / 4; ++kq) {
-            double s = 0.0;
-            if (4 * kq < p8) {
+            for (int kq = 0; kq < KQA; ++kq) {
                 const double *pp = pbuf + (size_t)g * PS + 4 * kq + t;
+                double s = 0.0;
 #pragma unroll
                 for (int c = 0; c < NWC; ++c) s += pp[(size_t)c * 8 * PS];
                 if (kl_s[4 * kq + t] == m) s -= 1.0;
+                qa[kq] = s;
             }
-            qa[kq] = s;
+            if (L::PB == 1) group_sync(1 + grp, 32 * NWC);
+        } else {
+            // two levels: this CTA's column warps first (fixed order), then the CTAs of the cluster
+            // through distributed shared memory (fixed order: every CTA forms bit-identical Q)
+            __syncthreads();
+            double *cp = cpart_s + (size_t)(it & 1) * 8 * PS;
+            for (int e = tid; e < 8 * 8 * NTA; e += NTHREADS) {
+                const int row = e / (8 * NTA), col = e % (8 * NTA);
+                double s = 0.0;
+#pragma unroll
+                for (int c = 0; c < NWC; ++c) s += pbuf[((size_t)c * 8 + row) * PS + col];
+                cp[row * PS + col] = s;
+            }
+            cluster_arrive();
+            cluster_wait();
+#pragma unroll
+            for (int kq = 0; kq < KQA; ++kq) {
+                const double *pp = cp + (size_t)g * PS + 4 * kq + t;
+                double s = 0.0;
+#pragma unroll
+                for (int c = 0; c < CS; ++c) s += (c == crank) ? *pp : ld_dsmem(pp, (uint32_t)c);
+                if (kl_s[4 * kq + t] == m) s -= 1.0;
+                qa[kq] = s;
+            }
         }
-        if (L::PB == 1) group_sync(1 + grp, 32 * NWC);
-        // T = Q S^-T (C fragments), negated
-        double tq[NT][2];
+        // step 2: B block -= Q R'; contraction index l = 4kq + t
 #pragma unroll
-        for (int nt = 0; nt < NT; ++nt) {
-            tq[nt][0] = tq[nt][1] = 0.0;
-            if (8 * nt < p) {
+        for (int kq = 0; kq < KQA; ++kq) {
+            const double af = -qa[kq];
 #pragma unroll
-                for (int kq = 0; kq < KPAD / 4; ++kq)
-                    if (4 * kq < p8) dmma884(tq[nt][0], tq[nt][1], qa[kq], sinv_s[(8 * nt + g) * SS + 4 * kq + t]);
-            }
-        }
-        // step 2: B block += (-T) Rows; contraction index l = 8nt + 2t + h
-#pragma unroll
-        for (int nt = 0; nt < NT; ++nt) {
-            if (8 * nt < p) {
-#pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    const double af = -tq[nt][h];
-                    const double *rp = rows_s + (8 * nt + 2 * t + h) * RS + col0 + g;
-#pragma unroll
-                    for (int i = 0; i < TW; ++i) dmma884(r[i].x, r[i].y, af, rp[8 * i]);
-                }
-            }
+            for (int i = 0; i < TW; ++i) dmma884(r[i].x, r[i].y, af, rfrag[4 * kq * RS + 8 * i]);
         }
         if (m < nel) {
             double *dst = walker_B + (size_t)m * LD;
@@ -253,6 +250,96 @@ __global__ void __launch_bounds__(32 * NWC * NG, 1) flush_dmma_kernel(FlushArgs 
         }
     }
     if (!staged) mbar_wait(mbar, 0);            // never leave with bulk copies in flight
+    if constexpr (CS > 1) {                     // ... nor while a peer may still read this CTA's partials
+        cluster_arrive();
+        cluster_wait();
+    }
+}
+
+// NWC column warps x TW 8-column tiles per warp = the CTA's LDC columns; NG row groups per CTA
+// (CS == 1 only); PF = prefetch the next row block into registers; CS = cluster size.
+template <int KPAD, int NWC, int TW, int NG, bool PF, int CS>
+__global__ void __launch_bounds__(32 * NWC * NG,
+                                  (2 * (FlushSmem<KPAD, NWC * TW * 8, NWC, NG, CS>::bytes + 1024) <= 228 * 1024 &&
+                                   2 * 32 * NWC * NG <= 1024) ? 2 : 1)
+flush_dmma_kernel(FlushArgs a)
+{
+    static_assert(CS == 1 || NG == 1, "a cluster exchanges partials with a cluster-wide barrier: one row group");
+    constexpr int LDC = NWC * TW * 8;
+    constexpr int LD = LDC * CS;
+    constexpr int NT = KPAD / 8;
+    using L = FlushSmem<KPAD, LDC, NWC, NG, CS>;
+    constexpr int RS = L::RS, VS = L::VS;
+    constexpr int NTHREADS = 32 * NWC * NG;
+    extern __shared__ __align__(128) unsigned char smem_flush[];
+    double *rows_s = reinterpret_cast<double *>(smem_flush + L::rows_off);
+    float *v_s = reinterpret_cast<float *>(smem_flush + L::v_off);
+    double *part_s = reinterpret_cast<double *>(smem_flush + L::part_off);
+    double *cpart_s = reinterpret_cast<double *>(smem_flush + L::cpart_off);
+    int *kl_s = reinterpret_cast<int *>(smem_flush + L::kl_off);
+    uint64_t *mbar = reinterpret_cast<uint64_t *>(smem_flush + L::mbar_off);
+
+    const int w = blockIdx.y;
+    const int p = a.win_count[w];
+    if (p == 0) return;                                            // the whole cluster leaves together
+    const int p8 = (p + 7) & ~7;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int K = a.K;
+    const int crank = CS > 1 ? (int)cluster_ctarank() : 0;
+    const int colbase = crank * LDC;                               // first column this CTA owns
+    const int nvec = max(0, min(a.np - colbase, LDC));             // its share of the vectors' np columns
+
+    // ---- stage the window: zero what the bulk copies do not write, then TMA the rows in
+    if (tid == 0) mbar_init(mbar, 1);
+    for (int e = tid; e < p * (LDC - nvec); e += NTHREADS) {       // pad columns of the vectors
+        const int l = e / (LDC - nvec), c = nvec + e % (LDC - nvec);
+        v_s[l * VS + c] = 0.f;
+    }
+    for (int e = tid; e < (p8 - p) * LDC; e += NTHREADS) {         // rows p..p8-1 of the last tile
+        const int l = p + e / LDC, c = e % LDC;
+        v_s[l * VS + c] = 0.f;
+        rows_s[l * RS + c] = 0.0;
+    }
+    if (tid < KPAD) kl_s[tid] = tid < p ? a.win_iel[(size_t)w * K + tid] : -1;
+    __syncthreads();
+    if (warp == 0) {
+        if (lane == 0)
+            mbar_arrive_expect_tx(mbar, (uint32_t)p * (uint32_t)(LDC * sizeof(double) + nvec * sizeof(float)));
+        __syncwarp();
+        const double *rows_g = a.win_rows + (size_t)w * K * LD + colbase;
+        const float *v_g = a.vec + (size_t)w * a.vec_wstride + colbase;
+        for (int l = lane; l < p; l += 32) {
+            const int slot = a.win_slot[(size_t)w * K + l];
+            bulk_g2s(rows_s + l * RS, rows_g + (size_t)l * LD, LDC * sizeof(double), mbar);
+            if (nvec) bulk_g2s(v_s + l * VS, v_g + (size_t)slot * a.vec_sstride, nvec * sizeof(float), mbar);
+        }
+    }
+
+    // ---- stream the row blocks with the tile count of this window
+    switch (p8 / 8) {
+    case 1: flush_stream<KPAD, NWC, TW, NG, PF, CS, 1>(a, w, rows_s, v_s, part_s, cpart_s, kl_s, mbar, crank, colbase); break;
+    case 2: if constexpr (NT >= 2) flush_stream<KPAD, NWC, TW, NG, PF, CS, 2>(a, w, rows_s, v_s, part_s, cpart_s, kl_s, mbar, crank, colbase); break;
+    case 3: if constexpr (NT >= 3) flush_stream<KPAD, NWC, TW, NG, PF, CS, 3>(a, w, rows_s, v_s, part_s, cpart_s, kl_s, mbar, crank, colbase); break;
+    case 4: if constexpr (NT >= 4) flush_stream<KPAD, NWC, TW, NG, PF, CS, 4>(a, w, rows_s, v_s, part_s, cpart_s, kl_s, mbar, crank, colbase); break;
+    }
+}
+
+// qmc_det_accept_update appended the raw rows B0[k_l] (row l) and kept S^-1: turn the rows into
+// R' = S^-T Rows in place before the flush.  One block per walker.
+template <int KMAX>
+__global__ void __launch_bounds__(256) rprime_kernel(int ld, int K, const int *win_count, const double *win_sinv,
+                                                     double *win_rows)
+{
+    constexpr int GS = KMAX + 1;
+    __shared__ double sinv_s[KMAX * GS];
+    __shared__ long long rowoff_s[KMAX];
+    const int w = blockIdx.x, p = win_count[w];
+    if (p == 0) return;
+    for (int e = threadIdx.x; e < p * p; e += 256) sinv_s[(e / p) * GS + e % p] = win_sinv[(size_t)w * K * K + (e / p) * K + e % p];
+    if (threadIdx.x < p) rowoff_s[threadIdx.x] = (long long)threadIdx.x * ld;
+    __syncthreads();
+    double *rows = win_rows + (size_t)w * K * ld;
+    rprime_warp<KMAX>(sinv_s, GS, p, rows, rowoff_s, rows, ld, threadIdx.x >> 5, 8, threadIdx.x & 31);
 }
 
 __global__ void reset_window_kernel(int nw, int *win_count)
@@ -261,30 +348,55 @@ __global__ void reset_window_kernel(int nw, int *win_count)
     if (w < nw) win_count[w] = 0;
 }
 
-// Launch shape for ld = 64 v: NWC column warps x TW 8-column tiles per warp, NG row groups per
-// CTA, PF = prefetch the next row block (needs 2 x 4 TW data registers per thread).
-struct FlushShape { int nwc, tw, ng; };
+// Launch shapes.  X(V, NWC, TW, NG, PF, CS): ld = 64 V doubles = CS * NWC * TW * 8.  Several shapes
+// may serve one ld, in order of measured preference; the first whose window fits shared memory is
+// used (a cluster shape stages only ld / CS columns per CTA, so it serves the larger ranks).
 #define QMC_FLUSH_SHAPES(X) \
-    X(1, 1, 8, 4, true) X(2, 2, 8, 4, true) X(3, 3, 8, 4, true) X(4, 4, 8, 4, true) X(6, 6, 8, 2, true) \
-    X(8, 8, 8, 2, true) X(12, 6, 16, 2, false) X(16, 8, 16, 2, false) X(24, 12, 16, 1, false) X(32, 16, 16, 1, false)
+    X(1, 1, 8, 4, true, 1) X(2, 2, 8, 4, true, 1) X(3, 3, 8, 4, true, 1) X(4, 4, 8, 4, true, 1) X(6, 6, 8, 2, true, 1) \
+    X(8, 8, 8, 2, true, 1) X(8, 8, 4, 1, true, 2) \
+    X(12, 6, 16, 2, false, 1) X(12, 6, 8, 1, true, 2) \
+    X(16, 8, 16, 2, false, 1) X(16, 8, 8, 1, true, 2) X(16, 8, 4, 1, true, 4) \
+    X(24, 12, 16, 1, false, 1) X(24, 6, 8, 1, true, 4) \
+    X(32, 16, 16, 1, false, 1) X(32, 8, 8, 1, true, 4) X(32, 8, 4, 1, true, 8)
 
-static FlushShape flush_shape(int v)
+struct FlushShape { int id, nwc, tw, ng, cs; };
+
+static size_t flush_smem_bytes(int kpad, const FlushShape &s)
 {
-    switch (v) {
-#define X(V, NWC, TW, NG, PF) case V: return {NWC, TW, NG};
-        QMC_FLUSH_SHAPES(X)
-#undef X
-    }
-    return {0, 0, 0};
+    const size_t ldc = (size_t)s.nwc * s.tw * 8, ps = kpad + 4;
+    const size_t base = (size_t)kpad * (ldc + 4) * 8 + (size_t)kpad * (ldc + 8) * 4;
+    const size_t part = (size_t)s.ng * s.nwc * 8 * ps * 8, tail = (size_t)kpad * 4 + 16;
+    if (s.cs > 1) return base + part + 2 * 8 * ps * 8 + tail;
+    return base + (base + 2 * part + tail <= kSmemMax ? 2 : 1) * part + tail;
 }
 
-static int kpad_of(int K) { return (K + 7) / 8 * 8; }
+// window ranks the flush kernel is instantiated for
+static int kpad_of(int K) { return K <= 8 ? 8 : (K <= 16 ? 16 : 32); }
 
-static size_t flush_smem_bytes(int kpad, int ld)
+// Shape for ld = 64 v and window rank kpad; id < 0 if none fits.
+static FlushShape flush_shape(int v, int kpad)
 {
-    const FlushShape s = flush_shape(ld / 64);
-    return (size_t)kpad * (ld + 2) * 8 + (size_t)kpad * (ld + 8) * 4 + (size_t)kpad * (kpad + 4) * 8 +
-           (size_t)s.ng * s.nwc * 8 * (kpad + 4) * 8 + (size_t)kpad * 4 + 16;
+    static const struct { int v; FlushShape s; } table[] = {
+#define X(V, NWC, TW, NG, PF, CS) {V, {0, NWC, TW, NG, CS}},
+        QMC_FLUSH_SHAPES(X)
+#undef X
+    };
+    const int n = (int)(sizeof(table) / sizeof(table[0]));
+    static const int forced = getenv("QMC_FLUSH_SHAPE") ? atoi(getenv("QMC_FLUSH_SHAPE")) : -1;   // nth shape of this ld
+    FlushShape fit{-1, 0, 0, 0, 0};
+    int nth = 0;
+    for (int i = 0; i < n; ++i) {
+        if (table[i].v != v) continue;
+        FlushShape s = table[i].s;
+        s.id = i;
+        const size_t b = flush_smem_bytes(kpad, s);
+        if (forced >= 0) {
+            if (nth++ == forced && b <= kSmemMax) return s;
+            continue;
+        }
+        if (b <= kSmemMax) return s;
+    }
+    return fit;
 }
 
 // Largest delay rank whose window fits the flush kernel's shared memory for this ld.
@@ -292,38 +404,47 @@ int delayed_max_rank(int ld)
 {
     int best = 0;
     for (int K = 2; K <= QMC_MAX_DELAY; ++K)
-        if (flush_smem_bytes(kpad_of(K), ld) <= kSmemMax) best = K;
+        if (flush_shape(ld / 64, kpad_of(K)).id >= 0) best = K;
     return best;
 }
 
-template <int KPAD, int NWC, int TW, int NG, bool PF>
+template <int KPAD, int NWC, int TW, int NG, bool PF, int CS>
 static cudaError_t launch_flush_t(const FlushArgs &a, int nw, cudaStream_t s)
 {
-    using L = FlushSmem<KPAD, NWC * TW * 8, NWC, NG>;
+    using L = FlushSmem<KPAD, NWC * TW * 8, NWC, NG, CS>;
     if constexpr (L::bytes > kSmemMax) {
         return cudaErrorInvalidValue;
     } else {
-        auto kern = flush_dmma_kernel<KPAD, NWC, TW, NG, PF>;
+        auto kern = flush_dmma_kernel<KPAD, NWC, TW, NG, PF, CS>;
         static bool configured = false;
         if (!configured) {
             cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L::bytes);
             if (e != cudaSuccess) return e;
             configured = true;
         }
-        dim3 grid((a.nel + a.rows_per_cta - 1) / a.rows_per_cta, nw);
-        kern<<<grid, 32 * NWC * NG, L::bytes, s>>>(a);
-        return cudaGetLastError();
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3(CS * ((a.nel + a.rows_per_cta - 1) / a.rows_per_cta), nw);
+        cfg.blockDim = dim3(32 * NWC * NG);
+        cfg.dynamicSmemBytes = L::bytes;
+        cfg.stream = s;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = CS;
+        attr[0].val.clusterDim.y = 1;
+        attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = CS > 1 ? 1 : 0;
+        return cudaLaunchKernelEx(&cfg, kern, a);
     }
 }
 
-template <int NWC, int TW, int NG, bool PF>
+template <int NWC, int TW, int NG, bool PF, int CS>
 static cudaError_t launch_flush_k(const FlushArgs &a, int nw, cudaStream_t s)
 {
     switch (kpad_of(a.K)) {
-    case 8: return launch_flush_t<8, NWC, TW, NG, PF>(a, nw, s);
-    case 16: return launch_flush_t<16, NWC, TW, NG, PF>(a, nw, s);
-    case 24: return launch_flush_t<24, NWC, TW, NG, PF>(a, nw, s);
-    case 32: return launch_flush_t<32, NWC, TW, NG, PF>(a, nw, s);
+    case 8: return launch_flush_t<8, NWC, TW, NG, PF, CS>(a, nw, s);
+    case 16: return launch_flush_t<16, NWC, TW, NG, PF, CS>(a, nw, s);
+    case 32: return launch_flush_t<32, NWC, TW, NG, PF, CS>(a, nw, s);
     }
     return cudaErrorInvalidValue;
 }
@@ -333,20 +454,30 @@ int delayed_flush(qmc_det *d, cudaStream_t s)
     if (!d->delay || d->host_pending == 0) return QMC_OK;
     FlushArgs a{};
     a.B = d->B; a.nel = d->nel; a.ld = d->ld; a.np = d->np; a.K = d->delay;
-    a.win_count = d->win_count; a.win_iel = d->win_iel; a.win_phi = d->win_phi;
-    a.win_rows = d->win_rows; a.win_sinv = d->win_sinv;
-    const FlushShape sh = flush_shape(d->ld / 64);
+    a.win_count = d->win_count; a.win_iel = d->win_iel; a.win_slot = d->win_slot;
+    a.vec = d->win_vec; a.vec_wstride = d->win_vec_wstride; a.vec_sstride = d->win_vec_sstride;
+    a.win_rows = d->win_rows;
+    const FlushShape sh = flush_shape(d->ld / 64, kpad_of(d->delay));
+    QMC_REQUIRE(sh.id >= 0, "qmc_det_flush: no kernel shape for ld=%d, rank %d", d->ld, d->delay);
     // rows per CTA: the window is staged once per CTA, so prefer long CTAs when the grid stays large
+    static const int rows_env = getenv("QMC_FLUSH_ROWS") ? atoi(getenv("QMC_FLUSH_ROWS")) : 0;
     a.rows_per_cta = ((long long)d->nw * d->nel >= 128LL * 148 * 8) ? 128 : 64;
+    if (rows_env) a.rows_per_cta = rows_env;
     if (a.rows_per_cta % (8 * sh.ng)) a.rows_per_cta = 8 * sh.ng * ((a.rows_per_cta + 8 * sh.ng - 1) / (8 * sh.ng));
-    cudaError_t e;
-    prof_start(d, kProfDelayedFlush, s);
-    switch (d->ld / 64) {
-#define X(V, NWC, TW, NG, PF) case V: e = launch_flush_k<NWC, TW, NG, PF>(a, d->nw, s); break;
-        QMC_FLUSH_SHAPES(X)
-#undef X
-    default: e = cudaErrorInvalidValue;
+    cudaError_t e = cudaErrorInvalidValue;
+    if (d->win_rows_raw) {
+        if (a.K <= 8) rprime_kernel<8><<<d->nw, 256, 0, s>>>(d->ld, a.K, d->win_count, d->win_sinv, d->win_rows);
+        else if (a.K <= 16) rprime_kernel<16><<<d->nw, 256, 0, s>>>(d->ld, a.K, d->win_count, d->win_sinv, d->win_rows);
+        else rprime_kernel<32><<<d->nw, 256, 0, s>>>(d->ld, a.K, d->win_count, d->win_sinv, d->win_rows);
+        QMC_LAUNCHED();
+        d->win_rows_raw = 0;
     }
+    prof_start(d, kProfDelayedFlush, s);
+    int id = 0;
+#define X(V, NWC, TW, NG, PF, CS) \
+    if (sh.id == id++) e = launch_flush_k<NWC, TW, NG, PF, CS>(a, d->nw, s);
+    QMC_FLUSH_SHAPES(X)
+#undef X
     prof_stop(d, s);
     count_launch();
     QMC_CUDA(e);

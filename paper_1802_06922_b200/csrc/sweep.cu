@@ -3,7 +3,8 @@
 //   K1 spo_batch_kernel      S0 proposal, S1 stencil, S2 SPO-VGL gather -- once per batch of steps
 //   K2 ratio_rowcopy_kernel  S3 ratio, copy of row k                    -- per electron step
 //   K3 sm_update_kernel      S4 Metropolis test, S5 rank-1 update       -- per electron step
-// (delayed mode: K2/K3 are delayed_step_kernel per step and flush_dmma_kernel per window)
+// (delayed mode, per window of K steps: K1, then delayed_window_kernel = S3 + S4 of the K steps,
+//  then flush_dmma_kernel = S5')
 #include "delayed_device.cuh"
 #include "spo_device.cuh"
 #include "update_device.cuh"
@@ -129,15 +130,18 @@ static int sweep_impl(qmc_det *d, const qmc_spline *sp, double *pos, const doubl
                                        rec ? rec + mv / nw * (size_t)nrec * nel : nullptr, nrec, s);
                 if (rc) return rc;
             }
-            const float *phi = d->vgl + slot * slot_stride;
-            if (d->delay) {           // K2: ratio against the window, decision, append (flushes every K steps)
-                int rc = delayed_sweep_step(d, pos, delta + 3 * mv, unif + mv, k, phi,
-                                            ratios_out ? ratios_out + mv : nullptr,
-                                            accept_out ? accept_out + mv : nullptr,
-                                            forced ? forced + mv : nullptr, s);
-                if (rc) return rc;
+            if (d->delay) {           // the whole window: ratios, decisions, moves; then the flush
+                if (slot == 0) {
+                    const int nb = min(batch, k0 + kn - k);
+                    int rc = delayed_sweep_window(d, pos, delta + 3 * mv, unif + mv, k, nb,
+                                                  ratios_out ? ratios_out + mv : nullptr,
+                                                  accept_out ? accept_out + mv : nullptr,
+                                                  forced ? forced + mv : nullptr, s);
+                    if (rc) return rc;
+                }
                 continue;
             }
+            const float *phi = d->vgl + slot * slot_stride;
             // K2: ratio + row copy, K3: decision + rank-1 update
             prof_start(d, kProfRatio, s);
             ratio_rowcopy_kernel<<<nw, 256, 0, s>>>(d->B, nel, d->ld, k, phi, (size_t)5 * d->np, d->rowk, d->rpart);
@@ -157,10 +161,6 @@ static int sweep_impl(qmc_det *d, const qmc_spline *sp, double *pos, const doubl
             cudaError_t ue = launch_sm_update<true>(u, nw, s);
             prof_stop(d, s);
             QMC_CUDA(ue);
-        }
-        if (d->delay) {
-            int rc = delayed_flush_reset_host(d, s);
-            if (rc) return rc;
         }
     }
     return QMC_OK;

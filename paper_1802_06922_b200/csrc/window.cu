@@ -1,0 +1,215 @@
+// One WINDOW of the delayed (rank-k) update inside qmc_sweep: the K consecutive electron steps
+// k0 .. k0+nb-1 of the lockstep sweep in ONE launch (DESIGN.md R:O7, R:A14).
+//
+// Every quantity the nb sequential ratios and decisions need is an entry of one small matrix:
+// the proposals of the window are known up front (r' = pos[w][k] + delta does not depend on the
+// outcome of earlier moves of OTHER electrons, and their orbital vectors v_i come from the batched
+// SPO-VGL launch), and every row of B0 the window touches is one of B0[k0 .. k0+nb-1].  With
+//
+//     G[i][j] = v_i . B0[k0+j]                 (nb x nb, one (nb x N)(N x nb) fp64 contraction)
+//
+// the ratio of step i against the accepted steps l_0 < l_1 < ... < l_{p-1} < i is
+//
+//     d = G[i][i],   x_m = G[i][l_m],   c_m = G[l_m][i],   R = d - x^T S^-1 c,   S[a][b] = G[l_a][l_b]
+//
+// so the steps are O(p^2) scalar work on S^-1 (grown by bordering), done by one warp with no
+// further pass over B0 or the vectors.  The kernel then leaves what the flush kernel consumes:
+// count, electron indices, slots (= step index in the window, where the flush finds v_l) and
+// R' = S^-T Rows (Rows[l] = B0[k_l]; the flush overwrites B in place and computes B -= Q R').
+#include "delayed_device.cuh"
+#include "dmma.cuh"
+#include "update_device.cuh"
+
+namespace qmc {
+
+constexpr int kWinThreads = 256;
+
+struct WindowArgs {
+    const double *B;              // [nw][nel][ld]  B0 of the window
+    int nw, nel, ld, np, K;
+    int iel0, nb;                 // electrons iel0 .. iel0+nb-1, nb <= K
+    const float *vgl;             // [nb][nw][5][np] SPO-VGL of the window's proposals (values first)
+    const double *unif;           // [nb][nw]
+    const unsigned char *forced;  // [nb][nw] or NULL
+    double *ratios_out;           // [nb][nw] or NULL
+    unsigned char *accept_out;    // [nb][nw] or NULL
+    double *pos;                  // [nw][nel][3]
+    const double *delta;          // [nb][nw][3]
+    double *logdet;
+    int *sign;
+    long long *naccept;
+    int *win_count;               // [nw]
+    int *win_iel;                 // [nw][K]
+    int *win_slot;                // [nw][K]
+    double *win_rows;             // [nw][K][ld]   row l <- R'[l]
+};
+
+// One block per walker, 8 warps.  Phase 1: warp q contracts the 16-column chunks q, q+8, ... with
+// DMMA.8x8x4 (the contraction index inside a chunk is permuted so that one lane's float4 / 2 x
+// double2 serve four k-steps).  Phase 2: fixed-order sum of the 8 partial G.  Phase 3: warp 0
+// walks the nb steps.  Phase 4: R' = S^-T Rows, 8-column tiles over the warps.
+template <int KMAX>
+__global__ void __launch_bounds__(kWinThreads) delayed_window_kernel(WindowArgs a)
+{
+    constexpr int MB = KMAX / 8;
+    constexpr int GS = KMAX + 1;
+    __shared__ double G_s[KMAX * GS];
+    __shared__ double sinv_s[KMAX * GS];
+    __shared__ long long rowoff_s[KMAX];
+    __shared__ int p_s;
+    const int w = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int g = lane >> 2, t = lane & 3;
+    const int nb = a.nb, ld = a.ld, np = a.np, K = a.K;
+    const size_t vstep = (size_t)a.nw * 5 * np;             // stride between steps in vgl
+    const float *v0 = a.vgl + (size_t)w * 5 * np;
+    const double *b0 = a.B + ((size_t)w * a.nel + a.iel0) * ld;
+
+    double acc[MB][MB][2];
+#pragma unroll
+    for (int i = 0; i < MB; ++i)
+#pragma unroll
+        for (int j = 0; j < MB; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+    for (int c0 = 16 * warp; c0 < np; c0 += 16 * (kWinThreads / 32)) {
+        const int col = c0 + 4 * t;
+        double av[MB][4], bv[MB][4];
+#pragma unroll
+        for (int jb = 0; jb < MB; ++jb) {
+            const int j = 8 * jb + g;
+            double2 lo = make_double2(0.0, 0.0), hi = lo;
+            if (j < nb) {
+                lo = *reinterpret_cast<const double2 *>(b0 + (size_t)j * ld + col);
+                hi = *reinterpret_cast<const double2 *>(b0 + (size_t)j * ld + col + 2);
+            }
+            bv[jb][0] = lo.x; bv[jb][1] = lo.y; bv[jb][2] = hi.x; bv[jb][3] = hi.y;
+        }
+#pragma unroll
+        for (int ib = 0; ib < MB; ++ib) {
+            const int i = 8 * ib + g;
+            float4 f = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (i < nb) f = *reinterpret_cast<const float4 *>(v0 + (size_t)i * vstep + col);
+            av[ib][0] = f.x; av[ib][1] = f.y; av[ib][2] = f.z; av[ib][3] = f.w;
+        }
+#pragma unroll
+        for (int s = 0; s < 4; ++s)
+#pragma unroll
+            for (int ib = 0; ib < MB; ++ib)
+#pragma unroll
+                for (int jb = 0; jb < MB; ++jb)
+                    if (8 * ib < nb && 8 * jb < nb) dmma884(acc[ib][jb][0], acc[ib][jb][1], av[ib][s], bv[jb][s]);
+    }
+    // ---- phase 2: G = sum over warps, fixed order
+    for (int q = 0; q < kWinThreads / 32; ++q) {
+        if (warp == q) {
+#pragma unroll
+            for (int ib = 0; ib < MB; ++ib)
+#pragma unroll
+                for (int jb = 0; jb < MB; ++jb) {
+                    double *dst = G_s + (8 * ib + g) * GS + 8 * jb + 2 * t;
+                    if (q == 0) { dst[0] = acc[ib][jb][0]; dst[1] = acc[ib][jb][1]; }
+                    else { dst[0] += acc[ib][jb][0]; dst[1] += acc[ib][jb][1]; }
+                }
+        }
+        __syncthreads();
+    }
+    // ---- phase 3: the nb steps in sequence; lane m owns accepted move m (its step index `mine`)
+    if (warp == 0) {
+    int p = 0, mine = 0;
+    double logdet_add = 0.0;
+    int flips = 0;
+    for (int i = 0; i < nb; ++i) {
+        const double c = lane < p ? G_s[mine * GS + i] : 0.0;     // c_m = v_{l_m} . B0[k_i]
+        const double x = lane < p ? G_s[i * GS + mine] : 0.0;     // x_m = v_i . B0[k_{l_m}]
+        double y = 0.0, z = 0.0;                                  // y = S^-1 c, z = S^-T x
+        for (int q = 0; q < p; ++q) {
+            const double cq = __shfl_sync(0xffffffffu, c, q), xq = __shfl_sync(0xffffffffu, x, q);
+            if (lane < p) {
+                y = fma(sinv_s[lane * GS + q], cq, y);
+                z = fma(sinv_s[q * GS + lane], xq, z);
+            }
+        }
+        const double R = G_s[i * GS + i] - warp_sum(x * y);
+        const size_t mv = (size_t)i * a.nw + w;
+        const bool acc_w = a.forced ? (a.forced[mv] != 0) : metropolis(R, a.unif[mv]);
+        if (lane == 0) {
+            if (a.ratios_out) a.ratios_out[mv] = R;
+            if (a.accept_out) a.accept_out[mv] = acc_w ? 1 : 0;
+        }
+        if (!acc_w) continue;
+        const double rinv = 1.0 / R;
+        __syncwarp();             // every lane has read the old S^-1
+        if (lane == 0) {
+            logdet_add += log(fabs(R));
+            if (R < 0.0) flips ^= 1;
+            double *r = a.pos + ((size_t)w * a.nel + a.iel0 + i) * 3;
+            r[0] += a.delta[3 * mv + 0];
+            r[1] += a.delta[3 * mv + 1];
+            r[2] += a.delta[3 * mv + 2];
+        }
+        // bordered inverse: S'^-1 = [[S^-1 + y z^T / R, -y / R], [-z^T / R, 1 / R]]
+        for (int q = 0; q < p; ++q) {
+            const double zq = __shfl_sync(0xffffffffu, z, q);
+            if (lane < p) sinv_s[lane * GS + q] += y * zq * rinv;
+        }
+        if (lane < p) {
+            sinv_s[lane * GS + p] = -y * rinv;
+            sinv_s[p * GS + lane] = -z * rinv;
+        }
+        if (lane == p) { sinv_s[p * GS + p] = rinv; mine = i; }
+        ++p;
+        __syncwarp();
+    }
+    if (lane == 0) {
+        a.win_count[w] = p;
+        p_s = p;
+        if (p) {
+            a.logdet[w] += logdet_add;
+            if (flips) a.sign[w] = -a.sign[w];
+            a.naccept[w] += p;
+        }
+    }
+    if (lane < p) {
+        a.win_iel[(size_t)w * K + lane] = a.iel0 + mine;
+        a.win_slot[(size_t)w * K + lane] = mine;
+        rowoff_s[lane] = (long long)mine * ld;
+    }
+    }
+    __syncthreads();
+
+    // ---- phase 4: R'[l] = sum_l' S^-1[l'][l] B0[k_l'] for the flush (pad columns of B are zero)
+    const int p = p_s;
+    if (p) rprime_warp<KMAX>(sinv_s, GS, p, b0, rowoff_s, a.win_rows + (size_t)w * K * ld, ld, warp, kWinThreads / 32, lane);
+}
+
+int delayed_sweep_window(qmc_det *d, double *pos, const double *delta, const double *unif, int iel0, int nb,
+                         double *ratios_out, unsigned char *accept_out, const unsigned char *forced, cudaStream_t s)
+{
+    if (d->host_pending) {        // rows pending from standalone qmc_det_accept_update calls
+        int rc = delayed_flush_reset_host(d, s);
+        if (rc) return rc;
+    }
+    WindowArgs a{};
+    a.B = d->B; a.nw = d->nw; a.nel = d->nel; a.ld = d->ld; a.np = d->np; a.K = d->delay;
+    a.iel0 = iel0; a.nb = nb;
+    a.vgl = d->vgl;
+    a.unif = unif; a.forced = forced; a.ratios_out = ratios_out; a.accept_out = accept_out;
+    a.pos = pos; a.delta = delta;
+    a.logdet = d->logdet; a.sign = d->sign; a.naccept = d->naccept;
+    a.win_count = d->win_count; a.win_iel = d->win_iel; a.win_slot = d->win_slot;
+    a.win_rows = d->win_rows;
+    prof_start(d, kProfDelayedRatio, s);
+    if (a.K <= 8) delayed_window_kernel<8><<<d->nw, kWinThreads, 0, s>>>(a);
+    else if (a.K <= 16) delayed_window_kernel<16><<<d->nw, kWinThreads, 0, s>>>(a);
+    else delayed_window_kernel<32><<<d->nw, kWinThreads, 0, s>>>(a);
+    prof_stop(d, s);
+    QMC_LAUNCHED();
+    // the flush takes the vectors of the accepted steps straight from the SPO-VGL scratch
+    d->host_pending = nb;
+    d->win_rows_raw = 0;
+    d->win_vec = d->vgl;
+    d->win_vec_wstride = (size_t)5 * d->np;
+    d->win_vec_sstride = (size_t)d->nw * 5 * d->np;
+    return delayed_flush_reset_host(d, s);
+}
+
+}  // namespace qmc
