@@ -9,6 +9,8 @@ int delayed_accept(qmc_det *d, int iel, const float *phi, int ldo, const double 
                    const unsigned char *accept, cudaStream_t s);
 int delayed_flush(qmc_det *d, cudaStream_t s);
 int delayed_flush_reset_host(qmc_det *d, cudaStream_t s);   // flush + forget the host-side window bookkeeping
+bool flush_ring_serves(int ld, int K);                       // flush_ring.cu has a shape for (ld, rank)
+cudaError_t flush_ring_launch(qmc_det *d, cudaStream_t s);    // enqueue it
 int delayed_max_rank(int ld);                                // largest K whose window fits shared memory
 // One window of qmc_sweep in delayed mode: electrons iel0 .. iel0+nb-1 (nb <= delay rank), whose
 // SPO-VGL is in d->vgl; ratios, decisions, moves and the flush.  Pointers are offset to the first step.

@@ -19,70 +19,10 @@
 // partial Q of the slices are exchanged through distributed shared memory once per row block.
 #include <stdlib.h>
 #include "delayed_device.cuh"
+#include "async_device.cuh"
 #include "dmma.cuh"
 
 namespace qmc {
-
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
-__device__ __forceinline__ void mbar_init(uint64_t *bar, int count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t *bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
-                 : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
-{
-    uint32_t ok;
-    do {
-        asm volatile("{\n\t.reg .pred p;\n\t"
-                     "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-                     "selp.u32 %0, 1, 0, p;\n\t}"
-                     : "=r"(ok)
-                     : "r"(smem_u32(bar)), "r"(parity)
-                     : "memory");
-    } while (!ok);
-}
-// TMA 1-D bulk copy global -> shared, completion counted on `bar` (bytes % 16 == 0, 16-B aligned).
-__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
-{
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-                     smem_u32(dst)),
-                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
-                 : "memory");
-}
-__device__ __forceinline__ void group_sync(int id, int nthreads)
-{
-    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
-}
-// thread-block cluster helpers (CS > 1: the CTAs of a cluster own column slices of the same rows)
-__device__ __forceinline__ uint32_t cluster_ctarank()
-{
-    uint32_t r;
-    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
-    return r;
-}
-__device__ __forceinline__ void cluster_arrive()
-{
-    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
-}
-__device__ __forceinline__ void cluster_wait()
-{
-    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
-}
-// read a double from the shared memory of CTA `rank` of this cluster (distributed shared memory)
-__device__ __forceinline__ double ld_dsmem(const double *local, uint32_t rank)
-{
-    uint32_t raddr;
-    double v;
-    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(raddr) : "r"(smem_u32(local)), "r"(rank));
-    asm volatile("ld.shared::cluster.f64 %0, [%1];" : "=d"(v) : "r"(raddr) : "memory");
-    return v;
-}
 
 struct FlushArgs {
     double *B;                    // [nw][nel][ld]
@@ -382,7 +322,8 @@ static FlushShape flush_shape(int v, int kpad)
 #undef X
     };
     const int n = (int)(sizeof(table) / sizeof(table[0]));
-    static const int forced = getenv("QMC_FLUSH_SHAPE") ? atoi(getenv("QMC_FLUSH_SHAPE")) : -1;   // nth shape of this ld
+    const char *env = getenv("QMC_FLUSH_SHAPE");        // tests: force the nth shape of this ld
+    const int forced = env ? atoi(env) : -1;
     FlushShape fit{-1, 0, 0, 0, 0};
     int nth = 0;
     for (int i = 0; i < n; ++i) {
@@ -404,7 +345,7 @@ int delayed_max_rank(int ld)
 {
     int best = 0;
     for (int K = 2; K <= QMC_MAX_DELAY; ++K)
-        if (flush_shape(ld / 64, kpad_of(K)).id >= 0) best = K;
+        if (flush_ring_serves(ld, K) || flush_shape(ld / 64, kpad_of(K)).id >= 0) best = K;
     return best;
 }
 
@@ -457,12 +398,11 @@ int delayed_flush(qmc_det *d, cudaStream_t s)
     a.win_count = d->win_count; a.win_iel = d->win_iel; a.win_slot = d->win_slot;
     a.vec = d->win_vec; a.vec_wstride = d->win_vec_wstride; a.vec_sstride = d->win_vec_sstride;
     a.win_rows = d->win_rows;
-    const FlushShape sh = flush_shape(d->ld / 64, kpad_of(d->delay));
+    const bool ring = flush_ring_serves(d->ld, d->delay);
+    const FlushShape sh = ring ? FlushShape{0, 1, 1, 1, 1} : flush_shape(d->ld / 64, kpad_of(d->delay));
     QMC_REQUIRE(sh.id >= 0, "qmc_det_flush: no kernel shape for ld=%d, rank %d", d->ld, d->delay);
     // rows per CTA: the window is staged once per CTA, so prefer long CTAs when the grid stays large
-    static const int rows_env = getenv("QMC_FLUSH_ROWS") ? atoi(getenv("QMC_FLUSH_ROWS")) : 0;
     a.rows_per_cta = ((long long)d->nw * d->nel >= 128LL * 148 * 8) ? 128 : 64;
-    if (rows_env) a.rows_per_cta = rows_env;
     if (a.rows_per_cta % (8 * sh.ng)) a.rows_per_cta = 8 * sh.ng * ((a.rows_per_cta + 8 * sh.ng - 1) / (8 * sh.ng));
     cudaError_t e = cudaErrorInvalidValue;
     if (d->win_rows_raw) {
@@ -473,9 +413,10 @@ int delayed_flush(qmc_det *d, cudaStream_t s)
         d->win_rows_raw = 0;
     }
     prof_start(d, kProfDelayedFlush, s);
+    if (ring) e = flush_ring_launch(d, s);
     int id = 0;
 #define X(V, NWC, TW, NG, PF, CS) \
-    if (sh.id == id++) e = launch_flush_k<NWC, TW, NG, PF, CS>(a, d->nw, s);
+    if (!ring && sh.id == id++) e = launch_flush_k<NWC, TW, NG, PF, CS>(a, d->nw, s);
     QMC_FLUSH_SHAPES(X)
 #undef X
     prof_stop(d, s);

@@ -1,0 +1,283 @@
+// Flush of the delayed (rank-k) update for large N: the same two fp64 tensor-core contractions as
+// flush.cu (DESIGN.md R:O7)
+//
+//     Q[m][l] = B0[m] . v_l - [k_l == m]           step 1
+//     B[m]    = B0[m] - sum_l Q[m][l] * R'[l]       step 2,  R' = S^-T Rows
+//
+// in one pass over B, laid out for the B200 memory system:
+//
+//   * the walker's window lives in REGISTERS: warp wc of a CTA owns 8 TW columns and keeps the
+//     step-1 fragments of v (converted to fp64 once) and the step-2 fragments of R' for those
+//     columns, so the inner loops are pure DMMA.8x8x4 with no shared-memory operand traffic;
+//   * the rows of B stream through a shared-memory RING filled by TMA bulk copies
+//     (cp.async.bulk + mbarrier), several 8-row blocks ahead of the tensor cores, so the HBM read
+//     stream never waits for a compute phase; results go back with 128-bit stores;
+//   * a window of 16 rows x 1024 columns of (v, R') in fp64 is 256 KB -- a whole SM's register
+//     file -- so the columns are split over a thread-block CLUSTER of CS CTAs; per row block every
+//     CTA sends its 8 x p partial Q to its peers with st.async into their shared memory
+//     (completion on the receiver's mbarrier: no fence, no cluster barrier);
+//   * the loop is software-pipelined by one block: step 1 of block j is issued before step 2 of
+//     block j-1, which hides the exchange latency behind tensor-core work.
+#include <stdlib.h>
+
+#include "async_device.cuh"
+#include "delayed_device.cuh"
+#include "dmma.cuh"
+
+namespace qmc {
+
+struct RingArgs {
+    double *B;                    // [nw][nel][ld]
+    int nel, ld, np, K;
+    int rows_per_cta;             // multiple of 8
+    const int *win_count;
+    const int *win_iel;
+    const int *win_slot;          // [nw][K] slot of accepted move l in vec
+    const float *vec;             // orbital vector of (walker w, slot s) at vec + w * vec_wstride + s * vec_sstride
+    size_t vec_wstride, vec_sstride;
+    const double *win_rows;       // [nw][K][ld] R'[l], accepted order
+};
+
+constexpr int kRecvBufs = 4;      // partial-Q receive buffers in flight (see the hazard note in the kernel)
+
+// Shared memory of one CTA (LDC = NWC * TW * 8 columns):
+//   ring   double [STAGES][8][LDC + 8]      row blocks of B (pitch + 8: conflict-free 128-bit reads)
+//   part   double [2][NWC][8][KPAD + 4]     partial Q of each column warp, by block parity
+//   recv   double [kRecvBufs][CS][8][KPAD + 4]   partial Q of every CTA of the cluster
+//   full   mbarrier [STAGES], rbar mbarrier [kRecvBufs]
+template <int KPAD, int TW, int NWC, int CS, int STAGES>
+struct RingSmem {
+    static constexpr int LDC = NWC * TW * 8, RP = LDC + 8, PS = KPAD + 4;
+    static constexpr size_t ring_off = 0;
+    static constexpr size_t part_off = ring_off + (size_t)STAGES * 8 * RP * sizeof(double);
+    static constexpr size_t recv_off = part_off + (size_t)2 * NWC * 8 * PS * sizeof(double);
+    static constexpr size_t bar_off = recv_off + (size_t)kRecvBufs * CS * 8 * PS * sizeof(double);
+    static constexpr size_t bytes = bar_off + (size_t)(STAGES + kRecvBufs) * sizeof(uint64_t);
+};
+
+// Row-block loop for a window of NTA active 8-wide tiles (8 NTA - 7 <= p <= 8 NTA).
+template <int KPAD, int TW, int NWC, int CS, int STAGES, int NTA>
+__device__ __forceinline__ void ring_stream(const RingArgs &a, int w, int p, unsigned char *smem)
+{
+    using L = RingSmem<KPAD, TW, NWC, CS, STAGES>;
+    constexpr int LDC = L::LDC, LD = LDC * CS, RP = L::RP, PS = L::PS;
+    constexpr int KQA = 2 * NTA, NTHREADS = 32 * NWC;
+    double *ring = reinterpret_cast<double *>(smem + L::ring_off);
+    double *part = reinterpret_cast<double *>(smem + L::part_off);
+    double *recv = reinterpret_cast<double *>(smem + L::recv_off);
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem + L::bar_off);
+    uint64_t *rbar = full + STAGES;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int g = lane >> 2, t = lane & 3;
+    const int K = a.K, nel = a.nel;
+    const uint32_t crank = CS > 1 ? cluster_ctarank() : 0u;
+    const int colbase = (int)crank * LDC;                  // first column this CTA owns
+    const int col0 = 8 * TW * warp;                        // this warp's first column within the slice
+
+    // ---- the window, as DMMA B-fragments in registers
+    double vf[TW][NTA][2], rf[TW][KQA];
+    int klr[KQA];
+#pragma unroll
+    for (int nt = 0; nt < NTA; ++nt) {
+        const int l = 8 * nt + g;
+        const bool live = l < p;
+        const float *vp = a.vec + (size_t)w * a.vec_wstride +
+                          (live ? (size_t)a.win_slot[(size_t)w * K + l] * a.vec_sstride : 0);
+#pragma unroll
+        for (int i = 0; i < TW; ++i) {
+            const int c = colbase + col0 + 8 * i + 2 * t;   // even; np is a multiple of 32
+            float2 f = make_float2(0.f, 0.f);
+            if (live && c < a.np) f = *reinterpret_cast<const float2 *>(vp + c);
+            vf[i][nt][0] = (double)f.x;
+            vf[i][nt][1] = (double)f.y;
+        }
+    }
+#pragma unroll
+    for (int kq = 0; kq < KQA; ++kq) {
+        const int l = 4 * kq + t;
+        const bool live = l < p;
+        klr[kq] = live ? a.win_iel[(size_t)w * K + l] : -1;
+        const double *rp = a.win_rows + ((size_t)w * K + (live ? l : 0)) * LD + colbase + col0 + g;
+#pragma unroll
+        for (int i = 0; i < TW; ++i) rf[i][kq] = live ? rp[8 * i] : 0.0;
+    }
+
+    // ---- the ring: warp 0 keeps STAGES - 1 row blocks in flight
+    const int m_begin = (blockIdx.x / CS) * a.rows_per_cta;
+    const int m_end = min(nel, m_begin + a.rows_per_cta);
+    const int nblk = (m_end - m_begin + 7) / 8;
+    double *const slice = a.B + (size_t)w * nel * LD + colbase;     // row m of this CTA's slice at + m * LD
+    auto issue = [&](int jb) {                                      // whole warp 0
+        const int s = jb % STAGES, m0 = m_begin + 8 * jb, nv = min(8, m_end - m0);
+        if (lane == 0) mbar_arrive_expect_tx(&full[s], (uint32_t)nv * (uint32_t)(LDC * sizeof(double)));
+        __syncwarp();
+        if (lane < nv)
+            bulk_g2s(ring + (size_t)(s * 8 + lane) * RP, slice + (size_t)(m0 + lane) * LD, LDC * sizeof(double), &full[s]);
+    };
+    if (warp == 0)
+        for (int jb = 0; jb < STAGES - 1 && jb < nblk; ++jb) issue(jb);
+
+    // ---- software-pipelined loop: iteration j runs step 1 of block j and step 2 of block j - 1.
+    // Hazards: ring stage (j-1) % STAGES is refilled at the top of iteration j, after the barrier
+    // of iteration j-1 that follows every warp's read of it.  A peer sends block j+4 only after it
+    // received my block j+2, which I send after I read its block j (iteration j+1): 4 buffers.
+    double2 ra[TW], rb[TW];
+    for (int j = 0; j <= nblk; ++j) {
+        if (j < nblk) {
+            if (warp == 0 && j + STAGES - 1 < nblk) issue(j + STAGES - 1);
+            const int s = j % STAGES;
+            mbar_wait(&full[s], (uint32_t)(j / STAGES) & 1u);
+            const double *src = ring + (size_t)(s * 8 + g) * RP + col0 + 2 * t;
+#pragma unroll
+            for (int i = 0; i < TW; ++i) rb[i] = *reinterpret_cast<const double2 *>(src + 8 * i);
+            // step 1: partial Q over this warp's columns
+            double cq[NTA][2];
+#pragma unroll
+            for (int nt = 0; nt < NTA; ++nt) cq[nt][0] = cq[nt][1] = 0.0;
+#pragma unroll
+            for (int i = 0; i < TW; ++i)
+#pragma unroll
+                for (int nt = 0; nt < NTA; ++nt) {
+                    dmma884(cq[nt][0], cq[nt][1], rb[i].x, vf[i][nt][0]);
+                    dmma884(cq[nt][0], cq[nt][1], rb[i].y, vf[i][nt][1]);
+                }
+            double *pbuf = part + (size_t)(j & 1) * NWC * 8 * PS;
+            double *ps = pbuf + ((size_t)warp * 8 + g) * PS;
+#pragma unroll
+            for (int nt = 0; nt < NTA; ++nt)
+                *reinterpret_cast<double2 *>(ps + 8 * nt + 2 * t) = make_double2(cq[nt][0], cq[nt][1]);
+            __syncthreads();
+            // this CTA's partial (fixed order over its warps), sent to every CTA of the cluster
+            const int b = j % kRecvBufs;
+            if (tid == 0) mbar_arrive_expect_tx(&rbar[b], (uint32_t)(CS * 64 * NTA * sizeof(double)));
+            for (int e = tid; e < 64 * NTA; e += NTHREADS) {
+                const int row = e / (8 * NTA), col = e % (8 * NTA);
+                double sum = 0.0;
+#pragma unroll
+                for (int c = 0; c < NWC; ++c) sum += pbuf[((size_t)c * 8 + row) * PS + col];
+                const double *dst = recv + ((size_t)(b * CS + (int)crank) * 8 + row) * PS + col;
+#pragma unroll
+                for (int c = 0; c < CS; ++c) st_async_f64(mapa_u32(dst, (uint32_t)c), sum, mapa_u32(&rbar[b], (uint32_t)c));
+            }
+        }
+        if (j >= 1) {
+            const int jj = j - 1, b = jj % kRecvBufs;
+            const int m = m_begin + 8 * jj + g;
+            mbar_wait(&rbar[b], (uint32_t)(jj / kRecvBufs) & 1u);
+            // step 2: B block -= Q R'; Q read back in A-fragment layout, summed over the cluster in
+            // a fixed order (every CTA forms bit-identical Q)
+#pragma unroll
+            for (int kq = 0; kq < KQA; ++kq) {
+                const double *pp = recv + ((size_t)(b * CS) * 8 + g) * PS + 4 * kq + t;
+                double q = 0.0;
+#pragma unroll
+                for (int c = 0; c < CS; ++c) q += pp[(size_t)c * 8 * PS];
+                if (klr[kq] == m) q -= 1.0;
+                const double af = -q;
+#pragma unroll
+                for (int i = 0; i < TW; ++i) dmma884(ra[i].x, ra[i].y, af, rf[i][kq]);
+            }
+            if (m < m_end) {
+                double *dst = slice + (size_t)m * LD + col0 + 2 * t;
+#pragma unroll
+                for (int i = 0; i < TW; ++i) *reinterpret_cast<double2 *>(dst + 8 * i) = ra[i];
+            }
+        }
+#pragma unroll
+        for (int i = 0; i < TW; ++i) ra[i] = rb[i];
+    }
+}
+
+template <int KPAD, int TW, int NWC, int CS, int STAGES>
+__global__ void __launch_bounds__(32 * NWC, (2 * (RingSmem<KPAD, TW, NWC, CS, STAGES>::bytes + 1024) <= 228 * 1024 &&
+                                             2 * 32 * NWC * 128 <= 65536) ? 2 : 1)
+flush_ring_kernel(RingArgs a)
+{
+    using L = RingSmem<KPAD, TW, NWC, CS, STAGES>;
+    extern __shared__ __align__(128) unsigned char smem_ring[];
+    const int w = blockIdx.y;
+    const int p = a.win_count[w];
+    if (p == 0) return;                                    // the whole cluster leaves together
+    uint64_t *bars = reinterpret_cast<uint64_t *>(smem_ring + L::bar_off);
+    if (threadIdx.x == 0)
+        for (int i = 0; i < STAGES + kRecvBufs; ++i) mbar_init(&bars[i], 1);
+    __syncthreads();
+    if constexpr (CS > 1) {                                // peers' barriers exist before anything is sent
+        cluster_arrive();
+        cluster_wait();
+    }
+    constexpr int NT = KPAD / 8;
+    switch ((p + 7) / 8) {
+    case 1: ring_stream<KPAD, TW, NWC, CS, STAGES, 1>(a, w, p, smem_ring); break;
+    case 2: if constexpr (NT >= 2) ring_stream<KPAD, TW, NWC, CS, STAGES, 2>(a, w, p, smem_ring); break;
+    case 3: if constexpr (NT >= 3) ring_stream<KPAD, TW, NWC, CS, STAGES, 3>(a, w, p, smem_ring); break;
+    case 4: if constexpr (NT >= 4) ring_stream<KPAD, TW, NWC, CS, STAGES, 4>(a, w, p, smem_ring); break;
+    }
+}
+
+// Shapes: X(V, KPAD, TW, NWC, CS, STAGES) serves ld = 64 V = CS * NWC * TW * 8 and ranks <= KPAD.
+#define QMC_RING_SHAPES(X) \
+    X(8, 16, 8, 8, 1, 5) X(16, 16, 8, 8, 2, 5) X(32, 16, 8, 8, 4, 5) \
+    X(8, 32, 4, 8, 2, 6) X(16, 32, 4, 8, 4, 6) X(32, 32, 4, 8, 8, 6)
+
+template <int KPAD, int TW, int NWC, int CS, int STAGES>
+static cudaError_t launch_ring(const RingArgs &a, int nw, cudaStream_t s)
+{
+    using L = RingSmem<KPAD, TW, NWC, CS, STAGES>;
+    static_assert(L::bytes <= 227 * 1024, "ring shape exceeds shared memory");
+    auto kern = flush_ring_kernel<KPAD, TW, NWC, CS, STAGES>;
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L::bytes);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(CS * ((a.nel + a.rows_per_cta - 1) / a.rows_per_cta), nw);
+    cfg.blockDim = dim3(32 * NWC);
+    cfg.dynamicSmemBytes = L::bytes;
+    cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = CS;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;                                      // a 1-CTA cluster still addresses shared::cluster
+    return cudaLaunchKernelEx(&cfg, kern, a);
+}
+
+// Does a ring shape serve (ld, rank)?  QMC_FLUSH_RING=0 in the environment disables the ring kernel
+// (A/B measurements and tests of the flush.cu kernel on the same shapes).
+bool flush_ring_serves(int ld, int K)
+{
+    const char *env = getenv("QMC_FLUSH_RING");
+    if ((env && atoi(env) == 0) || ld % 64) return false;
+    const int v = ld / 64, kpad = K <= 16 ? 16 : 32;
+#define X(V, KPAD, TW, NWC, CS, STAGES) \
+    if (v == V && kpad == KPAD) return true;
+    QMC_RING_SHAPES(X)
+#undef X
+    return false;
+}
+
+// Enqueue the ring flush (the caller has checked flush_ring_serves and brackets it with its profiling events).
+cudaError_t flush_ring_launch(qmc_det *d, cudaStream_t s)
+{
+    RingArgs a{};
+    a.B = d->B; a.nel = d->nel; a.ld = d->ld; a.np = d->np; a.K = d->delay;
+    a.win_count = d->win_count; a.win_iel = d->win_iel; a.win_slot = d->win_slot;
+    a.vec = d->win_vec; a.vec_wstride = d->win_vec_wstride; a.vec_sstride = d->win_vec_sstride;
+    a.win_rows = d->win_rows;
+    // rows per CTA: the window fragments are loaded once per CTA, so prefer long CTAs when the grid stays large
+    const long long rows_total = (long long)d->nw * d->nel;
+    a.rows_per_cta = rows_total >= 512LL * 148 * 4 ? 512 : (rows_total >= 128LL * 148 * 4 ? 128 : 64);
+    const int v = d->ld / 64, kpad = d->delay <= 16 ? 16 : 32;
+#define X(V, KPAD, TW, NWC, CS, STAGES) \
+    if (v == V && kpad == KPAD) return launch_ring<KPAD, TW, NWC, CS, STAGES>(a, d->nw, s);
+    QMC_RING_SHAPES(X)
+#undef X
+    return cudaErrorInvalidValue;
+}
+
+}  // namespace qmc

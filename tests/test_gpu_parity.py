@@ -294,3 +294,44 @@ def test_delayed_standalone_api():
     with pytest.raises(api.QmcError):
         api.Det.init(spline, pos_t, delay_rank=33)
     spline.destroy()
+
+
+# --------------------------------------------------- delayed rank-k at large N (cluster / ring flush shapes)
+@pytest.mark.parametrize("nel,K,nw,count,env", [
+    (512, 16, 6, 0, {}), (512, 32, 4, 0, {}), (1000, 16, 5, 0, {}), (1024, 16, 4, 0, {}), (1024, 32, 3, 0, {}),
+    (2048, 16, 2, 200, {}), (2048, 32, 2, 200, {}),
+    # the flush.cu kernel on the same shapes: one CTA per row block, then its cluster shapes
+    (1000, 16, 4, 0, {"QMC_FLUSH_RING": "0"}), (1024, 16, 3, 0, {"QMC_FLUSH_RING": "0", "QMC_FLUSH_SHAPE": "1"}),
+    (1024, 16, 3, 0, {"QMC_FLUSH_RING": "0", "QMC_FLUSH_SHAPE": "2"}), (1024, 32, 3, 0, {"QMC_FLUSH_RING": "0"}),
+    (2048, 16, 2, 200, {"QMC_FLUSH_RING": "0"})])
+def test_delayed_large_n_equals_rank1(nel, K, nw, count, env, monkeypatch):
+    """N >= 512 takes the flush kernels that split the columns of a row block over a thread-block
+    cluster (flush_ring.cu, or flush.cu's cluster shapes when the ring kernel is switched off): same
+    decisions, ratios and inverse as the rank-1 path on the same inputs, including a ragged N
+    (1000: partial last row block, zero pad columns) and a window that does not divide the
+    electron range."""
+    for k_, v_ in env.items():
+        monkeypatch.setenv(k_, v_)
+    cfg = inputs.custom_config(f"n{nel}", (24, 24, 24), nel, (9.0, 8.5, 9.5), nw=nw, nsweeps=1, sigma=0.3)
+    x = inputs.make_inputs(cfg, device=P.dev())
+    spline = api.Spline.create(x.coefs, x.lattice)
+    pos0, delta, unif = P.to_dev(x.pos), P.to_dev(x.delta), P.to_dev(x.unif)
+    res = {}
+    for k in (0, K):
+        det = api.Det.init(spline, pos0, delay_rank=k)
+        assert det.delay_rank == k
+        pos = pos0.clone()
+        R = torch.zeros_like(unif)
+        acc = torch.zeros(unif.shape, dtype=torch.uint8, device=P.dev())
+        api.sweep(det, pos, delta, unif, ratios_out=R, accept_out=acc, iel_begin=3 if count else 0, iel_count=count)
+        res[k] = (pos, R, acc, det.get_inverse(), det.get_stats())
+        det.destroy()
+    a, b = res[0], res[K]
+    assert 0.05 < float(a[2].float().mean()) if not count else True
+    assert torch.equal(a[2], b[2]) and torch.equal(a[0], b[0])
+    assert float((a[1] - b[1]).abs().max() / a[1].abs().max()) < 1e-10
+    scale = float(a[3].abs().max())
+    assert float((a[3] - b[3]).abs().max()) < 1e-9 * scale
+    assert float((a[4][0] - b[4][0]).abs().max()) < 1e-8
+    assert torch.equal(a[4][1], b[4][1]) and torch.equal(a[4][2], b[4][2])
+    spline.destroy()
