@@ -35,14 +35,11 @@ from paper_1802_06922_b200 import inputs, sharding  # noqa: E402
 
 METRIC = "electron moves/s at N=1024 (spline VGL+ratio+SM update); HBM GB/s vs peak"
 UNIT = "moves/s"
-# delayed rank measured by default per config (BASELINE.json: large = rank-16; xlarge asks for rank-32,
-# the flush kernel's shared-memory window holds rank 8 at N = 2048: DESIGN.md section 6)
-DEFAULT_DELAY = {"tiny": 0, "small": 16, "mid": 16, "large": 16, "xlarge": 8}
-# fp64 tensor-core peak measured with a DMMA.8x8x4 issue loop on this pool's B200 (profiles/r01_fp64_peak.md)
-FP64_DMMA_PEAK = 37.0
+# delayed rank measured by default per config (BASELINE.json: large = rank-16, very large = rank-32)
+DEFAULT_DELAY = {"tiny": 0, "small": 16, "mid": 16, "large": 16, "xlarge": 32}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures
-# (profiles/*.md), large config
-NCU_TRAFFIC = {"sm_update": 6.725e9}
+# (profiles/r01_*.md), config `large`
+NCU_TRAFFIC = {"sm_update": 6.725e9, "delayed_flush": 8.614e9, "spo_vgl": 2.303e9}
 
 
 def measured_peaks():
@@ -103,21 +100,29 @@ class ClockSampler:
 
 
 def cpu_sample(x, coefs_np, target_s=15.0):
-    """The oracle, as it stands, on a bounded sample of the workload: `cores` walkers (one per
-    thread) x the first M electron moves of a sweep.  Returns (moves/s, cores, sample text, seconds)."""
+    """The oracle, as it stands, on a bounded sample of the workload: W walkers (a whole number per
+    thread) x the first M electron moves of a sweep, sized for about `target_s` seconds.
+    Returns (moves/s, cores, sample text, seconds)."""
     import oracle
     cores = len(os.sched_getaffinity(0))
     nthreads = max(1, min(cores, oracle.max_threads(), 32, x.pos.shape[0]))
-    nwc, nel = nthreads, x.cfg.norb
-    pos = np.ascontiguousarray(x.pos[:nwc])
-    B, ld, sg = oracle.init_walkers(coefs_np, x.lattice, pos, nthreads=nthreads)       # untimed set-up
-    delta = np.ascontiguousarray(x.delta[:1, :, :nwc])
-    unif = np.ascontiguousarray(x.unif[:1, :, :nwc])
+    nel = x.cfg.norb
     probe = min(8, nel)
+
+    def setup(nwc):
+        pos = np.ascontiguousarray(x.pos[:nwc])
+        B, ld, sg = oracle.init_walkers(coefs_np, x.lattice, pos, nthreads=nthreads)       # untimed set-up
+        return pos, B, ld, sg, np.ascontiguousarray(x.delta[:1, :, :nwc]), np.ascontiguousarray(x.unif[:1, :, :nwc])
+
+    pos, B, ld, sg, delta, unif = setup(nthreads)
     t0 = time.perf_counter()
     oracle.sweep(coefs_np, x.lattice, pos, B, ld, sg, delta, unif, iel_count=probe, nthreads=nthreads)
-    t_probe = time.perf_counter() - t0
-    m = int(min(nel, max(probe, target_s / max(t_probe / probe, 1e-6))))
+    t_move = (time.perf_counter() - t0) / probe            # one electron step of `nthreads` walkers
+    m = int(min(nel, max(probe, target_s / max(t_move, 1e-6))))
+    per_thread = int(max(1, min(x.pos.shape[0] // nthreads, target_s / max(t_move * m, 1e-6))))
+    nwc = nthreads * per_thread
+    if per_thread > 1:
+        pos, B, ld, sg, delta, unif = setup(nwc)
     t0 = time.perf_counter()
     out = oracle.sweep(coefs_np, x.lattice, pos, B, ld, sg, delta, unif, iel_count=m, nthreads=nthreads)
     dt = time.perf_counter() - t0
@@ -216,6 +221,7 @@ def main():
     delta_h = torch.from_numpy(delta_np).pin_memory()
     unif_h = torch.from_numpy(unif_np).pin_memory()
     peak, peak_src = measured_peaks()
+    fp64_peak = api.probe_fp64_dmma()        # TFLOP/s, measured live (MEASURED_PEAKS.json has no fp64 figure)
 
     def barrier():
         torch.cuda.synchronize()
@@ -273,6 +279,8 @@ def main():
             "ratio_rowcopy": nw * (2 * 8 * ld + 4 * nel),
             "sm_update": (n_acc / max(prof["sm_update"][1], 1)) * (16 * nel * ld + 12 * nel),
             "delayed_flush": nw * 16 * nel * ld + (n_acc / max(prof["delayed_flush"][1], 1)) * (8 * ld + 4 * npitch),
+            # window: K rows of B0 and K vectors in, R' rows out
+            "delayed_window": nw * max(K, 1) * (8 * ld + 4 * npitch) + (n_acc / max(prof["delayed_window"][1], 1)) * 8 * ld,
         }
         kernels = {}
         for k, (kms, kn) in prof.items():
@@ -282,17 +290,29 @@ def main():
             if k in per_launch:
                 gbs = per_launch[k] / (kms / kn * 1e-3) / 1e9
                 kernels[k].update({"bytes_per_launch": per_launch[k], "GB/s": gbs, "frac_of_hbm_peak": gbs / peak})
-        if "delayed_flush" in kernels:   # two fp64 contractions on the tensor cores: 4 KPAD N ld flop / walker
-            kpad = (K + 7) // 8 * 8
-            fl = 4.0 * kpad * nel * ld * nw
-            kernels["delayed_flush"].update({"flops_per_launch": fl, "fp64_TFLOP/s": fl / (kernels["delayed_flush"]["avg_us"] * 1e-6) / 1e12,
-                                             "fp64_dmma_peak_TFLOP/s": FP64_DMMA_PEAK})
+        if "delayed_flush" in kernels:   # two fp64 contractions on the tensor cores: 4 p N^2 flop per walker
+            kf = kernels["delayed_flush"]
+            fl = 4.0 * (n_acc / kf["launches"]) * nel * nel
+            tf = fl / (kf["avg_us"] * 1e-6) / 1e12
+            kf.update({"flops_per_launch": fl, "fp64_TFLOP/s": tf, "fp64_dmma_peak_TFLOP/s": fp64_peak,
+                       "frac_of_fp64_dmma_peak": tf / fp64_peak,
+                       "min_ms_hbm": kf["bytes_per_launch"] / (peak * 1e9) * 1e3,
+                       "min_ms_fp64": fl / (fp64_peak * 1e12) * 1e3})
         dom = max(kernels, key=lambda k: kernels[k]["ms"])
         kd = kernels[dom]
-        roofline = {"bound": "hbm", "kernel": dom, "achieved": kd.get("GB/s"), "peak": peak, "unit": "GB/s",
-                    "frac": kd.get("frac_of_hbm_peak"), "traffic": NCU_TRAFFIC.get(dom), "peak_source": peak_src,
-                    "launches": kd["launches"], "avg_us": kd["avg_us"], "bytes_per_launch": kd.get("bytes_per_launch"),
-                    "share_of_step": kd["share_of_step"]}
+        traffic = NCU_TRAFFIC.get(dom) if (args.config == "large" and nw == cfg.nw) else None
+        if dom == "delayed_flush" and kd["min_ms_fp64"] > kd["min_ms_hbm"]:
+            # the contraction, not the pass over B, bounds this rank: report against the fp64 tensor peak
+            roofline = {"bound": "tensor", "kernel": dom, "achieved": kd["fp64_TFLOP/s"], "peak": fp64_peak,
+                        "unit": "TFLOP/s", "frac": kd["frac_of_fp64_dmma_peak"], "traffic": traffic,
+                        "peak_source": "measured live: qmc_probe_fp64_dmma (DMMA.8x8x4 issue loop)",
+                        "launches": kd["launches"], "avg_us": kd["avg_us"], "flops_per_launch": kd["flops_per_launch"],
+                        "share_of_step": kd["share_of_step"]}
+        else:
+            roofline = {"bound": "hbm", "kernel": dom, "achieved": kd.get("GB/s"), "peak": peak, "unit": "GB/s",
+                        "frac": kd.get("frac_of_hbm_peak"), "traffic": traffic, "peak_source": peak_src,
+                        "launches": kd["launches"], "avg_us": kd["avg_us"], "bytes_per_launch": kd.get("bytes_per_launch"),
+                        "share_of_step": kd["share_of_step"]}
 
         # ---- end to end through the C ABI with HOST buffers (pinned): H2D of pos/delta/unif and D2H
         #      of pos/ratios/decisions inside the timed region, every step

@@ -204,11 +204,19 @@ int qmc_det_info(const qmc_det_t *det, int *nwalkers, int *nel, int *ld, int *de
  *                             arrays of QMC_PROF_KINDS entries.  Kinds: 0 SPO-VGL of a batch of
  *                             electron steps, 1 rank-1 update, 2 delayed ratio/decide/append,
  *                             3 delayed accept (standalone), 4 delayed flush, 5 ratio + row copy.
+ *                             In qmc_sweep kind 2 is the one-launch-per-window kernel (ratios, decisions and
+ *                             moves of K steps).
  *                             Resets the recorder.
  */
 #define QMC_PROF_KINDS 6
 int qmc_det_profile(qmc_det_t *det, int enable);
 int qmc_det_profile_read(qmc_det_t *det, double *ms_host, long long *launches_host);
+
+/* Measured fp64 tensor-core peak of the current device in TFLOP/s (host pointer): an issue loop of
+ * mma.sync.m8n8k4.f64 with register operands, best of 5 after a warm-up, ~10 ms.  bench.py reports
+ * the delayed flush (the "genuine dense fp64 contraction" of north_star) against it,
+ * since MEASURED_PEAKS.json holds no fp64 figure.  Synchronises the stream. */
+int qmc_probe_fp64_dmma(double *tflops_host, void *stream);
 
 /* Number of kernel launches this library has enqueued since load (bench.py's gpu_launches). */
 long long qmc_launch_count(void);

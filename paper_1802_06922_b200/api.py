@@ -21,8 +21,9 @@ EXPORTS = [
     "qmc_det_init", "qmc_det_destroy", "qmc_det_ratio", "qmc_det_accept_update", "qmc_det_flush",
     "qmc_sweep", "qmc_sweep_ex", "qmc_sweep_host", "qmc_det_get_inverse", "qmc_det_set_inverse",
     "qmc_det_get_stats", "qmc_det_info", "qmc_launch_count", "qmc_det_profile", "qmc_det_profile_read",
+    "qmc_probe_fp64_dmma",
 ]
-PROF_KINDS = ["spo_vgl", "sm_update", "delayed_ratio", "delayed_accept", "delayed_flush", "ratio_rowcopy"]
+PROF_KINDS = ["spo_vgl", "sm_update", "delayed_window", "delayed_accept", "delayed_flush", "ratio_rowcopy"]
 
 
 class SweepOpts(ctypes.Structure):
@@ -69,6 +70,7 @@ def load_library(path=None):
         "qmc_det_info": [_vp] + [ctypes.POINTER(i)] * 4,
         "qmc_det_profile": [_vp, i],
         "qmc_det_profile_read": [_vp, ctypes.POINTER(d), ctypes.POINTER(ctypes.c_longlong)],
+        "qmc_probe_fp64_dmma": [ctypes.POINTER(d), _vp],
     }
     for name, args in sigs.items():
         fn = getattr(lib, name)
@@ -109,6 +111,13 @@ def _dev(t, dtype, allow_none=False):
 
 def launch_count():
     return int(load_library().qmc_launch_count())
+
+
+def probe_fp64_dmma(stream=None):
+    """qmc_probe_fp64_dmma: measured fp64 tensor-core (DMMA) peak of the current device, TFLOP/s."""
+    out = ctypes.c_double(0.0)
+    _check(load_library().qmc_probe_fp64_dmma(ctypes.byref(out), _stream(stream)), "qmc_probe_fp64_dmma")
+    return out.value
 
 
 class Spline:

@@ -44,7 +44,7 @@ constexpr int kRecvBufs = 4;      // partial-Q receive buffers in flight (see th
 //   ring   double [STAGES][8][LDC + 8]      row blocks of B (pitch + 8: conflict-free 128-bit reads)
 //   part   double [2][NWC][8][KPAD + 4]     partial Q of each column warp, by block parity
 //   recv   double [kRecvBufs][CS][8][KPAD + 4]   partial Q of every CTA of the cluster
-//   full   mbarrier [STAGES], rbar mbarrier [kRecvBufs]
+//   full   mbarrier [STAGES], rbar mbarrier [kRecvBufs], pbar mbarrier [2]
 template <int KPAD, int TW, int NWC, int CS, int STAGES>
 struct RingSmem {
     static constexpr int LDC = NWC * TW * 8, RP = LDC + 8, PS = KPAD + 4;
@@ -52,7 +52,7 @@ struct RingSmem {
     static constexpr size_t part_off = ring_off + (size_t)STAGES * 8 * RP * sizeof(double);
     static constexpr size_t recv_off = part_off + (size_t)2 * NWC * 8 * PS * sizeof(double);
     static constexpr size_t bar_off = recv_off + (size_t)kRecvBufs * CS * 8 * PS * sizeof(double);
-    static constexpr size_t bytes = bar_off + (size_t)(STAGES + kRecvBufs) * sizeof(uint64_t);
+    static constexpr size_t bytes = bar_off + (size_t)(STAGES + kRecvBufs + 2) * sizeof(uint64_t);
 };
 
 // Row-block loop for a window of NTA active 8-wide tiles (8 NTA - 7 <= p <= 8 NTA).
@@ -61,12 +61,14 @@ __device__ __forceinline__ void ring_stream(const RingArgs &a, int w, int p, uns
 {
     using L = RingSmem<KPAD, TW, NWC, CS, STAGES>;
     constexpr int LDC = L::LDC, LD = LDC * CS, RP = L::RP, PS = L::PS;
-    constexpr int KQA = 2 * NTA, NTHREADS = 32 * NWC;
+    constexpr int KQA = 2 * NTA;
+    constexpr int LW = NTA < NWC ? NTA : NWC;               // warps that reduce and send the partial Q
     double *ring = reinterpret_cast<double *>(smem + L::ring_off);
     double *part = reinterpret_cast<double *>(smem + L::part_off);
     double *recv = reinterpret_cast<double *>(smem + L::recv_off);
     uint64_t *full = reinterpret_cast<uint64_t *>(smem + L::bar_off);
     uint64_t *rbar = full + STAGES;
+    uint64_t *pbar = rbar + kRecvBufs;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int g = lane >> 2, t = lane & 3;
     const int K = a.K, nel = a.nel;
@@ -118,9 +120,12 @@ __device__ __forceinline__ void ring_stream(const RingArgs &a, int w, int p, uns
         for (int jb = 0; jb < STAGES - 1 && jb < nblk; ++jb) issue(jb);
 
     // ---- software-pipelined loop: iteration j runs step 1 of block j and step 2 of block j - 1.
-    // Hazards: ring stage (j-1) % STAGES is refilled at the top of iteration j, after the barrier
-    // of iteration j-1 that follows every warp's read of it.  A peer sends block j+4 only after it
-    // received my block j+2, which I send after I read its block j (iteration j+1): 4 buffers.
+    // Hazards: ring stage (j-1) % STAGES is refilled by warp 0 at the top of iteration j; warp 0 is a
+    // reducing warp, so in iteration j-1 it waited for every warp's partial of block j-1, which each
+    // warp writes after reading that stage.  part[j & 1] is rewritten in iteration j+2, which a warp
+    // reaches only after rbar of block j completed, i.e. after the reducers read part[j & 1].  A peer
+    // sends block j+4 only after it received my block j+2, which I send after I read its block j
+    // (iteration j+1): 4 receive buffers.
     double2 ra[TW], rb[TW];
     for (int j = 0; j <= nblk; ++j) {
         if (j < nblk) {
@@ -146,18 +151,25 @@ __device__ __forceinline__ void ring_stream(const RingArgs &a, int w, int p, uns
 #pragma unroll
             for (int nt = 0; nt < NTA; ++nt)
                 *reinterpret_cast<double2 *>(ps + 8 * nt + 2 * t) = make_double2(cq[nt][0], cq[nt][1]);
-            __syncthreads();
-            // this CTA's partial (fixed order over its warps), sent to every CTA of the cluster
-            const int b = j % kRecvBufs;
-            if (tid == 0) mbar_arrive_expect_tx(&rbar[b], (uint32_t)(CS * 64 * NTA * sizeof(double)));
-            for (int e = tid; e < 64 * NTA; e += NTHREADS) {
-                const int row = e / (8 * NTA), col = e % (8 * NTA);
-                double sum = 0.0;
+            // hand the partial to the reducing warps through an mbarrier: the other warps do not stop
+            // here (no CTA-wide barrier in the loop), so their DMMA work fills this exchange's bubbles
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&pbar[j & 1]);
+            if (warp < LW) {
+                // this CTA's partial (fixed order over its warps), sent to every CTA of the cluster
+                mbar_wait(&pbar[j & 1], (uint32_t)(j >> 1) & 1u);
+                const int b = j % kRecvBufs;
+                if (tid == 0) mbar_arrive_expect_tx(&rbar[b], (uint32_t)(CS * 64 * NTA * sizeof(double)));
+                for (int e = tid; e < 64 * NTA; e += 32 * LW) {
+                    const int row = e / (8 * NTA), col = e % (8 * NTA);
+                    double sum = 0.0;
 #pragma unroll
-                for (int c = 0; c < NWC; ++c) sum += pbuf[((size_t)c * 8 + row) * PS + col];
-                const double *dst = recv + ((size_t)(b * CS + (int)crank) * 8 + row) * PS + col;
+                    for (int c = 0; c < NWC; ++c) sum += pbuf[((size_t)c * 8 + row) * PS + col];
+                    const double *dst = recv + ((size_t)(b * CS + (int)crank) * 8 + row) * PS + col;
 #pragma unroll
-                for (int c = 0; c < CS; ++c) st_async_f64(mapa_u32(dst, (uint32_t)c), sum, mapa_u32(&rbar[b], (uint32_t)c));
+                    for (int c = 0; c < CS; ++c)
+                        st_async_f64(mapa_u32(dst, (uint32_t)c), sum, mapa_u32(&rbar[b], (uint32_t)c));
+                }
             }
         }
         if (j >= 1) {
@@ -199,8 +211,10 @@ flush_ring_kernel(RingArgs a)
     const int p = a.win_count[w];
     if (p == 0) return;                                    // the whole cluster leaves together
     uint64_t *bars = reinterpret_cast<uint64_t *>(smem_ring + L::bar_off);
-    if (threadIdx.x == 0)
+    if (threadIdx.x == 0) {
         for (int i = 0; i < STAGES + kRecvBufs; ++i) mbar_init(&bars[i], 1);
+        for (int i = 0; i < 2; ++i) mbar_init(&bars[STAGES + kRecvBufs + i], NWC);    // one arrival per warp
+    }
     __syncthreads();
     if constexpr (CS > 1) {                                // peers' barriers exist before anything is sent
         cluster_arrive();
