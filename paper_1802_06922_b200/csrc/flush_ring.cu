@@ -63,6 +63,9 @@ __device__ __forceinline__ void ring_stream(const RingArgs &a, int w, int p, uns
     constexpr int LDC = L::LDC, LD = LDC * CS, RP = L::RP, PS = L::PS;
     constexpr int KQA = 2 * NTA;
     constexpr int LW = NTA < NWC ? NTA : NWC;               // warps that reduce and send the partial Q
+    // small clusters: the reducers run their own step 2 first (the other warps' partials are in by
+    // then); larger clusters need the extra time for the exchange itself (measured both ways)
+    constexpr bool SEND_LATE = CS <= 2;
     double *ring = reinterpret_cast<double *>(smem + L::ring_off);
     double *part = reinterpret_cast<double *>(smem + L::part_off);
     double *recv = reinterpret_cast<double *>(smem + L::recv_off);
@@ -128,6 +131,23 @@ __device__ __forceinline__ void ring_stream(const RingArgs &a, int w, int p, uns
     // (iteration j+1): 4 receive buffers.
     double2 ra[TW], rb[TW];
     for (int j = 0; j <= nblk; ++j) {
+        double *pbuf = part + (size_t)(j & 1) * NWC * 8 * PS;
+        // the reducing warps: this CTA's partial (fixed order over its warps), sent to every CTA of the cluster
+        auto reduce_and_send = [&]() {
+            mbar_wait(&pbar[j & 1], (uint32_t)(j >> 1) & 1u);
+            const int b = j % kRecvBufs;
+            if (tid == 0) mbar_arrive_expect_tx(&rbar[b], (uint32_t)(CS * 64 * NTA * sizeof(double)));
+            for (int e = tid; e < 64 * NTA; e += 32 * LW) {
+                const int row = e / (8 * NTA), col = e % (8 * NTA);
+                double sum = 0.0;
+#pragma unroll
+                for (int c = 0; c < NWC; ++c) sum += pbuf[((size_t)c * 8 + row) * PS + col];
+                const double *dst = recv + ((size_t)(b * CS + (int)crank) * 8 + row) * PS + col;
+#pragma unroll
+                for (int c = 0; c < CS; ++c)
+                    st_async_f64(mapa_u32(dst, (uint32_t)c), sum, mapa_u32(&rbar[b], (uint32_t)c));
+            }
+        };
         if (j < nblk) {
             if (warp == 0 && j + STAGES - 1 < nblk) issue(j + STAGES - 1);
             const int s = j % STAGES;
@@ -146,7 +166,6 @@ __device__ __forceinline__ void ring_stream(const RingArgs &a, int w, int p, uns
                     dmma884(cq[nt][0], cq[nt][1], rb[i].x, vf[i][nt][0]);
                     dmma884(cq[nt][0], cq[nt][1], rb[i].y, vf[i][nt][1]);
                 }
-            double *pbuf = part + (size_t)(j & 1) * NWC * 8 * PS;
             double *ps = pbuf + ((size_t)warp * 8 + g) * PS;
 #pragma unroll
             for (int nt = 0; nt < NTA; ++nt)
@@ -155,22 +174,7 @@ __device__ __forceinline__ void ring_stream(const RingArgs &a, int w, int p, uns
             // here (no CTA-wide barrier in the loop), so their DMMA work fills this exchange's bubbles
             __syncwarp();
             if (lane == 0) mbar_arrive(&pbar[j & 1]);
-            if (warp < LW) {
-                // this CTA's partial (fixed order over its warps), sent to every CTA of the cluster
-                mbar_wait(&pbar[j & 1], (uint32_t)(j >> 1) & 1u);
-                const int b = j % kRecvBufs;
-                if (tid == 0) mbar_arrive_expect_tx(&rbar[b], (uint32_t)(CS * 64 * NTA * sizeof(double)));
-                for (int e = tid; e < 64 * NTA; e += 32 * LW) {
-                    const int row = e / (8 * NTA), col = e % (8 * NTA);
-                    double sum = 0.0;
-#pragma unroll
-                    for (int c = 0; c < NWC; ++c) sum += pbuf[((size_t)c * 8 + row) * PS + col];
-                    const double *dst = recv + ((size_t)(b * CS + (int)crank) * 8 + row) * PS + col;
-#pragma unroll
-                    for (int c = 0; c < CS; ++c)
-                        st_async_f64(mapa_u32(dst, (uint32_t)c), sum, mapa_u32(&rbar[b], (uint32_t)c));
-                }
-            }
+            if (!SEND_LATE && warp < LW) reduce_and_send();
         }
         if (j >= 1) {
             const int jj = j - 1, b = jj % kRecvBufs;
@@ -195,6 +199,7 @@ __device__ __forceinline__ void ring_stream(const RingArgs &a, int w, int p, uns
                 for (int i = 0; i < TW; ++i) *reinterpret_cast<double2 *>(dst + 8 * i) = ra[i];
             }
         }
+        if (SEND_LATE && j < nblk && warp < LW) reduce_and_send();
 #pragma unroll
         for (int i = 0; i < TW; ++i) ra[i] = rb[i];
     }
