@@ -117,11 +117,12 @@ def cpu_sample(x, coefs_np, target_s=15.0):
         return pos, B, ld, sg, np.ascontiguousarray(x.delta[:1, :, :nwc]), np.ascontiguousarray(x.unif[:1, :, :nwc])
 
     pos, B, ld, sg, delta, unif = setup(nthreads)
+    oracle.sweep(coefs_np, x.lattice, pos, B, ld, sg, delta, unif, iel_count=probe, nthreads=nthreads)   # page the table in
     t0 = time.perf_counter()
     oracle.sweep(coefs_np, x.lattice, pos, B, ld, sg, delta, unif, iel_count=probe, nthreads=nthreads)
     t_move = (time.perf_counter() - t0) / probe            # one electron step of `nthreads` walkers
     m = int(min(nel, max(probe, target_s / max(t_move, 1e-6))))
-    per_thread = int(max(1, min(x.pos.shape[0] // nthreads, target_s / max(t_move * m, 1e-6))))
+    per_thread = int(max(1, min(x.pos.shape[0] // nthreads, round(target_s / max(t_move * m, 1e-6)))))
     nwc = nthreads * per_thread
     if per_thread > 1:
         pos, B, ld, sg, delta, unif = setup(nwc)
