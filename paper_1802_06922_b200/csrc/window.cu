@@ -112,67 +112,79 @@ __global__ void __launch_bounds__(kWinThreads) delayed_window_kernel(WindowArgs 
         }
         __syncthreads();
     }
-    // ---- phase 3: the nb steps in sequence; lane m owns accepted move m (its step index `mine`)
+    // ---- phase 3: the nb steps in sequence; lane m owns accepted move m (its step index `mine`).
+    // Everything that lives in global memory stays outside the sequential loop: lane i fetches the
+    // uniform / forced decision of step i before it and writes ratio, decision and the moved
+    // position of step i after it, so a step costs shuffles, shared memory and fp64 arithmetic only.
     if (warp == 0) {
-    int p = 0, mine = 0;
-    double logdet_add = 0.0;
-    int flips = 0;
-    for (int i = 0; i < nb; ++i) {
-        const double c = lane < p ? G_s[mine * GS + i] : 0.0;     // c_m = v_{l_m} . B0[k_i]
-        const double x = lane < p ? G_s[i * GS + mine] : 0.0;     // x_m = v_i . B0[k_{l_m}]
-        double y = 0.0, z = 0.0;                                  // y = S^-1 c, z = S^-T x
-        for (int q = 0; q < p; ++q) {
-            const double cq = __shfl_sync(0xffffffffu, c, q), xq = __shfl_sync(0xffffffffu, x, q);
+        const size_t mv_l = (size_t)lane * a.nw + w;                  // move of step `lane`
+        const bool step_l = lane < nb;
+        const double u_l = (step_l && !a.forced) ? a.unif[mv_l] : 0.0;
+        const int f_l = (step_l && a.forced) ? (a.forced[mv_l] != 0) : 0;
+        double R_l = 1.0;                                             // ratio of step `lane`
+        unsigned acc_mask = 0;                                        // accepted steps (same in every lane)
+        int p = 0, mine = 0;
+        for (int i = 0; i < nb; ++i) {
+            const double c = lane < p ? G_s[mine * GS + i] : 0.0;     // c_m = v_{l_m} . B0[k_i]
+            const double x = lane < p ? G_s[i * GS + mine] : 0.0;     // x_m = v_i . B0[k_{l_m}]
+            double y = 0.0, z = 0.0;                                  // y = S^-1 c, z = S^-T x
+            for (int q = 0; q < p; ++q) {
+                const double cq = __shfl_sync(0xffffffffu, c, q), xq = __shfl_sync(0xffffffffu, x, q);
+                if (lane < p) {
+                    y = fma(sinv_s[lane * GS + q], cq, y);
+                    z = fma(sinv_s[q * GS + lane], xq, z);
+                }
+            }
+            const double R = G_s[i * GS + i] - warp_sum(x * y);
+            const double u_i = __shfl_sync(0xffffffffu, u_l, i);
+            const int f_i = __shfl_sync(0xffffffffu, f_l, i);
+            const bool acc_w = a.forced ? (f_i != 0) : metropolis(R, u_i);
+            if (lane == i) R_l = R;
+            if (!acc_w) continue;
+            acc_mask |= 1u << i;
+            const double rinv = 1.0 / R;
+            __syncwarp();             // every lane has read the old S^-1
+            // bordered inverse: S'^-1 = [[S^-1 + y z^T / R, -y / R], [-z^T / R, 1 / R]]
+            for (int q = 0; q < p; ++q) {
+                const double zq = __shfl_sync(0xffffffffu, z, q);
+                if (lane < p) sinv_s[lane * GS + q] += y * zq * rinv;
+            }
             if (lane < p) {
-                y = fma(sinv_s[lane * GS + q], cq, y);
-                z = fma(sinv_s[q * GS + lane], xq, z);
+                sinv_s[lane * GS + p] = -y * rinv;
+                sinv_s[p * GS + lane] = -z * rinv;
+            }
+            if (lane == p) { sinv_s[p * GS + p] = rinv; mine = i; }
+            ++p;
+            __syncwarp();
+        }
+        // results of step `lane`
+        const bool acc_l = step_l && ((acc_mask >> lane) & 1u);
+        if (step_l) {
+            if (a.ratios_out) a.ratios_out[mv_l] = R_l;
+            if (a.accept_out) a.accept_out[mv_l] = acc_l ? 1 : 0;
+        }
+        if (acc_l) {
+            double *r = a.pos + ((size_t)w * a.nel + a.iel0 + lane) * 3;
+            r[0] += a.delta[3 * mv_l + 0];
+            r[1] += a.delta[3 * mv_l + 1];
+            r[2] += a.delta[3 * mv_l + 2];
+        }
+        const double logdet_add = warp_sum(acc_l ? log(fabs(R_l)) : 0.0);     // fixed (butterfly) order
+        const unsigned neg = __ballot_sync(0xffffffffu, acc_l && R_l < 0.0);
+        if (lane == 0) {
+            a.win_count[w] = p;
+            p_s = p;
+            if (p) {
+                a.logdet[w] += logdet_add;
+                if (__popc(neg) & 1) a.sign[w] = -a.sign[w];
+                a.naccept[w] += p;
             }
         }
-        const double R = G_s[i * GS + i] - warp_sum(x * y);
-        const size_t mv = (size_t)i * a.nw + w;
-        const bool acc_w = a.forced ? (a.forced[mv] != 0) : metropolis(R, a.unif[mv]);
-        if (lane == 0) {
-            if (a.ratios_out) a.ratios_out[mv] = R;
-            if (a.accept_out) a.accept_out[mv] = acc_w ? 1 : 0;
-        }
-        if (!acc_w) continue;
-        const double rinv = 1.0 / R;
-        __syncwarp();             // every lane has read the old S^-1
-        if (lane == 0) {
-            logdet_add += log(fabs(R));
-            if (R < 0.0) flips ^= 1;
-            double *r = a.pos + ((size_t)w * a.nel + a.iel0 + i) * 3;
-            r[0] += a.delta[3 * mv + 0];
-            r[1] += a.delta[3 * mv + 1];
-            r[2] += a.delta[3 * mv + 2];
-        }
-        // bordered inverse: S'^-1 = [[S^-1 + y z^T / R, -y / R], [-z^T / R, 1 / R]]
-        for (int q = 0; q < p; ++q) {
-            const double zq = __shfl_sync(0xffffffffu, z, q);
-            if (lane < p) sinv_s[lane * GS + q] += y * zq * rinv;
-        }
         if (lane < p) {
-            sinv_s[lane * GS + p] = -y * rinv;
-            sinv_s[p * GS + lane] = -z * rinv;
+            a.win_iel[(size_t)w * K + lane] = a.iel0 + mine;
+            a.win_slot[(size_t)w * K + lane] = mine;
+            rowoff_s[lane] = (long long)mine * ld;
         }
-        if (lane == p) { sinv_s[p * GS + p] = rinv; mine = i; }
-        ++p;
-        __syncwarp();
-    }
-    if (lane == 0) {
-        a.win_count[w] = p;
-        p_s = p;
-        if (p) {
-            a.logdet[w] += logdet_add;
-            if (flips) a.sign[w] = -a.sign[w];
-            a.naccept[w] += p;
-        }
-    }
-    if (lane < p) {
-        a.win_iel[(size_t)w * K + lane] = a.iel0 + mine;
-        a.win_slot[(size_t)w * K + lane] = mine;
-        rowoff_s[lane] = (long long)mine * ld;
-    }
     }
     __syncthreads();
 

@@ -199,24 +199,28 @@ def test_sweep_control_flow():
 
 
 # ------------------------------------------------------------------------------- full sizes
-@pytest.mark.parametrize("name,nchk,npos", [("mid", 4, 48), ("large", 4, 32)])
-def test_full_size_sampled(name, nchk, npos):
+@pytest.mark.parametrize("name,nchk,npos,delay", [("mid", 4, 48, 0), ("large", 4, 32, 0), ("mid", 4, 0, 16),
+                                                  ("large", 4, 0, 16), ("large", 2, 0, 32)])
+def test_full_size_sampled(name, nchk, npos, delay):
     """BASELINE.json's full sizes in the launch configuration bench.py times (all walkers in
-    lockstep, one sweep): the oracle checks the SPO-VGL at sampled positions and replays the
-    first `nchk` walkers move by move (identical orbital vectors, decisions, inverse, residual)."""
+    lockstep, one sweep; rank-1 and the delayed ranks bench.py measures): the oracle checks the
+    SPO-VGL at sampled positions and replays the first `nchk` walkers move by move (identical
+    orbital vectors, decisions, inverse, residual)."""
     free_b = torch.cuda.mem_get_info()[0]
     cfg = inputs.CONFIGS[name]
     if free_b < 2.6 * cfg.table_bytes() + 4 * cfg.nw * cfg.norb ** 2 * 8:
         pytest.skip("not enough device memory")
     x = inputs.make_inputs(cfg, device=P.dev(), nsweeps=1)
     coefs_np = x.coefs_numpy()                  # the same bits for both sides
-    spline = api.Spline.create(x.coefs, x.lattice)
-    pos = x.pos.reshape(-1, 3)[:: max(1, x.pos.size // 3 // npos)][:npos]
-    v, g, l = api.spo_vgl(spline, P.to_dev(pos))
-    vo, go, lo = oracle.spline_vgl(coefs_np, x.lattice, pos)
-    print(name, "vgl rel err", P.check_vgl(v, g, l, vo, go, lo, cfg.norb))
-    spline.destroy()
-    out = P.run_protocol(x, walkers=nchk, free_oracle=(name == "mid"), coefs_np=coefs_np)
+    if npos:
+        spline = api.Spline.create(x.coefs, x.lattice)
+        pos = x.pos.reshape(-1, 3)[:: max(1, x.pos.size // 3 // npos)][:npos]
+        v, g, l = api.spo_vgl(spline, P.to_dev(pos))
+        vo, go, lo = oracle.spline_vgl(coefs_np, x.lattice, pos)
+        print(name, "vgl rel err", P.check_vgl(v, g, l, vo, go, lo, cfg.norb))
+        spline.destroy()
+    out = P.run_protocol(x, delay_rank=delay, walkers=nchk, free_oracle=(name == "mid" and not delay),
+                         coefs_np=coefs_np)
     print(name, out)
 
 
