@@ -50,7 +50,8 @@ def _load():
         lib.orc_sweep.restype = ctypes.c_int
         lib.orc_sweep.argtypes = ([ctypes.c_int] * 4 + [_dp, _fp, ctypes.c_int, ctypes.c_int,
                                   _dp, _dp, _dp, _dp, _ip, _dp, _dp, ctypes.c_int, ctypes.c_int,
-                                  _dp, _bp, _bp, _fp, _dp, ctypes.c_int, ctypes.c_int, _dp])
+                                  _dp, _bp, _bp, _fp, _dp, ctypes.c_int, ctypes.c_int, _dp,
+                                  ctypes.c_int, _dp])
         lib.orc_init_walkers.restype = ctypes.c_int
         lib.orc_init_walkers.argtypes = ([ctypes.c_int] * 4 + [_dp, _fp, ctypes.c_int, ctypes.c_int,
                                          _dp, _dp, _dp, _dp, _ip, ctypes.c_int])
@@ -178,9 +179,11 @@ def init_walkers(coefs, lattice, pos, nthreads=1, want_A=False):
 
 
 def sweep(coefs, lattice, pos, B, logdet, sign, delta, unif, A=None, iel_count=None,
-          forced=None, phi_in=None, want_phi=False, mode=0, nthreads=1, want_bnorm=False):
+          forced=None, phi_in=None, want_phi=False, mode=0, nthreads=1, want_bnorm=False,
+          fixed_node=False, want_force=False):
     """Run nsweeps particle-by-particle sweeps.  Inputs are copied; returns a dict with
-    pos, B, A, logdet, sign, ratios [nsweeps][nel][nw], accept (uint8, same shape), phi."""
+    pos, B, A, logdet, sign, ratios [nsweeps][nel][nw], accept (uint8, same shape), phi, force
+    (F = 2 grad log|Psi| of the moved electron at the proposed configuration, [nsweeps][nel][nw][3])."""
     lib = _load()
     coefs = _coefs(coefs)
     nx, ny, nz, norb = coefs.shape
@@ -211,11 +214,12 @@ def sweep(coefs, lattice, pos, B, logdet, sign, delta, unif, A=None, iel_count=N
         p_ptr = phi_in.ctypes.data_as(_fp)
     phi_out = np.zeros((nsweeps, nel, nw, nel)) if want_phi else None
     bnorm = np.zeros((nsweeps, nel, nw)) if want_bnorm else None
+    force = np.zeros((nsweeps, nel, nw, 3)) if want_force else None
     rc = lib.orc_sweep(nx, ny, nz, norb, _d(lat), coefs.ctypes.data_as(_fp), nw, nel,
                        _d(pos), _d(B), _d(A), _d(logdet), sign.ctypes.data_as(_ip),
                        _d(delta), _d(unif), nsweeps, int(iel_count), _d(ratios),
                        accept.ctypes.data_as(_bp), f_ptr, p_ptr, _d(phi_out), int(mode),
-                       int(nthreads), _d(bnorm))
+                       int(nthreads), _d(bnorm), int(bool(fixed_node)), _d(force))
     _check(rc, "sweep")
     return dict(pos=pos, B=B, A=A, logdet=logdet, sign=sign, ratios=ratios, accept=accept,
-                phi=phi_out, bnorm=bnorm)
+                phi=phi_out, bnorm=bnorm, force=force)

@@ -332,6 +332,16 @@ int orc_sm_update(int n, double *B, int k, const double *phi, double R)
  *   bnorm_out  NULL, or [nsweeps][nel][nw]: sum_j |B[k][j]| of the row used by each ratio (a
  *           diagnostic: it bounds how an error in phi propagates into R)
  *   nthreads  OpenMP threads over walkers (<=1: serial)
+ *   fixed_node  != 0: the fixed-node rule of PAPER.md L253 -- "proposed moves that result in a
+ *           nodal crossing are detected through the change in sign of the wavefunction and are
+ *           rejected": a move with R < 0 is rejected whatever u is (ignored when `forced`)
+ *   force_out  NULL, or double [nsweeps][nel][nw][3]: the "wavefunction force" F = 2 grad log Psi_T
+ *           (the F of eq. 11 / eq. 13) on the moved electron at the PROPOSED
+ *           configuration.  With Psi = det A, row k replaced by phi(r'):
+ *               grad_k log|det A'| = sum_j grad phi_j(r') (A'^-1)[j][k]
+ *                                  = sum_j grad phi_j(r') B[k][j] / R        (B'[k] = B[k] / R)
+ *           The gradients come from this oracle's own fp64 spline at r' (also in phi_in mode).
+ *           Written for every move, accepted or not; 0 when R == 0.
  *
  * Accept iff R*R > u; a non-finite R is rejected (R:A8).  On accept:
  * r_k <- r_k + delta (one fp64 add), row k of A <- phi, log|det| += log|R|,
@@ -341,7 +351,8 @@ int orc_sweep(int nx, int ny, int nz, int norb, const double lattice[9], const f
               int nw, int nel, double *pos, double *B, double *A, double *logdet, int *sign,
               const double *delta, const double *unif, int nsweeps, int iel_count,
               double *ratios_out, unsigned char *accept_out, const unsigned char *forced,
-              const float *phi_in, double *phi_out, int mode, int nthreads, double *bnorm_out)
+              const float *phi_in, double *phi_out, int mode, int nthreads, double *bnorm_out,
+              int fixed_node, double *force_out)
 {
     if (nel != norb || nw < 0 || nsweeps < 0 || iel_count < 0 || iel_count > nel) return -1;
     if (mode == 1 && !A) return -1;
@@ -353,9 +364,10 @@ int orc_sweep(int nx, int ny, int nz, int norb, const double lattice[9], const f
 #endif
     for (int w = 0; w < nw; ++w) {
         double *phi = (double *)malloc((size_t)nel * sizeof(double));
+        double *grad = force_out ? (double *)malloc((size_t)4 * nel * sizeof(double)) : NULL;   /* 3 gradients + scratch values */
         double *Bw = B + (size_t)w * nn;
         double *Aw = A ? A + (size_t)w * nn : NULL;
-        int rc = phi ? 0 : -2;
+        int rc = (phi && (grad || !force_out)) ? 0 : -2;
         for (int s = 0; s < nsweeps && rc == 0; ++s)
             for (int k = 0; k < iel_count && rc == 0; ++k) {
                 size_t mv = ((size_t)s * nel + k) * nw + w;
@@ -370,9 +382,18 @@ int orc_sweep(int nx, int ny, int nz, int norb, const double lattice[9], const f
                 }
                 if (phi_out) memcpy(phi_out + mv * nel, phi, (size_t)nel * sizeof(double));
                 double R = orc_det_ratio(nel, Bw, k, phi);
+                if (force_out) {       /* F = 2 grad_k log|det A'| at the proposed configuration */
+                    rc = orc_spline_vgl(nx, ny, nz, norb, lattice, coefs, 1, rnew, grad + (size_t)3 * nel, grad, NULL);
+                    if (rc) break;
+                    for (int d = 0; d < 3; ++d) {
+                        double gd = 0.0;
+                        for (int j = 0; j < nel; ++j) gd += grad[(size_t)d * nel + j] * Bw[(size_t)k * nel + j];
+                        force_out[3 * mv + d] = (R != 0.0) ? 2.0 * gd / R : 0.0;
+                    }
+                }
                 int acc;
                 if (forced) acc = forced[mv] != 0;
-                else acc = isfinite(R) && (R * R > unif[mv]);
+                else acc = isfinite(R) && (R * R > unif[mv]) && !(fixed_node && R < 0.0);
                 if (ratios_out) ratios_out[mv] = R;
                 if (bnorm_out) {
                     double bn = 0.0;
@@ -389,6 +410,7 @@ int orc_sweep(int nx, int ny, int nz, int norb, const double lattice[9], const f
                 else rc = orc_sm_update(nel, Bw, k, phi, R);
             }
         free(phi);
+        free(grad);
         if (rc) {
 #ifdef _OPENMP
 #pragma omp critical

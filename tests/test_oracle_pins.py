@@ -417,3 +417,66 @@ def test_bnorm_diagnostic(sweep_case):
         assert abs(out["bnorm"][0, 0, w] - np.sum(np.abs(B[w, 0]))) < 1e-12
     # |R - R'| <= bnorm * max|phi - phi'| for any perturbed orbital vector
     assert np.all(out["bnorm"] > 0)
+
+
+def test_wavefunction_force_against_finite_differences(sweep_case):
+    """F = 2 grad log Psi_T (the F of eq. 11/13) of the moved electron at the proposed
+    configuration.  Pin independent of the oracle's formula: F R / 2 = grad_r' (det A'(r') / det A),
+    a smooth function of r' even next to a node (where F itself diverges), against central finite
+    differences of that determinant ratio taken by numpy from Slater matrices at shifted positions
+    (the walk is followed with the oracle's own decisions so the configuration is known)."""
+    x, coefs, A, B, ld, sg = sweep_case
+    out = oracle.sweep(coefs, x.lattice, x.pos, B, ld, sg, x.delta, x.unif, want_force=True)
+    F, acc = out["force"], out["accept"]
+    assert np.isfinite(F).all() and np.abs(F).max() > 1e-3
+    nsw, nel, nw = x.unif.shape
+    h = 1e-5
+    checked = 0
+    for w in range(nw):
+        pos = x.pos[w].copy()
+        for s in range(nsw):
+            for k in range(nel):
+                rnew = pos[k] + x.delta[s, k, w]
+                if (s * nel + k) % 7 == w:            # a sample of moves, accepted and rejected ones
+                    s0, l0 = np.linalg.slogdet(oracle.slater_matrix(coefs, x.lattice, pos[None])[0])
+                    fd = np.zeros(3)
+                    for d in range(3):
+                        val = []
+                        for sgn in (+1.0, -1.0):
+                            trial = pos.copy()
+                            trial[k] = rnew
+                            trial[k, d] += sgn * h
+                            s1, l1 = np.linalg.slogdet(oracle.slater_matrix(coefs, x.lattice, trial[None])[0])
+                            val.append(s1 * s0 * np.exp(l1 - l0))
+                        fd[d] = (val[0] - val[1]) / (2.0 * h)
+                    got = 0.5 * F[s, k, w] * out["ratios"][s, k, w]
+                    scale = max(1.0, np.abs(fd).max())
+                    assert np.max(np.abs(got - fd)) < 1e-6 * scale, (s, k, w, got, fd)
+                    checked += 1
+                if acc[s, k, w]:
+                    pos[k] = rnew
+    assert checked >= 15
+
+
+def test_fixed_node_rule(sweep_case):
+    """moves that change the sign of the wavefunction are rejected.  With u = 0 every
+    move with R > 0 is accepted and every move with R < 0 rejected, so the sign of det A never
+    changes and log|det| telescopes over the accepted (positive) ratios; where the free run met no
+    negative ratio the flag changes nothing."""
+    x, coefs, A, B, ld, sg = sweep_case
+    zeros = np.zeros_like(x.unif)
+    fn = oracle.sweep(coefs, x.lattice, x.pos, B, ld, sg, x.delta, zeros, A=A, fixed_node=True)
+    assert np.array_equal(fn["accept"].astype(bool), fn["ratios"] > 0.0)
+    assert (fn["ratios"] < 0.0).any(), "the case should propose at least one nodal crossing"
+    assert np.array_equal(fn["sign"], sg)
+    for w in range(x.pos.shape[0]):
+        s_np, ld_np = np.linalg.slogdet(fn["A"][w])
+        assert s_np == sg[w] and abs(ld_np - fn["logdet"][w]) < 1e-9
+    free = oracle.sweep(coefs, x.lattice, x.pos, B, ld, sg, x.delta, x.unif)
+    fixed = oracle.sweep(coefs, x.lattice, x.pos, B, ld, sg, x.delta, x.unif, fixed_node=True)
+    for w in range(x.pos.shape[0]):
+        neg = (free["ratios"][:, :, w] < 0.0) & free["accept"][:, :, w].astype(bool)
+        if not neg.any():
+            assert np.array_equal(free["ratios"][:, :, w], fixed["ratios"][:, :, w])
+        else:
+            assert (fixed["ratios"][:, :, w][fixed["accept"][:, :, w].astype(bool)] > 0.0).all()
