@@ -143,7 +143,8 @@ int qmc_det_flush(qmc_det_t *det, void *stream);
  * Gaussian);  phi, grad, lap = SPO-VGL(r');  R = B_w[k] . phi;  accept iff R*R > u[s][k][w]
  * (eq. 12 with symmetric T and a determinant-only Psi, R:A8; non-finite R rejects); on accept
  * pos[w][k] = r' (stored unwrapped) and the inverse is updated as in qmc_det_accept_update.
- * Pending delayed updates are flushed at the end of every sweep.
+ * Pending delayed updates are flushed at the end of every sweep.  qmc_sweep_ex adds the fixed-node
+ * rule (L253) and the wavefunction force of every proposal (L155) as options.
  *
  *   pos            dev, double [nwalkers][nel][3], in/out.  Must be the positions the handle's
  *                  inverse corresponds to.
@@ -164,8 +165,14 @@ typedef struct qmc_sweep_opts {
     int iel_count;       /* electrons moved per sweep; 0 = nel - iel_begin                   */
     float *phi_record;   /* NULL, or dev float [nsweeps][nel][nrecord][nel]: the fp32 orbital */
     int nrecord;         /*   vector of every move of walkers 0..nrecord-1 (parity replay)   */
-    int use_graph;       /* 1: replay one electron step as a captured CUDA graph             */
-    int reserved[3];
+    int fixed_node;      /* != 0: fixed-node rule: a move that changes the   */
+                         /*   sign of the wavefunction (R < 0) is rejected whatever u is     */
+    double *force_out;   /* NULL, or dev double [nsweeps][nel][nwalkers][3]: the wavefunction */
+                         /*   force F = 2 grad log Psi_T (L155; the F of eq. 11 / eq. 13) on  */
+                         /*   the moved electron at the PROPOSED configuration,               */
+                         /*   F = 2 sum_j grad phi_j(r') B[k][j] / R, for every move          */
+                         /*   (accepted or not; 0 where R == 0)                               */
+    int reserved[2];
 } qmc_sweep_opts_t;
 
 int qmc_sweep_ex(qmc_det_t *det, const qmc_spline_t *spline, double *pos, const double *delta,

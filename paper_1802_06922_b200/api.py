@@ -28,8 +28,8 @@ PROF_KINDS = ["spo_vgl", "sm_update", "delayed_window", "delayed_accept", "delay
 
 class SweepOpts(ctypes.Structure):
     _fields_ = [("iel_begin", ctypes.c_int), ("iel_count", ctypes.c_int),
-                ("phi_record", _vp), ("nrecord", ctypes.c_int), ("use_graph", ctypes.c_int),
-                ("reserved", ctypes.c_int * 3)]
+                ("phi_record", _vp), ("nrecord", ctypes.c_int), ("fixed_node", ctypes.c_int),
+                ("force_out", _vp), ("reserved", ctypes.c_int * 2)]
 
 
 class QmcError(RuntimeError):
@@ -272,12 +272,13 @@ class Det:
 
 
 def sweep(det, pos, delta, unif, ratios_out=None, accept_out=None, forced_accept=None, iel_begin=0,
-          iel_count=0, phi_record=None, nrecord=0, stream=None):
+          iel_count=0, phi_record=None, nrecord=0, fixed_node=False, force_out=None, stream=None):
     """qmc_sweep / qmc_sweep_ex on device tensors (pos updated in place).
 
     pos double [nw][nel][3]; delta double [nsweeps][nel][nw][3]; unif double [nsweeps][nel][nw];
     ratios_out double / accept_out uint8 / forced_accept uint8: [nsweeps][nel][nw] or None;
-    phi_record float32 [nsweeps][nel][nrecord][nel] or None.
+    phi_record float32 [nsweeps][nel][nrecord][nel] or None; fixed_node: reject moves with R < 0;
+    force_out double [nsweeps][nel][nw][3] or None (F = 2 grad log|Psi| at the proposed configuration).
     """
     lib = load_library()
     nsweeps = delta.shape[0]
@@ -291,11 +292,15 @@ def sweep(det, pos, delta, unif, ratios_out=None, accept_out=None, forced_accept
     args = [det._h, det.spline._h, _dev(pos, torch.float64), _dev(delta, torch.float64),
             _dev(unif, torch.float64), nsweeps, _dev(ratios_out, torch.float64, True),
             _dev(accept_out, torch.uint8, True), _dev(forced_accept, torch.uint8, True)]
-    if iel_begin or iel_count or phi_record is not None:
+    if iel_begin or iel_count or phi_record is not None or fixed_node or force_out is not None:
         if phi_record is not None and tuple(phi_record.shape) != (nsweeps, det.nel, nrecord, det.nel):
             raise QmcError("phi_record must be [nsweeps][nel][nrecord][nel]")
+        if force_out is not None and tuple(force_out.shape) != tuple(unif.shape) + (3,):
+            raise QmcError("force_out must be [nsweeps][nel][nw][3]")
         opts = SweepOpts(int(iel_begin), int(iel_count),
-                         None if phi_record is None else phi_record.data_ptr(), int(nrecord), 0)
+                         None if phi_record is None else phi_record.data_ptr(), int(nrecord),
+                         1 if fixed_node else 0,
+                         None if force_out is None else _dev(force_out, torch.float64).value)
         rc = lib.qmc_sweep_ex(*args, ctypes.byref(opts), _stream(stream))
         _check(rc, "qmc_sweep_ex")
     else:

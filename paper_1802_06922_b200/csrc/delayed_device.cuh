@@ -14,7 +14,9 @@ cudaError_t flush_ring_launch(qmc_det *d, cudaStream_t s);    // enqueue it
 int delayed_max_rank(int ld);                                // largest K whose window fits shared memory
 // One window of qmc_sweep in delayed mode: electrons iel0 .. iel0+nb-1 (nb <= delay rank), whose
 // SPO-VGL is in d->vgl; ratios, decisions, moves and the flush.  Pointers are offset to the first step.
+// fixed_node: reject R < 0; force_out: NULL or [nb][nw][3], F = 2 grad log Psi_T at the proposed configuration.
 int delayed_sweep_window(qmc_det *d, double *pos, const double *delta, const double *unif, int iel0, int nb,
-                         double *ratios_out, unsigned char *accept_out, const unsigned char *forced, cudaStream_t s);
+                         double *ratios_out, unsigned char *accept_out, const unsigned char *forced,
+                         int fixed_node, double *force_out, cudaStream_t s);
 
 }  // namespace qmc

@@ -57,17 +57,21 @@ __global__ void __launch_bounds__(256) spo_batch_kernel(SpoBatchArgs a)
 }
 
 // S3 for the rank-1 path: R_w = B_w[iel] . phi_w (fp64, fixed order) and a copy of row iel, so that
-// the update kernel can overwrite B in place.  One block per walker.
+// the update kernel can overwrite B in place.  One block per walker.  With force_out the three
+// gradient vectors of the proposal (phi + np, + 2 np, + 3 np) are contracted with the same row:
+// F = 2 grad log Psi_T at the proposed configuration = 2 (B[iel] . grad phi) / R.
 __global__ void __launch_bounds__(256)
 ratio_rowcopy_kernel(const double *__restrict__ B, int nel, int ld, int iel, const float *__restrict__ phi,
-                     size_t ldphi, double *__restrict__ rowk, double *__restrict__ rpart)
+                     size_t ldphi, int np, double *__restrict__ rowk, double *__restrict__ rpart,
+                     double *__restrict__ force_out)
 {
     __shared__ double red[33];
     const int w = blockIdx.x;
     const double2 *row = reinterpret_cast<const double2 *>(B + ((size_t)w * nel + iel) * ld);
-    const float2 *ph = reinterpret_cast<const float2 *>(phi + (size_t)w * ldphi);
+    const float *pw = phi + (size_t)w * ldphi;
+    const float2 *ph = reinterpret_cast<const float2 *>(pw);
     double2 *dst = reinterpret_cast<double2 *>(rowk + (size_t)w * ld);
-    double acc = 0.0;
+    double acc = 0.0, g[3] = {0.0, 0.0, 0.0};
     for (int j = threadIdx.x; j < ld / 2; j += 256) {
         const double2 b = row[j];
         dst[j] = b;
@@ -75,10 +79,25 @@ ratio_rowcopy_kernel(const double *__restrict__ B, int nel, int ld, int iel, con
             const float2 f = ph[j];
             acc = fma(b.x, (double)f.x, acc);
             acc = fma(b.y, (double)f.y, acc);
+            if (force_out) {
+#pragma unroll
+                for (int d = 0; d < 3; ++d) {
+                    const float2 q = reinterpret_cast<const float2 *>(pw + (size_t)(1 + d) * np)[j];
+                    g[d] = fma(b.x, (double)q.x, g[d]);
+                    g[d] = fma(b.y, (double)q.y, g[d]);
+                }
+            }
         }
     }
     acc = block_sum(acc, red);
     if (threadIdx.x == 0) rpart[(size_t)w * kRatioTilesMax] = acc;
+    if (force_out) {
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            const double gd = block_sum(g[d], red);
+            if (threadIdx.x == 0) force_out[3 * (size_t)w + d] = acc != 0.0 ? 2.0 * gd / acc : 0.0;
+        }
+    }
 }
 
 int spo_batch_vgl(qmc_det *d, const qmc_spline *sp, const double *pos, const double *delta, int iel0, int nb,
@@ -109,8 +128,11 @@ static int sweep_impl(qmc_det *d, const qmc_spline *sp, double *pos, const doubl
     const int nw = d->nw, nel = d->nel;
     int k0 = 0, kn = nel;
     float *rec = nullptr;
-    int nrec = 0;
+    int nrec = 0, fixed_node = 0;
+    double *force = nullptr;
     if (opts) {
+        fixed_node = opts->fixed_node != 0;
+        force = opts->force_out;
         k0 = opts->iel_begin;
         kn = opts->iel_count ? opts->iel_count : nel - k0;
         rec = opts->phi_record;
@@ -136,7 +158,8 @@ static int sweep_impl(qmc_det *d, const qmc_spline *sp, double *pos, const doubl
                     int rc = delayed_sweep_window(d, pos, delta + 3 * mv, unif + mv, k, nb,
                                                   ratios_out ? ratios_out + mv : nullptr,
                                                   accept_out ? accept_out + mv : nullptr,
-                                                  forced ? forced + mv : nullptr, s);
+                                                  forced ? forced + mv : nullptr, fixed_node,
+                                                  force ? force + 3 * mv : nullptr, s);
                     if (rc) return rc;
                 }
                 continue;
@@ -144,7 +167,8 @@ static int sweep_impl(qmc_det *d, const qmc_spline *sp, double *pos, const doubl
             const float *phi = d->vgl + slot * slot_stride;
             // K2: ratio + row copy, K3: decision + rank-1 update
             prof_start(d, kProfRatio, s);
-            ratio_rowcopy_kernel<<<nw, 256, 0, s>>>(d->B, nel, d->ld, k, phi, (size_t)5 * d->np, d->rowk, d->rpart);
+            ratio_rowcopy_kernel<<<nw, 256, 0, s>>>(d->B, nel, d->ld, k, phi, (size_t)5 * d->np, d->np, d->rowk, d->rpart,
+                                                    force ? force + 3 * mv : nullptr);
             prof_stop(d, s);
             QMC_LAUNCHED();
             UpdateArgs u{};
@@ -153,6 +177,7 @@ static int sweep_impl(qmc_det *d, const qmc_spline *sp, double *pos, const doubl
             u.rpart = d->rpart; u.ntiles = 1;
             u.unif = unif + mv;
             u.forced = forced ? forced + mv : nullptr;
+            u.fixed_node = fixed_node;
             u.ratios_out = ratios_out ? ratios_out + mv : nullptr;
             u.accept_out = accept_out ? accept_out + mv : nullptr;
             u.pos = pos; u.delta = delta + 3 * mv;

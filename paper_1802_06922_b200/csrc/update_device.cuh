@@ -20,6 +20,7 @@ struct UpdateArgs {
     int ntiles;
     const double *unif;           // [nw]
     const unsigned char *forced;  // [nw] or NULL
+    int fixed_node;               // reject R < 0
     double *ratios_out;           // [nw] or NULL
     unsigned char *accept_out;    // [nw] or NULL
     double *pos;                  // [nw][nel][3]
@@ -49,7 +50,7 @@ __global__ void __launch_bounds__(kUpdThreads) sm_update_kernel(UpdateArgs a)
     if (DECIDE) {
         R = 0.0;
         for (int t = 0; t < a.ntiles; ++t) R += a.rpart[(size_t)w * kRatioTilesMax + t];
-        acc = a.forced ? (a.forced[w] != 0) : metropolis(R, a.unif[w]);
+        acc = a.forced ? (a.forced[w] != 0) : (metropolis(R, a.unif[w]) && !(a.fixed_node && R < 0.0));
     } else {
         R = a.ratio[w];
         acc = a.accept[w] != 0;

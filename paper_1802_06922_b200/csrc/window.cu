@@ -31,6 +31,8 @@ struct WindowArgs {
     const float *vgl;             // [nb][nw][5][np] SPO-VGL of the window's proposals (values first)
     const double *unif;           // [nb][nw]
     const unsigned char *forced;  // [nb][nw] or NULL
+    int fixed_node;               // reject R < 0
+    double *force_out;            // [nb][nw][3] or NULL: F = 2 grad log Psi_T at the proposed configuration
     double *ratios_out;           // [nb][nw] or NULL
     unsigned char *accept_out;    // [nb][nw] or NULL
     double *pos;                  // [nw][nel][3]
@@ -44,26 +46,18 @@ struct WindowArgs {
     double *win_rows;             // [nw][K][ld]   row l <- R'[l]
 };
 
-// One block per walker, 8 warps.  Phase 1: warp q contracts the 16-column chunks q, q+8, ... with
-// DMMA.8x8x4 (the contraction index inside a chunk is permuted so that one lane's float4 / 2 x
-// double2 serve four k-steps).  Phase 2: fixed-order sum of the 8 partial G.  Phase 3: warp 0
-// walks the nb steps.  Phase 4: R' = S^-T Rows, 8-column tiles over the warps.
+// G[i][j] = x_i . B0[iel0 + j] for the nb vectors x_i = x0 + i * vstep (fp32) of one walker, into
+// shared memory: warp q contracts the 16-column chunks q, q+8, ... with DMMA.8x8x4 (the contraction
+// index inside a chunk is permuted so that one lane's float4 / 2 x double2 serve four k-steps), then
+// the 8 partial G are summed in a fixed order.  Ends with a __syncthreads().
 template <int KMAX>
-__global__ void __launch_bounds__(kWinThreads) delayed_window_kernel(WindowArgs a)
+__device__ __forceinline__ void window_contract(const float *x0, size_t vstep, const double *b0, int nb, int ld,
+                                                int np, double *G_dst)
 {
     constexpr int MB = KMAX / 8;
     constexpr int GS = KMAX + 1;
-    __shared__ double G_s[KMAX * GS];
-    __shared__ double sinv_s[KMAX * GS];
-    __shared__ long long rowoff_s[KMAX];
-    __shared__ int p_s;
-    const int w = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int g = lane >> 2, t = lane & 3;
-    const int nb = a.nb, ld = a.ld, np = a.np, K = a.K;
-    const size_t vstep = (size_t)a.nw * 5 * np;             // stride between steps in vgl
-    const float *v0 = a.vgl + (size_t)w * 5 * np;
-    const double *b0 = a.B + ((size_t)w * a.nel + a.iel0) * ld;
-
     double acc[MB][MB][2];
 #pragma unroll
     for (int i = 0; i < MB; ++i)
@@ -87,7 +81,7 @@ __global__ void __launch_bounds__(kWinThreads) delayed_window_kernel(WindowArgs 
         for (int ib = 0; ib < MB; ++ib) {
             const int i = 8 * ib + g;
             float4 f = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (i < nb) f = *reinterpret_cast<const float4 *>(v0 + (size_t)i * vstep + col);
+            if (i < nb) f = *reinterpret_cast<const float4 *>(x0 + (size_t)i * vstep + col);
             av[ib][0] = f.x; av[ib][1] = f.y; av[ib][2] = f.z; av[ib][3] = f.w;
         }
 #pragma unroll
@@ -98,20 +92,43 @@ __global__ void __launch_bounds__(kWinThreads) delayed_window_kernel(WindowArgs 
                 for (int jb = 0; jb < MB; ++jb)
                     if (8 * ib < nb && 8 * jb < nb) dmma884(acc[ib][jb][0], acc[ib][jb][1], av[ib][s], bv[jb][s]);
     }
-    // ---- phase 2: G = sum over warps, fixed order
     for (int q = 0; q < kWinThreads / 32; ++q) {
         if (warp == q) {
 #pragma unroll
             for (int ib = 0; ib < MB; ++ib)
 #pragma unroll
                 for (int jb = 0; jb < MB; ++jb) {
-                    double *dst = G_s + (8 * ib + g) * GS + 8 * jb + 2 * t;
+                    double *dst = G_dst + (8 * ib + g) * GS + 8 * jb + 2 * t;
                     if (q == 0) { dst[0] = acc[ib][jb][0]; dst[1] = acc[ib][jb][1]; }
                     else { dst[0] += acc[ib][jb][0]; dst[1] += acc[ib][jb][1]; }
                 }
         }
         __syncthreads();
     }
+}
+
+// One block per walker, 8 warps.  Phases 1-2: G (and, with FORCE, the same contraction for the three
+// gradient vectors of every proposal).  Phase 3: warp 0 walks the nb steps.  Phase 4: R' = S^-T Rows,
+// 8-column tiles over the warps.
+template <int KMAX, bool FORCE>
+__global__ void __launch_bounds__(kWinThreads) delayed_window_kernel(WindowArgs a)
+{
+    constexpr int GS = KMAX + 1;
+    __shared__ double G_s[KMAX * GS];
+    __shared__ double Gd_s[FORCE ? 3 * KMAX * GS : 1];     // Gd[d][i][j] = d_d phi(r'_i) . B0[iel0 + j]
+    __shared__ double sinv_s[KMAX * GS];
+    __shared__ long long rowoff_s[KMAX];
+    __shared__ int p_s;
+    const int w = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int nb = a.nb, ld = a.ld, np = a.np, K = a.K;
+    const size_t vstep = (size_t)a.nw * 5 * np;             // stride between steps in vgl
+    const float *v0 = a.vgl + (size_t)w * 5 * np;
+    const double *b0 = a.B + ((size_t)w * a.nel + a.iel0) * ld;
+
+    window_contract<KMAX>(v0, vstep, b0, nb, ld, np, G_s);
+    if (FORCE)
+        for (int d = 0; d < 3; ++d) window_contract<KMAX>(v0 + (size_t)(1 + d) * np, vstep, b0, nb, ld, np, Gd_s + d * KMAX * GS);
+
     // ---- phase 3: the nb steps in sequence; lane m owns accepted move m (its step index `mine`).
     // Everything that lives in global memory stays outside the sequential loop: lane i fetches the
     // uniform / forced decision of step i before it and writes ratio, decision and the moved
@@ -122,6 +139,7 @@ __global__ void __launch_bounds__(kWinThreads) delayed_window_kernel(WindowArgs 
         const double u_l = (step_l && !a.forced) ? a.unif[mv_l] : 0.0;
         const int f_l = (step_l && a.forced) ? (a.forced[mv_l] != 0) : 0;
         double R_l = 1.0;                                             // ratio of step `lane`
+        double F_l[3] = {0.0, 0.0, 0.0};                              // force of step `lane`
         unsigned acc_mask = 0;                                        // accepted steps (same in every lane)
         int p = 0, mine = 0;
         for (int i = 0; i < nb; ++i) {
@@ -138,8 +156,18 @@ __global__ void __launch_bounds__(kWinThreads) delayed_window_kernel(WindowArgs 
             const double R = G_s[i * GS + i] - warp_sum(x * y);
             const double u_i = __shfl_sync(0xffffffffu, u_l, i);
             const int f_i = __shfl_sync(0xffffffffu, f_l, i);
-            const bool acc_w = a.forced ? (f_i != 0) : metropolis(R, u_i);
+            const bool acc_w = a.forced ? (f_i != 0) : (metropolis(R, u_i) && !(a.fixed_node && R < 0.0));
             if (lane == i) R_l = R;
+            if (FORCE) {
+                // grad phi(r'_i) . B_cur[k_i] = gd - xg^T S^-1 c with the same y = S^-1 c as the ratio
+#pragma unroll
+                for (int d = 0; d < 3; ++d) {
+                    const double *Gd = Gd_s + d * KMAX * GS;
+                    const double xg = lane < p ? Gd[i * GS + mine] : 0.0;
+                    const double gd = Gd[i * GS + i] - warp_sum(xg * y);
+                    if (lane == i) F_l[d] = R != 0.0 ? 2.0 * gd / R : 0.0;
+                }
+            }
             if (!acc_w) continue;
             acc_mask |= 1u << i;
             const double rinv = 1.0 / R;
@@ -162,6 +190,11 @@ __global__ void __launch_bounds__(kWinThreads) delayed_window_kernel(WindowArgs 
         if (step_l) {
             if (a.ratios_out) a.ratios_out[mv_l] = R_l;
             if (a.accept_out) a.accept_out[mv_l] = acc_l ? 1 : 0;
+            if (FORCE) {
+                a.force_out[3 * mv_l + 0] = F_l[0];
+                a.force_out[3 * mv_l + 1] = F_l[1];
+                a.force_out[3 * mv_l + 2] = F_l[2];
+            }
         }
         if (acc_l) {
             double *r = a.pos + ((size_t)w * a.nel + a.iel0 + lane) * 3;
@@ -194,7 +227,8 @@ __global__ void __launch_bounds__(kWinThreads) delayed_window_kernel(WindowArgs 
 }
 
 int delayed_sweep_window(qmc_det *d, double *pos, const double *delta, const double *unif, int iel0, int nb,
-                         double *ratios_out, unsigned char *accept_out, const unsigned char *forced, cudaStream_t s)
+                         double *ratios_out, unsigned char *accept_out, const unsigned char *forced,
+                         int fixed_node, double *force_out, cudaStream_t s)
 {
     if (d->host_pending) {        // rows pending from standalone qmc_det_accept_update calls
         int rc = delayed_flush_reset_host(d, s);
@@ -205,14 +239,21 @@ int delayed_sweep_window(qmc_det *d, double *pos, const double *delta, const dou
     a.iel0 = iel0; a.nb = nb;
     a.vgl = d->vgl;
     a.unif = unif; a.forced = forced; a.ratios_out = ratios_out; a.accept_out = accept_out;
+    a.fixed_node = fixed_node; a.force_out = force_out;
     a.pos = pos; a.delta = delta;
     a.logdet = d->logdet; a.sign = d->sign; a.naccept = d->naccept;
     a.win_count = d->win_count; a.win_iel = d->win_iel; a.win_slot = d->win_slot;
     a.win_rows = d->win_rows;
     prof_start(d, kProfDelayedRatio, s);
-    if (a.K <= 8) delayed_window_kernel<8><<<d->nw, kWinThreads, 0, s>>>(a);
-    else if (a.K <= 16) delayed_window_kernel<16><<<d->nw, kWinThreads, 0, s>>>(a);
-    else delayed_window_kernel<32><<<d->nw, kWinThreads, 0, s>>>(a);
+    if (force_out) {
+        if (a.K <= 8) delayed_window_kernel<8, true><<<d->nw, kWinThreads, 0, s>>>(a);
+        else if (a.K <= 16) delayed_window_kernel<16, true><<<d->nw, kWinThreads, 0, s>>>(a);
+        else delayed_window_kernel<32, true><<<d->nw, kWinThreads, 0, s>>>(a);
+    } else {
+        if (a.K <= 8) delayed_window_kernel<8, false><<<d->nw, kWinThreads, 0, s>>>(a);
+        else if (a.K <= 16) delayed_window_kernel<16, false><<<d->nw, kWinThreads, 0, s>>>(a);
+        else delayed_window_kernel<32, false><<<d->nw, kWinThreads, 0, s>>>(a);
+    }
     prof_stop(d, s);
     QMC_LAUNCHED();
     // the flush takes the vectors of the accepted steps straight from the SPO-VGL scratch

@@ -339,3 +339,85 @@ def test_delayed_large_n_equals_rank1(nel, K, nw, count, env, monkeypatch):
     assert float((a[4][0] - b[4][0]).abs().max()) < 1e-8
     assert torch.equal(a[4][1], b[4][1]) and torch.equal(a[4][2], b[4][2])
     spline.destroy()
+
+
+# --------------------------------------------- NEXT-1: wavefunction force and fixed-node rejection
+def _force_run(x, K, fixed_node=False, unif=None):
+    spline = api.Spline.create(x.coefs.to(P.dev()), x.lattice)
+    pos0, delta = P.to_dev(x.pos), P.to_dev(x.delta)
+    unif_t = P.to_dev(x.unif if unif is None else unif)
+    nsw, nel, nw = x.unif.shape
+    A0 = P.gpu_slater(spline, pos0)
+    det = api.Det.init(spline, pos0, delay_rank=K)
+    _, sg0, _ = (t.cpu().numpy() for t in det.get_stats())
+    pos = pos0.clone()
+    R = torch.zeros_like(unif_t)
+    acc = torch.zeros(unif_t.shape, dtype=torch.uint8, device=P.dev())
+    F = torch.full(tuple(unif_t.shape) + (3,), float("nan"), dtype=torch.float64, device=P.dev())
+    rec = torch.zeros((nsw, nel, nw, nel), dtype=torch.float32, device=P.dev())
+    api.sweep(det, pos, delta, unif_t, ratios_out=R, accept_out=acc, phi_record=rec, nrecord=nw,
+              fixed_node=fixed_node, force_out=F)
+    torch.cuda.synchronize()
+    _, sgf, _ = (t.cpu().numpy() for t in det.get_stats())
+    out = dict(A0=A0, R=R.cpu().numpy(), acc=acc.cpu().numpy(), F=F.cpu().numpy(), rec=rec.cpu().numpy(),
+               sign0=sg0, sign=sgf, pos=pos.cpu().numpy())
+    det.destroy()
+    spline.destroy()
+    return out
+
+
+@pytest.mark.parametrize("case,K", [("tiny", 0), ("tiny", 3), ("ragged37_skew", 0), ("ragged37_skew", 16),
+                                    ("n130_two_tiles", 0), ("n130_two_tiles", 7), ("small", 16)])
+def test_wavefunction_force_parity(case, K):
+    """qmc_sweep_ex force_out: F = 2 grad log Psi_T of the moved electron at the
+    proposed configuration, for every move, against the oracle replaying the GPU's decisions and
+    fp32 orbital vectors (its gradients come from its own fp64 spline).  Compared as F R / 2 =
+    grad_r' R, which stays smooth next to a node: the north_star gradient tolerance (2e-5 of
+    max|grad phi|) propagated through the dot product with row k of B, plus 1e-5 relative."""
+    x = CASES[case]()
+    g = _force_run(x, K)
+    assert np.isfinite(g["F"]).all()
+    coefs_np = x.coefs_numpy()
+    B0, ld0, sg0 = P.oracle_binv(g["A0"])
+    rep = oracle.sweep(coefs_np, x.lattice, x.pos, B0, ld0, sg0, x.delta, x.unif, forced=g["acc"], phi_in=g["rec"],
+                       want_force=True, want_bnorm=True, nthreads=oracle.max_threads())
+    _, go, _ = oracle.spline_vgl(coefs_np, x.lattice, x.pos.reshape(-1, 3)[:64])
+    gmax = float(np.max(np.abs(go)))
+    gR_g = 0.5 * g["F"] * g["R"][..., None]
+    gR_o = 0.5 * rep["force"] * rep["ratios"][..., None]
+    tol = rep["bnorm"][..., None] * 2e-5 * gmax + 1e-5 * np.abs(gR_o) + 1e-12
+    worst = float(np.max(np.abs(gR_g - gR_o) / tol))
+    big = np.abs(rep["ratios"]) > 0.1
+    rel = float(np.max(np.abs(g["F"] - rep["force"])[big] / np.maximum(1.0, np.abs(rep["force"])[big])))
+    print(case, K, "grad R err / tol", worst, "| F rel err where |R| > 0.1:", rel)
+    assert worst < 1.0
+    assert rel < 1e-3
+
+
+def test_force_delayed_equals_rank1():
+    x = CASES["n130_two_tiles"]()
+    a, b, c = _force_run(x, 0), _force_run(x, 5), _force_run(x, 16)
+    for o in (b, c):
+        assert np.array_equal(a["acc"], o["acc"])
+        assert np.max(np.abs(a["F"] - o["F"]) / np.maximum(1.0, np.abs(a["F"]))) < 1e-8
+
+
+@pytest.mark.parametrize("case,K", [("ragged37_skew", 0), ("ragged37_skew", 4), ("n130_two_tiles", 16)])
+def test_fixed_node_rejection(case, K):
+    """fixed_node: with u = 0 a move is accepted iff R > 0, so the sign of the
+    determinant never changes; with the seeded uniforms the decisions equal the oracle's (same rule,
+    identical orbital vectors) outside the 1e-6 band, and nothing else changes where no nodal
+    crossing was proposed."""
+    x = CASES[case]()
+    zeros = np.zeros_like(x.unif)
+    g0 = _force_run(x, K, fixed_node=True, unif=zeros)
+    assert (g0["R"] < 0).any(), "the case should propose at least one nodal crossing"
+    assert np.array_equal(g0["acc"].astype(bool), g0["R"] > 0.0)
+    assert np.array_equal(g0["sign"], g0["sign0"])
+    g = _force_run(x, K, fixed_node=True)
+    assert (g["R"][g["acc"].astype(bool)] > 0.0).all() and np.array_equal(g["sign"], g["sign0"])
+    B0, ld0, sg0 = P.oracle_binv(g["A0"])
+    dummy = np.zeros((1, 1, 1, x.cfg.norb), np.float32)
+    rep = oracle.sweep(dummy, x.lattice, x.pos, B0, ld0, sg0, x.delta, x.unif, phi_in=g["rec"], fixed_node=True,
+                       nthreads=oracle.max_threads())
+    P.compare_decisions(g["acc"], g["R"], rep["accept"], rep["ratios"], x.unif)
