@@ -126,9 +126,15 @@ def cpu_sample(x, coefs_np, target_s=15.0):
     nwc = nthreads * per_thread
     if per_thread > 1:
         pos, B, ld, sg, delta, unif = setup(nwc)
-    t0 = time.perf_counter()
-    out = oracle.sweep(coefs_np, x.lattice, pos, B, ld, sg, delta, unif, iel_count=m, nthreads=nthreads)
-    dt = time.perf_counter() - t0
+    for attempt in range(2):
+        t0 = time.perf_counter()
+        out = oracle.sweep(coefs_np, x.lattice, pos, B, ld, sg, delta, unif, iel_count=m, nthreads=nthreads)
+        dt = time.perf_counter() - t0
+        grow = int(min(x.pos.shape[0] // nthreads, per_thread * target_s / max(dt, 1e-3)))
+        if attempt or dt >= 0.6 * target_s or grow <= per_thread:
+            break
+        per_thread, nwc = grow, nthreads * grow          # the probe over-estimated the cost: enlarge the sample once
+        pos, B, ld, sg, delta, unif = setup(nwc)
     acc = float(out["accept"][0, :m].mean())
     text = (f"{nwc} walkers x first {m} electron moves of one sweep of config '{x.cfg.name}' "
             f"(accept {acc:.2f}), {nthreads} OpenMP threads, {dt:.1f} s")
