@@ -11,6 +11,7 @@ from .binding import (  # noqa: F401
     det_ratio,
     sm_update,
     slater_matrix,
+    det_kinetic,
     init_walkers,
     sweep,
     max_threads,

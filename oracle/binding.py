@@ -55,6 +55,8 @@ def _load():
         lib.orc_init_walkers.restype = ctypes.c_int
         lib.orc_init_walkers.argtypes = ([ctypes.c_int] * 4 + [_dp, _fp, ctypes.c_int, ctypes.c_int,
                                          _dp, _dp, _dp, _dp, _ip, ctypes.c_int])
+        lib.orc_det_kinetic.restype = ctypes.c_int
+        lib.orc_det_kinetic.argtypes = ([ctypes.c_int] * 4 + [_dp, _fp, ctypes.c_int, ctypes.c_int] + [_dp] * 6)
         lib.orc_max_threads.restype = ctypes.c_int
         lib.orc_max_threads.argtypes = []
         _lib = lib
@@ -158,6 +160,24 @@ def slater_matrix(coefs, lattice, pos):
                                _d(pos), _d(A))
     _check(rc, "slater_matrix")
     return A
+
+
+def det_kinetic(coefs, lattice, pos, B):
+    """Kinetic term of the local energy of Psi = det A (eq. 3, eq. 37): returns a dict with
+    grad [nw][nel][3] = grad_i det / det, lap [nw][nel] = lap_i det / det, one [nw][nel] (= 1 when B
+    is the transposed inverse at pos) and ekin [nw] = -1/2 sum_i lap."""
+    lib = _load()
+    coefs = _coefs(coefs)
+    nx, ny, nz, norb = coefs.shape
+    lat = _c64(lattice).reshape(9)
+    pos = _c64(pos)
+    nw, nel, _ = pos.shape
+    B = _c64(B, (nw, nel, nel))
+    grad, lap, one, ekin = np.empty((nw, nel, 3)), np.empty((nw, nel)), np.empty((nw, nel)), np.empty(nw)
+    rc = lib.orc_det_kinetic(nx, ny, nz, norb, _d(lat), coefs.ctypes.data_as(_fp), nw, nel, _d(pos), _d(B),
+                             _d(grad), _d(lap), _d(one), _d(ekin))
+    _check(rc, "det_kinetic")
+    return dict(grad=grad, lap=lap, one=one, ekin=ekin)
 
 
 def init_walkers(coefs, lattice, pos, nthreads=1, want_A=False):

@@ -458,6 +458,56 @@ int orc_init_walkers(int nx, int ny, int nz, int norb, const double lattice[9], 
     return rc_all;
 }
 
+/* ---------------------------------------------------------------------------
+ * orc_det_kinetic -- the determinant's contribution to the kinetic term of the local energy,
+ * E_L,kin = Psi^-1 (-1/2 sum_i lap_i) Psi (eq. 3 first term, eq. 37; L401: collected
+ * after all walkers have advanced one step).  For Psi = det A, A_ij = phi_j(r_i), only row i of A
+ * depends on r_i, so by the cofactor expansion along that row
+ *     grad_i det A / det A = sum_j grad phi_j(r_i) (A^-1)[j][i] = sum_j grad phi_j(r_i) B[i][j]
+ *     lap_i  det A / det A = sum_j lap  phi_j(r_i) B[i][j]
+ * and, as a consistency check of (pos, B), one[w][i] = sum_j phi_j(r_i) B[i][j] = 1.
+ *
+ *   pos  [nw][nel][3], B [nw][nel][nel] = (A^-1)^T
+ *   grad_out [nw][nel][3], lap_out [nw][nel], one_out [nw][nel] (any may be NULL)
+ *   ekin_out [nw] = -1/2 sum_i lap_out[w][i]                      (may be NULL)
+ */
+int orc_det_kinetic(int nx, int ny, int nz, int norb, const double lattice[9], const float *coefs,
+                    int nw, int nel, const double *pos, const double *B, double *grad_out,
+                    double *lap_out, double *one_out, double *ekin_out)
+{
+    if (nel != norb || nw < 0) return -1;
+    double *v = (double *)malloc((size_t)5 * nel * sizeof(double));
+    if (!v) return -2;
+    double *g = v + nel, *l = v + (size_t)4 * nel;
+    int rc = 0;
+    for (int w = 0; w < nw && rc == 0; ++w) {
+        double ek = 0.0;
+        for (int i = 0; i < nel && rc == 0; ++i) {
+            const double *Bi = B + ((size_t)w * nel + i) * nel;
+            rc = orc_spline_vgl(nx, ny, nz, norb, lattice, coefs, 1, pos + ((size_t)w * nel + i) * 3, v, g, l);
+            if (rc) break;
+            double one = 0.0, gx = 0.0, gy = 0.0, gz = 0.0, lp = 0.0;
+            for (int j = 0; j < nel; ++j) {
+                one += v[j] * Bi[j];
+                gx += g[j] * Bi[j];
+                gy += g[(size_t)nel + j] * Bi[j];
+                gz += g[(size_t)2 * nel + j] * Bi[j];
+                lp += l[j] * Bi[j];
+            }
+            if (grad_out) {
+                double *go = grad_out + ((size_t)w * nel + i) * 3;
+                go[0] = gx; go[1] = gy; go[2] = gz;
+            }
+            if (lap_out) lap_out[(size_t)w * nel + i] = lp;
+            if (one_out) one_out[(size_t)w * nel + i] = one;
+            ek += lp;
+        }
+        if (ekin_out) ekin_out[w] = -0.5 * ek;
+    }
+    free(v);
+    return rc;
+}
+
 int orc_max_threads(void)
 {
 #ifdef _OPENMP

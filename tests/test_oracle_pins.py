@@ -480,3 +480,36 @@ def test_fixed_node_rule(sweep_case):
             assert np.array_equal(free["ratios"][:, :, w], fixed["ratios"][:, :, w])
         else:
             assert (fixed["ratios"][:, :, w][fixed["accept"][:, :, w].astype(bool)] > 0.0).all()
+
+
+def test_det_kinetic_against_finite_differences(sweep_case):
+    """Kinetic term of the local energy of Psi = det A (eq. 3 first term, eq. 37):
+    grad_i det / det and lap_i det / det for every electron.  Pin independent of the cofactor formula:
+    first and second central differences of det A(r_i +- h e_d) / det A with the determinants taken
+    by numpy from Slater matrices at shifted positions; plus sum_j phi_j(r_i) B[i][j] = 1."""
+    x, coefs, A, B, ld, sg = sweep_case
+    out = oracle.det_kinetic(coefs, x.lattice, x.pos, B)
+    assert np.max(np.abs(out["one"] - 1.0)) < 1e-10
+    assert np.allclose(out["ekin"], -0.5 * out["lap"].sum(axis=1), rtol=0, atol=1e-9 * np.abs(out["lap"]).sum())
+    nw, nel, _ = x.pos.shape
+    h = 2e-4
+    for w in range(nw):
+        s0, l0 = np.linalg.slogdet(oracle.slater_matrix(coefs, x.lattice, x.pos[w][None])[0])
+        for i in range(0, nel, 5):
+            grad_fd, lap_fd = np.zeros(3), 0.0
+            for d in range(3):
+                r = []
+                for sgn in (+1.0, -1.0):
+                    trial = x.pos[w].copy()
+                    trial[i, d] += sgn * h
+                    s1, l1 = np.linalg.slogdet(oracle.slater_matrix(coefs, x.lattice, trial[None])[0])
+                    r.append(s1 * s0 * np.exp(l1 - l0))
+                grad_fd[d] = (r[0] - r[1]) / (2.0 * h)
+                lap_fd += (r[0] - 2.0 + r[1]) / (h * h)
+            gscale = max(1.0, np.abs(grad_fd).max())
+            assert np.max(np.abs(out["grad"][w, i] - grad_fd)) < 1e-6 * gscale, (w, i, out["grad"][w, i], grad_fd)
+            lscale = max(1.0, abs(lap_fd))
+            assert abs(out["lap"][w, i] - lap_fd) < 2e-5 * lscale, (w, i, out["lap"][w, i], lap_fd)
+    # a wrong inverse shows in `one`
+    bad = oracle.det_kinetic(coefs, x.lattice, x.pos, np.roll(B, 1, axis=1))
+    assert np.max(np.abs(bad["one"] - 1.0)) > 1e-3
