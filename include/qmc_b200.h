@@ -203,6 +203,24 @@ int qmc_det_get_stats(qmc_det_t *det, double *logdet, int *sign, long long *nacc
 int qmc_det_info(const qmc_det_t *det, int *nwalkers, int *nel, int *ld, int *delay_rank);
 
 /* ---------------------------------------------------------------------------------------
+ * qmc_det_kinetic -- the determinant's kinetic term of the local energy, eq. 3 (first
+ * term, -1/2 sum_i lap_i) and eq. 37 (E_L,n = Psi_T^-1 H_n Psi_T), "collected after all Monte Carlo
+ * walkers have advanced one step" (L401).  For Psi = det A only row i of A depends on r_i:
+ *     grad_out[w][i][:] = grad_i det A / det A = sum_j grad phi_j(r_i) B[i][j]
+ *     lap_out[w][i]     = lap_i  det A / det A = sum_j lap  phi_j(r_i) B[i][j]
+ *     one_out[w][i]     = sum_j phi_j(r_i) B[i][j]        (= 1 when B is the inverse at pos)
+ *     ekin_out[w]       = -1/2 sum_i lap_out[w][i]         (Hartree; determinant-only Psi)
+ * The SPO-VGL of the CURRENT positions is evaluated in fp32 by the sweep's batched gather kernel
+ * and contracted in fp64 (fixed order).  Pending delayed updates are flushed first.
+ *
+ *   pos       dev, double [nwalkers][nel][3]: the positions the handle's inverse corresponds to
+ *   grad_out  dev, double [nwalkers][nel][3] or NULL;   lap_out, one_out  dev, double [nwalkers][nel] or NULL
+ *   ekin_out  dev, double [nwalkers] or NULL            (at least one output must be given)
+ */
+int qmc_det_kinetic(qmc_det_t *det, const qmc_spline_t *spline, const double *pos, double *grad_out,
+                    double *lap_out, double *one_out, double *ekin_out, void *stream);
+
+/* ---------------------------------------------------------------------------------------
  * Per-kernel timing of qmc_sweep* (bench.py's roofline): with profiling enabled every kernel
  * launch of a sweep is bracketed by CUDA events on the launching stream.
  *   qmc_det_profile(det, 1)   enable and reset;  (det, 0) disable

@@ -21,7 +21,7 @@ EXPORTS = [
     "qmc_det_init", "qmc_det_destroy", "qmc_det_ratio", "qmc_det_accept_update", "qmc_det_flush",
     "qmc_sweep", "qmc_sweep_ex", "qmc_sweep_host", "qmc_det_get_inverse", "qmc_det_set_inverse",
     "qmc_det_get_stats", "qmc_det_info", "qmc_launch_count", "qmc_det_profile", "qmc_det_profile_read",
-    "qmc_probe_fp64_dmma",
+    "qmc_probe_fp64_dmma", "qmc_det_kinetic",
 ]
 PROF_KINDS = ["spo_vgl", "sm_update", "delayed_window", "delayed_accept", "delayed_flush", "ratio_rowcopy"]
 
@@ -71,6 +71,7 @@ def load_library(path=None):
         "qmc_det_profile": [_vp, i],
         "qmc_det_profile_read": [_vp, ctypes.POINTER(d), ctypes.POINTER(ctypes.c_longlong)],
         "qmc_probe_fp64_dmma": [ctypes.POINTER(d), _vp],
+        "qmc_det_kinetic": [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp],
     }
     for name, args in sigs.items():
         fn = getattr(lib, name)
@@ -246,6 +247,17 @@ class Det:
                                                 _dev(logdet, torch.float64, True),
                                                 _dev(sign, torch.int32, True), _stream(stream))
         _check(rc, "qmc_det_set_inverse")
+
+    def kinetic(self, pos, want_grad=True, stream=None):
+        """qmc_det_kinetic -> dict(grad [nw][nel][3] or None, lap [nw][nel], one [nw][nel], ekin [nw])."""
+        dev = torch.device("cuda", torch.cuda.current_device())
+        f64 = dict(dtype=torch.float64, device=dev)
+        grad = torch.empty((self.nw, self.nel, 3), **f64) if want_grad else None
+        lap, one, ekin = torch.empty((self.nw, self.nel), **f64), torch.empty((self.nw, self.nel), **f64), torch.empty(self.nw, **f64)
+        rc = load_library().qmc_det_kinetic(self._h, self.spline._h, _dev(pos, torch.float64), _dev(grad, None, True),
+                                            _dev(lap, None), _dev(one, None), _dev(ekin, None), _stream(stream))
+        _check(rc, "qmc_det_kinetic")
+        return dict(grad=grad, lap=lap, one=one, ekin=ekin)
 
     def profile(self, enable=True):
         """qmc_det_profile: bracket every sweep kernel with CUDA events (and reset the recorder)."""

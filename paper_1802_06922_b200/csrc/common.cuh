@@ -90,6 +90,7 @@ struct qmc_det {
     int *win_full;              // [1] set when any walker's window is full
     int host_pending;           // electron steps appended to the open window (host bookkeeping)
     unsigned char *win_host_iel;   // host [nel]: electrons touched in the open window
+    double *kin_lap;            // [nw][nel] scratch of qmc_det_kinetic (allocated on first use)
     // device staging of qmc_sweep_host (grown on demand)
     void *stage;
     size_t stage_bytes;

@@ -4,6 +4,11 @@
 
 namespace qmc {
 
+// SPO-VGL of electrons iel0 .. iel0+nb-1 of every walker at pos + delta (delta NULL: at pos) into d->vgl
+// (sweep.cu); nb <= d->spo_batch.
+int spo_batch_vgl(qmc_det *d, const qmc_spline *sp, const double *pos, const double *delta, int iel0, int nb,
+                  float *phi_record, int nrecord, cudaStream_t s);
+
 int delayed_ratio(qmc_det *d, int iel, const float *phi, int ldo, double *ratio, cudaStream_t s);
 int delayed_accept(qmc_det *d, int iel, const float *phi, int ldo, const double *ratio,
                    const unsigned char *accept, cudaStream_t s);

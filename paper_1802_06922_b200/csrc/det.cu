@@ -229,7 +229,7 @@ static void det_free(qmc_det *d)
     cudaFree(d->B); cudaFree(d->logdet); cudaFree(d->sign); cudaFree(d->naccept);
     cudaFree(d->vgl); cudaFree(d->rowk); cudaFree(d->rpart); cudaFree(d->ratio); cudaFree(d->acc);
     cudaFree(d->win_count); cudaFree(d->win_iel); cudaFree(d->win_slot); cudaFree(d->win_phi); cudaFree(d->win_rows);
-    cudaFree(d->win_sinv); cudaFree(d->win_full); cudaFree(d->stage);
+    cudaFree(d->win_sinv); cudaFree(d->win_full); cudaFree(d->stage); cudaFree(d->kin_lap);
     free(d->win_host_iel);
     delete d;
 }

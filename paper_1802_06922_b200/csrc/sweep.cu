@@ -20,7 +20,7 @@ void spo_launch_shape(int np, int *threads, int *tiles);
 struct SpoBatchArgs {
     SplineView sp;
     const double *pos;     // [nw][nel][3]
-    const double *delta;   // [nb][nw][3], offset to (sweep, first electron of the batch)
+    const double *delta;   // [nb][nw][3], offset to (sweep, first electron of the batch); NULL = the current positions
     int nel, iel0, nw;
     float *vgl;            // [nb][nw][5][np]
     float *phi_record;     // [nb][nrecord][nel], offset to (sweep, first electron), or NULL
@@ -34,8 +34,12 @@ __global__ void __launch_bounds__(256) spo_batch_kernel(SpoBatchArgs a)
     __shared__ StencilSmem st;
     const int w = blockIdx.y, j = blockIdx.z;
     const double *r = a.pos + ((size_t)w * a.nel + a.iel0 + j) * 3;
-    const double *dl = a.delta + 3 * ((size_t)j * a.nw + w);
-    stage_stencil(a.sp, r[0] + dl[0], r[1] + dl[1], r[2] + dl[2], st);
+    double dx = 0.0, dy = 0.0, dz = 0.0;
+    if (a.delta) {
+        const double *dl = a.delta + 3 * ((size_t)j * a.nw + w);
+        dx = dl[0]; dy = dl[1]; dz = dl[2];
+    }
+    stage_stencil(a.sp, r[0] + dx, r[1] + dy, r[2] + dz, st);
     const int np = a.sp.np;
     const int col = 4 * (blockIdx.x * blockDim.x + threadIdx.x);
     if (col >= np) return;

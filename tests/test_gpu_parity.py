@@ -421,3 +421,40 @@ def test_fixed_node_rejection(case, K):
     rep = oracle.sweep(dummy, x.lattice, x.pos, B0, ld0, sg0, x.delta, x.unif, phi_in=g["rec"], fixed_node=True,
                        nthreads=oracle.max_threads())
     P.compare_decisions(g["acc"], g["R"], rep["accept"], rep["ratios"], x.unif)
+
+
+# --------------------------------------------- NEXT-2 (first piece): kinetic term of the local energy
+@pytest.mark.parametrize("case,K", [("tiny", 0), ("ragged37_skew", 0), ("ragged37_skew", 4), ("n130_two_tiles", 16),
+                                    ("small", 0)])
+def test_det_kinetic_parity(case, K):
+    """qmc_det_kinetic after a sweep: grad_i det/det, lap_i det/det and E_kin = -1/2 sum_i lap_i
+    (eq. 3, eq. 37) against the oracle evaluated with the same inverse at the same positions
+    (its SPO-VGL in fp64): the north_star gradient / Laplacian tolerances (2e-5 of the max) propagated
+    through the dot product with row i of B; and sum_j phi_j(r_i) B[i][j] = 1."""
+    x = CASES[case]()
+    coefs_np = x.coefs_numpy()
+    spline = api.Spline.create(x.coefs.to(P.dev()), x.lattice)
+    pos = P.to_dev(x.pos)
+    det = api.Det.init(spline, pos, delay_rank=K)
+    api.sweep(det, pos, P.to_dev(x.delta), P.to_dev(x.unif))
+    k = det.kinetic(pos)
+    Bg = det.get_inverse().cpu().numpy()
+    ref = oracle.det_kinetic(coefs_np, x.lattice, pos.cpu().numpy(), Bg)
+    _, go, lo = oracle.spline_vgl(coefs_np, x.lattice, x.pos.reshape(-1, 3)[:64])
+    bnorm = np.abs(Bg).sum(axis=2)
+    tol_g = bnorm[..., None] * 2e-5 * float(np.max(np.abs(go))) + 1e-12
+    tol_l = bnorm * 2e-5 * float(np.max(np.abs(lo))) + 1e-12
+    eg = float(np.max(np.abs(k["grad"].cpu().numpy() - ref["grad"]) / tol_g))
+    el = float(np.max(np.abs(k["lap"].cpu().numpy() - ref["lap"]) / tol_l))
+    ee = float(np.max(np.abs(k["ekin"].cpu().numpy() - ref["ekin"]) / (0.5 * tol_l.sum(axis=1))))
+    one = float(np.max(np.abs(k["one"].cpu().numpy() - 1.0)))
+    print(case, K, "grad err/tol", eg, "lap err/tol", el, "ekin err/tol", ee, "|one - 1|", one,
+          "ekin[0]", float(k["ekin"][0]), float(ref["ekin"][0]))
+    assert eg < 1.0 and el < 1.0 and ee < 1.0 and one < 1e-6
+    # ekin only (no per-electron outputs requested) gives the same bits
+    ek2 = torch.empty(det.nw, dtype=torch.float64, device=P.dev())
+    rc = api.load_library().qmc_det_kinetic(det._h, spline._h, pos.data_ptr(), None, None, None, ek2.data_ptr(),
+                                            torch.cuda.current_stream().cuda_stream)
+    assert rc == 0 and torch.equal(ek2, k["ekin"])
+    det.destroy()
+    spline.destroy()
