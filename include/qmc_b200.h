@@ -118,6 +118,20 @@ int qmc_det_ratio(qmc_det_t *det, int iel, const float *phi, int ldo, double *ra
                   void *stream);
 
 /* ---------------------------------------------------------------------------------------
+ * qmc_det_ratio_points -- ratio-only evaluation of several trial positions of ONE electron against
+ * the same inverse row, with no update: the access pattern of the semi-local pseudopotential
+ * quadrature ("a 12 point angular integration used by default"), where every
+ * quadrature point needs det A'/det A = sum_j B[iel][j] * phi_q[j] (L299) and nothing else.
+ * Evaluate the orbital values of the nwalkers * npts points with qmc_spo_vgl (g = l = NULL) first.
+ *
+ *   phi     dev, float [nwalkers][npts][ldo], ldo >= nel
+ *   ratios  dev, double [nwalkers][npts] (out)
+ * With delay_rank >= 2 the pending accepted rows are applied first (the inverse is made current).
+ */
+int qmc_det_ratio_points(qmc_det_t *det, int iel, int npts, const float *phi, int ldo,
+                         double *ratios, void *stream);
+
+/* ---------------------------------------------------------------------------------------
  * qmc_det_accept_update -- L299 "for single electron moves, QMCPACK uses the Sherman-Morrison
  * algorithm": for every walker with accept[w] != 0, row iel of A_w is replaced by phi_w and
  *     B'[m][j] = B[m][j] - ((B[m] . phi) - delta_{m,iel}) * B[iel][j] / ratio_w

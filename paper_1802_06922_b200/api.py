@@ -21,7 +21,7 @@ EXPORTS = [
     "qmc_det_init", "qmc_det_destroy", "qmc_det_ratio", "qmc_det_accept_update", "qmc_det_flush",
     "qmc_sweep", "qmc_sweep_ex", "qmc_sweep_host", "qmc_det_get_inverse", "qmc_det_set_inverse",
     "qmc_det_get_stats", "qmc_det_info", "qmc_launch_count", "qmc_det_profile", "qmc_det_profile_read",
-    "qmc_probe_fp64_dmma", "qmc_det_kinetic",
+    "qmc_probe_fp64_dmma", "qmc_det_kinetic", "qmc_det_ratio_points",
 ]
 PROF_KINDS = ["spo_vgl", "sm_update", "delayed_window", "delayed_accept", "delayed_flush", "ratio_rowcopy"]
 
@@ -72,6 +72,7 @@ def load_library(path=None):
         "qmc_det_profile_read": [_vp, ctypes.POINTER(d), ctypes.POINTER(ctypes.c_longlong)],
         "qmc_probe_fp64_dmma": [ctypes.POINTER(d), _vp],
         "qmc_det_kinetic": [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp],
+        "qmc_det_ratio_points": [_vp, i, i, _vp, i, _vp, _vp],
     }
     for name, args in sigs.items():
         fn = getattr(lib, name)
@@ -223,6 +224,15 @@ class Det:
         rc = load_library().qmc_det_ratio(self._h, int(iel), _dev(phi, torch.float32), phi.shape[-1],
                                           _dev(out, None), _stream(stream))
         _check(rc, "qmc_det_ratio")
+        return out
+
+    def ratio_points(self, iel, phi, stream=None):
+        """qmc_det_ratio_points: phi float32 [nw][npts][ldo] -> ratios double [nw][npts] (no update)."""
+        npts = phi.shape[1]
+        out = torch.empty((self.nw, npts), dtype=torch.float64, device=phi.device)
+        rc = load_library().qmc_det_ratio_points(self._h, int(iel), int(npts), _dev(phi, torch.float32),
+                                                 phi.shape[-1], _dev(out, None), _stream(stream))
+        _check(rc, "qmc_det_ratio_points")
         return out
 
     def accept_update(self, iel, phi, ratio, accept, stream=None):

@@ -172,6 +172,23 @@ ratio_kernel(const double *__restrict__ B, int nel, int ld, int iel, const float
     if (threadIdx.x == 0) ratio[w] = acc;
 }
 
+// R[w][q] = sum_j B_w[iel][j] * (double)phi[w][q][j] for npts trial positions of the same electron: one
+// block per walker, one warp per point (the row stays in L1/L2), fixed summation order per point.
+__global__ void __launch_bounds__(256)
+ratio_points_kernel(const double *__restrict__ B, int nel, int ld, int iel, const float *__restrict__ phi,
+                    int npts, int ldphi, double *__restrict__ ratios)
+{
+    const int w = blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const double *row = B + ((size_t)w * nel + iel) * ld;
+    for (int q = warp; q < npts; q += 8) {
+        const float *ph = phi + ((size_t)w * npts + q) * ldphi;
+        double acc = 0.0;
+        for (int j = lane; j < nel; j += 32) acc = fma(row[j], (double)ph[j], acc);
+        acc = warp_sum(acc);
+        if (lane == 0) ratios[(size_t)w * npts + q] = acc;
+    }
+}
+
 __global__ void __launch_bounds__(256)
 copy_rowk_kernel(const double *__restrict__ B, int nel, int ld, int iel,
                  const unsigned char *__restrict__ accept, double *__restrict__ rowk)
@@ -415,6 +432,24 @@ extern "C" int qmc_det_ratio(qmc_det_t *d, int iel, const float *phi, int ldo, d
     cudaStream_t s = (cudaStream_t)stream;
     if (d->delay) return delayed_ratio(d, iel, phi, ldo, ratio, s);
     ratio_kernel<<<d->nw, 128, 0, s>>>(d->B, d->nel, d->ld, iel, phi, ldo, ratio);
+    QMC_LAUNCHED();
+    return QMC_OK;
+}
+
+extern "C" int qmc_det_ratio_points(qmc_det_t *d, int iel, int npts, const float *phi, int ldo, double *ratios,
+                                    void *stream)
+{
+    QMC_REQUIRE(d && phi && ratios, "qmc_det_ratio_points: NULL argument");
+    QMC_REQUIRE(iel >= 0 && iel < d->nel, "qmc_det_ratio_points: iel=%d out of range 0..%d", iel, d->nel - 1);
+    QMC_REQUIRE(npts >= 0, "qmc_det_ratio_points: npts=%d", npts);
+    QMC_REQUIRE(ldo >= d->nel, "qmc_det_ratio_points: ldo=%d < nel=%d", ldo, d->nel);
+    if (npts == 0) return QMC_OK;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (d->delay) {               // ratios against the current inverse: apply pending rows first
+        int rc = delayed_flush_reset_host(d, s);
+        if (rc) return rc;
+    }
+    ratio_points_kernel<<<d->nw, 256, 0, s>>>(d->B, d->nel, d->ld, iel, phi, npts, ldo, ratios);
     QMC_LAUNCHED();
     return QMC_OK;
 }
