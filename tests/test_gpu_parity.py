@@ -200,7 +200,7 @@ def test_sweep_control_flow():
 
 # ------------------------------------------------------------------------------- full sizes
 @pytest.mark.parametrize("name,nchk,npos,delay", [("mid", 4, 48, 0), ("large", 4, 32, 0), ("mid", 4, 0, 16),
-                                                  ("large", 4, 0, 16), ("large", 2, 0, 32)])
+                                                  ("large", 4, 0, 16), ("large", 2, 0, 32), ("xlarge", 2, 16, 16)])
 def test_full_size_sampled(name, nchk, npos, delay):
     """BASELINE.json's full sizes in the launch configuration bench.py times (all walkers in
     lockstep, one sweep; rank-1 and the delayed ranks bench.py measures): the oracle checks the
@@ -210,6 +210,9 @@ def test_full_size_sampled(name, nchk, npos, delay):
     cfg = inputs.CONFIGS[name]
     if free_b < 2.6 * cfg.table_bytes() + 4 * cfg.nw * cfg.norb ** 2 * 8:
         pytest.skip("not enough device memory")
+    import psutil
+    if psutil.virtual_memory().available < 2.5 * cfg.table_bytes():
+        pytest.skip("not enough host memory for the oracle's copy of the table")
     x = inputs.make_inputs(cfg, device=P.dev(), nsweeps=1)
     coefs_np = x.coefs_numpy()                  # the same bits for both sides
     if npos:
