@@ -241,8 +241,19 @@ flush_ring_kernel(RingArgs a)
     X(8, 32, 4, 8, 2, 6) X(16, 32, 4, 8, 4, 6) X(32, 32, 4, 8, 8, 6)
 
 template <int KPAD, int TW, int NWC, int CS, int STAGES>
-static cudaError_t launch_ring(const RingArgs &a, int nw, cudaStream_t s)
+static cudaError_t launch_ring(RingArgs a, int nw, cudaStream_t s)
 {
+    // rows per CTA: the window fragments are loaded and the ring is filled once per CTA (a few us), so
+    // prefer long CTAs as long as the grid still makes ~6 waves of one CTA per SM
+    static int nsm = 0;
+    if (!nsm) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        if (cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || nsm < 1) nsm = 148;
+    }
+    a.rows_per_cta = 64;
+    for (int r = 1024; r >= 128; r >>= 1)
+        if ((long long)nw * ((a.nel + r - 1) / r) * CS >= 6LL * nsm) { a.rows_per_cta = r; break; }
     using L = RingSmem<KPAD, TW, NWC, CS, STAGES>;
     static_assert(L::bytes <= 227 * 1024, "ring shape exceeds shared memory");
     auto kern = flush_ring_kernel<KPAD, TW, NWC, CS, STAGES>;
@@ -289,9 +300,6 @@ cudaError_t flush_ring_launch(qmc_det *d, cudaStream_t s)
     a.win_count = d->win_count; a.win_iel = d->win_iel; a.win_slot = d->win_slot;
     a.vec = d->win_vec; a.vec_wstride = d->win_vec_wstride; a.vec_sstride = d->win_vec_sstride;
     a.win_rows = d->win_rows;
-    // rows per CTA: the window fragments are loaded once per CTA, so prefer long CTAs when the grid stays large
-    const long long rows_total = (long long)d->nw * d->nel;
-    a.rows_per_cta = rows_total >= 512LL * 148 * 4 ? 512 : (rows_total >= 128LL * 148 * 4 ? 128 : 64);
     const int v = d->ld / 64, kpad = d->delay <= 16 ? 16 : 32;
 #define X(V, KPAD, TW, NWC, CS, STAGES) \
     if (v == V && kpad == KPAD) return launch_ring<KPAD, TW, NWC, CS, STAGES>(a, d->nw, s);
