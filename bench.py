@@ -41,7 +41,7 @@ UNIT = "moves/s"
 DEFAULT_DELAY = {"tiny": [0], "small": [16, 0], "mid": [16, 0], "large": [16, 0], "xlarge": [16, 32, 0]}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures
 # (profiles/r01_*.md), config `large`
-NCU_TRAFFIC = {"sm_update": 6.725e9, "delayed_flush": 8.613e9, "spo_vgl": 2.254e9, "delayed_window": 0.145e9}
+NCU_TRAFFIC = {"sm_update": 6.725e9, "delayed_flush": 8.612e9, "spo_vgl": 2.254e9, "delayed_window": 0.147e9}
 
 
 def measured_peaks():
