@@ -251,6 +251,12 @@ int qmc_det_kinetic(qmc_det_t *det, const qmc_spline_t *spline, const double *po
 int qmc_det_profile(qmc_det_t *det, int enable);
 int qmc_det_profile_read(qmc_det_t *det, double *ms_host, long long *launches_host);
 
+/* Environment variables read by qmc_det_flush / qmc_sweep (test and A/B-measurement hooks only; unset
+ * in production): QMC_FLUSH_RING=0 routes every shape to the shared-memory-window flush kernel
+ * (flush.cu) instead of the register-window / TMA-ring kernel (flush_ring.cu); QMC_FLUSH_SHAPE=n
+ * forces the n-th launch shape of flush.cu for the handle's leading dimension.  Results are the same
+ * to rounding with any setting (tests/test_gpu_parity.py::test_delayed_large_n_equals_rank1). */
+
 /* Measured fp64 tensor-core peak of the current device in TFLOP/s (host pointer): an issue loop of
  * mma.sync.m8n8k4.f64 with register operands, best of 5 after a warm-up, ~10 ms.  bench.py reports
  * the delayed flush (the "genuine dense fp64 contraction" of north_star) against it,

@@ -502,3 +502,11 @@ def test_ratio_points(case, K):
     assert np.max(np.abs(r1 - R[:, 0]) / np.abs(r1)) < 1e-12
     det.destroy()
     spline.destroy()
+
+
+def test_fp64_dmma_probe():
+    """qmc_probe_fp64_dmma: the roofline denominator bench.py uses for the delayed flush.  A B200
+    issues one DMMA.8x8x4 per 16 cycles per SM sub-partition: ~37 TFLOP/s at 1.9 GHz."""
+    tf = api.probe_fp64_dmma()
+    print("fp64 DMMA peak", tf, "TFLOP/s")
+    assert 15.0 < tf < 80.0
