@@ -111,7 +111,11 @@ int qmc_det_destroy(qmc_det_t *det);
  * the upcast fp32 orbital vector; warp-shuffle tree, fixed order).  With a delayed window open
  * the pending accepted rows are included (R:O7).
  *
- *   phi    dev, float [nwalkers][ldo], ldo >= nel
+ *   phi    dev, float [nwalkers][ldo], ldo >= nel.  With delay_rank >= 2 (here and in
+ *          qmc_det_accept_update) the vector is read with 128-bit loads up to the table pitch and
+ *          copied into the window: ldo >= the spline's row pitch (qmc_spline_info), ldo % 4 == 0,
+ *          phi 16-byte aligned, elements nel..pitch-1 finite (qmc_spo_vgl writes zeros there);
+ *          otherwise QMC_EINVAL.
  *   ratio  dev, double [nwalkers] (out)
  */
 int qmc_det_ratio(qmc_det_t *det, int iel, const float *phi, int ldo, double *ratio,
@@ -137,8 +141,10 @@ int qmc_det_ratio_points(qmc_det_t *det, int iel, int npts, const float *phi, in
  *     B'[m][j] = B[m][j] - ((B[m] . phi) - delta_{m,iel}) * B[iel][j] / ratio_w
  * in ONE pass over B (each row read once, dotted, updated, written: 16*nel*ld bytes per
  * accepted walker).  log|det| += log|ratio|, sign *= sgn(ratio), accept counter += 1.
- * Walkers with accept[w] == 0 are untouched.  With delay_rank >= 2 the row is appended to the
- * walker's window instead and the window is flushed when any walker's window is full.
+ * Walkers with accept[w] == 0 are untouched, and so are walkers whose ratio is zero or not finite
+ * (the update divides by it and the new Slater matrix would be singular: the accept is refused,
+ * R:A18; the same holds for forced_accept in qmc_sweep).  With delay_rank >= 2 the row is appended
+ * to the walker's window instead and the window is flushed when any walker's window is full.
  *
  *   phi, ldo  as in qmc_det_ratio (the vector the ratio was computed from)
  *   ratio     dev, double [nwalkers]: the values qmc_det_ratio returned
@@ -158,7 +164,7 @@ int qmc_det_flush(qmc_det_t *det, void *stream);
  * (eq. 12 with symmetric T and a determinant-only Psi, R:A8; non-finite R rejects); on accept
  * pos[w][k] = r' (stored unwrapped) and the inverse is updated as in qmc_det_accept_update.
  * Pending delayed updates are flushed at the end of every sweep.  qmc_sweep_ex adds the fixed-node
- * rule (L253) and the wavefunction force of every proposal (L155) as options.
+ * rule (L253) and the wavefunction force of every proposal (L156) as options.
  *
  *   pos            dev, double [nwalkers][nel][3], in/out.  Must be the positions the handle's
  *                  inverse corresponds to.
@@ -182,7 +188,7 @@ typedef struct qmc_sweep_opts {
     int fixed_node;      /* != 0: fixed-node rule: a move that changes the   */
                          /*   sign of the wavefunction (R < 0) is rejected whatever u is     */
     double *force_out;   /* NULL, or dev double [nsweeps][nel][nwalkers][3]: the wavefunction */
-                         /*   force F = 2 grad log Psi_T (L155; the F of eq. 11 / eq. 13) on  */
+                         /*   force F = 2 grad log Psi_T (L156; the F of eq. 11 / eq. 13) on  */
                          /*   the moved electron at the PROPOSED configuration,               */
                          /*   F = 2 sum_j grad phi_j(r') B[k][j] / R, for every move          */
                          /*   (accepted or not; 0 where R == 0)                               */

@@ -91,6 +91,7 @@ static void bspline_weights(double t, double b[4], double db[4], double d2b[4])
 /* Reduced coordinate -> (cell index, fraction) along one dimension (R:A7). */
 static void cell_of(double u, int n, int *i, double *t)
 {
+    if (!isfinite(u)) { *i = 0; *t = u - u; return; } /* NaN weights: every orbital is NaN (R:A18) */
     u -= floor(u);
     double s = u * (double)n;
     double fl = floor(s);
@@ -336,14 +337,16 @@ int orc_sm_update(int n, double *B, int k, const double *phi, double R)
  *           nodal crossing are detected through the change in sign of the wavefunction and are
  *           rejected": a move with R < 0 is rejected whatever u is (ignored when `forced`)
  *   force_out  NULL, or double [nsweeps][nel][nw][3]: the "wavefunction force" F = 2 grad log Psi_T
- *           (PAPER.md L155; the F of eq. 11 / eq. 13) on the moved electron at the PROPOSED
+ *           (PAPER.md L156; the F of eq. 11 / eq. 13) on the moved electron at the PROPOSED
  *           configuration.  With Psi = det A, row k replaced by phi(r'):
  *               grad_k log|det A'| = sum_j grad phi_j(r') (A'^-1)[j][k]
  *                                  = sum_j grad phi_j(r') B[k][j] / R        (B'[k] = B[k] / R)
  *           The gradients come from this oracle's own fp64 spline at r' (also in phi_in mode).
  *           Written for every move, accepted or not; 0 when R == 0.
  *
- * Accept iff R*R > u; a non-finite R is rejected (R:A8).  On accept:
+ * Accept iff R*R > u; a non-finite R is rejected (R:A8); an imposed accept (`forced`) of a move
+ * whose R is zero or not finite is refused -- the update divides by R and the new Slater matrix
+ * would be singular (R:A18).  On accept:
  * r_k <- r_k + delta (one fp64 add), row k of A <- phi, log|det| += log|R|,
  * sign *= sgn(R), B updated.  Returns 0 or the first error code met.
  */
@@ -392,7 +395,7 @@ int orc_sweep(int nx, int ny, int nz, int norb, const double lattice[9], const f
                     }
                 }
                 int acc;
-                if (forced) acc = forced[mv] != 0;
+                if (forced) acc = forced[mv] != 0 && isfinite(R) && R != 0.0; /* R:A18 */
                 else acc = isfinite(R) && (R * R > unif[mv]) && !(fixed_node && R < 0.0);
                 if (ratios_out) ratios_out[mv] = R;
                 if (bnorm_out) {

@@ -14,7 +14,6 @@ namespace qmc {
 
 constexpr int kWarp = 32;
 constexpr int kMaxNel = 2048;       // rows are held in registers: 64 doubles per lane at most
-constexpr int kRatioTilesMax = 8;   // partial-ratio slots per walker
 constexpr int kSpoBatch = 16;       // electron steps per SPO-VGL launch in rank-1 mode (delayed: the window)
 
 void set_error(const char *fmt, ...);
@@ -26,6 +25,18 @@ void count_launch(int n = 1);
         if (e__ != cudaSuccess) {                                                          \
             qmc::set_error("%s:%d: %s -> %s", __FILE__, __LINE__, #call,                   \
                            cudaGetErrorString(e__));                                       \
+            return QMC_ECUDA;                                                              \
+        }                                                                                  \
+    } while (0)
+
+// Same, running `cleanup` before the error return.
+#define QMC_CUDA_OR(call, cleanup)                                                         \
+    do {                                                                                   \
+        cudaError_t e__ = (call);                                                          \
+        if (e__ != cudaSuccess) {                                                          \
+            qmc::set_error("%s:%d: %s -> %s", __FILE__, __LINE__, #call,                   \
+                           cudaGetErrorString(e__));                                       \
+            cleanup;                                                                       \
             return QMC_ECUDA;                                                              \
         }                                                                                  \
     } while (0)
@@ -65,6 +76,7 @@ struct qmc_spline {
 struct qmc_det {
     const qmc_spline *spline;   // not owned; shape checks and det_init only
     int nw, nel, ld, delay;
+    int device, nsm;            // the CUDA device the handle lives on and its SM count (grid sizing)
     int np;                     // spline row pitch (floats)
     double *B;                  // [nw][nel][ld]   (A^-1)^T, pad columns zero
     double *logdet;             // [nw]
@@ -74,8 +86,7 @@ struct qmc_det {
     int spo_batch;              // electron steps whose SPO-VGL is evaluated per launch (qmc_sweep)
     float *vgl;                 // [spo_batch][nw][5][np]   v, gx, gy, gz, lap of the proposals of a batch
     double *rowk;               // [nw][ld]      copy of row iel of B taken before the update
-    double *rpart;              // [nw][kRatioTilesMax] partial ratios of the fused SPO kernel
-    double *ratio;              // [nw]
+    double *ratio;              // [nw]      ratio of the current step (ratio_rowcopy_kernel -> sm_update_kernel)
     unsigned char *acc;         // [nw]
     // delayed-update window (delay >= 2)
     int *win_count;             // [nw]           accepted rows pending

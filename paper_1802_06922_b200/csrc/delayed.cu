@@ -119,7 +119,7 @@ __global__ void __launch_bounds__(kStepThreads) delayed_step_kernel(DelayedStepA
         double R = s_tot[0];
         for (int m = 0; m < p; ++m) R -= s_tot[1 + m] * s_y[m];
         bool acc_w = false;
-        if (a.mode == 2) acc_w = a.accept_in[w] != 0;      // the caller's decision; R equals the ratio it was given
+        if (a.mode == 2) acc_w = a.accept_in[w] != 0 && usable_ratio(R);   // the caller's decision (R equals the ratio it was given); R:A18
         else a.ratio_io[w] = R;
         s_tot[0] = R;
         s_flag = acc_w;
@@ -179,6 +179,7 @@ static void fill_common(DelayedStepArgs &a, qmc_det *d, int iel, const float *ph
 int delayed_ratio(qmc_det *d, int iel, const float *phi, int ldo, double *ratio, cudaStream_t s)
 {
     QMC_REQUIRE(ldo >= d->np, "qmc_det_ratio (delayed): ldo=%d must be >= the table pitch %d", ldo, d->np);
+    QMC_REQUIRE(ldo % 4 == 0 && ((uintptr_t)phi & 15) == 0, "qmc_det_ratio (delayed): phi must be 16-byte aligned with ldo %% 4 == 0 (ldo=%d)", ldo);
     // a second move of an electron already in the window would break row distinctness: flush first
     if (d->host_pending && d->win_host_iel[iel]) {
         int rc = delayed_flush_reset_host(d, s);
@@ -199,6 +200,7 @@ int delayed_accept(qmc_det *d, int iel, const float *phi, int ldo, const double 
                    const unsigned char *accept, cudaStream_t s)
 {
     QMC_REQUIRE(ldo >= d->np, "qmc_det_accept_update (delayed): ldo=%d must be >= the table pitch %d", ldo, d->np);
+    QMC_REQUIRE(ldo % 4 == 0 && ((uintptr_t)phi & 15) == 0, "qmc_det_accept_update (delayed): phi must be 16-byte aligned with ldo %% 4 == 0 (ldo=%d)", ldo);
     if (d->host_pending >= d->delay || (d->host_pending && d->win_host_iel[iel])) {
         int rc = delayed_flush_reset_host(d, s);
         if (rc) return rc;

@@ -244,7 +244,7 @@ static void det_free(qmc_det *d)
         delete d->prof_kinds;
     }
     cudaFree(d->B); cudaFree(d->logdet); cudaFree(d->sign); cudaFree(d->naccept);
-    cudaFree(d->vgl); cudaFree(d->rowk); cudaFree(d->rpart); cudaFree(d->ratio); cudaFree(d->acc);
+    cudaFree(d->vgl); cudaFree(d->rowk); cudaFree(d->ratio); cudaFree(d->acc);
     cudaFree(d->win_count); cudaFree(d->win_iel); cudaFree(d->win_slot); cudaFree(d->win_phi); cudaFree(d->win_rows);
     cudaFree(d->win_sinv); cudaFree(d->win_full); cudaFree(d->stage); cudaFree(d->kin_lap);
     free(d->win_host_iel);
@@ -309,6 +309,8 @@ extern "C" int qmc_det_init(qmc_det_t **out, const qmc_spline_t *sp, int nw, int
     qmc_det *d = new (std::nothrow) qmc_det();
     if (!d) { set_error("qmc_det_init: host allocation failed"); return QMC_ENOMEM; }
     d->spline = sp;
+    QMC_CUDA_OR(cudaGetDevice(&d->device), det_free(d));
+    QMC_CUDA_OR(cudaDeviceGetAttribute(&d->nsm, cudaDevAttrMultiProcessorCount, d->device), det_free(d));
     d->nw = nw; d->nel = nel; d->ld = update_ld(nel); d->np = sp->view.np;
     d->delay = delay_rank <= 1 ? 0 : delay_rank;
     d->spo_batch = d->delay ? d->delay : kSpoBatch;
@@ -317,7 +319,7 @@ extern "C" int qmc_det_init(qmc_det_t **out, const qmc_spline_t *sp, int nw, int
     if ((rc = dev_alloc(&d->B, (size_t)nw * nel * ld, "B")) || (rc = dev_alloc(&d->logdet, nw, "logdet")) ||
         (rc = dev_alloc(&d->sign, nw, "sign")) || (rc = dev_alloc(&d->naccept, nw, "naccept")) ||
         (rc = dev_alloc(&d->vgl, (size_t)d->spo_batch * nw * 5 * np, "vgl")) || (rc = dev_alloc(&d->rowk, (size_t)nw * ld, "rowk")) ||
-        (rc = dev_alloc(&d->rpart, (size_t)nw * kRatioTilesMax, "rpart")) || (rc = dev_alloc(&d->ratio, nw, "ratio")) ||
+        (rc = dev_alloc(&d->ratio, nw, "ratio")) ||
         (rc = dev_alloc(&d->acc, nw, "acc"))) {
         det_free(d);
         return rc;
@@ -345,7 +347,6 @@ extern "C" int qmc_det_init(qmc_det_t **out, const qmc_spline_t *sp, int nw, int
     }
     cudaError_t e = cudaMemsetAsync(d->B, 0, (size_t)nw * nel * ld * sizeof(double), s);
     if (e == cudaSuccess) e = cudaMemsetAsync(d->rowk, 0, (size_t)nw * ld * sizeof(double), s);
-    if (e == cudaSuccess) e = cudaMemsetAsync(d->rpart, 0, (size_t)nw * kRatioTilesMax * sizeof(double), s);
     if (e == cudaSuccess) e = cudaMemsetAsync(d->vgl, 0, (size_t)d->spo_batch * nw * 5 * np * sizeof(float), s);
     if (e == cudaSuccess && K) e = cudaMemsetAsync(d->win_count, 0, (size_t)nw * sizeof(int), s);
     if (e == cudaSuccess && K) e = cudaMemsetAsync(d->win_full, 0, sizeof(int), s);

@@ -357,12 +357,9 @@ static cudaError_t launch_flush_t(const FlushArgs &a, int nw, cudaStream_t s)
         return cudaErrorInvalidValue;
     } else {
         auto kern = flush_dmma_kernel<KPAD, NWC, TW, NG, PF, CS>;
-        static bool configured = false;
-        if (!configured) {
-            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L::bytes);
-            if (e != cudaSuccess) return e;
-            configured = true;
-        }
+        // the opt-in is per device, not per process: set it on every launch (a host-side table write)
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L::bytes);
+        if (e != cudaSuccess) return e;
         cudaLaunchConfig_t cfg{};
         cfg.gridDim = dim3(CS * ((a.nel + a.rows_per_cta - 1) / a.rows_per_cta), nw);
         cfg.blockDim = dim3(32 * NWC * NG);
@@ -402,7 +399,7 @@ int delayed_flush(qmc_det *d, cudaStream_t s)
     const FlushShape sh = ring ? FlushShape{0, 1, 1, 1, 1} : flush_shape(d->ld / 64, kpad_of(d->delay));
     QMC_REQUIRE(sh.id >= 0, "qmc_det_flush: no kernel shape for ld=%d, rank %d", d->ld, d->delay);
     // rows per CTA: the window is staged once per CTA, so prefer long CTAs when the grid stays large
-    a.rows_per_cta = ((long long)d->nw * d->nel >= 128LL * 148 * 8) ? 128 : 64;
+    a.rows_per_cta = ((long long)d->nw * d->nel >= 128LL * d->nsm * 8) ? 128 : 64;
     if (a.rows_per_cta % (8 * sh.ng)) a.rows_per_cta = 8 * sh.ng * ((a.rows_per_cta + 8 * sh.ng - 1) / (8 * sh.ng));
     cudaError_t e = cudaErrorInvalidValue;
     if (d->win_rows_raw) {

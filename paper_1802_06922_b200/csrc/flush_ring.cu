@@ -241,28 +241,19 @@ flush_ring_kernel(RingArgs a)
     X(8, 32, 4, 8, 2, 6) X(16, 32, 4, 8, 4, 6) X(32, 32, 4, 8, 8, 6)
 
 template <int KPAD, int TW, int NWC, int CS, int STAGES>
-static cudaError_t launch_ring(RingArgs a, int nw, cudaStream_t s)
+static cudaError_t launch_ring(RingArgs a, int nw, int nsm, cudaStream_t s)
 {
     // rows per CTA: the window fragments are loaded and the ring is filled once per CTA (a few us), so
     // prefer long CTAs as long as the grid still makes ~6 waves of one CTA per SM
-    static int nsm = 0;
-    if (!nsm) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        if (cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || nsm < 1) nsm = 148;
-    }
     a.rows_per_cta = 64;
     for (int r = 1024; r >= 128; r >>= 1)
         if ((long long)nw * ((a.nel + r - 1) / r) * CS >= 6LL * nsm) { a.rows_per_cta = r; break; }
     using L = RingSmem<KPAD, TW, NWC, CS, STAGES>;
     static_assert(L::bytes <= 227 * 1024, "ring shape exceeds shared memory");
     auto kern = flush_ring_kernel<KPAD, TW, NWC, CS, STAGES>;
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L::bytes);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
+    // the opt-in is per device, not per process: set it on every launch (a host-side table write)
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L::bytes);
+    if (e != cudaSuccess) return e;
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3(CS * ((a.nel + a.rows_per_cta - 1) / a.rows_per_cta), nw);
     cfg.blockDim = dim3(32 * NWC);
@@ -302,7 +293,7 @@ cudaError_t flush_ring_launch(qmc_det *d, cudaStream_t s)
     a.win_rows = d->win_rows;
     const int v = d->ld / 64, kpad = d->delay <= 16 ? 16 : 32;
 #define X(V, KPAD, TW, NWC, CS, STAGES) \
-    if (v == V && kpad == KPAD) return launch_ring<KPAD, TW, NWC, CS, STAGES>(a, d->nw, s);
+    if (v == V && kpad == KPAD) return launch_ring<KPAD, TW, NWC, CS, STAGES>(a, d->nw, d->nsm, s);
     QMC_RING_SHAPES(X)
 #undef X
     return cudaErrorInvalidValue;

@@ -1,5 +1,5 @@
 // Device side of the SPO-VGL gather: stencil weights and the 64-row gather.
-// Shared by the standalone qmc_spo_vgl kernel and the fused SPO+ratio kernel of qmc_sweep.
+// Shared by the standalone qmc_spo_vgl kernel and the batched gather of qmc_sweep (sweep.cu).
 #pragma once
 #include "common.cuh"
 

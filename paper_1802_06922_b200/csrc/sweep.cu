@@ -63,10 +63,10 @@ __global__ void __launch_bounds__(256) spo_batch_kernel(SpoBatchArgs a)
 // S3 for the rank-1 path: R_w = B_w[iel] . phi_w (fp64, fixed order) and a copy of row iel, so that
 // the update kernel can overwrite B in place.  One block per walker.  With force_out the three
 // gradient vectors of the proposal (phi + np, + 2 np, + 3 np) are contracted with the same row:
-// F = 2 grad log Psi_T at the proposed configuration = 2 (B[iel] . grad phi) / R  (PAPER.md L155).
+// F = 2 grad log Psi_T at the proposed configuration = 2 (B[iel] . grad phi) / R  (PAPER.md L156).
 __global__ void __launch_bounds__(256)
 ratio_rowcopy_kernel(const double *__restrict__ B, int nel, int ld, int iel, const float *__restrict__ phi,
-                     size_t ldphi, int np, double *__restrict__ rowk, double *__restrict__ rpart,
+                     size_t ldphi, int np, double *__restrict__ rowk, double *__restrict__ ratio,
                      double *__restrict__ force_out)
 {
     __shared__ double red[33];
@@ -94,7 +94,7 @@ ratio_rowcopy_kernel(const double *__restrict__ B, int nel, int ld, int iel, con
         }
     }
     acc = block_sum(acc, red);
-    if (threadIdx.x == 0) rpart[(size_t)w * kRatioTilesMax] = acc;
+    if (threadIdx.x == 0) ratio[w] = acc;
     if (force_out) {
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
@@ -171,14 +171,14 @@ static int sweep_impl(qmc_det *d, const qmc_spline *sp, double *pos, const doubl
             const float *phi = d->vgl + slot * slot_stride;
             // K2: ratio + row copy, K3: decision + rank-1 update
             prof_start(d, kProfRatio, s);
-            ratio_rowcopy_kernel<<<nw, 256, 0, s>>>(d->B, nel, d->ld, k, phi, (size_t)5 * d->np, d->np, d->rowk, d->rpart,
+            ratio_rowcopy_kernel<<<nw, 256, 0, s>>>(d->B, nel, d->ld, k, phi, (size_t)5 * d->np, d->np, d->rowk, d->ratio,
                                                     force ? force + 3 * mv : nullptr);
             prof_stop(d, s);
             QMC_LAUNCHED();
             UpdateArgs u{};
             u.B = d->B; u.nel = nel; u.ld = d->ld; u.iel = k;
             u.phi = phi; u.ldphi = (size_t)5 * d->np; u.rowk = d->rowk;
-            u.rpart = d->rpart; u.ntiles = 1;
+            u.ratio = d->ratio;
             u.unif = unif + mv;
             u.forced = forced ? forced + mv : nullptr;
             u.fixed_node = fixed_node;

@@ -1,6 +1,6 @@
 // Sherman-Morrison rank-1 update of B = (A^-1)^T in one pass (S4+S5 of the hot
 // path).  Used by qmc_det_accept_update (decision given) and qmc_sweep (decision taken here from
-// the partial ratios of the fused SPO kernel).
+// the ratio ratio_rowcopy_kernel left in d->ratio).
 #pragma once
 #include "common.cuh"
 
@@ -12,12 +12,10 @@ struct UpdateArgs {
     const float *phi;             // [nw][ldphi] orbital vector of the proposal (fp32)
     size_t ldphi;                 //   walker stride in floats
     const double *rowk;           // [nw][ld] row iel of B before the update
+    const double *ratio;          // [nw] det A'/det A of the proposal
     // decision given (qmc_det_accept_update)
-    const double *ratio;          // [nw]
     const unsigned char *accept;  // [nw]
     // decision taken here (qmc_sweep): all pointers already offset to (sweep, electron)
-    const double *rpart;          // [nw][kRatioTilesMax]
-    int ntiles;
     const double *unif;           // [nw]
     const unsigned char *forced;  // [nw] or NULL
     int fixed_node;               // reject R < 0
@@ -36,6 +34,11 @@ constexpr int kUpdRowsPerCta = 64;
 
 // Metropolis test of eq. 12 with symmetric T and a determinant-only Psi (R:A8).
 __device__ __forceinline__ bool metropolis(double R, double u) { return isfinite(R) && (R * R > u); }
+// A move may be applied only if its ratio is finite and non-zero: the update divides by R and the
+// new Slater matrix would be singular otherwise (R:A18).  The Metropolis test already implies it
+// (R * R > u >= 0); decisions imposed by the caller (forced_accept, qmc_det_accept_update) are
+// filtered with it.
+__device__ __forceinline__ bool usable_ratio(double R) { return isfinite(R) && R != 0.0; }
 
 // One warp per row m: the row (ld = 64*VPT doubles) is read once into registers as VPT double2
 // per lane, dotted with phi (warp-shuffle tree), updated with the old row iel, and written back:
@@ -45,16 +48,11 @@ __global__ void __launch_bounds__(kUpdThreads) sm_update_kernel(UpdateArgs a)
 {
     extern __shared__ double smem_upd[];
     const int w = blockIdx.y;
-    double R;
+    const double R = a.ratio[w];
     bool acc;
-    if (DECIDE) {
-        R = 0.0;
-        for (int t = 0; t < a.ntiles; ++t) R += a.rpart[(size_t)w * kRatioTilesMax + t];
-        acc = a.forced ? (a.forced[w] != 0) : (metropolis(R, a.unif[w]) && !(a.fixed_node && R < 0.0));
-    } else {
-        R = a.ratio[w];
-        acc = a.accept[w] != 0;
-    }
+    if (DECIDE) acc = a.forced ? (a.forced[w] != 0) : (metropolis(R, a.unif[w]) && !(a.fixed_node && R < 0.0));
+    else acc = a.accept[w] != 0;
+    acc = acc && usable_ratio(R);     // an imposed accept of a singular / non-finite move is refused (R:A18)
     if (blockIdx.x == 0 && threadIdx.x == 0) {
         if (DECIDE) {
             if (a.ratios_out) a.ratios_out[w] = R;

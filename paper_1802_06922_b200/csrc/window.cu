@@ -156,7 +156,7 @@ __global__ void __launch_bounds__(kWinThreads) delayed_window_kernel(WindowArgs 
             const double R = G_s[i * GS + i] - warp_sum(x * y);
             const double u_i = __shfl_sync(0xffffffffu, u_l, i);
             const int f_i = __shfl_sync(0xffffffffu, f_l, i);
-            const bool acc_w = a.forced ? (f_i != 0) : (metropolis(R, u_i) && !(a.fixed_node && R < 0.0));
+            const bool acc_w = (a.forced ? (f_i != 0) : (metropolis(R, u_i) && !(a.fixed_node && R < 0.0))) && usable_ratio(R);
             if (lane == i) R_l = R;
             if (FORCE) {
                 // grad phi(r'_i) . B_cur[k_i] = gd - xg^T S^-1 c with the same y = S^-1 c as the ratio

@@ -372,7 +372,7 @@ def _force_run(x, K, fixed_node=False, unif=None):
 @pytest.mark.parametrize("case,K", [("tiny", 0), ("tiny", 3), ("ragged37_skew", 0), ("ragged37_skew", 16),
                                     ("n130_two_tiles", 0), ("n130_two_tiles", 7), ("small", 16)])
 def test_wavefunction_force_parity(case, K):
-    """qmc_sweep_ex force_out: F = 2 grad log Psi_T (PAPER.md L155) of the moved electron at the
+    """qmc_sweep_ex force_out: F = 2 grad log Psi_T (PAPER.md L156) of the moved electron at the
     proposed configuration, for every move, against the oracle replaying the GPU's decisions and
     fp32 orbital vectors (its gradients come from its own fp64 spline).  Compared as F R / 2 =
     grad_r' R, which stays smooth next to a node: the north_star gradient tolerance (2e-5 of

@@ -137,6 +137,68 @@ def test_planewave_nodes_closed_form():
         assert abs(v[p, 0] - acc) < 1e-14
 
 
+def test_planewave_general_t_closed_form():
+    """Same table at GENERAL fractions t (the closed form of SURVEY P-d): with weights b_a(t_d),
+    phi = Re[ e^{i(kappa.i + theta)} prod_d sum_a b_a(t_d) e^{i kappa_d a} ], where the b_a are taken
+    from scipy's de Boor recursion (not from the oracle's polynomials); first s-derivatives likewise
+    with scipy's derivative basis.  Positions include cells that wrap in x and z."""
+    grid = (16, 12, 20)
+    nvec, theta = np.array([3, -2, 5]), 0.7
+    kap = 2 * np.pi * nvec / np.array(grid)
+    I = np.stack(np.meshgrid(*[np.arange(n) for n in grid], indexing="ij"), axis=-1)
+    exact = np.cos(I @ kap + theta)
+    coefs = exact[..., None].astype(np.float32)
+    lat = SKEW
+    rng = np.random.default_rng(21)
+    cells = np.array([[2, 3, 4], [15, 5, 19], [14, 11, 18], [13, 0, 17], [0, 0, 0], [15, 11, 19]])
+    tt = rng.uniform(0.02, 0.98, size=cells.shape)
+    pos = ((cells + tt) / np.array(grid)) @ lat
+    v, g, l = oracle.spline_vgl(coefs, lat, pos)
+    s, J = grid_coords(lat, grid, pos)
+    for p, (nd, t) in enumerate(zip(cells, tt)):
+        assert np.allclose(s[p], nd + t, atol=1e-9)
+        fac, dfac = [], []
+        for d in range(3):
+            b = _scipy_basis(grid[d], np.array([nd[d] + t[d]]), 0)[0]      # weights of control points by index
+            db = _scipy_basis(grid[d], np.array([nd[d] + t[d]]), 1)[0]
+            ph = np.exp(1j * kap[d] * np.arange(grid[d] + 3))     # extended control points m = 0..n+2
+            fac.append(np.sum(b * ph))
+            dfac.append(np.sum(db * ph))
+        e0 = np.exp(1j * theta)
+        phi = (e0 * fac[0] * fac[1] * fac[2]).real
+        d1 = np.array([(e0 * dfac[0] * fac[1] * fac[2]).real, (e0 * fac[0] * dfac[1] * fac[2]).real,
+                       (e0 * fac[0] * fac[1] * dfac[2]).real])
+        assert abs(v[p, 0] - phi) < 2e-7          # fp32 rounding of the table: |dc| <= 6e-8
+        assert np.allclose(g[p, :, 0], J @ d1, atol=5e-6)
+
+
+def test_cell_face_rounding_and_nonfinite_positions():
+    """R:A7 / R:A18.  A reduced coordinate that rounds UP to 1.0 (r = -1e-18 a0: u = -tiny,
+    u - floor(u) = 1.0 in fp64) is the point u = 0: cell 0, t = 0, the same bits as r = 0, and the
+    node weights (1,4,1,0)/6 applied to control points 0,1,2 give the value.  A non-finite position
+    gives NaN orbitals (never an out-of-range table read)."""
+    rng = np.random.default_rng(3)
+    grid, norb = (6, 5, 7), 4
+    coefs = rand_table(rng, grid, norb)
+    for lat in (ORTHO, SKEW):
+        for d in range(3):
+            eps = -1e-18 * lat[d]
+            u = eps @ np.linalg.inv(lat)
+            assert (u[d] - np.floor(u[d])) == 1.0                      # the case is really exercised
+            v, g, l = oracle.spline_vgl(coefs, lat, np.stack([eps, np.zeros(3), lat[d]]))
+            assert np.array_equal(v[0], v[1]) or np.max(np.abs(v[0] - v[1])) < 1e-15
+            assert np.max(np.abs(v[0] - v[2])) < 1e-14 and np.max(np.abs(g[0] - g[1])) < 1e-12
+            assert np.max(np.abs(l[0] - l[1])) < 1e-10
+        w = np.array([1, 4, 1]) / 6.0
+        cd = coefs.astype(np.float64)
+        ref = np.einsum("a,b,c,abcn->n", w, w, w, cd[:3, :3, :3])
+        v0 = oracle.spline_vgl(coefs, lat, np.zeros((1, 3)), want_gl=False)
+        assert np.max(np.abs(v0[0] - ref)) < 1e-15
+    for bad in (np.nan, np.inf, -np.inf):
+        v, g, l = oracle.spline_vgl(coefs, ORTHO, np.array([[0.3, bad, 0.1]]))
+        assert np.isnan(v).all() and np.isnan(g).all() and np.isnan(l).all()
+
+
 # ----------------------------------------------------------------------------- P-e, P-f
 def test_periodicity_and_continuity():
     rng = np.random.default_rng(3)
@@ -400,6 +462,34 @@ def test_accept_control_flow(sweep_case):
     assert np.array_equal(out_mt["B"], out_st["B"]) and np.array_equal(out_mt["ratios"], out_st["ratios"])
 
 
+def test_sweep_singular_and_nonfinite_moves(sweep_case):
+    """R:A8 / R:A18.  A NaN displacement gives a NaN ratio: rejected, nothing changes for that
+    walker at that step.  An IMPOSED accept of a move with R = 0 (orbital vector identically zero)
+    or NaN is refused: B, positions, log-det untouched; everything else proceeds as without it."""
+    x, coefs, A, B, ld, sg = sweep_case
+    delta = x.delta.copy()
+    delta[0, 3, 1, 2] = np.nan
+    out = oracle.sweep(coefs, x.lattice, x.pos, B, ld, sg, delta[:1], np.zeros_like(x.unif[:1]), iel_count=4)
+    assert np.isnan(out["ratios"][0, 3, 1]) and out["accept"][0, 3, 1] == 0
+    assert out["accept"][0, :3].all() and out["accept"][0, 3, [0, 2]].all()
+    assert np.array_equal(out["pos"][1, 3], x.pos[1, 3]) and np.isfinite(out["B"]).all()
+    ref = oracle.sweep(coefs, x.lattice, x.pos, B, ld, sg, x.delta[:1], np.zeros_like(x.unif[:1]), iel_count=3)
+    assert np.array_equal(out["B"][1], ref["B"][1]) and out["logdet"][1] == ref["logdet"][1]
+    # forced accept of R == 0 and of R = NaN
+    nel, nw = x.cfg.norb, x.cfg.nw
+    phi = np.ascontiguousarray(oracle.sweep(coefs, x.lattice, x.pos, B, ld, sg, x.delta[:1], x.unif[:1],
+                                            want_phi=True)["phi"].astype(np.float32))
+    phi[0, 2, 0, :] = 0.0
+    phi[0, 4, 2, 5] = np.nan
+    forced = np.ones((1, nel, nw), dtype=np.uint8)
+    out = oracle.sweep(coefs, x.lattice, x.pos, B, ld, sg, x.delta[:1], x.unif[:1], forced=forced, phi_in=phi)
+    assert out["ratios"][0, 2, 0] == 0.0 and out["accept"][0, 2, 0] == 0
+    assert np.isnan(out["ratios"][0, 4, 2]) and out["accept"][0, 4, 2] == 0
+    assert out["accept"].sum() == nel * nw - 2
+    assert np.isfinite(out["B"]).all() and np.isfinite(out["logdet"]).all()
+    assert np.array_equal(out["pos"][0, 2], x.pos[0, 2]) and np.array_equal(out["pos"][2, 4], x.pos[2, 4])
+
+
 def test_init_walkers_matches_numpy(sweep_case):
     x, coefs, A, B, ld, sg = sweep_case
     B2, ld2, sg2, A2 = oracle.init_walkers(coefs, x.lattice, x.pos, nthreads=2, want_A=True)
@@ -420,7 +510,7 @@ def test_bnorm_diagnostic(sweep_case):
 
 
 def test_wavefunction_force_against_finite_differences(sweep_case):
-    """F = 2 grad log Psi_T (PAPER.md L155, the F of eq. 11/13) of the moved electron at the proposed
+    """F = 2 grad log Psi_T (PAPER.md L156, the F of eq. 11/13) of the moved electron at the proposed
     configuration.  Pin independent of the oracle's formula: F R / 2 = grad_r' (det A'(r') / det A),
     a smooth function of r' even next to a node (where F itself diverges), against central finite
     differences of that determinant ratio taken by numpy from Slater matrices at shifted positions
