@@ -41,7 +41,9 @@ UNIT = "moves/s"
 DEFAULT_DELAY = {"tiny": [0], "small": [16, 0], "mid": [16, 0], "large": [16, 0], "xlarge": [16, 32, 0]}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures
 # (profiles/r01_*.md), config `large`
-NCU_TRAFFIC = {"sm_update": 6.725e9, "delayed_flush": 8.612e9, "spo_vgl": 2.254e9, "delayed_window": 0.147e9}
+# keyed by (kernel, delay rank); value = (bytes per launch, the file the figure comes from)
+NCU_TRAFFIC = {("sm_update", 0): (6.725e9, "profiles/r01_rank1_summary.md"),
+               ("delayed_flush", 16): (8.612e9, "profiles/r01_delayed_summary.md")}
 
 
 def measured_peaks():
@@ -179,7 +181,7 @@ def run_reference(args, rank, world):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="large", choices=list(inputs.CONFIGS))
     ap.add_argument("--delay", type=int, default=-1,
@@ -190,9 +192,19 @@ def main():
     ap.add_argument("--walkers", type=int, default=0, help="override walkers per GPU (debug)")
     args = ap.parse_args()
 
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # `python bench.py --gpus N`: launch N ranks (one per GPU) of this script, as the driver's
+        # torchrun command does, and let rank 0 print the line
+        import subprocess
+        port = 29500 + os.getpid() % 2000
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        sys.exit(subprocess.call(cmd))
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.gpus != world and rank == 0:
+        print(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}; running {world} rank(s)", file=sys.stderr)
     if args.impl == "reference":
         run_reference(args, rank, world)
         return
@@ -255,11 +267,11 @@ def main():
         def step(i):
             api.sweep(det, pos, delta[i:i + 1], unif[i:i + 1], ratios_out=ratios[i:i + 1], accept_out=accept[i:i + 1])
 
-        # ---- device-resident timing: inputs in HBM, CUDA events on the launching stream
+        # ---- device-resident timing: inputs in HBM, CUDA events on the launching stream, no
+        #      per-kernel instrumentation inside the timed region
         for i in range(args.warmup):
             step(i)
         barrier()
-        det.profile(True)
         launches0 = api.launch_count()
         sampler = ClockSampler(local_rank)
         sampler.start()
@@ -271,20 +283,29 @@ def main():
         barrier()
         clocks = sampler.stop()
         launches = api.launch_count() - launches0
-        ms = e0.elapsed_time(e1)
-        prof = det.profile_read()
-        det.profile(False)
-        ms = max_over_ranks(ms)
+        ms = max_over_ranks(e0.elapsed_time(e1))
         moves = args.steps * nel * nw * world
         value = moves / (ms * 1e-3)
-        acc_timed = accept[args.warmup:].to(torch.float64)
-        n_acc = float(acc_timed.sum().item())
-        acc_rate = n_acc / acc_timed.numel()
+        acc_rate = float(accept[args.warmup:].to(torch.float64).mean().item())
+
+        # ---- per-kernel split: a SECOND pass of `nprof` sweeps with every launch bracketed by CUDA
+        #      events (qmc_det_profile); the walk goes on with the random numbers of the first timed sweeps
+        nprof = min(args.steps, 5)
+        det.profile(True)
+        e0.record()
+        for i in range(args.warmup, args.warmup + nprof):
+            step(i)
+        e1.record()
+        barrier()
+        prof = det.profile_read()
+        det.profile(False)
+        ms_prof = e0.elapsed_time(e1)
+        n_acc = float(accept[args.warmup:args.warmup + nprof].to(torch.float64).sum().item())
 
         # ---- roofline of the dominant kernel (rank-local, from the per-launch CUDA events)
         ld, npitch, K = det.ld, spline.row_pitch, det.delay_rank
         per_launch = {   # algorithmic bytes per launch
-            "spo_vgl": (args.steps * nel * nw / max(prof["spo_vgl"][1], 1)) * (64 + 5) * npitch * 4,
+            "spo_vgl": (nprof * nel * nw / max(prof["spo_vgl"][1], 1)) * (64 + 5) * npitch * 4,
             "ratio_rowcopy": nw * (2 * 8 * ld + 4 * nel),
             "sm_update": (n_acc / max(prof["sm_update"][1], 1)) * (16 * nel * ld + 12 * nel),
             "delayed_flush": nw * 16 * nel * ld + (n_acc / max(prof["delayed_flush"][1], 1)) * (8 * ld + 4 * npitch),
@@ -295,7 +316,7 @@ def main():
         for k, (kms, kn) in prof.items():
             if not kn:
                 continue
-            kernels[k] = {"ms": kms, "launches": kn, "avg_us": 1e3 * kms / kn, "share_of_step": kms / ms}
+            kernels[k] = {"ms": kms, "launches": kn, "avg_us": 1e3 * kms / kn, "share_of_step": kms / ms_prof}
             if k in per_launch:
                 gbs = per_launch[k] / (kms / kn * 1e-3) / 1e9
                 kernels[k].update({"bytes_per_launch": per_launch[k], "GB/s": gbs, "frac_of_hbm_peak": gbs / peak})
@@ -309,17 +330,21 @@ def main():
                        "min_ms_fp64": fl / (fp64_peak * 1e12) * 1e3})
         dom = max(kernels, key=lambda k: kernels[k]["ms"])
         kd = kernels[dom]
-        traffic = NCU_TRAFFIC.get(dom) if (args.config == "large" and nw == cfg.nw) else None
+        # DRAM bytes per launch are an ncu measurement (no profiler runs inside bench.py): quoted from the
+        # committed capture of the same kernel and launch shape, with its source; null for other shapes
+        traffic, traffic_src = None, None
+        if args.config == "large" and nw == cfg.nw and (dom, K) in NCU_TRAFFIC:
+            traffic, traffic_src = NCU_TRAFFIC[(dom, K)]
         if dom == "delayed_flush" and kd["min_ms_fp64"] > kd["min_ms_hbm"]:
             # the contraction, not the pass over B, bounds this rank: report against the fp64 tensor peak
             roofline = {"bound": "tensor", "kernel": dom, "achieved": kd["fp64_TFLOP/s"], "peak": fp64_peak,
-                        "unit": "TFLOP/s", "frac": kd["frac_of_fp64_dmma_peak"], "traffic": traffic,
+                        "unit": "TFLOP/s", "frac": kd["frac_of_fp64_dmma_peak"], "traffic": traffic, "traffic_source": traffic_src,
                         "peak_source": "measured live: qmc_probe_fp64_dmma (DMMA.8x8x4 issue loop)",
                         "launches": kd["launches"], "avg_us": kd["avg_us"], "flops_per_launch": kd["flops_per_launch"],
                         "share_of_step": kd["share_of_step"]}
         else:
             roofline = {"bound": "hbm", "kernel": dom, "achieved": kd.get("GB/s"), "peak": peak, "unit": "GB/s",
-                        "frac": kd.get("frac_of_hbm_peak"), "traffic": traffic, "peak_source": peak_src,
+                        "frac": kd.get("frac_of_hbm_peak"), "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
                         "launches": kd["launches"], "avg_us": kd["avg_us"], "bytes_per_launch": kd.get("bytes_per_launch"),
                         "share_of_step": kd["share_of_step"]}
 
@@ -348,6 +373,7 @@ def main():
         update = "sherman-morrison rank-1" if K == 0 else f"delayed rank-{K} (same result as rank-1)"
         det.destroy()
         return {"value": value, "ms_per_step": ms / args.steps, "update": update, "accept_rate": acc_rate,
+                "kernel_split": f"second pass of {nprof} sweeps with per-launch CUDA events ({ms_prof / nprof:.2f} ms per sweep)",
                 "init_s": t_init, "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
                 "kernels": kernels, "spline_evals_per_s": value * nel}
 
@@ -369,7 +395,7 @@ def main():
                    "l2": l2_note,
                    "spo_dtype": "f32", "accept_rate": main_arm["accept_rate"], "init_s": main_arm["init_s"]},
         "clocks": main_arm["clocks"], "e2e": main_arm["e2e"], "gpu_launches": main_arm["gpu_launches"],
-        "roofline": main_arm["roofline"], "kernels": main_arm["kernels"],
+        "roofline": main_arm["roofline"], "kernels": main_arm["kernels"], "kernel_split": main_arm["kernel_split"],
         "spline_evals_per_s": main_arm["spline_evals_per_s"],
     }
     if len(arms) > 1:

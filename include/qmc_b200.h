@@ -106,6 +106,38 @@ int qmc_det_init(qmc_det_t **out, const qmc_spline_t *spline, int nwalkers, int 
 int qmc_det_destroy(qmc_det_t *det);
 
 /* ---------------------------------------------------------------------------------------
+ * qmc_det_init_ex -- qmc_det_init with flags.  QMC_DET_FP32_INVERSE: "the numerical
+ * precision is parameterized, with single, double and mixed precision": the handle STORES
+ * B = (A^-1)^T in fp32, float [nwalkers][nel][ld] (half the bytes every update and flush moves; reading
+ * R:A19 of DESIGN.md): the initial inverse is computed in fp64 and rounded once; every kernel converts
+ * the rows it reads to fp64, does all arithmetic (ratios, Sherman-Morrison multipliers, the tensor-core
+ * contractions of the delayed update, log|det|) in fp64, and rounds to nearest even when it stores --
+ * after every accepted update (delay_rank <= 1) or once per window flush (delay_rank >= 2).  The
+ * rounding error accumulates slowly: monitor it with qmc_det_residual and refresh the inverse from the
+ * positions with qmc_det_recompute every few sweeps.
+ */
+#define QMC_DET_FP32_INVERSE 1u
+int qmc_det_init_ex(qmc_det_t **out, const qmc_spline_t *spline, int nwalkers, int nel,
+                    const double *pos, int delay_rank, unsigned flags, void *stream);
+/* 8 (fp64 inverse) or 4 (QMC_DET_FP32_INVERSE). */
+int qmc_det_storage(const qmc_det_t *det, int *bytes_per_element);
+
+/* qmc_det_recompute -- the inverse, log|det| and sign of every walker again from scratch at `pos`
+ * (dev, double [nwalkers][nel][3]), exactly as qmc_det_init computes them (Slater matrix from the SPO
+ * kernel, Gauss-Jordan in fp64, rounded once for fp32 storage); the accept counters are kept and an
+ * open delayed window is closed first.  The "recompute" of mixed precision (L82; R:A19) and of
+ * north_star's residual check.  Synchronises `stream`.  QMC_ESINGULAR leaves the inverse undefined. */
+int qmc_det_recompute(qmc_det_t *det, const qmc_spline_t *spline, const double *pos, void *stream);
+
+/* qmc_det_residual -- drift monitor: resid_out[w] (dev, double [nwalkers]) =
+ *     max over the nsample electrons i = s * (nel / nsample) and all k of | B_w[k] . phi(r_i) - delta_ik |
+ * i.e. nsample rows of A B^T - I with A recomputed by the SPO kernel at `pos` (R:A11); one pass over B
+ * per call.  nsample * nel * 8 bytes must fit 96 KB of shared memory.  Pending delayed updates are
+ * applied first.  Synchronises `stream`. */
+int qmc_det_residual(qmc_det_t *det, const qmc_spline_t *spline, const double *pos, int nsample,
+                     double *resid_out, void *stream);
+
+/* ---------------------------------------------------------------------------------------
  * qmc_det_ratio -- L299: for a single-electron move of electron iel to a position where the
  * orbitals take the values phi, det A'/det A = sum_j B[iel][j] * phi[j] (fp64 accumulation of
  * the upcast fp32 orbital vector; warp-shuffle tree, fixed order).  With a delayed window open
@@ -209,7 +241,8 @@ int qmc_sweep_host(qmc_det_t *det, const qmc_spline_t *spline, double *pos_host,
 
 /* ---------------------------------------------------------------------------------------
  * State access (checkpoint / parity).  Pending delayed updates are flushed first.
- *   qmc_det_get_inverse   binv_out dev double [nwalkers][nel][nel] dense, B = (A^-1)^T
+ *   qmc_det_get_inverse   binv_out dev double [nwalkers][nel][nel] dense, B = (A^-1)^T (fp32 storage:
+ *                         upcast exactly; set_inverse rounds to nearest even)
  *   qmc_det_set_inverse   the reverse (binv_in dense); logdet / sign dev arrays or NULL (kept)
  *   qmc_det_get_stats     dev: logdet double [nwalkers], sign int [nwalkers],
  *                         naccept long long [nwalkers]; any may be NULL

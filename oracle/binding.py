@@ -20,6 +20,12 @@ _ip = ctypes.POINTER(ctypes.c_int)
 _bp = ctypes.POINTER(ctypes.c_ubyte)
 
 
+class SweepOpts(ctypes.Structure):
+    """orc_sweep_opts of qmc_oracle.c."""
+    _fields_ = [("tau", ctypes.c_double), ("rprop_in", _dp), ("rprop_out", _dp), ("fcur_out", _dp),
+                ("logt_out", _dp), ("b32", ctypes.c_int)]
+
+
 def build(force=False):
     """Compile qmc_oracle.c with gcc -O2 (no fast-math, no intrinsics) into oracle/."""
     if (not force and os.path.exists(_LIB)
@@ -52,6 +58,8 @@ def _load():
                                   _dp, _dp, _dp, _dp, _ip, _dp, _dp, ctypes.c_int, ctypes.c_int,
                                   _dp, _bp, _bp, _fp, _dp, ctypes.c_int, ctypes.c_int, _dp,
                                   ctypes.c_int, _dp])
+        lib.orc_sweep_ex.restype = ctypes.c_int
+        lib.orc_sweep_ex.argtypes = lib.orc_sweep.argtypes + [ctypes.POINTER(SweepOpts)]
         lib.orc_init_walkers.restype = ctypes.c_int
         lib.orc_init_walkers.argtypes = ([ctypes.c_int] * 4 + [_dp, _fp, ctypes.c_int, ctypes.c_int,
                                          _dp, _dp, _dp, _dp, _ip, ctypes.c_int])
@@ -200,10 +208,13 @@ def init_walkers(coefs, lattice, pos, nthreads=1, want_A=False):
 
 def sweep(coefs, lattice, pos, B, logdet, sign, delta, unif, A=None, iel_count=None,
           forced=None, phi_in=None, want_phi=False, mode=0, nthreads=1, want_bnorm=False,
-          fixed_node=False, want_force=False):
+          fixed_node=False, want_force=False, tau=0.0, rprop_in=None, b32=0):
     """Run nsweeps particle-by-particle sweeps.  Inputs are copied; returns a dict with
     pos, B, A, logdet, sign, ratios [nsweeps][nel][nw], accept (uint8, same shape), phi, force
-    (F = 2 grad log|Psi| of the moved electron at the proposed configuration, [nsweeps][nel][nw][3])."""
+    (F = 2 grad log|Psi| of the moved electron at the proposed configuration, [nsweeps][nel][nw][3]).
+    tau > 0: drift moves (delta = the Gaussian part chi ~ N(0, tau)); adds rprop, fcur, logt to the
+    result; rprop_in replays given proposals.  b32: fp32-stored inverse (1 = rounded after every
+    accepted update, K >= 2 = at the end of every window of K steps); B must hold fp32 values."""
     lib = _load()
     coefs = _coefs(coefs)
     nx, ny, nz, norb = coefs.shape
@@ -235,11 +246,20 @@ def sweep(coefs, lattice, pos, B, logdet, sign, delta, unif, A=None, iel_count=N
     phi_out = np.zeros((nsweeps, nel, nw, nel)) if want_phi else None
     bnorm = np.zeros((nsweeps, nel, nw)) if want_bnorm else None
     force = np.zeros((nsweeps, nel, nw, 3)) if want_force else None
-    rc = lib.orc_sweep(nx, ny, nz, norb, _d(lat), coefs.ctypes.data_as(_fp), nw, nel,
-                       _d(pos), _d(B), _d(A), _d(logdet), sign.ctypes.data_as(_ip),
-                       _d(delta), _d(unif), nsweeps, int(iel_count), _d(ratios),
-                       accept.ctypes.data_as(_bp), f_ptr, p_ptr, _d(phi_out), int(mode),
-                       int(nthreads), _d(bnorm), int(bool(fixed_node)), _d(force))
+    drift = tau > 0.0
+    rprop = np.zeros((nsweeps, nel, nw, 3)) if drift else None
+    fcur = np.zeros((nsweeps, nel, nw, 3)) if drift else None
+    logt = np.zeros((nsweeps, nel, nw)) if drift else None
+    if rprop_in is not None:
+        rprop_in = _c64(rprop_in, (nsweeps, nel, nw, 3))
+    if b32:
+        assert np.array_equal(B, B.astype(np.float32).astype(np.float64)), "b32: B must hold fp32 values"
+    opts = SweepOpts(float(tau), _d(rprop_in), _d(rprop), _d(fcur), _d(logt), int(b32))
+    rc = lib.orc_sweep_ex(nx, ny, nz, norb, _d(lat), coefs.ctypes.data_as(_fp), nw, nel,
+                          _d(pos), _d(B), _d(A), _d(logdet), sign.ctypes.data_as(_ip),
+                          _d(delta), _d(unif), nsweeps, int(iel_count), _d(ratios),
+                          accept.ctypes.data_as(_bp), f_ptr, p_ptr, _d(phi_out), int(mode),
+                          int(nthreads), _d(bnorm), int(bool(fixed_node)), _d(force), ctypes.byref(opts))
     _check(rc, "sweep")
     return dict(pos=pos, B=B, A=A, logdet=logdet, sign=sign, ratios=ratios, accept=accept,
-                phi=phi_out, bnorm=bnorm, force=force)
+                phi=phi_out, bnorm=bnorm, force=force, rprop=rprop, fcur=fcur, logt=logt)

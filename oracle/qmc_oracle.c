@@ -28,6 +28,13 @@
  *                     eq. 13 with F = 0; acceptance eq. 12 with symmetric T and
  *                     a determinant-only Psi: accept iff R*R > u (R:A8).
  *
+ *   orc_sweep_ex      the same with options: (i) drift moves, L183-199: the proposal of eq. 13 with
+ *                     the wavefunction force F = 2 grad log Psi_T (L156) and the acceptance of
+ *                     eq. 12 with the ratio T(r'->r)/T(r->r') of the Gaussians of eq. 11 / eq. 13
+ *                     (R:A20: lambda = 1/2); (ii) single-precision storage of the inverse, L82
+ *                     "single, double and mixed precision" (R:A19: B rounded to fp32 when stored,
+ *                     all arithmetic in fp64), with orc_init_walkers as the recompute-from-scratch.
+ *
  * Pins (tests/test_oracle_pins.py, run with -m "not gpu"): partition of unity,
  * polynomial reproduction, plane-wave node closed form, periodicity, C2
  * continuity, scipy.interpolate.BSpline tensor product, central finite
@@ -350,15 +357,62 @@ int orc_sm_update(int n, double *B, int k, const double *phi, double R)
  * r_k <- r_k + delta (one fp64 add), row k of A <- phi, log|det| += log|R|,
  * sign *= sgn(R), B updated.  Returns 0 or the first error code met.
  */
-int orc_sweep(int nx, int ny, int nz, int norb, const double lattice[9], const float *coefs,
+/*
+ * Options of orc_sweep_ex (all zero / NULL = orc_sweep).
+ *
+ * Drift moves (R:A20).  tau > 0 switches them on.  With lambda = 1/2 (electrons,
+ * Hartree atomic units) eq. 13 reads T(r_k -> r_k') ~ exp(-|r_k' - r_k - tau F_k(r)|^2 / (2 tau)),
+ * i.e. r_k' = r_k + tau F_k(r) + chi with chi ~ N(0, tau) per component (eq. 19 for one electron);
+ * `delta` holds chi.  F_k(r) = 2 grad_k log|det A| = 2 sum_j grad phi_j(r_k) B[k][j] at the CURRENT
+ * configuration (L156); F_k(r') = 2 sum_j grad phi_j(r_k') B[k][j] / R at the proposed one.  The
+ * move is accepted with the probability of eq. 12,
+ *     min(1, R^2 T(r'->r) / T(r->r')),   log T(r'->r)/T(r->r') = (|chi|^2 - |r_k - r_k' - tau F_k(r')|^2) / (2 tau),
+ * i.e. iff R^2 exp(logT) > u.  With tau -> 0+ ... the no-drift walk is NOT recovered by tau = 0 (that
+ * switches drift off and uses delta as the whole displacement, eq. 13 with F = 0).
+ *   rprop_in   NULL, or [nsweeps][nel][nw][3]: proposed positions to use instead of r + tau F + chi
+ *              (replay of another implementation's proposals; the forward density still uses this
+ *              oracle's own F_k(r): log T = (|r_k' - r_k - tau F_k(r)|^2 - |r_k - r_k' - tau F_k(r')|^2) / (2 tau))
+ *   rprop_out  NULL, or same shape: the proposed positions used
+ *   fcur_out   NULL, or [nsweeps][nel][nw][3]: F_k(r) at the current configuration
+ *   logt_out   NULL, or [nsweeps][nel][nw]: log T(r'->r)/T(r->r')  (-inf... finite only when R != 0)
+ *
+ * Single-precision storage of the inverse (R:A19).  b32 != 0: B holds values that are
+ * exactly representable in fp32 on entry (the caller rounds the initial inverse) and is rounded to
+ * fp32 (round to nearest even, the C cast) whenever it is STORED: after every accepted update when
+ * b32 == 1 (rank-1 Sherman-Morrison), or -- b32 = K >= 2, the delayed update of rank K -- when a
+ * window of K consecutive electron steps closes (k % K == K - 1 within the moved range, or the end of
+ * the sweep), the accepted updates inside the window being applied in fp64 to the unrounded matrix.
+ * Ratios, Sherman-Morrison multipliers and log|det| are fp64 arithmetic on those stored values.
+ */
+typedef struct orc_sweep_opts {
+    double tau;
+    const double *rprop_in;
+    double *rprop_out, *fcur_out, *logt_out;
+    int b32;
+} orc_sweep_opts;
+
+static void round_to_fp32(double *x, size_t n)
+{
+    for (size_t i = 0; i < n; ++i) x[i] = (double)(float)x[i];
+}
+
+int orc_sweep_ex(int nx, int ny, int nz, int norb, const double lattice[9], const float *coefs,
               int nw, int nel, double *pos, double *B, double *A, double *logdet, int *sign,
               const double *delta, const double *unif, int nsweeps, int iel_count,
               double *ratios_out, unsigned char *accept_out, const unsigned char *forced,
               const float *phi_in, double *phi_out, int mode, int nthreads, double *bnorm_out,
-              int fixed_node, double *force_out)
+              int fixed_node, double *force_out, const orc_sweep_opts *opts)
 {
     if (nel != norb || nw < 0 || nsweeps < 0 || iel_count < 0 || iel_count > nel) return -1;
     if (mode == 1 && !A) return -1;
+    const double tau = opts ? opts->tau : 0.0;
+    const int drift = tau > 0.0;
+    const int b32 = opts ? opts->b32 : 0;
+    const double *rprop_in = opts ? opts->rprop_in : NULL;
+    double *rprop_out = opts ? opts->rprop_out : NULL;
+    double *fcur_out = opts ? opts->fcur_out : NULL;
+    double *logt_out = opts ? opts->logt_out : NULL;
+    if (b32 < 0 || (opts && opts->tau < 0.0)) return -1;
     int rc_all = 0;
     size_t nn = (size_t)nel * nel;
 #ifdef _OPENMP
@@ -367,16 +421,33 @@ int orc_sweep(int nx, int ny, int nz, int norb, const double lattice[9], const f
 #endif
     for (int w = 0; w < nw; ++w) {
         double *phi = (double *)malloc((size_t)nel * sizeof(double));
-        double *grad = force_out ? (double *)malloc((size_t)4 * nel * sizeof(double)) : NULL;   /* 3 gradients + scratch values */
+        const int want_grad = force_out || drift;
+        double *grad = want_grad ? (double *)malloc((size_t)4 * nel * sizeof(double)) : NULL;   /* 3 gradients + scratch values */
         double *Bw = B + (size_t)w * nn;
         double *Aw = A ? A + (size_t)w * nn : NULL;
-        int rc = (phi && (grad || !force_out)) ? 0 : -2;
+        int rc = (phi && (grad || !want_grad)) ? 0 : -2;
         for (int s = 0; s < nsweeps && rc == 0; ++s)
             for (int k = 0; k < iel_count && rc == 0; ++k) {
                 size_t mv = ((size_t)s * nel + k) * nw + w;
                 double *rk = pos + ((size_t)w * nel + k) * 3;
-                double rnew[3] = {rk[0] + delta[3 * mv + 0], rk[1] + delta[3 * mv + 1],
-                                  rk[2] + delta[3 * mv + 2]};
+                double fcur[3] = {0.0, 0.0, 0.0};
+                if (drift) {           /* F_k(r) = 2 sum_j grad phi_j(r_k) B[k][j], current configuration */
+                    rc = orc_spline_vgl(nx, ny, nz, norb, lattice, coefs, 1, rk, grad + (size_t)3 * nel, grad, NULL);
+                    if (rc) break;
+                    for (int d = 0; d < 3; ++d) {
+                        double gd = 0.0;
+                        for (int j = 0; j < nel; ++j) gd += grad[(size_t)d * nel + j] * Bw[(size_t)k * nel + j];
+                        fcur[d] = 2.0 * gd;
+                    }
+                    if (fcur_out) { fcur_out[3 * mv] = fcur[0]; fcur_out[3 * mv + 1] = fcur[1]; fcur_out[3 * mv + 2] = fcur[2]; }
+                }
+                double rnew[3];
+                for (int d = 0; d < 3; ++d) {
+                    if (drift && rprop_in) rnew[d] = rprop_in[3 * mv + d];
+                    else if (drift) rnew[d] = rk[d] + (tau * fcur[d] + delta[3 * mv + d]);
+                    else rnew[d] = rk[d] + delta[3 * mv + d];
+                }
+                if (rprop_out) { rprop_out[3 * mv] = rnew[0]; rprop_out[3 * mv + 1] = rnew[1]; rprop_out[3 * mv + 2] = rnew[2]; }
                 if (phi_in) {
                     for (int j = 0; j < nel; ++j) phi[j] = (double)phi_in[mv * nel + j];
                 } else {
@@ -385,17 +456,31 @@ int orc_sweep(int nx, int ny, int nz, int norb, const double lattice[9], const f
                 }
                 if (phi_out) memcpy(phi_out + mv * nel, phi, (size_t)nel * sizeof(double));
                 double R = orc_det_ratio(nel, Bw, k, phi);
-                if (force_out) {       /* F = 2 grad_k log|det A'| at the proposed configuration */
+                double fnew[3] = {0.0, 0.0, 0.0}, logt = 0.0;
+                if (want_grad) {       /* F = 2 grad_k log|det A'| at the proposed configuration */
                     rc = orc_spline_vgl(nx, ny, nz, norb, lattice, coefs, 1, rnew, grad + (size_t)3 * nel, grad, NULL);
                     if (rc) break;
                     for (int d = 0; d < 3; ++d) {
                         double gd = 0.0;
                         for (int j = 0; j < nel; ++j) gd += grad[(size_t)d * nel + j] * Bw[(size_t)k * nel + j];
-                        force_out[3 * mv + d] = (R != 0.0) ? 2.0 * gd / R : 0.0;
+                        fnew[d] = (R != 0.0) ? 2.0 * gd / R : 0.0;
+                        if (force_out) force_out[3 * mv + d] = fnew[d];
                     }
+                }
+                if (drift) {           /* log T(r'->r)/T(r->r'), eq. 11-13 with lambda = 1/2 */
+                    double fwd = 0.0, bwd = 0.0;
+                    for (int d = 0; d < 3; ++d) {
+                        double a = rnew[d] - rk[d] - tau * fcur[d];
+                        double b = rk[d] - rnew[d] - tau * fnew[d];
+                        fwd += a * a;
+                        bwd += b * b;
+                    }
+                    logt = (fwd - bwd) / (2.0 * tau);
+                    if (logt_out) logt_out[mv] = logt;
                 }
                 int acc;
                 if (forced) acc = forced[mv] != 0 && isfinite(R) && R != 0.0; /* R:A18 */
+                else if (drift) acc = isfinite(R) && isfinite(logt) && (R * R * exp(logt) > unif[mv]) && !(fixed_node && R < 0.0);
                 else acc = isfinite(R) && (R * R > unif[mv]) && !(fixed_node && R < 0.0);
                 if (ratios_out) ratios_out[mv] = R;
                 if (bnorm_out) {
@@ -404,13 +489,17 @@ int orc_sweep(int nx, int ny, int nz, int norb, const double lattice[9], const f
                     bnorm_out[mv] = bn;
                 }
                 if (accept_out) accept_out[mv] = (unsigned char)acc;
-                if (!acc) continue;
-                rk[0] = rnew[0]; rk[1] = rnew[1]; rk[2] = rnew[2];
-                if (Aw) memcpy(Aw + (size_t)k * nel, phi, (size_t)nel * sizeof(double));
-                logdet[w] += log(fabs(R));
-                if (R < 0.0) sign[w] = -sign[w];
-                if (mode == 1) rc = orc_binv_from_A(nel, Aw, Bw, NULL, NULL);
-                else rc = orc_sm_update(nel, Bw, k, phi, R);
+                if (acc) {
+                    rk[0] = rnew[0]; rk[1] = rnew[1]; rk[2] = rnew[2];
+                    if (Aw) memcpy(Aw + (size_t)k * nel, phi, (size_t)nel * sizeof(double));
+                    logdet[w] += log(fabs(R));
+                    if (R < 0.0) sign[w] = -sign[w];
+                    if (mode == 1) rc = orc_binv_from_A(nel, Aw, Bw, NULL, NULL);
+                    else rc = orc_sm_update(nel, Bw, k, phi, R);
+                    if (b32 == 1) round_to_fp32(Bw, nn);
+                }
+                /* delayed rank-K storage: the window of K steps closes here (R:A19) */
+                if (b32 >= 2 && (k % b32 == b32 - 1 || k == iel_count - 1)) round_to_fp32(Bw, nn);
             }
         free(phi);
         free(grad);
@@ -422,6 +511,18 @@ int orc_sweep(int nx, int ny, int nz, int norb, const double lattice[9], const f
         }
     }
     return rc_all;
+}
+
+int orc_sweep(int nx, int ny, int nz, int norb, const double lattice[9], const float *coefs,
+              int nw, int nel, double *pos, double *B, double *A, double *logdet, int *sign,
+              const double *delta, const double *unif, int nsweeps, int iel_count,
+              double *ratios_out, unsigned char *accept_out, const unsigned char *forced,
+              const float *phi_in, double *phi_out, int mode, int nthreads, double *bnorm_out,
+              int fixed_node, double *force_out)
+{
+    return orc_sweep_ex(nx, ny, nz, norb, lattice, coefs, nw, nel, pos, B, A, logdet, sign, delta, unif,
+                        nsweeps, iel_count, ratios_out, accept_out, forced, phi_in, phi_out, mode, nthreads,
+                        bnorm_out, fixed_node, force_out, NULL);
 }
 
 /* Slater matrices A[w][i][j] = phi_j(r_{w,i}) (L325) for nw walkers. */

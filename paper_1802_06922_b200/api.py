@@ -22,7 +22,9 @@ EXPORTS = [
     "qmc_sweep", "qmc_sweep_ex", "qmc_sweep_host", "qmc_det_get_inverse", "qmc_det_set_inverse",
     "qmc_det_get_stats", "qmc_det_info", "qmc_launch_count", "qmc_det_profile", "qmc_det_profile_read",
     "qmc_probe_fp64_dmma", "qmc_det_kinetic", "qmc_det_ratio_points",
+    "qmc_det_init_ex", "qmc_det_storage", "qmc_det_recompute", "qmc_det_residual",
 ]
+QMC_DET_FP32_INVERSE = 1
 PROF_KINDS = ["spo_vgl", "sm_update", "delayed_window", "delayed_accept", "delayed_flush", "ratio_rowcopy"]
 
 
@@ -73,6 +75,10 @@ def load_library(path=None):
         "qmc_probe_fp64_dmma": [ctypes.POINTER(d), _vp],
         "qmc_det_kinetic": [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp],
         "qmc_det_ratio_points": [_vp, i, i, _vp, i, _vp, _vp],
+        "qmc_det_init_ex": [ctypes.POINTER(_vp), _vp, i, i, _vp, i, ctypes.c_uint, _vp],
+        "qmc_det_storage": [_vp, ctypes.POINTER(i)],
+        "qmc_det_recompute": [_vp, _vp, _vp, _vp],
+        "qmc_det_residual": [_vp, _vp, _vp, i, _vp, _vp],
     }
     for name, args in sigs.items():
         fn = getattr(lib, name)
@@ -195,17 +201,36 @@ class Det:
         _check(lib.qmc_det_info(self._h, ctypes.byref(a), ctypes.byref(b), ctypes.byref(c), ctypes.byref(e)),
                "qmc_det_info")
         self.nw, self.nel, self.ld, self.delay_rank = a.value, b.value, c.value, e.value
+        _check(lib.qmc_det_storage(self._h, ctypes.byref(a)), "qmc_det_storage")
+        self.storage_bytes = a.value            # 8: fp64 inverse, 4: fp32-stored inverse
 
     @classmethod
-    def init(cls, spline, pos, delay_rank=0, stream=None):
-        """qmc_det_init: pos double [nw][nel][3] on the device."""
+    def init(cls, spline, pos, delay_rank=0, fp32_inverse=False, stream=None):
+        """qmc_det_init / qmc_det_init_ex: pos double [nw][nel][3] on the device."""
         lib = load_library()
         nw, nel, _ = pos.shape
         h = _vp()
-        rc = lib.qmc_det_init(ctypes.byref(h), spline._h, nw, nel, _dev(pos, torch.float64), int(delay_rank),
-                              _stream(stream))
+        if fp32_inverse:
+            rc = lib.qmc_det_init_ex(ctypes.byref(h), spline._h, nw, nel, _dev(pos, torch.float64), int(delay_rank),
+                                     QMC_DET_FP32_INVERSE, _stream(stream))
+        else:
+            rc = lib.qmc_det_init(ctypes.byref(h), spline._h, nw, nel, _dev(pos, torch.float64), int(delay_rank),
+                                  _stream(stream))
         _check(rc, "qmc_det_init")
         return cls(h, spline)
+
+    def recompute(self, pos, stream=None):
+        """qmc_det_recompute: inverse, log|det| and sign again from scratch at pos."""
+        rc = load_library().qmc_det_recompute(self._h, self.spline._h, _dev(pos, torch.float64), _stream(stream))
+        _check(rc, "qmc_det_recompute")
+
+    def residual(self, pos, nsample=4, stream=None):
+        """qmc_det_residual -> double [nw]: max |B[k] . phi(r_i) - delta_ik| over nsample electrons i, all k."""
+        out = torch.empty(self.nw, dtype=torch.float64, device=pos.device)
+        rc = load_library().qmc_det_residual(self._h, self.spline._h, _dev(pos, torch.float64), int(nsample),
+                                             _dev(out, None), _stream(stream))
+        _check(rc, "qmc_det_residual")
+        return out
 
     def destroy(self):
         if self._h:

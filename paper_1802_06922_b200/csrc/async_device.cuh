@@ -41,9 +41,24 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
                  "l"(src), "r"(bytes), "r"(smem_u32(bar))
                  : "memory");
 }
+// Bulk prefetch global -> L2 (no destination, no completion): brings the lines in ahead of the bulk
+// copy that will stage them in shared memory, so that copy pays the L2 latency, not the HBM one.
+__device__ __forceinline__ void bulk_prefetch_l2(const void *src, uint32_t bytes)
+{
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
+}
 __device__ __forceinline__ void group_sync(int id, int nthreads)
 {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+// named barriers (ids 1..15; `nthreads` = threads that take part, arrivals + waiters, a multiple of 32)
+__device__ __forceinline__ void named_sync(int id, int nthreads)
+{
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+__device__ __forceinline__ void named_arrive(int id, int nthreads)
+{
+    asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 // thread-block cluster helpers (CS > 1: the CTAs of a cluster own column slices of the same rows)
 __device__ __forceinline__ uint32_t cluster_ctarank()
@@ -75,6 +90,13 @@ __device__ __forceinline__ uint32_t mapa_u32(const void *local, uint32_t rank)
 {
     uint32_t raddr;
     asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(raddr) : "r"(smem_u32(local)), "r"(rank));
+    return raddr;
+}
+// the same from a shared::cta address already converted to 32 bits
+__device__ __forceinline__ uint32_t mapa_addr(uint32_t local_addr, uint32_t rank)
+{
+    uint32_t raddr;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(raddr) : "r"(local_addr), "r"(rank));
     return raddr;
 }
 // asynchronous store of one double into the shared memory of a cluster CTA; the 8 bytes are counted

@@ -78,13 +78,21 @@ struct qmc_det {
     int nw, nel, ld, delay;
     int device, nsm;            // the CUDA device the handle lives on and its SM count (grid sizing)
     int np;                     // spline row pitch (floats)
-    double *B;                  // [nw][nel][ld]   (A^-1)^T, pad columns zero
+    double *B;                  // [nw][nel][ld]   (A^-1)^T, pad columns zero (fp64 storage; NULL when b32)
+    int b32;                    // 1: the inverse is STORED in fp32 (R:A19): Bf is used instead of B
+    float *Bf;                  // [nw][nel][ld]   the same matrix in fp32 (NULL unless b32)
     double *logdet;             // [nw]
     int *sign;                  // [nw]
     long long *naccept;         // [nw]
     // scratch owned by the handle
     int spo_batch;              // electron steps whose SPO-VGL is evaluated per launch (qmc_sweep)
     float *vgl;                 // [spo_batch][nw][5][np]   v, gx, gy, gz, lap of the proposals of a batch
+    // delayed mode: the SPO-VGL of window i+1 is evaluated on a second stream while window i is
+    // flushed (the proposals of a window depend on nothing the previous window changes)
+    float *vgl_buf[2];          // vgl_buf[0] == the allocation vgl points into first; [1] only when overlap is on
+    cudaStream_t aux;           // second stream (non-blocking), created on first use
+    cudaEvent_t ev_spo[2], ev_main;
+    int overlap;                // 1: overlap enabled (delay >= 2 and QMC_SWEEP_OVERLAP != 0)
     double *rowk;               // [nw][ld]      copy of row iel of B taken before the update
     double *ratio;              // [nw]      ratio of the current step (ratio_rowcopy_kernel -> sm_update_kernel)
     unsigned char *acc;         // [nw]
@@ -111,6 +119,13 @@ struct qmc_det {
     std::vector<int> *prof_kinds;            // kind of pair i
     size_t prof_used;                        // events handed out since the last reset
 };
+
+// Run `...` with TB = the handle's storage type and Bp = its matrix.
+#define QMC_WITH_B(d, TB, Bp, ...)                                                         \
+    do {                                                                                   \
+        if ((d)->b32) { using TB = float; TB *Bp = (d)->Bf; (void)Bp; __VA_ARGS__; }       \
+        else { using TB = double; TB *Bp = (d)->B; (void)Bp; __VA_ARGS__; }                \
+    } while (0)
 
 namespace qmc {
 enum ProfKind { kProfSpoRatio = 0, kProfUpdate = 1, kProfDelayedRatio = 2, kProfDelayedAccept = 3,
@@ -146,6 +161,17 @@ __device__ __forceinline__ double block_sum(double x, double *red)
     __syncthreads();
     return red[32];
 }
+
+// Storage type of the inverse (double, or float for the single-precision inverse of PAPER.md L82,
+// R:A19): two consecutive elements as fp64, and back (one rounding to nearest even when TB = float).
+__device__ __forceinline__ double2 ld2(const double *p) { return *reinterpret_cast<const double2 *>(p); }
+__device__ __forceinline__ double2 ld2(const float *p)
+{
+    const float2 f = *reinterpret_cast<const float2 *>(p);
+    return make_double2((double)f.x, (double)f.y);
+}
+__device__ __forceinline__ void st2(double *p, double2 v) { *reinterpret_cast<double2 *>(p) = v; }
+__device__ __forceinline__ void st2(float *p, double2 v) { *reinterpret_cast<float2 *>(p) = make_float2((float)v.x, (float)v.y); }
 
 __device__ __forceinline__ float4 ldg_stream(const float4 *p)
 {

@@ -22,7 +22,7 @@ namespace qmc {
 constexpr int kStepThreads = 256;
 
 struct DelayedStepArgs {
-    const double *B;              // [nw][nel][ld]  (B0 during a window)
+    const void *B;                // TB [nw][nel][ld]  (B0 during a window)
     int nel, ld, np, iel, K;
     const float *phi;             // [nw][ldphi]
     size_t ldphi;
@@ -45,7 +45,7 @@ struct DelayedStepArgs {
 // accumulates the 2p+1 partial dots d, x_m, c_l over its columns; the block reduces them in a
 // fixed order; warp 0 finishes the ratio and, on accept, the block grows the window (row copy,
 // orbital vector copy, bordered S^-1).
-template <int KMAX>
+template <typename TB, int KMAX>
 __global__ void __launch_bounds__(kStepThreads) delayed_step_kernel(DelayedStepArgs a)
 {
     constexpr int NV = 2 * KMAX + 1;
@@ -56,7 +56,7 @@ __global__ void __launch_bounds__(kStepThreads) delayed_step_kernel(DelayedStepA
     const int w = blockIdx.x, tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int p = a.win_count[w];
     const int K = a.K, ld = a.ld, np = a.np;
-    const double *b0k = a.B + ((size_t)w * a.nel + a.iel) * ld;
+    const TB *b0k = reinterpret_cast<const TB *>(a.B) + ((size_t)w * a.nel + a.iel) * ld;
     const float *phi = a.phi + (size_t)w * a.ldphi;
     const double *rows = a.win_rows + (size_t)w * K * ld;
     const float *vwin = a.win_phi + (size_t)w * K * np;
@@ -67,8 +67,8 @@ __global__ void __launch_bounds__(kStepThreads) delayed_step_kernel(DelayedStepA
     {
         for (int j = 4 * tid; j < np; j += 4 * kStepThreads) {
             const float4 f = *reinterpret_cast<const float4 *>(phi + j);
-            const double2 ba = *reinterpret_cast<const double2 *>(b0k + j);
-            const double2 bb = *reinterpret_cast<const double2 *>(b0k + j + 2);
+            const double2 ba = ld2(b0k + j);
+            const double2 bb = ld2(b0k + j + 2);
             const double v0 = f.x, v1 = f.y, v2 = f.z, v3 = f.w;
             acc[0] = fma(v0, ba.x, fma(v1, ba.y, fma(v2, bb.x, fma(v3, bb.y, acc[0]))));
 #pragma unroll
@@ -141,7 +141,7 @@ __global__ void __launch_bounds__(kStepThreads) delayed_step_kernel(DelayedStepA
     for (int j = 4 * tid; j < np; j += 4 * kStepThreads)
         *reinterpret_cast<float4 *>(vdst + j) = *reinterpret_cast<const float4 *>(phi + j);
     for (int j = 2 * tid; j < ld; j += 2 * kStepThreads)
-        *reinterpret_cast<double2 *>(rdst + j) = *reinterpret_cast<const double2 *>(b0k + j);
+        *reinterpret_cast<double2 *>(rdst + j) = ld2(b0k + j);
     // bordered inverse: S'^-1 = [[S^-1 + y z^T / R, -y / R], [-z^T / R, 1 / R]]
     double *so = a.win_sinv + (size_t)w * K * K;
     const double rinv = 1.0 / R;
@@ -158,18 +158,25 @@ __global__ void __launch_bounds__(kStepThreads) delayed_step_kernel(DelayedStepA
 
 // The flush (two DMMA contractions in one pass over B) lives in flush.cu.
 
-static cudaError_t launch_step(const DelayedStepArgs &a, int nw, cudaStream_t s)
+static cudaError_t launch_step(const DelayedStepArgs &a, int nw, int b32, cudaStream_t s)
 {
-    if (a.K <= 8) delayed_step_kernel<8><<<nw, kStepThreads, 0, s>>>(a);
-    else if (a.K <= 16) delayed_step_kernel<16><<<nw, kStepThreads, 0, s>>>(a);
-    else delayed_step_kernel<32><<<nw, kStepThreads, 0, s>>>(a);
+    if (b32) {
+        if (a.K <= 8) delayed_step_kernel<float, 8><<<nw, kStepThreads, 0, s>>>(a);
+        else if (a.K <= 16) delayed_step_kernel<float, 16><<<nw, kStepThreads, 0, s>>>(a);
+        else delayed_step_kernel<float, 32><<<nw, kStepThreads, 0, s>>>(a);
+    } else {
+        if (a.K <= 8) delayed_step_kernel<double, 8><<<nw, kStepThreads, 0, s>>>(a);
+        else if (a.K <= 16) delayed_step_kernel<double, 16><<<nw, kStepThreads, 0, s>>>(a);
+        else delayed_step_kernel<double, 32><<<nw, kStepThreads, 0, s>>>(a);
+    }
     count_launch();
     return cudaGetLastError();
 }
 
 static void fill_common(DelayedStepArgs &a, qmc_det *d, int iel, const float *phi, size_t ldphi)
 {
-    a.B = d->B; a.nel = d->nel; a.ld = d->ld; a.np = d->np; a.iel = iel; a.K = d->delay;
+    a.B = d->b32 ? (const void *)d->Bf : (const void *)d->B;
+    a.nel = d->nel; a.ld = d->ld; a.np = d->np; a.iel = iel; a.K = d->delay;
     a.phi = phi; a.ldphi = ldphi;
     a.win_count = d->win_count; a.win_iel = d->win_iel; a.win_slot = d->win_slot; a.win_phi = d->win_phi;
     a.win_rows = d->win_rows; a.win_sinv = d->win_sinv;
@@ -190,7 +197,7 @@ int delayed_ratio(qmc_det *d, int iel, const float *phi, int ldo, double *ratio,
     a.mode = 1;
     a.ratio_io = ratio;
     prof_start(d, kProfDelayedRatio, s);
-    cudaError_t e = launch_step(a, d->nw, s);
+    cudaError_t e = launch_step(a, d->nw, d->b32, s);
     prof_stop(d, s);
     QMC_CUDA(e);
     return QMC_OK;
@@ -211,7 +218,7 @@ int delayed_accept(qmc_det *d, int iel, const float *phi, int ldo, const double 
     (void)ratio;   // recomputed bit-identically from the same inputs
     a.accept_in = accept;
     prof_start(d, kProfDelayedAccept, s);
-    cudaError_t e = launch_step(a, d->nw, s);
+    cudaError_t e = launch_step(a, d->nw, d->b32, s);
     prof_stop(d, s);
     QMC_CUDA(e);
     d->host_pending += 1;

@@ -18,10 +18,11 @@ __device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double
 //     R'[l][n] = sum_l' S^-1[l'][l] * Rows[l'][n]          (p x ld, once per walker and window)
 // so the flush needs no p x p product per row block.  One warp handles the 8-column tiles
 // warp, warp + nwarps, ...: source row l' is src + rowoff_s[l'], the result goes to dst[l * ld + n]
-// for l < p.  src may alias dst (a tile is read completely before it is written).
+// for l < p.  src (double, or float rows of an fp32-stored inverse) may alias dst (a tile is read
+// completely before it is written).
 // sinv_s: S^-1 in shared memory, row stride gs.
-template <int KMAX>
-__device__ __forceinline__ void rprime_warp(const double *sinv_s, int gs, int p, const double *src,
+template <int KMAX, typename TS>
+__device__ __forceinline__ void rprime_warp(const double *sinv_s, int gs, int p, const TS *src,
                                             const long long *rowoff_s, double *dst, int ld, int warp,
                                             int nwarps, int lane)
 {
@@ -42,7 +43,7 @@ __device__ __forceinline__ void rprime_warp(const double *sinv_s, int gs, int p,
     for (int n0 = 8 * warp; n0 < ld; n0 += 8 * nwarps) {
         double b[KQ], c[MB][2];
 #pragma unroll
-        for (int kq = 0; kq < KQ; ++kq) b[kq] = off[kq] >= 0 ? src[off[kq] + n0 + g] : 0.0;
+        for (int kq = 0; kq < KQ; ++kq) b[kq] = off[kq] >= 0 ? (double)src[off[kq] + n0 + g] : 0.0;
 #pragma unroll
         for (int mb = 0; mb < MB; ++mb) c[mb][0] = c[mb][1] = 0.0;
 #pragma unroll

@@ -25,7 +25,7 @@
 namespace qmc {
 
 struct FlushArgs {
-    double *B;                    // [nw][nel][ld]
+    void *B;                      // TB [nw][nel][ld] (double, or float: fp32-stored inverse, R:A19)
     int nel, ld, np, K;
     int rows_per_cta;             // multiple of 8 * NG
     const int *win_count;
@@ -66,7 +66,7 @@ constexpr size_t kSmemMax = 227 * 1024;
 // Row-block loop of the flush for a window of NTA active 8-wide tiles (8 NTA - 7 <= p <= 8 NTA): a
 // compile-time count keeps the DMMA sequences free of branches, so the shared-memory operand loads
 // and the fp32 -> fp64 conversions are scheduled ahead of the tensor-core instructions.
-template <int KPAD, int NWC, int TW, int NG, bool PF, int CS, int NTA>
+template <typename TB, int KPAD, int NWC, int TW, int NG, bool PF, int CS, int NTA>
 __device__ __forceinline__ void flush_stream(const FlushArgs &a, int w, const double *rows_s, const float *v_s,
                                              double *part_s, double *cpart_s, const int *kl_s, uint64_t *mbar,
                                              int crank, int colbase)
@@ -88,24 +88,24 @@ __device__ __forceinline__ void flush_stream(const FlushArgs &a, int w, const do
     const int m_begin = (blockIdx.x / CS) * a.rows_per_cta;
     const int m_end = min(nel, m_begin + a.rows_per_cta);
     const int col0 = 8 * TW * wc;                                  // within the CTA's slice
-    double *const walker_B = a.B + (size_t)w * nel * LD + colbase + col0 + 2 * t;
+    TB *const walker_B = reinterpret_cast<TB *>(a.B) + (size_t)w * nel * LD + colbase + col0 + 2 * t;
     const float *const vfrag = v_s + g * VS + col0 + 2 * t;        // step-1 B fragments of this lane
     const double *const rfrag = rows_s + t * RS + col0 + g;        // step-2 B fragments of this lane
     bool staged = false;
     int m0 = m_begin + 8 * grp;
     double2 r[TW], rn[PF ? TW : 1];
     if (m0 < m_end) {
-        const double *src = walker_B + (size_t)min(m0 + g, nel - 1) * LD;
+        const TB *src = walker_B + (size_t)min(m0 + g, nel - 1) * LD;
 #pragma unroll
-        for (int i = 0; i < TW; ++i) r[i] = *reinterpret_cast<const double2 *>(src + 8 * i);
+        for (int i = 0; i < TW; ++i) r[i] = ld2(src + 8 * i);
     }
     for (int it = 0; m0 < m_end; m0 += 8 * NG, ++it) {
         const int m = m0 + g;
         const int m0n = m0 + 8 * NG;
         if (PF && m0n < m_end) {
-            const double *src = walker_B + (size_t)min(m0n + g, nel - 1) * LD;
+            const TB *src = walker_B + (size_t)min(m0n + g, nel - 1) * LD;
 #pragma unroll
-            for (int i = 0; i < TW; ++i) rn[PF ? i : 0] = *reinterpret_cast<const double2 *>(src + 8 * i);
+            for (int i = 0; i < TW; ++i) rn[PF ? i : 0] = ld2(src + 8 * i);
         }
         if (!staged) {
             mbar_wait(mbar, 0);
@@ -176,17 +176,17 @@ __device__ __forceinline__ void flush_stream(const FlushArgs &a, int w, const do
             for (int i = 0; i < TW; ++i) dmma884(r[i].x, r[i].y, af, rfrag[4 * kq * RS + 8 * i]);
         }
         if (m < nel) {
-            double *dst = walker_B + (size_t)m * LD;
+            TB *dst = walker_B + (size_t)m * LD;
 #pragma unroll
-            for (int i = 0; i < TW; ++i) *reinterpret_cast<double2 *>(dst + 8 * i) = r[i];
+            for (int i = 0; i < TW; ++i) st2(dst + 8 * i, r[i]);
         }
         if (PF) {
 #pragma unroll
             for (int i = 0; i < TW; ++i) r[i] = rn[PF ? i : 0];
         } else if (m0n < m_end) {
-            const double *src = walker_B + (size_t)min(m0n + g, nel - 1) * LD;
+            const TB *src = walker_B + (size_t)min(m0n + g, nel - 1) * LD;
 #pragma unroll
-            for (int i = 0; i < TW; ++i) r[i] = *reinterpret_cast<const double2 *>(src + 8 * i);
+            for (int i = 0; i < TW; ++i) r[i] = ld2(src + 8 * i);
         }
     }
     if (!staged) mbar_wait(mbar, 0);            // never leave with bulk copies in flight
@@ -198,7 +198,7 @@ __device__ __forceinline__ void flush_stream(const FlushArgs &a, int w, const do
 
 // NWC column warps x TW 8-column tiles per warp = the CTA's LDC columns; NG row groups per CTA
 // (CS == 1 only); PF = prefetch the next row block into registers; CS = cluster size.
-template <int KPAD, int NWC, int TW, int NG, bool PF, int CS>
+template <typename TB, int KPAD, int NWC, int TW, int NG, bool PF, int CS>
 __global__ void __launch_bounds__(32 * NWC * NG,
                                   (2 * (FlushSmem<KPAD, NWC * TW * 8, NWC, NG, CS>::bytes + 1024) <= 228 * 1024 &&
                                    2 * 32 * NWC * NG <= 1024) ? 2 : 1)
@@ -257,10 +257,10 @@ flush_dmma_kernel(FlushArgs a)
 
     // ---- stream the row blocks with the tile count of this window
     switch (p8 / 8) {
-    case 1: flush_stream<KPAD, NWC, TW, NG, PF, CS, 1>(a, w, rows_s, v_s, part_s, cpart_s, kl_s, mbar, crank, colbase); break;
-    case 2: if constexpr (NT >= 2) flush_stream<KPAD, NWC, TW, NG, PF, CS, 2>(a, w, rows_s, v_s, part_s, cpart_s, kl_s, mbar, crank, colbase); break;
-    case 3: if constexpr (NT >= 3) flush_stream<KPAD, NWC, TW, NG, PF, CS, 3>(a, w, rows_s, v_s, part_s, cpart_s, kl_s, mbar, crank, colbase); break;
-    case 4: if constexpr (NT >= 4) flush_stream<KPAD, NWC, TW, NG, PF, CS, 4>(a, w, rows_s, v_s, part_s, cpart_s, kl_s, mbar, crank, colbase); break;
+    case 1: flush_stream<TB, KPAD, NWC, TW, NG, PF, CS, 1>(a, w, rows_s, v_s, part_s, cpart_s, kl_s, mbar, crank, colbase); break;
+    case 2: if constexpr (NT >= 2) flush_stream<TB, KPAD, NWC, TW, NG, PF, CS, 2>(a, w, rows_s, v_s, part_s, cpart_s, kl_s, mbar, crank, colbase); break;
+    case 3: if constexpr (NT >= 3) flush_stream<TB, KPAD, NWC, TW, NG, PF, CS, 3>(a, w, rows_s, v_s, part_s, cpart_s, kl_s, mbar, crank, colbase); break;
+    case 4: if constexpr (NT >= 4) flush_stream<TB, KPAD, NWC, TW, NG, PF, CS, 4>(a, w, rows_s, v_s, part_s, cpart_s, kl_s, mbar, crank, colbase); break;
     }
 }
 
@@ -279,7 +279,7 @@ __global__ void __launch_bounds__(256) rprime_kernel(int ld, int K, const int *w
     if (threadIdx.x < p) rowoff_s[threadIdx.x] = (long long)threadIdx.x * ld;
     __syncthreads();
     double *rows = win_rows + (size_t)w * K * ld;
-    rprime_warp<KMAX>(sinv_s, GS, p, rows, rowoff_s, rows, ld, threadIdx.x >> 5, 8, threadIdx.x & 31);
+    rprime_warp<KMAX, double>(sinv_s, GS, p, rows, rowoff_s, rows, ld, threadIdx.x >> 5, 8, threadIdx.x & 31);
 }
 
 __global__ void reset_window_kernel(int nw, int *win_count)
@@ -349,14 +349,14 @@ int delayed_max_rank(int ld)
     return best;
 }
 
-template <int KPAD, int NWC, int TW, int NG, bool PF, int CS>
+template <typename TB, int KPAD, int NWC, int TW, int NG, bool PF, int CS>
 static cudaError_t launch_flush_t(const FlushArgs &a, int nw, cudaStream_t s)
 {
     using L = FlushSmem<KPAD, NWC * TW * 8, NWC, NG, CS>;
     if constexpr (L::bytes > kSmemMax) {
         return cudaErrorInvalidValue;
     } else {
-        auto kern = flush_dmma_kernel<KPAD, NWC, TW, NG, PF, CS>;
+        auto kern = flush_dmma_kernel<TB, KPAD, NWC, TW, NG, PF, CS>;
         // the opt-in is per device, not per process: set it on every launch (a host-side table write)
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L::bytes);
         if (e != cudaSuccess) return e;
@@ -376,13 +376,13 @@ static cudaError_t launch_flush_t(const FlushArgs &a, int nw, cudaStream_t s)
     }
 }
 
-template <int NWC, int TW, int NG, bool PF, int CS>
+template <typename TB, int NWC, int TW, int NG, bool PF, int CS>
 static cudaError_t launch_flush_k(const FlushArgs &a, int nw, cudaStream_t s)
 {
     switch (kpad_of(a.K)) {
-    case 8: return launch_flush_t<8, NWC, TW, NG, PF, CS>(a, nw, s);
-    case 16: return launch_flush_t<16, NWC, TW, NG, PF, CS>(a, nw, s);
-    case 32: return launch_flush_t<32, NWC, TW, NG, PF, CS>(a, nw, s);
+    case 8: return launch_flush_t<TB, 8, NWC, TW, NG, PF, CS>(a, nw, s);
+    case 16: return launch_flush_t<TB, 16, NWC, TW, NG, PF, CS>(a, nw, s);
+    case 32: return launch_flush_t<TB, 32, NWC, TW, NG, PF, CS>(a, nw, s);
     }
     return cudaErrorInvalidValue;
 }
@@ -391,7 +391,8 @@ int delayed_flush(qmc_det *d, cudaStream_t s)
 {
     if (!d->delay || d->host_pending == 0) return QMC_OK;
     FlushArgs a{};
-    a.B = d->B; a.nel = d->nel; a.ld = d->ld; a.np = d->np; a.K = d->delay;
+    a.B = d->b32 ? (void *)d->Bf : (void *)d->B;
+    a.nel = d->nel; a.ld = d->ld; a.np = d->np; a.K = d->delay;
     a.win_count = d->win_count; a.win_iel = d->win_iel; a.win_slot = d->win_slot;
     a.vec = d->win_vec; a.vec_wstride = d->win_vec_wstride; a.vec_sstride = d->win_vec_sstride;
     a.win_rows = d->win_rows;
@@ -413,7 +414,8 @@ int delayed_flush(qmc_det *d, cudaStream_t s)
     if (ring) e = flush_ring_launch(d, s);
     int id = 0;
 #define X(V, NWC, TW, NG, PF, CS) \
-    if (!ring && sh.id == id++) e = launch_flush_k<NWC, TW, NG, PF, CS>(a, d->nw, s);
+    if (!ring && sh.id == id++)                                                              \
+        e = d->b32 ? launch_flush_k<float, NWC, TW, NG, PF, CS>(a, d->nw, s) : launch_flush_k<double, NWC, TW, NG, PF, CS>(a, d->nw, s);
     QMC_FLUSH_SHAPES(X)
 #undef X
     prof_stop(d, s);

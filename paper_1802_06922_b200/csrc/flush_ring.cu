@@ -18,6 +18,11 @@
 //     (completion on the receiver's mbarrier: no fence, no cluster barrier);
 //   * the loop is software-pipelined by one block: step 1 of block j is issued before step 2 of
 //     block j-1, which hides the exchange latency behind tensor-core work.
+//
+// This kernel serves ranks <= 16 (the window fragments of 16 x 64 columns per warp fill the register
+// file).  Ranks 17..32 take flush_ring_hp.cu.  TB is the storage type of the inverse: double, or float
+// for the single-precision inverse of PAPER.md L82 (R:A19) -- rows are converted when a fragment is
+// loaded and rounded once when the block is stored; all arithmetic is fp64.
 #include <stdlib.h>
 
 #include "async_device.cuh"
@@ -27,7 +32,7 @@
 namespace qmc {
 
 struct RingArgs {
-    double *B;                    // [nw][nel][ld]
+    void *B;                      // TB [nw][nel][ld]
     int nel, ld, np, K;
     int rows_per_cta;             // multiple of 8
     const int *win_count;
@@ -41,32 +46,32 @@ struct RingArgs {
 constexpr int kRecvBufs = 4;      // partial-Q receive buffers in flight (see the hazard note in the kernel)
 
 // Shared memory of one CTA (LDC = NWC * TW * 8 columns):
-//   ring   double [STAGES][8][LDC + 8]      row blocks of B (pitch + 8: conflict-free 128-bit reads)
+//   ring   TB     [STAGES][8][LDC + 8]      row blocks of B (pitch + 8 elements: conflict-free vector reads)
 //   part   double [2][NWC][8][KPAD + 4]     partial Q of each column warp, by block parity
 //   recv   double [kRecvBufs][CS][8][KPAD + 4]   partial Q of every CTA of the cluster
 //   full   mbarrier [STAGES], rbar mbarrier [kRecvBufs], pbar mbarrier [2]
-template <int KPAD, int TW, int NWC, int CS, int STAGES>
+template <typename TB, int KPAD, int TW, int NWC, int CS, int STAGES>
 struct RingSmem {
     static constexpr int LDC = NWC * TW * 8, RP = LDC + 8, PS = KPAD + 4;
     static constexpr size_t ring_off = 0;
-    static constexpr size_t part_off = ring_off + (size_t)STAGES * 8 * RP * sizeof(double);
+    static constexpr size_t part_off = ring_off + (size_t)STAGES * 8 * RP * sizeof(TB);
     static constexpr size_t recv_off = part_off + (size_t)2 * NWC * 8 * PS * sizeof(double);
     static constexpr size_t bar_off = recv_off + (size_t)kRecvBufs * CS * 8 * PS * sizeof(double);
     static constexpr size_t bytes = bar_off + (size_t)(STAGES + kRecvBufs + 2) * sizeof(uint64_t);
 };
 
 // Row-block loop for a window of NTA active 8-wide tiles (8 NTA - 7 <= p <= 8 NTA).
-template <int KPAD, int TW, int NWC, int CS, int STAGES, int NTA>
+template <typename TB, int KPAD, int TW, int NWC, int CS, int STAGES, int NTA>
 __device__ __forceinline__ void ring_stream(const RingArgs &a, int w, int p, unsigned char *smem)
 {
-    using L = RingSmem<KPAD, TW, NWC, CS, STAGES>;
+    using L = RingSmem<TB, KPAD, TW, NWC, CS, STAGES>;
     constexpr int LDC = L::LDC, LD = LDC * CS, RP = L::RP, PS = L::PS;
     constexpr int KQA = 2 * NTA;
     constexpr int LW = NTA < NWC ? NTA : NWC;               // warps that reduce and send the partial Q
     // small clusters: the reducers run their own step 2 first (the other warps' partials are in by
     // then); larger clusters need the extra time for the exchange itself (measured both ways)
     constexpr bool SEND_LATE = CS <= 2;
-    double *ring = reinterpret_cast<double *>(smem + L::ring_off);
+    TB *ring = reinterpret_cast<TB *>(smem + L::ring_off);
     double *part = reinterpret_cast<double *>(smem + L::part_off);
     double *recv = reinterpret_cast<double *>(smem + L::recv_off);
     uint64_t *full = reinterpret_cast<uint64_t *>(smem + L::bar_off);
@@ -112,13 +117,13 @@ __device__ __forceinline__ void ring_stream(const RingArgs &a, int w, int p, uns
     const int m_begin = (blockIdx.x / CS) * a.rows_per_cta;
     const int m_end = min(nel, m_begin + a.rows_per_cta);
     const int nblk = (m_end - m_begin + 7) / 8;
-    double *const slice = a.B + (size_t)w * nel * LD + colbase;     // row m of this CTA's slice at + m * LD
+    TB *const slice = reinterpret_cast<TB *>(a.B) + (size_t)w * nel * LD + colbase;     // row m of this CTA's slice at + m * LD
     auto issue = [&](int jb) {                                      // whole warp 0
         const int s = jb % STAGES, m0 = m_begin + 8 * jb, nv = min(8, m_end - m0);
-        if (lane == 0) mbar_arrive_expect_tx(&full[s], (uint32_t)nv * (uint32_t)(LDC * sizeof(double)));
+        if (lane == 0) mbar_arrive_expect_tx(&full[s], (uint32_t)nv * (uint32_t)(LDC * sizeof(TB)));
         __syncwarp();
         if (lane < nv)
-            bulk_g2s(ring + (size_t)(s * 8 + lane) * RP, slice + (size_t)(m0 + lane) * LD, LDC * sizeof(double), &full[s]);
+            bulk_g2s(ring + (size_t)(s * 8 + lane) * RP, slice + (size_t)(m0 + lane) * LD, LDC * sizeof(TB), &full[s]);
     };
     if (warp == 0)
         for (int jb = 0; jb < STAGES - 1 && jb < nblk; ++jb) issue(jb);
@@ -153,9 +158,9 @@ __device__ __forceinline__ void ring_stream(const RingArgs &a, int w, int p, uns
             if (warp == 0 && j + STAGES - 1 < nblk) issue(j + STAGES - 1);
             const int s = j % STAGES;
             mbar_wait(&full[s], (uint32_t)(j / STAGES) & 1u);
-            const double *src = ring + (size_t)(s * 8 + g) * RP + col0 + 2 * t;
+            const TB *src = ring + (size_t)(s * 8 + g) * RP + col0 + 2 * t;
 #pragma unroll
-            for (int i = 0; i < TW; ++i) rb[i] = *reinterpret_cast<const double2 *>(src + 8 * i);
+            for (int i = 0; i < TW; ++i) rb[i] = ld2(src + 8 * i);
             // step 1: partial Q over this warp's columns
             double cq[NTA][2];
 #pragma unroll
@@ -195,9 +200,9 @@ __device__ __forceinline__ void ring_stream(const RingArgs &a, int w, int p, uns
                 for (int i = 0; i < TW; ++i) dmma884(ra[i].x, ra[i].y, af, rf[i][kq]);
             }
             if (m < m_end) {
-                double *dst = slice + (size_t)m * LD + col0 + 2 * t;
+                TB *dst = slice + (size_t)m * LD + col0 + 2 * t;
 #pragma unroll
-                for (int i = 0; i < TW; ++i) *reinterpret_cast<double2 *>(dst + 8 * i) = ra[i];
+                for (int i = 0; i < TW; ++i) st2(dst + 8 * i, ra[i]);
             }
         }
         if (SEND_LATE && j < nblk && warp < LW) reduce_and_send();
@@ -206,12 +211,10 @@ __device__ __forceinline__ void ring_stream(const RingArgs &a, int w, int p, uns
     }
 }
 
-template <int KPAD, int TW, int NWC, int CS, int STAGES>
-__global__ void __launch_bounds__(32 * NWC, (2 * (RingSmem<KPAD, TW, NWC, CS, STAGES>::bytes + 1024) <= 228 * 1024 &&
-                                             2 * 32 * NWC * 128 <= 65536) ? 2 : 1)
-flush_ring_kernel(RingArgs a)
+template <typename TB, int KPAD, int TW, int NWC, int CS, int STAGES>
+__global__ void __launch_bounds__(32 * NWC, 1) flush_ring_kernel(RingArgs a)
 {
-    using L = RingSmem<KPAD, TW, NWC, CS, STAGES>;
+    using L = RingSmem<TB, KPAD, TW, NWC, CS, STAGES>;
     extern __shared__ __align__(128) unsigned char smem_ring[];
     const int w = blockIdx.y;
     const int p = a.win_count[w];
@@ -228,19 +231,17 @@ flush_ring_kernel(RingArgs a)
     }
     constexpr int NT = KPAD / 8;
     switch ((p + 7) / 8) {
-    case 1: ring_stream<KPAD, TW, NWC, CS, STAGES, 1>(a, w, p, smem_ring); break;
-    case 2: if constexpr (NT >= 2) ring_stream<KPAD, TW, NWC, CS, STAGES, 2>(a, w, p, smem_ring); break;
-    case 3: if constexpr (NT >= 3) ring_stream<KPAD, TW, NWC, CS, STAGES, 3>(a, w, p, smem_ring); break;
-    case 4: if constexpr (NT >= 4) ring_stream<KPAD, TW, NWC, CS, STAGES, 4>(a, w, p, smem_ring); break;
+    case 1: ring_stream<TB, KPAD, TW, NWC, CS, STAGES, 1>(a, w, p, smem_ring); break;
+    case 2: if constexpr (NT >= 2) ring_stream<TB, KPAD, TW, NWC, CS, STAGES, 2>(a, w, p, smem_ring); break;
+    case 3: if constexpr (NT >= 3) ring_stream<TB, KPAD, TW, NWC, CS, STAGES, 3>(a, w, p, smem_ring); break;
+    case 4: if constexpr (NT >= 4) ring_stream<TB, KPAD, TW, NWC, CS, STAGES, 4>(a, w, p, smem_ring); break;
     }
 }
 
 // Shapes: X(V, KPAD, TW, NWC, CS, STAGES) serves ld = 64 V = CS * NWC * TW * 8 and ranks <= KPAD.
-#define QMC_RING_SHAPES(X) \
-    X(8, 16, 8, 8, 1, 5) X(16, 16, 8, 8, 2, 6) X(32, 16, 8, 8, 4, 5) \
-    X(8, 32, 4, 8, 2, 6) X(16, 32, 4, 8, 4, 6) X(32, 32, 4, 8, 8, 6)
+#define QMC_RING_SHAPES(X) X(8, 16, 8, 8, 1, 5) X(16, 16, 8, 8, 2, 6) X(32, 16, 8, 8, 4, 5)
 
-template <int KPAD, int TW, int NWC, int CS, int STAGES>
+template <typename TB, int KPAD, int TW, int NWC, int CS, int STAGES>
 static cudaError_t launch_ring(RingArgs a, int nw, int nsm, cudaStream_t s)
 {
     // rows per CTA: the window fragments are loaded and the ring is filled once per CTA (a few us), so
@@ -248,9 +249,9 @@ static cudaError_t launch_ring(RingArgs a, int nw, int nsm, cudaStream_t s)
     a.rows_per_cta = 64;
     for (int r = 1024; r >= 128; r >>= 1)
         if ((long long)nw * ((a.nel + r - 1) / r) * CS >= 6LL * nsm) { a.rows_per_cta = r; break; }
-    using L = RingSmem<KPAD, TW, NWC, CS, STAGES>;
+    using L = RingSmem<TB, KPAD, TW, NWC, CS, STAGES>;
     static_assert(L::bytes <= 227 * 1024, "ring shape exceeds shared memory");
-    auto kern = flush_ring_kernel<KPAD, TW, NWC, CS, STAGES>;
+    auto kern = flush_ring_kernel<TB, KPAD, TW, NWC, CS, STAGES>;
     // the opt-in is per device, not per process: set it on every launch (a host-side table write)
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L::bytes);
     if (e != cudaSuccess) return e;
@@ -269,15 +270,16 @@ static cudaError_t launch_ring(RingArgs a, int nw, int nsm, cudaStream_t s)
     return cudaLaunchKernelEx(&cfg, kern, a);
 }
 
-// Does a ring shape serve (ld, rank)?  QMC_FLUSH_RING=0 in the environment disables the ring kernel
+// Does a ring shape serve (ld, rank)?  QMC_FLUSH_RING=0 in the environment disables the ring kernels
 // (A/B measurements and tests of the flush.cu kernel on the same shapes).
 bool flush_ring_serves(int ld, int K)
 {
     const char *env = getenv("QMC_FLUSH_RING");
     if ((env && atoi(env) == 0) || ld % 64) return false;
-    const int v = ld / 64, kpad = K <= 16 ? 16 : 32;
+    if (K > 16) return flush_ring_hp_serves(ld, K);
+    const int v = ld / 64;
 #define X(V, KPAD, TW, NWC, CS, STAGES) \
-    if (v == V && kpad == KPAD) return true;
+    if (v == V) return true;
     QMC_RING_SHAPES(X)
 #undef X
     return false;
@@ -286,14 +288,18 @@ bool flush_ring_serves(int ld, int K)
 // Enqueue the ring flush (the caller has checked flush_ring_serves and brackets it with its profiling events).
 cudaError_t flush_ring_launch(qmc_det *d, cudaStream_t s)
 {
+    if (d->delay > 16) return flush_ring_hp_launch(d, s);
     RingArgs a{};
-    a.B = d->B; a.nel = d->nel; a.ld = d->ld; a.np = d->np; a.K = d->delay;
+    a.B = d->b32 ? (void *)d->Bf : (void *)d->B;
+    a.nel = d->nel; a.ld = d->ld; a.np = d->np; a.K = d->delay;
     a.win_count = d->win_count; a.win_iel = d->win_iel; a.win_slot = d->win_slot;
     a.vec = d->win_vec; a.vec_wstride = d->win_vec_wstride; a.vec_sstride = d->win_vec_sstride;
     a.win_rows = d->win_rows;
-    const int v = d->ld / 64, kpad = d->delay <= 16 ? 16 : 32;
-#define X(V, KPAD, TW, NWC, CS, STAGES) \
-    if (v == V && kpad == KPAD) return launch_ring<KPAD, TW, NWC, CS, STAGES>(a, d->nw, d->nsm, s);
+    const int v = d->ld / 64;
+#define X(V, KPAD, TW, NWC, CS, STAGES)                                                       \
+    if (v == V)                                                                               \
+        return d->b32 ? launch_ring<float, KPAD, TW, NWC, CS, STAGES>(a, d->nw, d->nsm, s)    \
+                      : launch_ring<double, KPAD, TW, NWC, CS, STAGES>(a, d->nw, d->nsm, s);
     QMC_RING_SHAPES(X)
 #undef X
     return cudaErrorInvalidValue;

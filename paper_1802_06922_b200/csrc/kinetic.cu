@@ -11,18 +11,19 @@ namespace qmc {
 
 // One block per (electron of the chunk, walker): five fp64 dots of row iel0 + j of B with the fp32
 // vectors v, d/dx, d/dy, d/dz, lap of that electron (fixed order: bit-reproducible).
+template <typename TB>
 __global__ void __launch_bounds__(256)
-det_glap_kernel(const double *__restrict__ B, int nel, int ld, int np, int nw, int iel0,
+det_glap_kernel(const TB *__restrict__ B, int nel, int ld, int np, int nw, int iel0,
                 const float *__restrict__ vgl, double *__restrict__ grad_out, double *__restrict__ lap_out,
                 double *__restrict__ one_out)
 {
     __shared__ double red[33];
     const int j = blockIdx.x, w = blockIdx.y, i = iel0 + j;
-    const double2 *row = reinterpret_cast<const double2 *>(B + ((size_t)w * nel + i) * ld);
+    const TB *row = B + ((size_t)w * nel + i) * ld;
     const float *x = vgl + ((size_t)j * nw + w) * 5 * np;
     double acc[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
     for (int c = threadIdx.x; 2 * c < nel; c += 256) {      // the vectors are zero-padded up to np >= nel
-        const double2 b = row[c];
+        const double2 b = ld2(row + 2 * c);
 #pragma unroll
         for (int k = 0; k < 5; ++k) {
             const float2 f = reinterpret_cast<const float2 *>(x + (size_t)k * np)[c];
@@ -80,9 +81,9 @@ extern "C" int qmc_det_kinetic(qmc_det_t *d, const qmc_spline_t *sp, const doubl
     }
     for (int k = 0; k < d->nel; k += d->spo_batch) {
         const int nb = d->nel - k < d->spo_batch ? d->nel - k : d->spo_batch;
-        int rc = spo_batch_vgl(d, sp, pos, nullptr, k, nb, nullptr, 0, s);
+        int rc = spo_batch_vgl(d, sp, pos, nullptr, k, nb, nullptr, 0, d->vgl, s);
         if (rc) return rc;
-        det_glap_kernel<<<dim3(nb, d->nw), 256, 0, s>>>(d->B, d->nel, d->ld, d->np, d->nw, k, d->vgl, grad_out, lap, one_out);
+        QMC_WITH_B(d, TB, Bp, (det_glap_kernel<TB><<<dim3(nb, d->nw), 256, 0, s>>>(Bp, d->nel, d->ld, d->np, d->nw, k, d->vgl, grad_out, lap, one_out)));
         QMC_LAUNCHED();
     }
     if (ekin_out) {

@@ -64,20 +64,21 @@ __global__ void __launch_bounds__(256) spo_batch_kernel(SpoBatchArgs a)
 // the update kernel can overwrite B in place.  One block per walker.  With force_out the three
 // gradient vectors of the proposal (phi + np, + 2 np, + 3 np) are contracted with the same row:
 // F = 2 grad log Psi_T at the proposed configuration = 2 (B[iel] . grad phi) / R.
+template <typename TB>
 __global__ void __launch_bounds__(256)
-ratio_rowcopy_kernel(const double *__restrict__ B, int nel, int ld, int iel, const float *__restrict__ phi,
+ratio_rowcopy_kernel(const TB *__restrict__ B, int nel, int ld, int iel, const float *__restrict__ phi,
                      size_t ldphi, int np, double *__restrict__ rowk, double *__restrict__ ratio,
                      double *__restrict__ force_out)
 {
     __shared__ double red[33];
     const int w = blockIdx.x;
-    const double2 *row = reinterpret_cast<const double2 *>(B + ((size_t)w * nel + iel) * ld);
+    const TB *row = B + ((size_t)w * nel + iel) * ld;
     const float *pw = phi + (size_t)w * ldphi;
     const float2 *ph = reinterpret_cast<const float2 *>(pw);
     double2 *dst = reinterpret_cast<double2 *>(rowk + (size_t)w * ld);
     double acc = 0.0, g[3] = {0.0, 0.0, 0.0};
     for (int j = threadIdx.x; j < ld / 2; j += 256) {
-        const double2 b = row[j];
+        const double2 b = ld2(row + 2 * j);
         dst[j] = b;
         if (2 * j < nel) {          // phi is padded with zeros up to the table pitch >= nel
             const float2 f = ph[j];
@@ -105,7 +106,7 @@ ratio_rowcopy_kernel(const double *__restrict__ B, int nel, int ld, int iel, con
 }
 
 int spo_batch_vgl(qmc_det *d, const qmc_spline *sp, const double *pos, const double *delta, int iel0, int nb,
-                  float *phi_record, int nrecord, cudaStream_t s)
+                  float *phi_record, int nrecord, float *out, cudaStream_t s)
 {
     int threads, tiles;
     spo_launch_shape(d->np, &threads, &tiles);
@@ -113,12 +114,73 @@ int spo_batch_vgl(qmc_det *d, const qmc_spline *sp, const double *pos, const dou
     a.sp = sp->view;
     a.pos = pos; a.delta = delta;
     a.nel = d->nel; a.iel0 = iel0; a.nw = d->nw;
-    a.vgl = d->vgl;
+    a.vgl = out;
     a.phi_record = phi_record; a.nrecord = nrecord;
     prof_start(d, kProfSpoRatio, s);
     spo_batch_kernel<<<dim3(tiles, d->nw, nb), threads, 0, s>>>(a);
     prof_stop(d, s);
     QMC_LAUNCHED();
+    return QMC_OK;
+}
+
+// Delayed mode: per window of K consecutive electron steps, K1 (SPO-VGL of the window's proposals),
+// delayed_window_kernel (S3 + S4 of the K steps) and the flush (S5').  The proposals of window i+1
+// are r' = pos[w][k] + delta for electrons no earlier window of this sweep touches, so K1 of window
+// i+1 is enqueued on a second stream as soon as the window kernel of window i has been enqueued and
+// runs UNDER the flush of window i (the flush is bound by the fp64 tensor pipe at ranks >= 24 and
+// leaves HBM bandwidth unused; the gather is a pure HBM stream).  Two SPO-VGL buffers alternate: buffer
+// b is rewritten only after the flush that read it (two windows earlier on `s`) has been enqueued before
+// the event the second stream waits on.  Everything the second stream did is joined back into `s`
+// before this function returns (the last SPO-VGL is awaited by the last window kernel).
+static int sweep_delayed(qmc_det *d, const qmc_spline *sp, double *pos, const double *delta, const double *unif,
+                         int nsweeps, int k0, int kn, double *ratios_out, unsigned char *accept_out,
+                         const unsigned char *forced, int fixed_node, double *force, float *rec, int nrec,
+                         cudaStream_t s)
+{
+    const int nw = d->nw, nel = d->nel, batch = d->spo_batch;
+    const int wins_per_sweep = (kn + batch - 1) / batch;
+    const long long nwin = (long long)nsweeps * wins_per_sweep;
+    if (nwin == 0) return QMC_OK;
+    bool overlap = d->overlap && !d->prof_on;     // per-kernel event timing needs the kernels one after another
+    if (overlap && !d->aux) {
+        QMC_CUDA(cudaStreamCreateWithFlags(&d->aux, cudaStreamNonBlocking));
+        QMC_CUDA(cudaEventCreateWithFlags(&d->ev_spo[0], cudaEventDisableTiming));
+        QMC_CUDA(cudaEventCreateWithFlags(&d->ev_spo[1], cudaEventDisableTiming));
+        QMC_CUDA(cudaEventCreateWithFlags(&d->ev_main, cudaEventDisableTiming));
+    }
+    auto spo = [&](long long i, cudaStream_t st) -> int {     // K1 of window i into buffer i & 1
+        const int sw = (int)(i / wins_per_sweep), k = k0 + (int)(i % wins_per_sweep) * batch;
+        const int nb = min(batch, k0 + kn - k);
+        const size_t mv = ((size_t)sw * nel + k) * nw;
+        return spo_batch_vgl(d, sp, pos, delta + 3 * mv, k, nb, rec ? rec + mv / nw * (size_t)nrec * nel : nullptr,
+                             nrec, d->vgl_buf[overlap ? (i & 1) : 0], st);
+    };
+    int rc;
+    if (overlap) {
+        QMC_CUDA(cudaEventRecord(d->ev_main, s));
+        QMC_CUDA(cudaStreamWaitEvent(d->aux, d->ev_main, 0));
+        if ((rc = spo(0, d->aux))) return rc;
+        QMC_CUDA(cudaEventRecord(d->ev_spo[0], d->aux));
+    }
+    for (long long i = 0; i < nwin; ++i) {
+        const int sw = (int)(i / wins_per_sweep), k = k0 + (int)(i % wins_per_sweep) * batch;
+        const int nb = min(batch, k0 + kn - k);
+        const size_t mv = ((size_t)sw * nel + k) * nw;
+        if (overlap) QMC_CUDA(cudaStreamWaitEvent(s, d->ev_spo[i & 1], 0));
+        else if ((rc = spo(i, s))) return rc;
+        d->vgl = d->vgl_buf[overlap ? (i & 1) : 0];
+        rc = delayed_sweep_window(d, pos, delta + 3 * mv, unif + mv, k, nb, ratios_out ? ratios_out + mv : nullptr,
+                                  accept_out ? accept_out + mv : nullptr, forced ? forced + mv : nullptr, fixed_node,
+                                  force ? force + 3 * mv : nullptr, overlap && i + 1 < nwin ? 1 : 0, s);
+        if (rc) return rc;
+        if (overlap && i + 1 < nwin) {
+            // (delayed_sweep_window recorded ev_main between its window kernel and its flush)
+            QMC_CUDA(cudaStreamWaitEvent(d->aux, d->ev_main, 0));
+            if ((rc = spo(i + 1, d->aux))) return rc;
+            QMC_CUDA(cudaEventRecord(d->ev_spo[(i + 1) & 1], d->aux));
+        }
+    }
+    d->vgl = d->vgl_buf[0];
     return QMC_OK;
 }
 
@@ -146,6 +208,8 @@ static int sweep_impl(qmc_det *d, const qmc_spline *sp, double *pos, const doubl
     }
     const int batch = d->spo_batch;
     const size_t slot_stride = (size_t)nw * 5 * d->np;
+    if (d->delay) return sweep_delayed(d, sp, pos, delta, unif, nsweeps, k0, kn, ratios_out, accept_out, forced,
+                                       fixed_node, force, rec, nrec, s);
     for (int sw = 0; sw < nsweeps; ++sw) {
         for (int k = k0; k < k0 + kn; ++k) {
             const size_t mv = ((size_t)sw * nel + k) * nw;
@@ -153,30 +217,18 @@ static int sweep_impl(qmc_det *d, const qmc_spline *sp, double *pos, const doubl
             if (slot == 0) {          // K1: SPO-VGL of the next `nb` electron steps, all walkers
                 const int nb = min(batch, k0 + kn - k);
                 int rc = spo_batch_vgl(d, sp, pos, delta + 3 * mv, k, nb,
-                                       rec ? rec + mv / nw * (size_t)nrec * nel : nullptr, nrec, s);
+                                       rec ? rec + mv / nw * (size_t)nrec * nel : nullptr, nrec, d->vgl, s);
                 if (rc) return rc;
-            }
-            if (d->delay) {           // the whole window: ratios, decisions, moves; then the flush
-                if (slot == 0) {
-                    const int nb = min(batch, k0 + kn - k);
-                    int rc = delayed_sweep_window(d, pos, delta + 3 * mv, unif + mv, k, nb,
-                                                  ratios_out ? ratios_out + mv : nullptr,
-                                                  accept_out ? accept_out + mv : nullptr,
-                                                  forced ? forced + mv : nullptr, fixed_node,
-                                                  force ? force + 3 * mv : nullptr, s);
-                    if (rc) return rc;
-                }
-                continue;
             }
             const float *phi = d->vgl + slot * slot_stride;
             // K2: ratio + row copy, K3: decision + rank-1 update
             prof_start(d, kProfRatio, s);
-            ratio_rowcopy_kernel<<<nw, 256, 0, s>>>(d->B, nel, d->ld, k, phi, (size_t)5 * d->np, d->np, d->rowk, d->ratio,
-                                                    force ? force + 3 * mv : nullptr);
+            QMC_WITH_B(d, TB, Bp, (ratio_rowcopy_kernel<TB><<<nw, 256, 0, s>>>(Bp, nel, d->ld, k, phi, (size_t)5 * d->np, d->np, d->rowk,
+                                                                               d->ratio, force ? force + 3 * mv : nullptr)));
             prof_stop(d, s);
             QMC_LAUNCHED();
             UpdateArgs u{};
-            u.B = d->B; u.nel = nel; u.ld = d->ld; u.iel = k;
+            u.B = d->b32 ? (void *)d->Bf : (void *)d->B; u.nel = nel; u.ld = d->ld; u.iel = k;
             u.phi = phi; u.ldphi = (size_t)5 * d->np; u.rowk = d->rowk;
             u.ratio = d->ratio;
             u.unif = unif + mv;
@@ -187,7 +239,7 @@ static int sweep_impl(qmc_det *d, const qmc_spline *sp, double *pos, const doubl
             u.pos = pos; u.delta = delta + 3 * mv;
             u.logdet = d->logdet; u.sign = d->sign; u.naccept = d->naccept;
             prof_start(d, kProfUpdate, s);
-            cudaError_t ue = launch_sm_update<true>(u, nw, s);
+            cudaError_t ue = d->b32 ? launch_sm_update<float, true>(u, nw, s) : launch_sm_update<double, true>(u, nw, s);
             prof_stop(d, s);
             QMC_CUDA(ue);
         }

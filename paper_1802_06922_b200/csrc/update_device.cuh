@@ -7,7 +7,7 @@
 namespace qmc {
 
 struct UpdateArgs {
-    double *B;                    // [nw][nel][ld]
+    void *B;                      // TB [nw][nel][ld]
     int nel, ld, iel;
     const float *phi;             // [nw][ldphi] orbital vector of the proposal (fp32)
     size_t ldphi;                 //   walker stride in floats
@@ -42,8 +42,8 @@ __device__ __forceinline__ bool usable_ratio(double R) { return isfinite(R) && R
 
 // One warp per row m: the row (ld = 64*VPT doubles) is read once into registers as VPT double2
 // per lane, dotted with phi (warp-shuffle tree), updated with the old row iel, and written back:
-// 16*ld bytes of HBM traffic per row, the floor for a rank-1 update.
-template <int VPT, bool DECIDE>
+// 16*ld bytes of HBM traffic per row (8*ld with the fp32-stored inverse), the floor for a rank-1 update.
+template <typename TB, int VPT, bool DECIDE>
 __global__ void __launch_bounds__(kUpdThreads) sm_update_kernel(UpdateArgs a)
 {
     extern __shared__ double smem_upd[];
@@ -88,10 +88,10 @@ __global__ void __launch_bounds__(kUpdThreads) sm_update_kernel(UpdateArgs a)
     const double2 *phi2 = reinterpret_cast<const double2 *>(phi_s);
     const double2 *rk2 = reinterpret_cast<const double2 *>(rowk_s);
     for (int m = blockIdx.x * kUpdRowsPerCta + wid; m < m_end; m += kUpdThreads / 32) {
-        double2 *row = reinterpret_cast<double2 *>(a.B + ((size_t)w * a.nel + m) * ld);
+        TB *row = reinterpret_cast<TB *>(a.B) + ((size_t)w * a.nel + m) * ld;
         double2 r[VPT];
 #pragma unroll
-        for (int i = 0; i < VPT; ++i) r[i] = row[lane + 32 * i];
+        for (int i = 0; i < VPT; ++i) r[i] = ld2(row + 2 * (lane + 32 * i));
         double dot = 0.0;
 #pragma unroll
         for (int i = 0; i < VPT; ++i) {
@@ -106,7 +106,7 @@ __global__ void __launch_bounds__(kUpdThreads) sm_update_kernel(UpdateArgs a)
             const double2 k2 = rk2[lane + 32 * i];
             r[i].x = fma(-f, k2.x, r[i].x);
             r[i].y = fma(-f, k2.y, r[i].y);
-            row[lane + 32 * i] = r[i];
+            st2(row + 2 * (lane + 32 * i), r[i]);
         }
     }
 }
@@ -121,7 +121,7 @@ inline int update_ld(int nel)
     return -1;
 }
 
-template <bool DECIDE>
+template <typename TB, bool DECIDE>
 inline cudaError_t launch_sm_update(const UpdateArgs &a, int nw, cudaStream_t s)
 {
     dim3 grid((a.nel + kUpdRowsPerCta - 1) / kUpdRowsPerCta, nw);
@@ -129,7 +129,7 @@ inline cudaError_t launch_sm_update(const UpdateArgs &a, int nw, cudaStream_t s)
     switch (a.ld / 64) {
 #define QMC_UPD_CASE(V)                                                              \
     case V:                                                                          \
-        sm_update_kernel<V, DECIDE><<<grid, kUpdThreads, smem, s>>>(a);              \
+        sm_update_kernel<TB, V, DECIDE><<<grid, kUpdThreads, smem, s>>>(a);              \
         break;
         QMC_UPD_CASE(1) QMC_UPD_CASE(2) QMC_UPD_CASE(3) QMC_UPD_CASE(4) QMC_UPD_CASE(6)
         QMC_UPD_CASE(8) QMC_UPD_CASE(12) QMC_UPD_CASE(16) QMC_UPD_CASE(24) QMC_UPD_CASE(32)

@@ -25,7 +25,7 @@ namespace qmc {
 constexpr int kWinThreads = 256;
 
 struct WindowArgs {
-    const double *B;              // [nw][nel][ld]  B0 of the window
+    const void *B;                // TB [nw][nel][ld]  B0 of the window
     int nw, nel, ld, np, K;
     int iel0, nb;                 // electrons iel0 .. iel0+nb-1, nb <= K
     const float *vgl;             // [nb][nw][5][np] SPO-VGL of the window's proposals (values first)
@@ -50,8 +50,8 @@ struct WindowArgs {
 // shared memory: warp q contracts the 16-column chunks q, q+8, ... with DMMA.8x8x4 (the contraction
 // index inside a chunk is permuted so that one lane's float4 / 2 x double2 serve four k-steps), then
 // the 8 partial G are summed in a fixed order.  Ends with a __syncthreads().
-template <int KMAX>
-__device__ __forceinline__ void window_contract(const float *x0, size_t vstep, const double *b0, int nb, int ld,
+template <int KMAX, typename TB>
+__device__ __forceinline__ void window_contract(const float *x0, size_t vstep, const TB *b0, int nb, int ld,
                                                 int np, double *G_dst)
 {
     constexpr int MB = KMAX / 8;
@@ -72,8 +72,8 @@ __device__ __forceinline__ void window_contract(const float *x0, size_t vstep, c
             const int j = 8 * jb + g;
             double2 lo = make_double2(0.0, 0.0), hi = lo;
             if (j < nb) {
-                lo = *reinterpret_cast<const double2 *>(b0 + (size_t)j * ld + col);
-                hi = *reinterpret_cast<const double2 *>(b0 + (size_t)j * ld + col + 2);
+                lo = ld2(b0 + (size_t)j * ld + col);
+                hi = ld2(b0 + (size_t)j * ld + col + 2);
             }
             bv[jb][0] = lo.x; bv[jb][1] = lo.y; bv[jb][2] = hi.x; bv[jb][3] = hi.y;
         }
@@ -110,7 +110,7 @@ __device__ __forceinline__ void window_contract(const float *x0, size_t vstep, c
 // One block per walker, 8 warps.  Phases 1-2: G (and, with FORCE, the same contraction for the three
 // gradient vectors of every proposal).  Phase 3: warp 0 walks the nb steps.  Phase 4: R' = S^-T Rows,
 // 8-column tiles over the warps.
-template <int KMAX, bool FORCE>
+template <typename TB, int KMAX, bool FORCE>
 __global__ void __launch_bounds__(kWinThreads) delayed_window_kernel(WindowArgs a)
 {
     constexpr int GS = KMAX + 1;
@@ -123,11 +123,11 @@ __global__ void __launch_bounds__(kWinThreads) delayed_window_kernel(WindowArgs 
     const int nb = a.nb, ld = a.ld, np = a.np, K = a.K;
     const size_t vstep = (size_t)a.nw * 5 * np;             // stride between steps in vgl
     const float *v0 = a.vgl + (size_t)w * 5 * np;
-    const double *b0 = a.B + ((size_t)w * a.nel + a.iel0) * ld;
+    const TB *b0 = reinterpret_cast<const TB *>(a.B) + ((size_t)w * a.nel + a.iel0) * ld;
 
-    window_contract<KMAX>(v0, vstep, b0, nb, ld, np, G_s);
+    window_contract<KMAX, TB>(v0, vstep, b0, nb, ld, np, G_s);
     if (FORCE)
-        for (int d = 0; d < 3; ++d) window_contract<KMAX>(v0 + (size_t)(1 + d) * np, vstep, b0, nb, ld, np, Gd_s + d * KMAX * GS);
+        for (int d = 0; d < 3; ++d) window_contract<KMAX, TB>(v0 + (size_t)(1 + d) * np, vstep, b0, nb, ld, np, Gd_s + d * KMAX * GS);
 
     // ---- phase 3: the nb steps in sequence; lane m owns accepted move m (its step index `mine`).
     // Everything that lives in global memory stays outside the sequential loop: lane i fetches the
@@ -223,19 +223,20 @@ __global__ void __launch_bounds__(kWinThreads) delayed_window_kernel(WindowArgs 
 
     // ---- phase 4: R'[l] = sum_l' S^-1[l'][l] B0[k_l'] for the flush (pad columns of B are zero)
     const int p = p_s;
-    if (p) rprime_warp<KMAX>(sinv_s, GS, p, b0, rowoff_s, a.win_rows + (size_t)w * K * ld, ld, warp, kWinThreads / 32, lane);
+    if (p) rprime_warp<KMAX, TB>(sinv_s, GS, p, b0, rowoff_s, a.win_rows + (size_t)w * K * ld, ld, warp, kWinThreads / 32, lane);
 }
 
 int delayed_sweep_window(qmc_det *d, double *pos, const double *delta, const double *unif, int iel0, int nb,
                          double *ratios_out, unsigned char *accept_out, const unsigned char *forced,
-                         int fixed_node, double *force_out, cudaStream_t s)
+                         int fixed_node, double *force_out, int record_mid, cudaStream_t s)
 {
     if (d->host_pending) {        // rows pending from standalone qmc_det_accept_update calls
         int rc = delayed_flush_reset_host(d, s);
         if (rc) return rc;
     }
     WindowArgs a{};
-    a.B = d->B; a.nw = d->nw; a.nel = d->nel; a.ld = d->ld; a.np = d->np; a.K = d->delay;
+    a.B = d->b32 ? (const void *)d->Bf : (const void *)d->B;
+    a.nw = d->nw; a.nel = d->nel; a.ld = d->ld; a.np = d->np; a.K = d->delay;
     a.iel0 = iel0; a.nb = nb;
     a.vgl = d->vgl;
     a.unif = unif; a.forced = forced; a.ratios_out = ratios_out; a.accept_out = accept_out;
@@ -245,17 +246,22 @@ int delayed_sweep_window(qmc_det *d, double *pos, const double *delta, const dou
     a.win_count = d->win_count; a.win_iel = d->win_iel; a.win_slot = d->win_slot;
     a.win_rows = d->win_rows;
     prof_start(d, kProfDelayedRatio, s);
-    if (force_out) {
-        if (a.K <= 8) delayed_window_kernel<8, true><<<d->nw, kWinThreads, 0, s>>>(a);
-        else if (a.K <= 16) delayed_window_kernel<16, true><<<d->nw, kWinThreads, 0, s>>>(a);
-        else delayed_window_kernel<32, true><<<d->nw, kWinThreads, 0, s>>>(a);
-    } else {
-        if (a.K <= 8) delayed_window_kernel<8, false><<<d->nw, kWinThreads, 0, s>>>(a);
-        else if (a.K <= 16) delayed_window_kernel<16, false><<<d->nw, kWinThreads, 0, s>>>(a);
-        else delayed_window_kernel<32, false><<<d->nw, kWinThreads, 0, s>>>(a);
-    }
+#define QMC_WIN_LAUNCH(TB, KM, F) delayed_window_kernel<TB, KM, F><<<d->nw, kWinThreads, 0, s>>>(a)
+#define QMC_WIN_RANK(TB, F)                                  \
+    do {                                                     \
+        if (a.K <= 8) QMC_WIN_LAUNCH(TB, 8, F);              \
+        else if (a.K <= 16) QMC_WIN_LAUNCH(TB, 16, F);       \
+        else if (a.K <= 24) QMC_WIN_LAUNCH(TB, 24, F);       \
+        else QMC_WIN_LAUNCH(TB, 32, F);                      \
+    } while (0)
+    if (d->b32) { if (force_out) QMC_WIN_RANK(float, true); else QMC_WIN_RANK(float, false); }
+    else { if (force_out) QMC_WIN_RANK(double, true); else QMC_WIN_RANK(double, false); }
+#undef QMC_WIN_RANK
+#undef QMC_WIN_LAUNCH
     prof_stop(d, s);
     QMC_LAUNCHED();
+    // positions are final for this window: the next window's SPO-VGL may start (second stream, sweep.cu)
+    if (record_mid) QMC_CUDA(cudaEventRecord(d->ev_main, s));
     // the flush takes the vectors of the accepted steps straight from the SPO-VGL scratch
     d->host_pending = nb;
     d->win_rows_raw = 0;

@@ -13,6 +13,11 @@ TOL_RATIO = 1e-5    # determinant ratio, relative (floor 1e-2 on |R| end to end,
 TOL_BINV = 1e-9     # inverse after a sweep, identical orbital vectors (max-abs; R:A12)
 TOL_RESID = 1e-6    # ||Binv^T A - I||_inf with A recomputed from scratch (R:A11)
 BAND = 1e-6         # accept decisions may differ only where |R^2 - u| < BAND
+# Quantities that are dot products of an fp32 gradient / Laplacian vector with a row of B are compared
+# with |B[k]|_1 * TOL_GL_PROP * max|grad phi| (or max|lap phi|): 10x the worst error measured on the
+# B200 over every case of the suite (7e-8; gpurun log of round 2).  north_star's
+# per-orbital tolerance (2e-5) would allow 20x more.
+TOL_GL_PROP = 1e-6
 
 
 def dev():
@@ -179,6 +184,15 @@ def run_protocol(x, delay_rank=0, walkers=None, free_oracle=True, coefs_np=None)
         out["ratio_e2e_over_tol"] = float(np.max(err / tol))
         out["ratio_e2e_rel_floor"] = float(np.max(err / np.maximum(np.abs(frc["ratios"]), 1e-2)))
         out["ratio_e2e_frac_within_1e-5"] = float(np.mean(err <= TOL_RATIO * np.maximum(np.abs(frc["ratios"]), 1e-2)))
+        # measured propagation factor: |dR| / (||B[k]||_1 max|phi|), to be compared with TOL_V
+        out["ratio_e2e_prop_factor"] = float(np.max(err / (frc["bnorm"] * phimax)))
+        out["bnorm_max"] = float(np.max(frc["bnorm"]))
+        # moves outside SURVEY A10's plain bound are the ones with a large inverse row: every one of
+        # them must be explained by the propagated term, and they must be a small minority
+        plain = err <= TOL_RATIO * np.maximum(np.abs(frc["ratios"]), 1e-2)
+        out["bnorm_min_of_exceptions"] = float(np.min(frc["bnorm"][~plain])) if (~plain).any() else float("inf")
+        out["bnorm_median"] = float(np.median(frc["bnorm"]))
+        assert out["ratio_e2e_frac_within_1e-5"] >= 0.9, out
         assert out["ratio_e2e_over_tol"] < 1.0, out
         assert np.array_equal(pos_g.cpu().numpy()[:nchk], frc["pos"])
         out["binv_e2e_rel"] = float(np.max(np.abs(Bf_g[:nchk] - frc["B"])) / max(1.0, np.max(np.abs(frc["B"]))))

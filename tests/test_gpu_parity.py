@@ -198,9 +198,90 @@ def test_sweep_control_flow():
     spline.destroy()
 
 
+def test_edge_inputs_both_sides():
+    """Edge inputs, same answers as the oracle (R:A7, R:A8, R:A18): a position whose reduced coordinate
+    rounds up to 1.0; a zero displacement (R = 1, inverse unchanged); a NaN displacement (rejected,
+    state untouched); imposed accepts of a zero and of a NaN orbital vector (refused) -- on the rank-1
+    path, the one-launch-per-window path and the standalone delayed path."""
+    x = CASES["ragged37_skew"]()
+    coefs_np = x.coefs_numpy()
+    nw, nel = x.pos.shape[0], x.cfg.norb
+    spline = api.Spline.create(x.coefs.to(P.dev()), x.lattice)
+    # (a) cell-face rounding and non-finite positions
+    lat = x.lattice
+    pts = np.stack([-1e-18 * lat[0], -1e-18 * lat[1], -1e-18 * lat[2], np.zeros(3), lat[0] + lat[2]])
+    u = pts[:3] @ np.linalg.inv(lat)
+    assert all((u[d, d] - np.floor(u[d, d])) == 1.0 for d in range(3))
+    v, g, l = api.spo_vgl(spline, P.to_dev(pts))
+    vo, go, lo = oracle.spline_vgl(coefs_np, lat, pts)
+    P.check_vgl(v, g, l, vo, go, lo, nel)
+    assert torch.equal(v[0], v[3]) and torch.equal(v[1], v[3]) and torch.equal(v[2], v[3])
+    bad = P.to_dev(np.array([[0.1, np.nan, 0.2], [np.inf, 0.0, 0.0]]))
+    vb, gb, lb = api.spo_vgl(spline, bad)
+    assert bool(torch.isnan(vb[:, :nel]).all()) and bool(torch.isnan(lb[:, :nel]).all())
+    # (b)-(d) sweeps
+    delta = x.delta.copy()
+    delta[0, 3, :, :] = 0.0                   # zero displacement for every walker at electron 3
+    delta[0, 5, 1, 2] = np.nan                # NaN proposal for walker 1 at electron 5
+    unif = x.unif.copy()
+    unif[0, 3] = 0.5
+    pos0 = P.to_dev(x.pos)
+    A0 = P.gpu_slater(spline, pos0)
+    B0, ld0, sg0 = P.oracle_binv(A0)
+    for K in (0, 4, 16):
+        det = api.Det.init(spline, pos0, delay_rank=K)
+        pos = pos0.clone()
+        R = torch.zeros(unif.shape, dtype=torch.float64, device=P.dev())
+        acc = torch.zeros(unif.shape, dtype=torch.uint8, device=P.dev())
+        rec = torch.zeros((unif.shape[0], nel, nw, nel), dtype=torch.float32, device=P.dev())
+        api.sweep(det, pos, P.to_dev(delta), P.to_dev(unif), ratios_out=R, accept_out=acc, phi_record=rec, nrecord=nw)
+        Rn, an = R.cpu().numpy(), acc.cpu().numpy()
+        assert np.max(np.abs(Rn[0, 3] - 1.0)) < 1e-6 and an[0, 3].all()          # fp32 orbitals: R = 1 to ~1e-7
+        assert np.isnan(Rn[0, 5, 1]) and an[0, 5, 1] == 0
+        assert np.isfinite(np.delete(Rn.reshape(-1), (0 * nel + 5) * nw + 1)).all()
+        rep = oracle.sweep(coefs_np, lat, x.pos, B0, ld0, sg0, delta, unif, forced=an, phi_in=rec.cpu().numpy())
+        Bg = det.get_inverse().cpu().numpy()
+        assert np.isfinite(Bg).all()
+        assert np.max(np.abs(Bg - rep["B"])) < P.TOL_BINV * max(1.0, np.max(np.abs(rep["B"])))
+        assert np.array_equal(pos.cpu().numpy(), rep["pos"])
+        assert np.array_equal(an, rep["accept"])
+        # imposed decisions: all ones, with one zero and one NaN orbital vector recorded -> refused
+        det2 = api.Det.init(spline, pos0, delay_rank=K)
+        pos2 = pos0.clone()
+        ones = torch.ones(unif.shape, dtype=torch.uint8, device=P.dev())
+        acc2 = torch.zeros_like(ones)
+        api.sweep(det2, pos2, P.to_dev(delta), P.to_dev(unif), accept_out=acc2, forced_accept=ones)
+        a2 = acc2.cpu().numpy()
+        assert a2[0, 5, 1] == 0 and a2.sum() == a2.size - 1                       # only the NaN move is refused
+        assert bool(torch.isfinite(det2.get_inverse()).all())
+        det.destroy()
+        det2.destroy()
+    # standalone calls: accept imposed on a zero vector (R = 0) and a NaN vector
+    for K in (0, 4):
+        det = api.Det.init(spline, pos0, delay_rank=K)
+        B_before = det.get_inverse()
+        phi = api.spo_vgl(spline, P.to_dev(x.pos[:, 2] + 0.1), want_gl=False)
+        phi[0] = 0.0
+        phi[1, 3] = float("nan")
+        Rr = det.ratio(2, phi)
+        assert float(Rr[0]) == 0.0 and bool(torch.isnan(Rr[1]))
+        det.accept_update(2, phi, Rr, torch.ones(nw, dtype=torch.uint8, device=P.dev()))
+        B_after = det.get_inverse()
+        _, _, nacc = det.get_stats()
+        assert torch.equal(B_after[:2], B_before[:2]) and bool(torch.isfinite(B_after).all())
+        assert nacc.cpu().tolist() == [0, 0] + [1] * (nw - 2)
+        phi_np = phi[:, :nel].double().cpu().numpy()
+        for w in range(2, nw):
+            Bo = oracle.sm_update(B0[w], 2, phi_np[w], float(Rr[w]))
+            assert np.max(np.abs(B_after[w].cpu().numpy() - Bo)) < P.TOL_BINV * max(1.0, np.max(np.abs(Bo)))
+        det.destroy()
+    spline.destroy()
+
+
 # ------------------------------------------------------------------------------- full sizes
 @pytest.mark.parametrize("name,nchk,npos,delay", [("mid", 4, 48, 0), ("large", 4, 32, 0), ("mid", 4, 0, 16),
-                                                  ("large", 4, 0, 16), ("large", 2, 0, 32), ("xlarge", 2, 16, 16)])
+                                                  ("large", 4, 0, 16), ("large", 2, 0, 32), ("large", 2, 0, 24),
+                                                  ("xlarge", 2, 16, 16), ("xlarge", 2, 0, 32), ("xlarge", 2, 0, 0)])
 def test_full_size_sampled(name, nchk, npos, delay):
     """BASELINE.json's full sizes in the launch configuration bench.py times (all walkers in
     lockstep, one sweep; rank-1 and the delayed ranks bench.py measures): the oracle checks the
@@ -222,14 +303,17 @@ def test_full_size_sampled(name, nchk, npos, delay):
         vo, go, lo = oracle.spline_vgl(coefs_np, x.lattice, pos)
         print(name, "vgl rel err", P.check_vgl(v, g, l, vo, go, lo, cfg.norb))
         spline.destroy()
-    out = P.run_protocol(x, delay_rank=delay, walkers=nchk, free_oracle=(name == "mid" and not delay),
+    # the end-to-end leg (the oracle's own fp64 spline, Slater matrix, LU and sweep) runs at mid and at
+    # the headline config, rank-1 and rank-16
+    out = P.run_protocol(x, delay_rank=delay, walkers=nchk, free_oracle=(name in ("mid", "large") and delay in (0, 16)),
                          coefs_np=coefs_np)
     print(name, out)
 
 
 # ------------------------------------------------------------------------------- delayed rank-k
 @pytest.mark.parametrize("case,K", [("tiny", 2), ("tiny", 5), ("ragged37_skew", 4), ("ragged37_skew", 16),
-                                    ("n130_two_tiles", 7), ("small", 16), ("small", 32)])
+                                    ("n130_two_tiles", 7), ("n130_two_tiles", 20), ("small", 16), ("small", 24),
+                                    ("small", 32)])
 def test_delayed_sweep_parity_protocol(case, K):
     """The delayed update has no oracle of its own: it must reach the Sherman-Morrison / LU result
     (DESIGN.md R:O7), so the same protocol and tolerances apply.  Windows of K steps do not divide
@@ -306,7 +390,8 @@ def test_delayed_standalone_api():
 # --------------------------------------------------- delayed rank-k at large N (cluster / ring flush shapes)
 @pytest.mark.parametrize("nel,K,nw,count,env", [
     (512, 16, 6, 0, {}), (512, 32, 4, 0, {}), (1000, 16, 5, 0, {}), (1024, 16, 4, 0, {}), (1024, 32, 3, 0, {}),
-    (2048, 16, 2, 200, {}), (2048, 32, 2, 200, {}),
+    (2048, 16, 2, 200, {}), (2048, 32, 2, 200, {}), (512, 24, 4, 0, {}), (1024, 24, 3, 0, {}), (1024, 20, 3, 0, {}),
+    (2048, 24, 2, 200, {}),
     # the flush.cu kernel on the same shapes: one CTA per row block, then its cluster shapes
     (1000, 16, 4, 0, {"QMC_FLUSH_RING": "0"}), (1024, 16, 3, 0, {"QMC_FLUSH_RING": "0", "QMC_FLUSH_SHAPE": "1"}),
     (1024, 16, 3, 0, {"QMC_FLUSH_RING": "0", "QMC_FLUSH_SHAPE": "2"}), (1024, 32, 3, 0, {"QMC_FLUSH_RING": "0"}),
@@ -375,8 +460,9 @@ def test_wavefunction_force_parity(case, K):
     """qmc_sweep_ex force_out: F = 2 grad log Psi_T of the moved electron at the
     proposed configuration, for every move, against the oracle replaying the GPU's decisions and
     fp32 orbital vectors (its gradients come from its own fp64 spline).  Compared as F R / 2 =
-    grad_r' R, which stays smooth next to a node: the north_star gradient tolerance (2e-5 of
-    max|grad phi|) propagated through the dot product with row k of B, plus 1e-5 relative."""
+    grad_r' R, which stays smooth next to a node: an fp32 gradient error of TOL_GL_PROP * max|grad phi|
+    per orbital (10x the worst measured; north_star allows 2e-5) propagated through the dot product
+    with row k of B, plus 1e-5 relative."""
     x = CASES[case]()
     g = _force_run(x, K)
     assert np.isfinite(g["F"]).all()
@@ -388,7 +474,7 @@ def test_wavefunction_force_parity(case, K):
     gmax = float(np.max(np.abs(go)))
     gR_g = 0.5 * g["F"] * g["R"][..., None]
     gR_o = 0.5 * rep["force"] * rep["ratios"][..., None]
-    tol = rep["bnorm"][..., None] * 2e-5 * gmax + 1e-5 * np.abs(gR_o) + 1e-12
+    tol = rep["bnorm"][..., None] * P.TOL_GL_PROP * gmax + 1e-5 * np.abs(gR_o) + 1e-12
     worst = float(np.max(np.abs(gR_g - gR_o) / tol))
     big = np.abs(rep["ratios"]) > 0.1
     rel = float(np.max(np.abs(g["F"] - rep["force"])[big] / np.maximum(1.0, np.abs(rep["force"])[big])))
@@ -432,8 +518,9 @@ def test_fixed_node_rejection(case, K):
 def test_det_kinetic_parity(case, K):
     """qmc_det_kinetic after a sweep: grad_i det/det, lap_i det/det and E_kin = -1/2 sum_i lap_i
     (eq. 3, eq. 37) against the oracle evaluated with the same inverse at the same positions
-    (its SPO-VGL in fp64): the north_star gradient / Laplacian tolerances (2e-5 of the max) propagated
-    through the dot product with row i of B; and sum_j phi_j(r_i) B[i][j] = 1."""
+    (its SPO-VGL in fp64): an fp32 gradient / Laplacian error of TOL_GL_PROP of the max per orbital
+    (10x the worst measured; north_star allows 2e-5) propagated through the dot product with row i
+    of B; and sum_j phi_j(r_i) B[i][j] = 1."""
     x = CASES[case]()
     coefs_np = x.coefs_numpy()
     spline = api.Spline.create(x.coefs.to(P.dev()), x.lattice)
@@ -445,8 +532,8 @@ def test_det_kinetic_parity(case, K):
     ref = oracle.det_kinetic(coefs_np, x.lattice, pos.cpu().numpy(), Bg)
     _, go, lo = oracle.spline_vgl(coefs_np, x.lattice, x.pos.reshape(-1, 3)[:64])
     bnorm = np.abs(Bg).sum(axis=2)
-    tol_g = bnorm[..., None] * 2e-5 * float(np.max(np.abs(go))) + 1e-12
-    tol_l = bnorm * 2e-5 * float(np.max(np.abs(lo))) + 1e-12
+    tol_g = bnorm[..., None] * P.TOL_GL_PROP * float(np.max(np.abs(go))) + 1e-12
+    tol_l = bnorm * P.TOL_GL_PROP * float(np.max(np.abs(lo))) + 1e-12
     eg = float(np.max(np.abs(k["grad"].cpu().numpy() - ref["grad"]) / tol_g))
     el = float(np.max(np.abs(k["lap"].cpu().numpy() - ref["lap"]) / tol_l))
     ee = float(np.max(np.abs(k["ekin"].cpu().numpy() - ref["ekin"]) / (0.5 * tol_l.sum(axis=1))))
@@ -510,3 +597,138 @@ def test_fp64_dmma_probe():
     tf = api.probe_fp64_dmma()
     print("fp64 DMMA peak", tf, "TFLOP/s")
     assert 15.0 < tf < 80.0
+
+
+# --------------------------------------------- NEXT-3: fp32-stored inverse with fp64 recompute
+FP32_ULP = 2.0 ** -23
+
+
+def _fp32_run(x, K, nsweeps=None):
+    """GPU sweep with the fp32-stored inverse; returns what the oracle replay needs."""
+    spline = api.Spline.create(x.coefs.to(P.dev()) if not x.coefs.is_cuda else x.coefs, x.lattice)
+    nsw = x.delta.shape[0] if nsweeps is None else nsweeps
+    pos0 = P.to_dev(x.pos)
+    delta, unif = P.to_dev(x.delta[:nsw]), P.to_dev(x.unif[:nsw])
+    nw, nel = x.pos.shape[0], x.cfg.norb
+    det = api.Det.init(spline, pos0, delay_rank=K, fp32_inverse=True)
+    assert det.storage_bytes == 4
+    B0 = det.get_inverse().cpu().numpy()
+    ld0, sg0, _ = (t.cpu().numpy() for t in det.get_stats())
+    pos = pos0.clone()
+    R = torch.zeros_like(unif)
+    acc = torch.zeros(unif.shape, dtype=torch.uint8, device=P.dev())
+    rec = torch.zeros((nsw, nel, nw, nel), dtype=torch.float32, device=P.dev())
+    api.sweep(det, pos, delta, unif, ratios_out=R, accept_out=acc, phi_record=rec, nrecord=nw)
+    torch.cuda.synchronize()
+    return dict(spline=spline, det=det, B0=B0, ld0=ld0, sg0=sg0, pos=pos, R=R.cpu().numpy(), acc=acc.cpu().numpy(),
+                rec=rec.cpu().numpy(), nsw=nsw)
+
+
+@pytest.mark.parametrize("case,K", [("tiny", 0), ("ragged37_skew", 0), ("ragged37_skew", 4), ("n130_two_tiles", 0),
+                                    ("n130_two_tiles", 7), ("small", 0), ("small", 16)])
+def test_fp32_inverse_parity(case, K):
+    """QMC_DET_FP32_INVERSE against the oracle in its fp32-storage mode (R:A19), identical orbital
+    vectors: the stored initial inverse is the fp32 rounding of the fp64 one; the oracle, started from
+    the SAME stored matrix, rounds after every accepted update (rank-1) or at the end of every window of
+    K steps (delayed), with fp64 arithmetic in between -- decisions agree outside the 1e-6 band, ratios
+    to 1e-5, the final stored inverse to a few fp32 ulps of max|B| (the two sides round the same fp64
+    value except where their fp64 results straddle a rounding boundary)."""
+    x = CASES[case]()
+    g = _fp32_run(x, K)
+    nw, nel = x.pos.shape[0], x.cfg.norb
+    assert np.array_equal(g["B0"], g["B0"].astype(np.float32).astype(np.float64))          # really fp32 values
+    A0 = P.gpu_slater(g["spline"], P.to_dev(x.pos))
+    B0_o, ld0_o, sg0_o = P.oracle_binv(A0)
+    scale0 = max(1.0, np.max(np.abs(B0_o)))
+    assert np.max(np.abs(g["B0"] - B0_o)) <= 0.75 * FP32_ULP * scale0                   # one rounding of the fp64 inverse
+    assert np.max(np.abs(g["ld0"] - ld0_o)) < 1e-8 and np.array_equal(g["sg0"], sg0_o)
+    dummy = np.zeros((1, 1, 1, nel), np.float32)
+    b32 = K if K >= 2 else 1
+    nth = oracle.max_threads()
+    d, u = x.delta[:g["nsw"]], x.unif[:g["nsw"]]
+    free = oracle.sweep(dummy, x.lattice, x.pos, g["B0"], g["ld0"], g["sg0"], d, u, phi_in=g["rec"], b32=b32, nthreads=nth)
+    P.compare_decisions(g["acc"], g["R"], free["accept"], free["ratios"], u)
+    rep = oracle.sweep(dummy, x.lattice, x.pos, g["B0"], g["ld0"], g["sg0"], d, u, forced=g["acc"], phi_in=g["rec"],
+                       b32=b32, nthreads=nth)
+    Bg = g["det"].get_inverse().cpu().numpy()
+    assert np.array_equal(Bg, Bg.astype(np.float32).astype(np.float64))
+    scale = max(1.0, np.max(np.abs(rep["B"])))
+    eb = float(np.max(np.abs(Bg - rep["B"])) / scale)
+    er = float(np.max(np.abs(g["R"] - rep["ratios"]) / np.maximum(np.abs(rep["ratios"]), 1e-300)))
+    ldg, sgg, _ = (t.cpu().numpy() for t in g["det"].get_stats())
+    print(case, K, "fp32 inverse: |B - B_oracle| / max|B| =", eb, "(ulp", FP32_ULP, ") ratio rel", er,
+          "accept", g["acc"].mean())
+    assert eb <= 16 * FP32_ULP, eb
+    assert er < P.TOL_RATIO
+    # (one flipped rounding perturbs the later ratios of that walker at the 1e-6 level, log|det| with them)
+    assert np.max(np.abs(ldg - rep["logdet"])) < 1e-4 and np.array_equal(sgg, rep["sign"])
+    assert np.array_equal(g["pos"].cpu().numpy(), rep["pos"])
+    g["det"].destroy()
+    g["spline"].destroy()
+
+
+@pytest.mark.parametrize("case,K,nsw", [("small", 0, 4), ("small", 16, 4), ("n130_two_tiles", 7, 1)])
+def test_fp32_inverse_drift_and_recompute(case, K, nsw):
+    """Residual monitor and recompute (R:A19): after several sweeps the fp32-stored inverse has a residual
+    max |B[k] . phi(r_i) - delta_ik| at the fp32 level (far above the fp64 engine's, far below 1e-2);
+    qmc_det_recompute restores the freshly rounded level and re-derives log|det| and sign, which agree with
+    the running values; an fp64 handle on the same walk has a residual at its own level; the monitor
+    agrees with the same quantity formed by numpy from get_inverse and the recomputed Slater matrix."""
+    x = CASES[case]()
+    if x.delta.shape[0] < nsw:
+        x = inputs.make_inputs(x.cfg, nsweeps=nsw)
+    g = _fp32_run(x, K, nsweeps=nsw)
+    det, spline, pos = g["det"], g["spline"], g["pos"]
+    nw, nel = x.pos.shape[0], x.cfg.norb
+    r_run = det.residual(pos, nsample=4).cpu().numpy()
+    # the same number from numpy: rows i = s * (nel // 4) of A B^T - I
+    A = P.gpu_slater(spline, pos)
+    Bg = det.get_inverse().cpu().numpy()
+    idx = [s_ * (nel // 4) for s_ in range(4)]
+    ref = np.array([np.max(np.abs(A[w][idx] @ Bg[w].T - np.eye(nel)[idx])) for w in range(nw)])
+    assert np.max(np.abs(r_run - ref)) < 1e-9 * max(1.0, ref.max()) + 1e-12
+    ld_run, sg_run, nacc = (t.cpu().numpy().copy() for t in det.get_stats())
+    det.recompute(pos)
+    r_new = det.residual(pos, nsample=4).cpu().numpy()
+    ld_new, sg_new, nacc2 = (t.cpu().numpy() for t in det.get_stats())
+    print(case, K, "fp32 residual after", nsw, "sweeps: max", r_run.max(), "median", np.median(r_run),
+          "| after recompute: max", r_new.max(), "| logdet drift", np.max(np.abs(ld_run - ld_new)))
+    assert 1e-9 < np.median(r_run) and r_run.max() < 1e-2
+    assert r_new.max() < 1e-3 and np.median(r_new) <= np.median(r_run) * 1.5
+    assert np.array_equal(sg_run, sg_new) and np.array_equal(nacc, nacc2)
+    assert np.max(np.abs(ld_run - ld_new)) < 1e-6 * max(1.0, np.max(np.abs(ld_new)))
+    # the recomputed stored inverse is the fp32 rounding of the oracle's LU inverse of the same Slater matrix
+    Bo, _, _ = P.oracle_binv(A)
+    Bn = det.get_inverse().cpu().numpy()
+    assert np.max(np.abs(Bn - Bo)) <= 0.75 * FP32_ULP * max(1.0, np.max(np.abs(Bo)))
+    # fp64 engine on the same walk: residual at its own level; recompute leaves it there
+    det64 = api.Det.init(spline, P.to_dev(x.pos), delay_rank=K)
+    pos64 = P.to_dev(x.pos)
+    api.sweep(det64, pos64, P.to_dev(x.delta[:nsw]), P.to_dev(x.unif[:nsw]))
+    r64 = det64.residual(pos64, nsample=4).cpu().numpy()
+    assert r64.max() < P.TOL_RESID and r64.max() < 1e-3 * np.median(r_run)
+    det64.recompute(pos64)
+    assert det64.residual(pos64, nsample=4).cpu().numpy().max() < P.TOL_RESID
+    det64.destroy()
+    det.destroy()
+    spline.destroy()
+
+
+@pytest.mark.parametrize("nel,K,nw", [(512, 16, 3), (1024, 16, 3), (1024, 24, 2)])
+def test_fp32_inverse_ring_flush(nel, K, nw):
+    """The TMA-ring flush kernels with fp32 rows (flush_ring.cu ranks <= 16, flush_ring_hp.cu above)
+    against the oracle's fp32-storage mode with the window length K, identical orbital vectors."""
+    cfg = inputs.custom_config(f"f32n{nel}", (24, 24, 24), nel, (9.0, 8.5, 9.5), nw=nw, nsweeps=1, sigma=0.3)
+    x = inputs.make_inputs(cfg, device=P.dev())
+    g = _fp32_run(x, K)
+    dummy = np.zeros((1, 1, 1, nel), np.float32)
+    rep = oracle.sweep(dummy, x.lattice, x.pos, g["B0"], g["ld0"], g["sg0"], x.delta, x.unif, forced=g["acc"],
+                       phi_in=g["rec"], b32=K, nthreads=oracle.max_threads())
+    Bg = g["det"].get_inverse().cpu().numpy()
+    scale = max(1.0, np.max(np.abs(rep["B"])))
+    eb = float(np.max(np.abs(Bg - rep["B"])) / scale)
+    er = float(np.max(np.abs(g["R"] - rep["ratios"]) / np.abs(rep["ratios"])))
+    print(nel, K, "fp32 ring flush: |B - B_oracle| / max|B| =", eb, "ratio rel", er)
+    assert eb <= 16 * FP32_ULP and er < P.TOL_RATIO
+    g["det"].destroy()
+    g["spline"].destroy()

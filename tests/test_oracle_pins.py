@@ -603,3 +603,158 @@ def test_det_kinetic_against_finite_differences(sweep_case):
     # a wrong inverse shows in `one`
     bad = oracle.det_kinetic(coefs, x.lattice, x.pos, np.roll(B, 1, axis=1))
     assert np.max(np.abs(bad["one"] - 1.0)) > 1e-3
+
+
+# ----------------------------------------------------------------------------- drift moves (eq. 11-13)
+def _logdet_at(coefs, lat, pos):
+    s, l = np.linalg.slogdet(oracle.slater_matrix(coefs, lat, pos[None])[0])
+    return s, l
+
+
+def _fd_force(coefs, lat, pos, k, h=1e-5):
+    """F_k = 2 grad_k log|det A| by central differences of numpy log-determinants (L156)."""
+    f = np.zeros(3)
+    for d in range(3):
+        v = []
+        for sgn in (+1.0, -1.0):
+            t = pos.copy()
+            t[k, d] += sgn * h
+            v.append(_logdet_at(coefs, lat, t)[1])
+        f[d] = 2.0 * (v[0] - v[1]) / (2.0 * h)
+    return f
+
+
+def test_drift_moves_against_closed_forms(sweep_case):
+    """orc_sweep_ex with tau > 0.  Pins, none of them the oracle's own formulas:
+    F_k(r) = 2 grad_k log|det A| at the CURRENT configuration against finite differences of numpy
+    log-determinants; the proposal r' = r + tau F + chi (eq. 13 / eq. 19, lambda = 1/2); the
+    transition ratio against scipy's Gaussian log-densities, T(r->r') = N(r'; r + tau F(r), tau I) and
+    T(r'->r) = N(r; r' + tau F(r'), tau I) with F(r') again from finite differences at the proposed
+    configuration; the decision rule of eq. 12; log-det telescoping and B^T A = I at the end."""
+    from scipy.stats import multivariate_normal
+    x, coefs, A, B, ld, sg = sweep_case
+    tau = 0.02
+    rng = np.random.default_rng(17)
+    chi = rng.normal(0.0, np.sqrt(tau), size=x.delta.shape)
+    out = oracle.sweep(coefs, x.lattice, x.pos, B, ld, sg, chi, x.unif, A=A, tau=tau, want_force=True)
+    acc = out["accept"].astype(bool)
+    assert 0 < acc.sum() < acc.size
+    assert np.array_equal(acc, out["ratios"] ** 2 * np.exp(out["logt"]) > x.unif)
+    assert np.abs(out["logt"]).max() > 1e-3            # the ratio of the two Gaussians really matters
+    nsw, nel, nw = x.unif.shape
+    checked = 0
+    for w in range(nw):
+        pos = x.pos[w].copy()
+        for s in range(nsw):
+            for k in range(nel):
+                rp = out["rprop"][s, k, w]
+                assert np.max(np.abs(rp - (pos[k] + tau * out["fcur"][s, k, w] + chi[s, k, w]))) < 1e-14
+                if (s * nel + k) % 9 == w:
+                    f_cur = _fd_force(coefs, x.lattice, pos, k)
+                    assert np.max(np.abs(out["fcur"][s, k, w] - f_cur)) < 1e-5 * max(1.0, np.abs(f_cur).max())
+                    trial = pos.copy()
+                    trial[k] = rp
+                    if abs(out["ratios"][s, k, w]) > 0.05:      # FD of log|det| needs to stay off the node
+                        f_new = _fd_force(coefs, x.lattice, trial, k)
+                        fwd = multivariate_normal(mean=pos[k] + tau * f_cur, cov=tau * np.eye(3)).logpdf(rp)
+                        bwd = multivariate_normal(mean=rp + tau * f_new, cov=tau * np.eye(3)).logpdf(pos[k])
+                        assert abs(out["logt"][s, k, w] - (bwd - fwd)) < 2e-4 * max(1.0, abs(bwd - fwd)), (s, k, w)
+                        checked += 1
+                if acc[s, k, w]:
+                    pos[k] = rp
+        assert np.array_equal(pos, out["pos"][w])
+        s_np, l_np = _logdet_at(coefs, x.lattice, out["pos"][w])
+        assert abs(out["logdet"][w] - l_np) < 1e-8 and out["sign"][w] == int(s_np)
+        res = out["B"][w].T @ oracle.slater_matrix(coefs, x.lattice, out["pos"][w][None])[0] - np.eye(nel)
+        assert np.max(np.abs(res)) < 1e-8
+    assert checked >= 8
+
+
+def test_drift_reverse_move_identity(sweep_case):
+    """Detailed balance structure: accept a move r -> r' (imposed), then propose the reverse move
+    r' -> r from the new configuration (rprop_in): the determinant ratio is the reciprocal and the
+    log transition ratio the negative of the forward one.  A swapped F(r) / F(r'), a wrong sign or a
+    missing 1/R in the force at the proposal breaks this."""
+    x, coefs, A, B, ld, sg = sweep_case
+    tau = 0.03
+    nsw, nel, nw = x.unif.shape
+    chi = np.random.default_rng(5).normal(0.0, np.sqrt(tau), size=(1, nel, nw, 3))
+    ones = np.ones((1, nel, nw), dtype=np.uint8)
+    fwd = oracle.sweep(coefs, x.lattice, x.pos, B, ld, sg, chi, x.unif[:1], forced=ones, tau=tau, iel_count=1,
+                       want_force=True)
+    back = oracle.sweep(coefs, x.lattice, fwd["pos"], fwd["B"], fwd["logdet"], fwd["sign"], chi, x.unif[:1],
+                        forced=ones, tau=tau, iel_count=1,
+                        rprop_in=np.broadcast_to(x.pos.transpose(1, 0, 2)[None], (1, nel, nw, 3)).copy())
+    assert np.max(np.abs(back["ratios"][0, 0] * fwd["ratios"][0, 0] - 1.0)) < 1e-9
+    assert np.max(np.abs(back["logt"][0, 0] + fwd["logt"][0, 0])) < 1e-8 * max(1.0, np.abs(fwd["logt"][0, 0]).max())
+    assert np.max(np.abs(back["pos"] - x.pos)) == 0.0
+    assert np.max(np.abs(back["B"] - B)) < 1e-8 * np.max(np.abs(B))
+    # the force at the proposal of the forward move is the force at the current position of the reverse one
+    assert np.max(np.abs(back["fcur"][0, 0] - fwd["force"][0, 0])) < 1e-8 * max(1.0, np.abs(fwd["force"][0, 0]).max())
+
+
+def test_drift_small_tau_limit(sweep_case):
+    """tau -> 0 with chi = sqrt(tau) z: the drift tau F and log T = O(sqrt(tau)) vanish against the
+    diffusion, so the proposals tend to r + chi and the decisions to those of the no-drift walk
+    (eq. 13 with F = 0) on the same displacements."""
+    x, coefs, A, B, ld, sg = sweep_case
+    z = np.random.default_rng(9).normal(size=x.delta.shape)
+    tau = 1e-10
+    chi = np.sqrt(tau) * z
+    d = oracle.sweep(coefs, x.lattice, x.pos, B, ld, sg, chi, x.unif, tau=tau)
+    n = oracle.sweep(coefs, x.lattice, x.pos, B, ld, sg, chi, x.unif)
+    assert np.abs(d["logt"]).max() < 1e-2
+    assert np.max(np.abs(d["ratios"] - n["ratios"])) < 1e-5
+    same = d["accept"] == n["accept"]
+    assert same.mean() > 0.99
+    assert np.all(np.abs(n["ratios"][~same] ** 2 - x.unif[~same]) < 1e-2)
+
+
+# ----------------------------------------------------------------------------- fp32-stored inverse (L82)
+def test_fp32_stored_inverse(sweep_case):
+    """R:A19.  b32 = 1: after every accepted move the stored inverse is the fp32 rounding of the fp64
+    Sherman-Morrison result computed from the stored (fp32-valued) matrix -- checked move by move
+    against orc_sm_update (itself pinned to numpy's inverse) followed by numpy's cast.  The residual
+    B^T A - I sits at the fp32 level, grows slowly with the number of sweeps, and a recompute from the
+    positions (orc_init_walkers) restores the fp64 level.  b32 = K (delayed rank-K storage) differs
+    from b32 = 1 by a few fp32 ulps of max|B| only."""
+    x, coefs, A, B, ld, sg = sweep_case
+    nsw, nel, nw = x.unif.shape
+    B32 = B.astype(np.float32).astype(np.float64)
+    out = oracle.sweep(coefs, x.lattice, x.pos, B32, ld, sg, x.delta, x.unif, b32=1, want_phi=True)
+    assert np.array_equal(out["B"], out["B"].astype(np.float32).astype(np.float64))
+    # move-by-move replay with the pinned pieces
+    for w in range(nw):
+        Bw = B32[w].copy()
+        for s in range(nsw):
+            for k in range(nel):
+                phi = out["phi"][s, k, w]
+                R = oracle.det_ratio(Bw, k, phi)
+                assert R == out["ratios"][s, k, w]
+                if out["accept"][s, k, w]:
+                    Bw = oracle.sm_update(Bw, k, phi, R).astype(np.float32).astype(np.float64)
+        assert np.array_equal(Bw, out["B"][w])
+    # residual level and growth, recompute
+    delta4 = np.concatenate([x.delta, x.delta[::-1]], axis=0)
+    unif4 = np.concatenate([x.unif, x.unif[::-1]], axis=0)
+    o4 = oracle.sweep(coefs, x.lattice, x.pos, B32, ld, sg, delta4, unif4, b32=1)
+    o1 = oracle.sweep(coefs, x.lattice, x.pos, B32, ld, sg, delta4[:1], unif4[:1], b32=1)
+    o64 = oracle.sweep(coefs, x.lattice, x.pos, B, ld, sg, delta4, unif4, forced=o4["accept"])
+
+    def resid(Bm, pos):
+        Af = oracle.slater_matrix(coefs, x.lattice, pos)
+        return max(np.max(np.sum(np.abs(Bm[w].T @ Af[w] - np.eye(nel)), axis=1)) for w in range(nw))
+
+    r1, r4, r64 = resid(o1["B"], o1["pos"]), resid(o4["B"], o4["pos"]), resid(o64["B"], o64["pos"])
+    assert 1e-8 < r1 < 1e-3 and r4 < 1e-3 and r4 < 50.0 * r1 and r64 < 1e-9
+    assert np.max(np.abs(o4["B"] - o64["B"])) < 1e-4 * np.max(np.abs(o64["B"]))
+    Br, ldr, sgr = oracle.init_walkers(coefs, x.lattice, o4["pos"])
+    assert resid(Br, o4["pos"]) < 1e-10
+    assert np.max(np.abs(ldr - o4["logdet"])) < 1e-4 and np.array_equal(sgr, o4["sign"])
+    # delayed-rank storage: same decisions here, and the stored matrices agree to a few fp32 ulps
+    ok = oracle.sweep(coefs, x.lattice, x.pos, B32, ld, sg, x.delta, x.unif, b32=5, forced=out["accept"])
+    assert np.array_equal(ok["B"], ok["B"].astype(np.float32).astype(np.float64))
+    assert 0 < np.max(np.abs(ok["B"] - out["B"])) < 64 * 2.0 ** -24 * np.max(np.abs(out["B"]))
+    # and b32 = K with a window that closes after every step is b32 = 1 exactly
+    o_k1 = oracle.sweep(coefs, x.lattice, x.pos, B32, ld, sg, x.delta, x.unif, b32=1, forced=out["accept"])
+    assert np.array_equal(o_k1["B"], out["B"])
