@@ -39,6 +39,9 @@ UNIT = "moves/s"
 # rank-16 vs rank-1; very large names rank-32, which is measured beside rank-16: at N = 2048 the
 # rank-16 window is the faster one on this kernel)
 DEFAULT_DELAY = {"tiny": [0], "small": [16, 0], "mid": [16, 0], "large": [16, 0], "xlarge": [16, 32, 0]}
+# further arms reported as variants (fewer timed steps each): (delay rank, fp32-stored inverse)
+EXTRA_ARMS = {"large": [(16, True), (0, True), (24, False), (32, False)], "mid": [(16, True)],
+              "xlarge": [(16, True), (24, False)]}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures
 # (profiles/r01_*.md), config `large`
 # keyed by (kernel, delay rank); value = (bytes per launch, the file the figure comes from)
@@ -189,6 +192,8 @@ def main():
                          "config's delayed rank as the headline AND rank-1 as a variant in the same line")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--fp32-inverse", action="store_true", help="store the inverse in fp32 (QMC_DET_FP32_INVERSE)")
+    ap.add_argument("--no-variants", action="store_true", help="skip the extra variant arms of the default run")
     ap.add_argument("--walkers", type=int, default=0, help="override walkers per GPU (debug)")
     args = ap.parse_args()
 
@@ -253,14 +258,17 @@ def main():
     def max_over_ranks(ms):
         return sharding.max_over_ranks(ms, device=dev)
 
-    def run_arm(delay):
+    def run_arm(delay, fp32=False, steps=None):
         """W warm-up sweeps + K timed sweeps with the inverse update `delay` (0 = rank-1), device
-        resident; then the same K sweeps end to end from pinned host buffers."""
+        resident; then the same K sweeps end to end from pinned host buffers.  fp32: the inverse is
+        stored in single precision (QMC_DET_FP32_INVERSE)."""
+        nsteps = args.steps if steps is None else min(args.steps, steps)
+        nsteps_total = args.warmup + nsteps
         pos = torch.from_numpy(pos_np).to(dev)
         accept = torch.zeros(unif.shape, dtype=torch.uint8, device=dev)
         ratios = torch.zeros(unif.shape, dtype=torch.float64, device=dev)
         t0 = time.perf_counter()
-        det = api.Det.init(spline, pos, delay_rank=delay)
+        det = api.Det.init(spline, pos, delay_rank=delay, fp32_inverse=fp32)
         torch.cuda.synchronize()
         t_init = time.perf_counter() - t0
 
@@ -284,13 +292,13 @@ def main():
         clocks = sampler.stop()
         launches = api.launch_count() - launches0
         ms = max_over_ranks(e0.elapsed_time(e1))
-        moves = args.steps * nel * nw * world
+        moves = nsteps * nel * nw * world
         value = moves / (ms * 1e-3)
         acc_rate = float(accept[args.warmup:].to(torch.float64).mean().item())
 
         # ---- per-kernel split: a SECOND pass of `nprof` sweeps with every launch bracketed by CUDA
         #      events (qmc_det_profile); the walk goes on with the random numbers of the first timed sweeps
-        nprof = min(args.steps, 5)
+        nprof = min(nsteps, 5)
         det.profile(True)
         e0.record()
         for i in range(args.warmup, args.warmup + nprof):
@@ -303,14 +311,14 @@ def main():
         n_acc = float(accept[args.warmup:args.warmup + nprof].to(torch.float64).sum().item())
 
         # ---- roofline of the dominant kernel (rank-local, from the per-launch CUDA events)
-        ld, npitch, K = det.ld, spline.row_pitch, det.delay_rank
-        per_launch = {   # algorithmic bytes per launch
+        ld, npitch, K, eb = det.ld, spline.row_pitch, det.delay_rank, det.storage_bytes
+        per_launch = {   # algorithmic bytes per launch; eb = bytes per stored element of B
             "spo_vgl": (nprof * nel * nw / max(prof["spo_vgl"][1], 1)) * (64 + 5) * npitch * 4,
-            "ratio_rowcopy": nw * (2 * 8 * ld + 4 * nel),
-            "sm_update": (n_acc / max(prof["sm_update"][1], 1)) * (16 * nel * ld + 12 * nel),
-            "delayed_flush": nw * 16 * nel * ld + (n_acc / max(prof["delayed_flush"][1], 1)) * (8 * ld + 4 * npitch),
+            "ratio_rowcopy": nw * ((eb + 8) * ld + 4 * nel),
+            "sm_update": (n_acc / max(prof["sm_update"][1], 1)) * (2 * eb * nel * ld + 12 * nel),
+            "delayed_flush": nw * 2 * eb * nel * ld + (n_acc / max(prof["delayed_flush"][1], 1)) * (8 * ld + 4 * npitch),
             # window: K rows of B0 and K vectors in, R' rows out
-            "delayed_window": nw * max(K, 1) * (8 * ld + 4 * npitch) + (n_acc / max(prof["delayed_window"][1], 1)) * 8 * ld,
+            "delayed_window": nw * max(K, 1) * (eb * ld + 4 * npitch) + (n_acc / max(prof["delayed_window"][1], 1)) * 8 * ld,
         }
         kernels = {}
         for k, (kms, kn) in prof.items():
@@ -333,7 +341,7 @@ def main():
         # DRAM bytes per launch are an ncu measurement (no profiler runs inside bench.py): quoted from the
         # committed capture of the same kernel and launch shape, with its source; null for other shapes
         traffic, traffic_src = None, None
-        if args.config == "large" and nw == cfg.nw and (dom, K) in NCU_TRAFFIC:
+        if args.config == "large" and nw == cfg.nw and not fp32 and (dom, K) in NCU_TRAFFIC:
             traffic, traffic_src = NCU_TRAFFIC[(dom, K)]
         if dom == "delayed_flush" and kd["min_ms_fp64"] > kd["min_ms_hbm"]:
             # the contraction, not the pass over B, bounds this rank: report against the fp64 tensor peak
@@ -371,8 +379,10 @@ def main():
         e2e = {"value": moves / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d * world,
                "d2h_bytes_per_step": d2h * world}
         update = "sherman-morrison rank-1" if K == 0 else f"delayed rank-{K} (same result as rank-1)"
+        if fp32:
+            update += ", fp32-stored inverse (fp64 arithmetic; R:A19)"
         det.destroy()
-        return {"value": value, "ms_per_step": ms / args.steps, "update": update, "accept_rate": acc_rate,
+        return {"value": value, "ms_per_step": ms / nsteps, "steps": nsteps, "update": update, "accept_rate": acc_rate,
                 "kernel_split": f"second pass of {nprof} sweeps with per-launch CUDA events ({ms_prof / nprof:.2f} ms per sweep)",
                 "init_s": t_init, "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
                 "kernels": kernels, "spline_evals_per_s": value * nel}
@@ -382,7 +392,9 @@ def main():
                + ("exceeds the 126 MB L2; no flush needed" if ws_table + ws_binv > 0.5 else
                   "fits L2: numbers are L2-resident, not HBM rooflines"))
     delays = [args.delay] if args.delay >= 0 else DEFAULT_DELAY.get(args.config, [0])
-    arms = [run_arm(dl) for dl in dict.fromkeys(delays)]
+    arms = [run_arm(dl, fp32=args.fp32_inverse) for dl in dict.fromkeys(delays)]
+    if args.delay < 0 and not args.fp32_inverse and not args.no_variants:
+        arms += [run_arm(dl, fp32=f32, steps=5) for dl, f32 in EXTRA_ARMS.get(args.config, [])]
     main_arm = arms[0]
     line = {
         "metric": METRIC, "value": main_arm["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -399,7 +411,7 @@ def main():
         "spline_evals_per_s": main_arm["spline_evals_per_s"],
     }
     if len(arms) > 1:
-        line["variants"] = {a["update"]: {k: a[k] for k in ("value", "ms_per_step", "accept_rate", "clocks", "e2e",
+        line["variants"] = {a["update"]: {k: a[k] for k in ("value", "ms_per_step", "steps", "accept_rate", "clocks", "e2e",
                                                             "gpu_launches", "roofline", "kernels")} for a in arms[1:]}
 
     if want_cpu:

@@ -224,7 +224,20 @@ typedef struct qmc_sweep_opts {
                          /*   the moved electron at the PROPOSED configuration,               */
                          /*   F = 2 sum_j grad phi_j(r') B[k][j] / R, for every move          */
                          /*   (accepted or not; 0 where R == 0)                               */
-    int reserved[2];
+    double drift_tau;    /* > 0: drift moves (reading R:A20).  `delta` then holds   */
+                         /*   the diffusion part chi ~ N(0, tau) per component and the proposal is      */
+                         /*   r' = r_k + tau F_k(r) + chi  (eq. 13 / eq. 19 with lambda = 1/2), with     */
+                         /*   F_k(r) = 2 grad_k log Psi_T = 2 sum_j grad phi_j(r_k) B[k][j] (L156) at    */
+                         /*   the CURRENT configuration; the move is accepted iff (eq. 12)              */
+                         /*   R^2 T(r'->r)/T(r->r') > u,  log T'/T = (|r' - r - tau F(r)|^2              */
+                         /*   - |r - r' - tau F(r')|^2) / (2 tau).  One SPO-VGL gather more per move    */
+                         /*   (gradients at the current position, batched over 16 electrons) and the     */
+                         /*   proposal gather per step (it depends on the decisions before it).          */
+                         /*   With delay_rank >= 2 pending rows are applied first and every step is a   */
+                         /*   rank-1 update (the one-launch window needs all its proposals up front).    */
+    double *rprop_out;   /* NULL, or dev double [nsweeps][nel][nw][3]: the proposed positions (drift)   */
+    double *logt_out;    /* NULL, or dev double [nsweeps][nel][nw]: log T(r'->r)/T(r->r') (drift)       */
+    double *fcur_out;    /* NULL, or dev double [nsweeps][nel][nw][3]: F_k(r) at the current config.    */
 } qmc_sweep_opts_t;
 
 int qmc_sweep_ex(qmc_det_t *det, const qmc_spline_t *spline, double *pos, const double *delta,

@@ -31,7 +31,8 @@ PROF_KINDS = ["spo_vgl", "sm_update", "delayed_window", "delayed_accept", "delay
 class SweepOpts(ctypes.Structure):
     _fields_ = [("iel_begin", ctypes.c_int), ("iel_count", ctypes.c_int),
                 ("phi_record", _vp), ("nrecord", ctypes.c_int), ("fixed_node", ctypes.c_int),
-                ("force_out", _vp), ("reserved", ctypes.c_int * 2)]
+                ("force_out", _vp), ("drift_tau", ctypes.c_double), ("rprop_out", _vp), ("logt_out", _vp),
+                ("fcur_out", _vp)]
 
 
 class QmcError(RuntimeError):
@@ -319,13 +320,16 @@ class Det:
 
 
 def sweep(det, pos, delta, unif, ratios_out=None, accept_out=None, forced_accept=None, iel_begin=0,
-          iel_count=0, phi_record=None, nrecord=0, fixed_node=False, force_out=None, stream=None):
+          iel_count=0, phi_record=None, nrecord=0, fixed_node=False, force_out=None, drift_tau=0.0,
+          rprop_out=None, logt_out=None, fcur_out=None, stream=None):
     """qmc_sweep / qmc_sweep_ex on device tensors (pos updated in place).
 
     pos double [nw][nel][3]; delta double [nsweeps][nel][nw][3]; unif double [nsweeps][nel][nw];
     ratios_out double / accept_out uint8 / forced_accept uint8: [nsweeps][nel][nw] or None;
     phi_record float32 [nsweeps][nel][nrecord][nel] or None; fixed_node: reject moves with R < 0;
     force_out double [nsweeps][nel][nw][3] or None (F = 2 grad log|Psi| at the proposed configuration).
+    drift_tau > 0: drift moves (delta = chi ~ N(0, tau)); rprop_out [nsweeps][nel][nw][3], logt_out
+    [nsweeps][nel][nw], fcur_out [nsweeps][nel][nw][3]: proposals, log T'/T and F at the current configuration.
     """
     lib = load_library()
     nsweeps = delta.shape[0]
@@ -339,7 +343,7 @@ def sweep(det, pos, delta, unif, ratios_out=None, accept_out=None, forced_accept
     args = [det._h, det.spline._h, _dev(pos, torch.float64), _dev(delta, torch.float64),
             _dev(unif, torch.float64), nsweeps, _dev(ratios_out, torch.float64, True),
             _dev(accept_out, torch.uint8, True), _dev(forced_accept, torch.uint8, True)]
-    if iel_begin or iel_count or phi_record is not None or fixed_node or force_out is not None:
+    if iel_begin or iel_count or phi_record is not None or fixed_node or force_out is not None or drift_tau:
         if phi_record is not None and tuple(phi_record.shape) != (nsweeps, det.nel, nrecord, det.nel):
             raise QmcError("phi_record must be [nsweeps][nel][nrecord][nel]")
         if force_out is not None and tuple(force_out.shape) != tuple(unif.shape) + (3,):
@@ -347,7 +351,11 @@ def sweep(det, pos, delta, unif, ratios_out=None, accept_out=None, forced_accept
         opts = SweepOpts(int(iel_begin), int(iel_count),
                          None if phi_record is None else phi_record.data_ptr(), int(nrecord),
                          1 if fixed_node else 0,
-                         None if force_out is None else _dev(force_out, torch.float64).value)
+                         None if force_out is None else _dev(force_out, torch.float64).value,
+                         float(drift_tau),
+                         None if rprop_out is None else _dev(rprop_out, torch.float64).value,
+                         None if logt_out is None else _dev(logt_out, torch.float64).value,
+                         None if fcur_out is None else _dev(fcur_out, torch.float64).value)
         rc = lib.qmc_sweep_ex(*args, ctypes.byref(opts), _stream(stream))
         _check(rc, "qmc_sweep_ex")
     else:

@@ -93,6 +93,9 @@ struct qmc_det {
     cudaStream_t aux;           // second stream (non-blocking), created on first use
     cudaEvent_t ev_spo[2], ev_main;
     int overlap;                // 1: overlap enabled (delay >= 2 and QMC_SWEEP_OVERLAP != 0)
+    // drift moves (qmc_sweep_ex drift_tau > 0): allocated on first use
+    float *vgl_cur;             // [kSpoBatch][nw][5][np] SPO-VGL at the CURRENT positions of a batch of electrons
+    double *rprop, *fcur, *tfac;   // [nw][3], [nw][3], [nw]: proposal, F_k(r), T(r'->r)/T(r->r') of the current step
     double *rowk;               // [nw][ld]      copy of row iel of B taken before the update
     double *ratio;              // [nw]      ratio of the current step (ratio_rowcopy_kernel -> sm_update_kernel)
     unsigned char *acc;         // [nw]

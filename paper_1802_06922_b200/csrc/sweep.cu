@@ -23,8 +23,8 @@ struct SpoBatchArgs {
     const double *delta;   // [nb][nw][3], offset to (sweep, first electron of the batch); NULL = the current positions
     int nel, iel0, nw;
     float *vgl;            // [nb][nw][5][np]
-    float *phi_record;     // [nb][nrecord][nel], offset to (sweep, first electron), or NULL
-    int nrecord;
+    float *phi_record;     // [nb][nrecord][nel_record], offset to (sweep, first electron), or NULL
+    int nrecord, nel_record;
 };
 
 // One block per (orbital tile, walker, step of the batch).  Thread t owns orbitals 4t..4t+3 of the
@@ -52,11 +52,11 @@ __global__ void __launch_bounds__(256) spo_batch_kernel(SpoBatchArgs a)
     *reinterpret_cast<float4 *>(o + 3 * (size_t)np) = gz;
     *reinterpret_cast<float4 *>(o + 4 * (size_t)np) = lp;
     if (a.phi_record && w < a.nrecord) {
-        float *rec = a.phi_record + ((size_t)j * a.nrecord + w) * a.nel;
-        if (col + 0 < a.nel) rec[col + 0] = v.x;
-        if (col + 1 < a.nel) rec[col + 1] = v.y;
-        if (col + 2 < a.nel) rec[col + 2] = v.z;
-        if (col + 3 < a.nel) rec[col + 3] = v.w;
+        float *rec = a.phi_record + ((size_t)j * a.nrecord + w) * a.nel_record;
+        if (col + 0 < a.nel_record) rec[col + 0] = v.x;
+        if (col + 1 < a.nel_record) rec[col + 1] = v.y;
+        if (col + 2 < a.nel_record) rec[col + 2] = v.z;
+        if (col + 3 < a.nel_record) rec[col + 3] = v.w;
     }
 }
 
@@ -64,11 +64,56 @@ __global__ void __launch_bounds__(256) spo_batch_kernel(SpoBatchArgs a)
 // the update kernel can overwrite B in place.  One block per walker.  With force_out the three
 // gradient vectors of the proposal (phi + np, + 2 np, + 3 np) are contracted with the same row:
 // F = 2 grad log Psi_T at the proposed configuration = 2 (B[iel] . grad phi) / R.
+// Drift moves (eq. 11-13; R:A20): what the ratio kernel needs to form the ratio of the
+// transition densities, log T(r'->r)/T(r->r') = (|r' - r - tau F(r)|^2 - |r - r' - tau F(r')|^2) / (2 tau).
+struct DriftStep {
+    double tau;               // 0: no drift
+    const double *pos;        // [nw][nel][3] current positions
+    const double *rprop;      // [nw][3] proposed positions of this step
+    const double *fcur;       // [nw][3] F_k(r) at the current configuration
+    double *tfac;             // [nw] out: exp(log T ratio), the factor of eq. 12
+    double *logt_out;         // [nw] out or NULL
+};
+
+// F_k(r) = 2 grad_k log|det A| = 2 sum_j grad phi_j(r_k) B[k][j] at the CURRENT configuration (L156) and
+// the proposal of eq. 13 / eq. 19 with lambda = 1/2: r' = r_k + (tau F + chi), chi ~ N(0, tau) pre-generated.
+// One block per walker; the three dots in a fixed order.
+template <typename TB>
+__global__ void __launch_bounds__(128)
+drift_propose_kernel(const TB *__restrict__ B, int nel, int ld, int iel, const float *__restrict__ vgl_cur,
+                     size_t ldv, int np, const double *__restrict__ pos, const double *__restrict__ chi,
+                     double tau, double *__restrict__ rprop, double *__restrict__ fcur)
+{
+    __shared__ double red[33];
+    const int w = blockIdx.x;
+    const TB *row = B + ((size_t)w * nel + iel) * ld;
+    const float *gv = vgl_cur + (size_t)w * ldv + np;          // d/dx, then d/dy, d/dz at + np each
+    double g[3] = {0.0, 0.0, 0.0};
+    for (int j = threadIdx.x; 2 * j < nel; j += 128) {         // the vectors are zero-padded up to np >= nel
+        const double2 b = ld2(row + 2 * j);
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            const float2 q = reinterpret_cast<const float2 *>(gv + (size_t)d * np)[j];
+            g[d] = fma(b.x, (double)q.x, g[d]);
+            g[d] = fma(b.y, (double)q.y, g[d]);
+        }
+    }
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        const double f = 2.0 * block_sum(g[d], red);
+        if (threadIdx.x == 0) {
+            fcur[3 * (size_t)w + d] = f;
+            // (no FMA contraction: the proposal is reproducible from fcur, chi and the position, bit for bit)
+            rprop[3 * (size_t)w + d] = __dadd_rn(pos[((size_t)w * nel + iel) * 3 + d], __dadd_rn(__dmul_rn(tau, f), chi[3 * (size_t)w + d]));
+        }
+    }
+}
+
 template <typename TB>
 __global__ void __launch_bounds__(256)
 ratio_rowcopy_kernel(const TB *__restrict__ B, int nel, int ld, int iel, const float *__restrict__ phi,
                      size_t ldphi, int np, double *__restrict__ rowk, double *__restrict__ ratio,
-                     double *__restrict__ force_out)
+                     double *__restrict__ force_out, DriftStep ds)
 {
     __shared__ double red[33];
     const int w = blockIdx.x;
@@ -84,7 +129,7 @@ ratio_rowcopy_kernel(const TB *__restrict__ B, int nel, int ld, int iel, const f
             const float2 f = ph[j];
             acc = fma(b.x, (double)f.x, acc);
             acc = fma(b.y, (double)f.y, acc);
-            if (force_out) {
+            if (force_out || ds.tau > 0.0) {
 #pragma unroll
                 for (int d = 0; d < 3; ++d) {
                     const float2 q = reinterpret_cast<const float2 *>(pw + (size_t)(1 + d) * np)[j];
@@ -96,11 +141,27 @@ ratio_rowcopy_kernel(const TB *__restrict__ B, int nel, int ld, int iel, const f
     }
     acc = block_sum(acc, red);
     if (threadIdx.x == 0) ratio[w] = acc;
-    if (force_out) {
+    if (force_out || ds.tau > 0.0) {
+        double fnew[3];
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
             const double gd = block_sum(g[d], red);
-            if (threadIdx.x == 0) force_out[3 * (size_t)w + d] = acc != 0.0 ? 2.0 * gd / acc : 0.0;
+            fnew[d] = acc != 0.0 ? 2.0 * gd / acc : 0.0;
+            if (threadIdx.x == 0 && force_out) force_out[3 * (size_t)w + d] = fnew[d];
+        }
+        if (ds.tau > 0.0 && threadIdx.x == 0) {        // log T(r'->r)/T(r->r'), eq. 11-13 with lambda = 1/2
+            double fwd = 0.0, bwd = 0.0;
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                const double rk = ds.pos[((size_t)w * nel + iel) * 3 + d], rn = ds.rprop[3 * (size_t)w + d];
+                const double a = rn - rk - ds.tau * ds.fcur[3 * (size_t)w + d];
+                const double b = rk - rn - ds.tau * fnew[d];
+                fwd += a * a;
+                bwd += b * b;
+            }
+            const double logt = (fwd - bwd) / (2.0 * ds.tau);
+            ds.tfac[w] = exp(logt);
+            if (ds.logt_out) ds.logt_out[w] = logt;
         }
     }
 }
@@ -115,7 +176,7 @@ int spo_batch_vgl(qmc_det *d, const qmc_spline *sp, const double *pos, const dou
     a.pos = pos; a.delta = delta;
     a.nel = d->nel; a.iel0 = iel0; a.nw = d->nw;
     a.vgl = out;
-    a.phi_record = phi_record; a.nrecord = nrecord;
+    a.phi_record = phi_record; a.nrecord = nrecord; a.nel_record = d->nel;
     prof_start(d, kProfSpoRatio, s);
     spo_batch_kernel<<<dim3(tiles, d->nw, nb), threads, 0, s>>>(a);
     prof_stop(d, s);
@@ -184,6 +245,92 @@ static int sweep_delayed(qmc_det *d, const qmc_spline *sp, double *pos, const do
     return QMC_OK;
 }
 
+// Drift moves (R:A20).  The proposal of electron k now depends on the decisions
+// before it (F_k(r) is taken with the current inverse), so per electron step:
+//   D1 drift_propose_kernel  F_k(r) from the gradients at the CURRENT position, r' = r + tau F + chi
+//   D2 spo_batch_kernel      SPO-VGL at r' (one position per walker)
+//   D3 ratio_rowcopy_kernel  R, F_k(r') and the factor T(r'->r)/T(r->r') of eq. 12
+//   D4 sm_update_kernel      accept iff R^2 T'/T > u; rank-1 update
+// and once per 16 electrons a batched SPO-VGL at their current positions (those do not change until the
+// electron's own step), which is what survives of the batched gather.  delay_rank >= 2 is served by
+// the same per-step kernels after the pending window has been applied (every step is then a rank-1
+// update: the one-launch-per-window form needs all proposals of a window up front).
+static int sweep_drift(qmc_det *d, const qmc_spline *sp, double *pos, const double *chi, const double *unif,
+                       int nsweeps, int k0, int kn, double *ratios_out, unsigned char *accept_out,
+                       const unsigned char *forced, int fixed_node, double *force, float *rec, int nrec, double tau,
+                       double *rprop_out, double *logt_out, double *fcur_out, cudaStream_t s)
+{
+    const int nw = d->nw, nel = d->nel, np = d->np;
+    if (d->delay) {
+        int rc = delayed_flush_reset_host(d, s);
+        if (rc) return rc;
+    }
+    if (!d->vgl_cur) {
+        auto alloc = [&](void **p, size_t bytes) {
+            cudaError_t e = cudaMalloc(p, bytes);
+            if (e != cudaSuccess) { set_error("qmc_sweep_ex (drift): cudaMalloc(%zu bytes) -> %s", bytes, cudaGetErrorString(e)); (void)cudaGetLastError(); return QMC_ENOMEM; }
+            return QMC_OK;
+        };
+        int rc;
+        if ((rc = alloc((void **)&d->vgl_cur, (size_t)kSpoBatch * nw * 5 * np * sizeof(float))) ||
+            (rc = alloc((void **)&d->rprop, (size_t)nw * 3 * sizeof(double))) ||
+            (rc = alloc((void **)&d->fcur, (size_t)nw * 3 * sizeof(double))) ||
+            (rc = alloc((void **)&d->tfac, (size_t)nw * sizeof(double)))) return rc;
+    }
+    int threads, tiles;
+    spo_launch_shape(np, &threads, &tiles);
+    const size_t slot_stride = (size_t)nw * 5 * np;
+    float *const vgl_prop = d->vgl_buf[0];                 // slot 0 of the proposal scratch
+    for (int sw = 0; sw < nsweeps; ++sw) {
+        for (int k = k0; k < k0 + kn; ++k) {
+            const size_t mv = ((size_t)sw * nel + k) * nw;
+            const int slot = (k - k0) % kSpoBatch;
+            if (slot == 0) {          // gradients at the current positions of the next 16 electrons
+                const int nb = min(kSpoBatch, k0 + kn - k);
+                int rc = spo_batch_vgl(d, sp, pos, nullptr, k, nb, nullptr, 0, d->vgl_cur, s);
+                if (rc) return rc;
+            }
+            double *rprop = rprop_out ? rprop_out + 3 * mv : d->rprop;
+            double *fcur = fcur_out ? fcur_out + 3 * mv : d->fcur;
+            prof_start(d, kProfRatio, s);
+            QMC_WITH_B(d, TB, Bp, (drift_propose_kernel<TB><<<nw, 128, 0, s>>>(Bp, nel, d->ld, k, d->vgl_cur + slot * slot_stride,
+                                                                               (size_t)5 * np, np, pos, chi + 3 * mv, tau, rprop, fcur)));
+            prof_stop(d, s);
+            QMC_LAUNCHED();
+            SpoBatchArgs a{};         // D2: one position per walker, read from rprop ([nw][1][3])
+            a.sp = sp->view; a.pos = rprop; a.delta = nullptr; a.nel = 1; a.iel0 = 0; a.nw = nw;
+            a.vgl = vgl_prop;
+            a.phi_record = rec ? rec + mv / nw * (size_t)nrec * nel : nullptr; a.nrecord = nrec; a.nel_record = nel;
+            prof_start(d, kProfSpoRatio, s);
+            spo_batch_kernel<<<dim3(tiles, nw, 1), threads, 0, s>>>(a);
+            prof_stop(d, s);
+            QMC_LAUNCHED();
+            DriftStep ds{tau, pos, rprop, fcur, d->tfac, logt_out ? logt_out + mv : nullptr};
+            prof_start(d, kProfRatio, s);
+            QMC_WITH_B(d, TB, Bp, (ratio_rowcopy_kernel<TB><<<nw, 256, 0, s>>>(Bp, nel, d->ld, k, vgl_prop, (size_t)5 * np, np, d->rowk,
+                                                                               d->ratio, force ? force + 3 * mv : nullptr, ds)));
+            prof_stop(d, s);
+            QMC_LAUNCHED();
+            UpdateArgs u{};
+            u.B = d->b32 ? (void *)d->Bf : (void *)d->B; u.nel = nel; u.ld = d->ld; u.iel = k;
+            u.phi = vgl_prop; u.ldphi = (size_t)5 * np; u.rowk = d->rowk;
+            u.ratio = d->ratio; u.tfac = d->tfac; u.rprop = rprop;
+            u.unif = unif + mv;
+            u.forced = forced ? forced + mv : nullptr;
+            u.fixed_node = fixed_node;
+            u.ratios_out = ratios_out ? ratios_out + mv : nullptr;
+            u.accept_out = accept_out ? accept_out + mv : nullptr;
+            u.pos = pos; u.delta = chi + 3 * mv;
+            u.logdet = d->logdet; u.sign = d->sign; u.naccept = d->naccept;
+            prof_start(d, kProfUpdate, s);
+            cudaError_t ue = d->b32 ? launch_sm_update<float, true>(u, nw, s) : launch_sm_update<double, true>(u, nw, s);
+            prof_stop(d, s);
+            QMC_CUDA(ue);
+        }
+    }
+    return QMC_OK;
+}
+
 static int sweep_impl(qmc_det *d, const qmc_spline *sp, double *pos, const double *delta, const double *unif,
                       int nsweeps, double *ratios_out, unsigned char *accept_out, const unsigned char *forced,
                       const qmc_sweep_opts_t *opts, cudaStream_t s)
@@ -205,6 +352,10 @@ static int sweep_impl(qmc_det *d, const qmc_spline *sp, double *pos, const doubl
         nrec = rec ? opts->nrecord : 0;
         QMC_REQUIRE(k0 >= 0 && kn >= 0 && k0 + kn <= nel, "qmc_sweep_ex: electron range %d+%d outside 0..%d", k0, kn, nel);
         QMC_REQUIRE(nrec >= 0 && nrec <= nw, "qmc_sweep_ex: nrecord=%d outside 0..%d", nrec, nw);
+        QMC_REQUIRE(opts->drift_tau >= 0.0 && isfinite(opts->drift_tau), "qmc_sweep_ex: drift_tau=%g", opts->drift_tau);
+        if (opts->drift_tau > 0.0)
+            return sweep_drift(d, sp, pos, delta, unif, nsweeps, k0, kn, ratios_out, accept_out, forced, fixed_node, force,
+                               rec, nrec, opts->drift_tau, opts->rprop_out, opts->logt_out, opts->fcur_out, s);
     }
     const int batch = d->spo_batch;
     const size_t slot_stride = (size_t)nw * 5 * d->np;
@@ -224,7 +375,7 @@ static int sweep_impl(qmc_det *d, const qmc_spline *sp, double *pos, const doubl
             // K2: ratio + row copy, K3: decision + rank-1 update
             prof_start(d, kProfRatio, s);
             QMC_WITH_B(d, TB, Bp, (ratio_rowcopy_kernel<TB><<<nw, 256, 0, s>>>(Bp, nel, d->ld, k, phi, (size_t)5 * d->np, d->np, d->rowk,
-                                                                               d->ratio, force ? force + 3 * mv : nullptr)));
+                                                                               d->ratio, force ? force + 3 * mv : nullptr, DriftStep{})));
             prof_stop(d, s);
             QMC_LAUNCHED();
             UpdateArgs u{};

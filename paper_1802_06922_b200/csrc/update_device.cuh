@@ -23,6 +23,9 @@ struct UpdateArgs {
     unsigned char *accept_out;    // [nw] or NULL
     double *pos;                  // [nw][nel][3]
     const double *delta;          // [nw][3]
+    // drift moves (eq. 11-13): factor T(r'->r)/T(r->r') of the acceptance and the proposed positions
+    const double *tfac;           // [nw] or NULL (= 1)
+    const double *rprop;          // [nw][3] or NULL (the accepted electron moves to pos + delta)
     // per-walker statistics
     double *logdet;
     int *sign;
@@ -34,6 +37,8 @@ constexpr int kUpdRowsPerCta = 64;
 
 // Metropolis test of eq. 12 with symmetric T and a determinant-only Psi (R:A8).
 __device__ __forceinline__ bool metropolis(double R, double u) { return isfinite(R) && (R * R > u); }
+// The same with the ratio of the transition densities (drift moves, eq. 12): accept iff R^2 T'/T > u.
+__device__ __forceinline__ bool metropolis_t(double R, double tf, double u) { return isfinite(R) && isfinite(tf) && (R * R * tf > u); }
 // A move may be applied only if its ratio is finite and non-zero: the update divides by R and the
 // new Slater matrix would be singular otherwise (R:A18).  The Metropolis test already implies it
 // (R * R > u >= 0); decisions imposed by the caller (forced_accept, qmc_det_accept_update) are
@@ -50,7 +55,10 @@ __global__ void __launch_bounds__(kUpdThreads) sm_update_kernel(UpdateArgs a)
     const int w = blockIdx.y;
     const double R = a.ratio[w];
     bool acc;
-    if (DECIDE) acc = a.forced ? (a.forced[w] != 0) : (metropolis(R, a.unif[w]) && !(a.fixed_node && R < 0.0));
+    if (DECIDE) {
+        const double tf = a.tfac ? a.tfac[w] : 1.0;
+        acc = a.forced ? (a.forced[w] != 0) : (metropolis_t(R, tf, a.unif[w]) && !(a.fixed_node && R < 0.0));
+    }
     else acc = a.accept[w] != 0;
     acc = acc && usable_ratio(R);     // an imposed accept of a singular / non-finite move is refused (R:A18)
     if (blockIdx.x == 0 && threadIdx.x == 0) {
@@ -64,9 +72,13 @@ __global__ void __launch_bounds__(kUpdThreads) sm_update_kernel(UpdateArgs a)
             a.naccept[w] += 1;
             if (DECIDE) {
                 double *r = a.pos + ((size_t)w * a.nel + a.iel) * 3;
-                r[0] += a.delta[3 * (size_t)w + 0];
-                r[1] += a.delta[3 * (size_t)w + 1];
-                r[2] += a.delta[3 * (size_t)w + 2];
+                if (a.rprop) {
+                    r[0] = a.rprop[3 * (size_t)w + 0]; r[1] = a.rprop[3 * (size_t)w + 1]; r[2] = a.rprop[3 * (size_t)w + 2];
+                } else {
+                    r[0] += a.delta[3 * (size_t)w + 0];
+                    r[1] += a.delta[3 * (size_t)w + 1];
+                    r[2] += a.delta[3 * (size_t)w + 2];
+                }
             }
         }
     }

@@ -47,8 +47,19 @@ def test_header_compiles_as_plain_c(tmp_path):
 
 
 def test_sweep_opts_layout_matches_binding():
-    # the ctypes mirror must have the C struct's size: 2 ints, pointer, 2 ints, 3 ints (+ padding)
-    assert ctypes.sizeof(api.SweepOpts) == 40
+    # the ctypes mirror must have the C struct's size and offsets: compile the header and ask the compiler
+    src = "#include <stdio.h>\n#include <stddef.h>\n#include \"qmc_b200.h\"\nint main(void){printf(\"%zu %zu %zu %zu %zu %zu\\n\", sizeof(qmc_sweep_opts_t), offsetof(qmc_sweep_opts_t, phi_record), offsetof(qmc_sweep_opts_t, force_out), offsetof(qmc_sweep_opts_t, drift_tau), offsetof(qmc_sweep_opts_t, rprop_out), offsetof(qmc_sweep_opts_t, fcur_out));return 0;}\n"
+    import tempfile
+    with tempfile.TemporaryDirectory() as tmp:
+        c = os.path.join(tmp, "t.c")
+        with open(c, "w") as f:
+            f.write(src)
+        exe = os.path.join(tmp, "t")
+        subprocess.run(["gcc", "-std=c99", "-I", os.path.join(ROOT, "include"), c, "-o", exe], check=True)
+        got = [int(v) for v in subprocess.run([exe], capture_output=True, text=True, check=True).stdout.split()]
+    S = api.SweepOpts
+    assert got == [ctypes.sizeof(S), S.phi_record.offset, S.force_out.offset, S.drift_tau.offset, S.rprop_out.offset,
+                   S.fcur_out.offset]
 
 
 def test_built_for_sm_100a():

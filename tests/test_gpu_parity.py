@@ -647,19 +647,22 @@ def test_fp32_inverse_parity(case, K):
     nth = oracle.max_threads()
     d, u = x.delta[:g["nsw"]], x.unif[:g["nsw"]]
     free = oracle.sweep(dummy, x.lattice, x.pos, g["B0"], g["ld0"], g["sg0"], d, u, phi_in=g["rec"], b32=b32, nthreads=nth)
-    P.compare_decisions(g["acc"], g["R"], free["accept"], free["ratios"], u)
     rep = oracle.sweep(dummy, x.lattice, x.pos, g["B0"], g["ld0"], g["sg0"], d, u, forced=g["acc"], phi_in=g["rec"],
                        b32=b32, nthreads=nth)
     Bg = g["det"].get_inverse().cpu().numpy()
     assert np.array_equal(Bg, Bg.astype(np.float32).astype(np.float64))
     scale = max(1.0, np.max(np.abs(rep["B"])))
+    # ratio tolerance in fp32-storage mode: 1e-5 relative plus what a few flipped fp32 roundings of the
+    # stored rows can do to the dot product, 32 ulp * max|B| * max|phi| (absolute)
+    rtol = lambda Ro: P.TOL_RATIO * np.abs(Ro) + 32 * FP32_ULP * scale * float(np.max(np.abs(g["rec"])))
+    P.compare_decisions(g["acc"], g["R"], free["accept"], free["ratios"], u, tol=rtol(free["ratios"]))
     eb = float(np.max(np.abs(Bg - rep["B"])) / scale)
-    er = float(np.max(np.abs(g["R"] - rep["ratios"]) / np.maximum(np.abs(rep["ratios"]), 1e-300)))
+    er = float(np.max(np.abs(g["R"] - rep["ratios"]) / rtol(rep["ratios"])))
     ldg, sgg, _ = (t.cpu().numpy() for t in g["det"].get_stats())
-    print(case, K, "fp32 inverse: |B - B_oracle| / max|B| =", eb, "(ulp", FP32_ULP, ") ratio rel", er,
+    print(case, K, "fp32 inverse: |B - B_oracle| / max|B| =", eb, "(ulp", FP32_ULP, ") ratio err / tol", er,
           "accept", g["acc"].mean())
     assert eb <= 16 * FP32_ULP, eb
-    assert er < P.TOL_RATIO
+    assert er < 1.0
     # (one flipped rounding perturbs the later ratios of that walker at the 1e-6 level, log|det| with them)
     assert np.max(np.abs(ldg - rep["logdet"])) < 1e-4 and np.array_equal(sgg, rep["sign"])
     assert np.array_equal(g["pos"].cpu().numpy(), rep["pos"])
@@ -696,7 +699,9 @@ def test_fp32_inverse_drift_and_recompute(case, K, nsw):
     assert 1e-9 < np.median(r_run) and r_run.max() < 1e-2
     assert r_new.max() < 1e-3 and np.median(r_new) <= np.median(r_run) * 1.5
     assert np.array_equal(sg_run, sg_new) and np.array_equal(nacc, nacc2)
-    assert np.max(np.abs(ld_run - ld_new)) < 1e-6 * max(1.0, np.max(np.abs(ld_new)))
+    # the running log|det| (sum of log|R| over ~100 accepted moves per sweep, each R carrying the fp32
+    # storage error of a row) drifts from the recomputed one at the 1e-4 level; measured 1.7e-4 after 4 sweeps
+    assert np.max(np.abs(ld_run - ld_new)) < 2e-3
     # the recomputed stored inverse is the fp32 rounding of the oracle's LU inverse of the same Slater matrix
     Bo, _, _ = P.oracle_binv(A)
     Bn = det.get_inverse().cpu().numpy()
@@ -727,8 +732,124 @@ def test_fp32_inverse_ring_flush(nel, K, nw):
     Bg = g["det"].get_inverse().cpu().numpy()
     scale = max(1.0, np.max(np.abs(rep["B"])))
     eb = float(np.max(np.abs(Bg - rep["B"])) / scale)
-    er = float(np.max(np.abs(g["R"] - rep["ratios"]) / np.abs(rep["ratios"])))
-    print(nel, K, "fp32 ring flush: |B - B_oracle| / max|B| =", eb, "ratio rel", er)
-    assert eb <= 16 * FP32_ULP and er < P.TOL_RATIO
+    # At N = 1024 on this 24^3 toy table the Slater matrices are badly conditioned and ~800 rounded
+    # updates amplify a single flipped fp32 rounding into hundreds of ulps.  The yardstick is therefore
+    # the oracle's own sensitivity to WHERE it rounds: the same walk with the inverse rounded after every
+    # accepted move (b32 = 1) instead of once per window.  The GPU must be as close to the window-mode
+    # oracle as that.
+    alt = oracle.sweep(dummy, x.lattice, x.pos, g["B0"], g["ld0"], g["sg0"], x.delta, x.unif, forced=g["acc"],
+                       phi_in=g["rec"], b32=1, nthreads=oracle.max_threads())
+    sens_b = float(np.max(np.abs(alt["B"] - rep["B"])) / scale)
+    sens_r = np.abs(alt["ratios"] - rep["ratios"])
+    tol = P.TOL_RATIO * np.abs(rep["ratios"]) + 32 * FP32_ULP * scale * float(np.max(np.abs(g["rec"]))) + 2.0 * sens_r.max()
+    er = float(np.max(np.abs(g["R"] - rep["ratios"]) / tol))
+    print(nel, K, "fp32 ring flush: |B - B_oracle| / max|B| =", eb, "(oracle window vs per-move rounding:", sens_b,
+          ") ratio err / tol", er)
+    assert eb <= max(16 * FP32_ULP, 2.0 * sens_b) and er < 1.0
     g["det"].destroy()
     g["spline"].destroy()
+
+
+# --------------------------------------------- NEXT-1: drift moves with the T'/T acceptance (eq. 11-13)
+@pytest.mark.parametrize("case,K", [("tiny", 0), ("ragged37_skew", 0), ("n130_two_tiles", 0), ("n130_two_tiles", 7),
+                                    ("small", 0), ("small", 16)])
+def test_drift_sweep_parity(case, K):
+    """qmc_sweep_ex drift_tau (R:A20) against orc_sweep_ex replaying the GPU's proposals
+    (rprop_in), fp32 orbital vectors and decisions: the proposal obeys r' = r + (tau F + chi) bitwise with
+    the GPU's own F; F_k(r) and log T'/T agree with the oracle's (fp64 gradients) within the propagated
+    gradient tolerance; ratios 1e-5, final inverse 1e-9, positions bitwise; the oracle deciding for itself
+    takes the same decisions except where R^2 T'/T is within the band of u."""
+    x = CASES[case]()
+    coefs_np = x.coefs_numpy()
+    nw, nel, nsw = x.pos.shape[0], x.cfg.norb, x.delta.shape[0]
+    tau = float(x.cfg.sigma) ** 2
+    chi = np.random.default_rng(123).normal(0.0, np.sqrt(tau), size=x.delta.shape)
+    spline = api.Spline.create(x.coefs.to(P.dev()), x.lattice)
+    pos0 = P.to_dev(x.pos)
+    A0 = P.gpu_slater(spline, pos0)
+    B0, ld0, sg0 = P.oracle_binv(A0)
+    det = api.Det.init(spline, pos0, delay_rank=K)
+    pos = pos0.clone()
+    shp = x.unif.shape
+    f64 = dict(dtype=torch.float64, device=P.dev())
+    R, logt = torch.zeros(shp, **f64), torch.zeros(shp, **f64)
+    rprop, fcur, fnew = torch.zeros(shp + (3,), **f64), torch.zeros(shp + (3,), **f64), torch.zeros(shp + (3,), **f64)
+    acc = torch.zeros(shp, dtype=torch.uint8, device=P.dev())
+    rec = torch.zeros((nsw, nel, nw, nel), dtype=torch.float32, device=P.dev())
+    api.sweep(det, pos, P.to_dev(chi), P.to_dev(x.unif), ratios_out=R, accept_out=acc, phi_record=rec, nrecord=nw,
+              force_out=fnew, drift_tau=tau, rprop_out=rprop, logt_out=logt, fcur_out=fcur)
+    torch.cuda.synchronize()
+    R, logt, rprop, fcur, fnew, acc, rec = (t.cpu().numpy() for t in (R, logt, rprop, fcur, fnew, acc, rec))
+    assert 0.05 < acc.mean() < 0.999 and np.isfinite(logt).all() and np.abs(logt).max() > 1e-3
+    # the proposal, from the GPU's own force: positions before each step are the replayed ones
+    rep = oracle.sweep(coefs_np, x.lattice, x.pos, B0, ld0, sg0, chi, x.unif, forced=acc, phi_in=rec, tau=tau,
+                       rprop_in=rprop, want_force=True, want_bnorm=True, nthreads=oracle.max_threads())
+    cur = x.pos.copy()
+    for s_ in range(nsw):
+        for k in range(nel):
+            assert np.array_equal(rprop[s_, k], cur[:, k] + (tau * fcur[s_, k] + chi[s_, k])), (s_, k)
+            a_ = acc[s_, k].astype(bool)
+            cur[a_, k] = rprop[s_, k][a_]
+    assert np.array_equal(cur, pos.cpu().numpy()) and np.array_equal(cur, rep["pos"])
+    # ratios (identical vectors), inverse, log-det
+    assert np.max(np.abs(R - rep["ratios"]) / np.abs(rep["ratios"])) < P.TOL_RATIO
+    Bg = det.get_inverse().cpu().numpy()
+    assert np.max(np.abs(Bg - rep["B"])) < P.TOL_BINV * max(1.0, np.max(np.abs(rep["B"])))
+    ldg, sgg, _ = (t.cpu().numpy() for t in det.get_stats())
+    assert np.max(np.abs(ldg - rep["logdet"])) < 1e-7 and np.array_equal(sgg, rep["sign"])
+    # forces and the transition ratio: fp32 gradients propagated through row k of B
+    _, go, _ = oracle.spline_vgl(coefs_np, x.lattice, x.pos.reshape(-1, 3)[:64])
+    gmax = float(np.max(np.abs(go)))
+    tol_f = 2.0 * rep["bnorm"] * P.TOL_GL_PROP * gmax + 1e-10                      # |dF_k(r)| per component
+    tol_fn = tol_f / np.abs(rep["ratios"]) + 1e-5 * np.abs(rep["force"]).max(axis=-1)  # |dF_k(r')|
+    ef = float(np.max(np.abs(fcur - rep["fcur"]).max(axis=-1) / tol_f))
+    rk = np.zeros_like(rprop)                                                       # r_k before each step
+    cur = x.pos.copy()
+    for s_ in range(nsw):
+        for k in range(nel):
+            rk[s_, k] = cur[:, k]
+            a_ = acc[s_, k].astype(bool)
+            cur[a_, k] = rprop[s_, k][a_]
+    a1 = np.abs(rprop - rk - tau * rep["fcur"]).sum(axis=-1)
+    b1 = np.abs(rk - rprop - tau * rep["force"]).sum(axis=-1)
+    tol_lt = a1 * tol_f + b1 * tol_fn + 1e-9
+    el = float(np.max(np.abs(logt - rep["logt"]) / tol_lt))
+    print(case, K, "drift: accept", acc.mean(), "F err/tol", ef, "logT err/tol", el, "max|logT|", np.abs(logt).max())
+    assert ef < 1.0 and el < 1.0
+    # the oracle deciding for itself
+    free = oracle.sweep(coefs_np, x.lattice, x.pos, B0, ld0, sg0, chi, x.unif, phi_in=rec, tau=tau, rprop_in=rprop,
+                        nthreads=oracle.max_threads())
+    ag, ao = acc.reshape(-1, nw), free["accept"].reshape(-1, nw)
+    Ro, lo, u = free["ratios"].reshape(-1, nw), free["logt"].reshape(-1, nw), x.unif.reshape(-1, nw)
+    tl = tol_lt.reshape(-1, nw)
+    for w in range(nw):
+        mism = np.nonzero(ag[:, w] != ao[:, w])[0]
+        if len(mism):            # up to the first mismatch both saw the same state (rprop_in is the GPU's walk)
+            m = mism[0]
+            val = Ro[m, w] ** 2 * np.exp(lo[m, w])
+            assert abs(val - u[m, w]) < P.BAND + val * (2 * P.TOL_RATIO + 2 * tl[m, w]), (w, m, val, u[m, w])
+    det.destroy()
+    spline.destroy()
+
+
+def test_drift_tau_to_zero_and_delayed_handle():
+    """A drift sweep on a delay_rank = 16 handle gives the same bits as on a rank-1 handle (pending rows
+    are applied first, every step is a rank-1 update), and leaves the handle usable for a plain delayed
+    sweep afterwards."""
+    x = CASES["n130_two_tiles"]()
+    tau = 0.02
+    chi = np.random.default_rng(3).normal(0.0, np.sqrt(tau), size=x.delta.shape)
+    spline = api.Spline.create(x.coefs.to(P.dev()), x.lattice)
+    out = {}
+    for K in (0, 16):
+        det = api.Det.init(spline, P.to_dev(x.pos), delay_rank=K)
+        pos = P.to_dev(x.pos)
+        acc = torch.zeros(x.unif.shape, dtype=torch.uint8, device=P.dev())
+        api.sweep(det, pos, P.to_dev(chi), P.to_dev(x.unif), accept_out=acc, drift_tau=tau)
+        api.sweep(det, pos, P.to_dev(x.delta), P.to_dev(x.unif))           # plain sweep afterwards
+        out[K] = (pos.clone(), acc.clone(), det.get_inverse())
+        det.destroy()
+    assert torch.equal(out[0][0], out[16][0]) and torch.equal(out[0][1], out[16][1])
+    scale = float(out[0][2].abs().max())
+    assert float((out[0][2] - out[16][2]).abs().max()) < 1e-9 * scale
+    spline.destroy()
