@@ -287,6 +287,36 @@ int qmc_det_kinetic(qmc_det_t *det, const qmc_spline_t *spline, const double *po
                     double *lap_out, double *one_out, double *ekin_out, void *stream);
 
 /* ---------------------------------------------------------------------------------------
+ * qmc_wf_* -- the product of two spin determinants, Psi_T = D_up D_dn: PAPER.md eq. 26 (L295),
+ * Psi_T = sum_i c_i D_i^up D_i^dn e^J with one determinant per spin and no Jastrow factor.  A sweep
+ * iterates "sequentially over all electrons" (L195): the nup electrons of the up determinant, then the
+ * ndn of the down determinant; moving an up electron leaves D_dn unchanged, so the ratio of the move is
+ * D_up'/D_up and only that inverse is updated.  The handle does NOT own the determinants or the splines
+ * (each spin has its own orbital set; pass the same spline twice for a closed shell), which must have
+ * the same walker count and live on the same device.
+ *
+ *   qmc_wf_sweep    pos_up dev double [nw][nup][3], pos_dn dev double [nw][ndn][3] (in/out);
+ *                   delta dev double [nsweeps][nup+ndn][nw][3], uniforms / ratios_out / accept_out /
+ *                   forced_accept [nsweeps][nup+ndn][nw] (electron index: up first); opts as in
+ *                   qmc_sweep_ex (fixed_node, force_out, drift_tau and its outputs, with the
+ *                   [nup+ndn] electron axis; iel_begin / iel_count / phi_record must be 0 / NULL).
+ *   qmc_wf_kinetic  ekin_out dev double [nw] = -1/2 sum over ALL electrons of lap_i Psi / Psi (eq. 3),
+ *                   the sum of the two determinants' qmc_det_kinetic.
+ *   qmc_wf_get_stats  logpsi dev double [nw] = log|D_up| + log|D_dn|, sign dev int [nw] = their
+ *                   product; either may be NULL.
+ */
+typedef struct qmc_wf qmc_wf_t;
+int qmc_wf_create(qmc_wf_t **out, qmc_det_t *det_up, const qmc_spline_t *spline_up, qmc_det_t *det_dn,
+                  const qmc_spline_t *spline_dn);
+int qmc_wf_destroy(qmc_wf_t *wf);
+int qmc_wf_info(const qmc_wf_t *wf, int *nwalkers, int *nup, int *ndn);
+int qmc_wf_sweep(qmc_wf_t *wf, double *pos_up, double *pos_dn, const double *delta, const double *uniforms,
+                 int nsweeps, double *ratios_out, unsigned char *accept_out,
+                 const unsigned char *forced_accept, const qmc_sweep_opts_t *opts, void *stream);
+int qmc_wf_kinetic(qmc_wf_t *wf, const double *pos_up, const double *pos_dn, double *ekin_out, void *stream);
+int qmc_wf_get_stats(qmc_wf_t *wf, double *logpsi, int *sign, void *stream);
+
+/* ---------------------------------------------------------------------------------------
  * Per-kernel timing of qmc_sweep* (bench.py's roofline): with profiling enabled every kernel
  * launch of a sweep is bracketed by CUDA events on the launching stream.
  *   qmc_det_profile(det, 1)   enable and reset;  (det, 0) disable

@@ -14,5 +14,6 @@ from .binding import (  # noqa: F401
     det_kinetic,
     init_walkers,
     sweep,
+    wf_sweep,
     max_threads,
 )

@@ -263,3 +263,34 @@ def sweep(coefs, lattice, pos, B, logdet, sign, delta, unif, A=None, iel_count=N
     _check(rc, "sweep")
     return dict(pos=pos, B=B, A=A, logdet=logdet, sign=sign, ratios=ratios, accept=accept,
                 phi=phi_out, bnorm=bnorm, force=force, rprop=rprop, fcur=fcur, logt=logt)
+
+
+def wf_sweep(spin, delta, unif, forced=None, phi_in=None, nthreads=1, **kw):
+    """Psi_T = D_up D_dn (eq. 26 with one determinant per spin, no Jastrow): a sweep iterates over
+    the up electrons, then the down electrons (L195); moving an up electron leaves D_dn unchanged, so the
+    sweep IS the up sweep followed by the down sweep.  Marshalling only: the arrays are sliced per spin and
+    `sweep` is called once per spin and sweep.
+
+    spin: two dicts (up, down) with coefs, lattice, pos, B, logdet, sign.  delta [nsweeps][nup+ndn][nw][3],
+    unif / forced [nsweeps][nup+ndn][nw]; phi_in: None or a pair of float32 [nsweeps][n_s][nw][n_s].
+    Returns (up result, down result, ratios [nsweeps][nup+ndn][nw], accept likewise)."""
+    nup, ndn = spin[0]["pos"].shape[1], spin[1]["pos"].shape[1]
+    nsweeps, n, nw, _ = delta.shape
+    assert n == nup + ndn
+    state = [dict(pos=s_["pos"], B=s_["B"], logdet=s_["logdet"], sign=s_["sign"]) for s_ in spin]
+    ratios = np.zeros((nsweeps, n, nw))
+    accept = np.zeros((nsweeps, n, nw), dtype=np.uint8)
+    out = [None, None]
+    for sw in range(nsweeps):
+        for sp, (lo, hi) in enumerate(((0, nup), (nup, n))):
+            st = state[sp]
+            r = sweep(spin[sp]["coefs"], spin[sp]["lattice"], st["pos"], st["B"], st["logdet"], st["sign"],
+                      np.ascontiguousarray(delta[sw:sw + 1, lo:hi]), np.ascontiguousarray(unif[sw:sw + 1, lo:hi]),
+                      forced=None if forced is None else np.ascontiguousarray(forced[sw:sw + 1, lo:hi]),
+                      phi_in=None if phi_in is None else np.ascontiguousarray(phi_in[sp][sw:sw + 1]),
+                      nthreads=nthreads, **kw)
+            state[sp] = dict(pos=r["pos"], B=r["B"], logdet=r["logdet"], sign=r["sign"])
+            ratios[sw, lo:hi] = r["ratios"][0]
+            accept[sw, lo:hi] = r["accept"][0]
+            out[sp] = r
+    return out[0], out[1], ratios, accept

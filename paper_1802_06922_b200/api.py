@@ -23,6 +23,7 @@ EXPORTS = [
     "qmc_det_get_stats", "qmc_det_info", "qmc_launch_count", "qmc_det_profile", "qmc_det_profile_read",
     "qmc_probe_fp64_dmma", "qmc_det_kinetic", "qmc_det_ratio_points",
     "qmc_det_init_ex", "qmc_det_storage", "qmc_det_recompute", "qmc_det_residual",
+    "qmc_wf_create", "qmc_wf_destroy", "qmc_wf_info", "qmc_wf_sweep", "qmc_wf_kinetic", "qmc_wf_get_stats",
 ]
 QMC_DET_FP32_INVERSE = 1
 PROF_KINDS = ["spo_vgl", "sm_update", "delayed_window", "delayed_accept", "delayed_flush", "ratio_rowcopy"]
@@ -80,6 +81,12 @@ def load_library(path=None):
         "qmc_det_storage": [_vp, ctypes.POINTER(i)],
         "qmc_det_recompute": [_vp, _vp, _vp, _vp],
         "qmc_det_residual": [_vp, _vp, _vp, i, _vp, _vp],
+        "qmc_wf_create": [ctypes.POINTER(_vp), _vp, _vp, _vp, _vp],
+        "qmc_wf_destroy": [_vp],
+        "qmc_wf_info": [_vp] + [ctypes.POINTER(i)] * 3,
+        "qmc_wf_sweep": [_vp, _vp, _vp, _vp, _vp, i, _vp, _vp, _vp, ctypes.POINTER(SweepOpts), _vp],
+        "qmc_wf_kinetic": [_vp, _vp, _vp, _vp, _vp],
+        "qmc_wf_get_stats": [_vp, _vp, _vp, _vp],
     }
     for name, args in sigs.items():
         fn = getattr(lib, name)
@@ -373,3 +380,57 @@ def sweep_host(det, pos, delta, unif, ratios_out=None, accept_out=None, stream=N
                             _ptr(unif, torch.float64), nsweeps, _ptr(ratios_out, torch.float64, True),
                             _ptr(accept_out, torch.uint8, True), _stream(stream))
     _check(rc, "qmc_sweep_host")
+
+
+class Wavefunction:
+    """qmc_wf_t: Psi_T = D_up D_dn (eq. 26); does not own its determinants."""
+
+    def __init__(self, det_up, det_dn):
+        h = _vp()
+        rc = load_library().qmc_wf_create(ctypes.byref(h), det_up._h, det_up.spline._h, det_dn._h, det_dn.spline._h)
+        _check(rc, "qmc_wf_create")
+        self._h, self.up, self.dn = h, det_up, det_dn
+        self.nw, self.nup, self.ndn = det_up.nw, det_up.nel, det_dn.nel
+
+    def destroy(self):
+        if self._h:
+            _check(load_library().qmc_wf_destroy(self._h), "qmc_wf_destroy")
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def sweep(self, pos_up, pos_dn, delta, unif, ratios_out=None, accept_out=None, forced_accept=None,
+              fixed_node=False, force_out=None, drift_tau=0.0, stream=None):
+        """qmc_wf_sweep: delta [nsweeps][nup+ndn][nw][3], unif / outputs [nsweeps][nup+ndn][nw]."""
+        n, nsweeps = self.nup + self.ndn, delta.shape[0]
+        if tuple(delta.shape) != (nsweeps, n, self.nw, 3) or tuple(unif.shape) != (nsweeps, n, self.nw):
+            raise QmcError("delta / unif shapes do not match the wavefunction")
+        opts = None
+        if fixed_node or force_out is not None or drift_tau:
+            opts = ctypes.byref(SweepOpts(0, 0, None, 0, 1 if fixed_node else 0,
+                                          None if force_out is None else _dev(force_out, torch.float64).value,
+                                          float(drift_tau), None, None, None))
+        rc = load_library().qmc_wf_sweep(self._h, _dev(pos_up, torch.float64), _dev(pos_dn, torch.float64),
+                                         _dev(delta, torch.float64), _dev(unif, torch.float64), nsweeps,
+                                         _dev(ratios_out, torch.float64, True), _dev(accept_out, torch.uint8, True),
+                                         _dev(forced_accept, torch.uint8, True), opts, _stream(stream))
+        _check(rc, "qmc_wf_sweep")
+
+    def kinetic(self, pos_up, pos_dn, stream=None):
+        out = torch.empty(self.nw, dtype=torch.float64, device=pos_up.device)
+        rc = load_library().qmc_wf_kinetic(self._h, _dev(pos_up, torch.float64), _dev(pos_dn, torch.float64),
+                                           _dev(out, None), _stream(stream))
+        _check(rc, "qmc_wf_kinetic")
+        return out
+
+    def get_stats(self, stream=None):
+        """(log|Psi| double [nw], sign int32 [nw])."""
+        dev = torch.device("cuda", torch.cuda.current_device())
+        lp = torch.empty(self.nw, dtype=torch.float64, device=dev)
+        sg = torch.empty(self.nw, dtype=torch.int32, device=dev)
+        _check(load_library().qmc_wf_get_stats(self._h, _dev(lp, None), _dev(sg, None), _stream(stream)), "qmc_wf_get_stats")
+        return lp, sg

@@ -853,3 +853,70 @@ def test_drift_tau_to_zero_and_delayed_handle():
     scale = float(out[0][2].abs().max())
     assert float((out[0][2] - out[16][2]).abs().max()) < 1e-9 * scale
     spline.destroy()
+
+
+# --------------------------------------------- NEXT-2: two spin determinants, Psi_T = D_up D_dn (eq. 26)
+@pytest.mark.parametrize("K", [0, 4])
+def test_wavefunction_updn_parity(K):
+    """qmc_wf_sweep / qmc_wf_kinetic / qmc_wf_get_stats with N_up = 37 (skewed cell) and N_dn = 29, each spin
+    with its own orbital set: against oracle.wf_sweep (two independent oracle sweeps, pinned to the block-
+    diagonal determinant) replaying the recorded vectors and decisions per spin, and free-running in fp64
+    within the end-to-end bound; the kinetic energy is the sum of the two determinants' terms."""
+    cfgs = [inputs.custom_config("up", (12, 10, 14), 37, SKEW, nw=5, nsweeps=2, sigma=0.25, index=301),
+            inputs.custom_config("dn", (12, 10, 14), 29, SKEW, nw=5, nsweeps=2, sigma=0.25, index=302)]
+    xs = [inputs.make_inputs(c) for c in cfgs]
+    nup, ndn, nw, nsw = 37, 29, 5, 2
+    delta = np.concatenate([xs[0].delta, xs[1].delta], axis=1)
+    unif = np.concatenate([xs[0].unif, xs[1].unif], axis=1)
+    splines = [api.Spline.create(x.coefs.to(P.dev()), x.lattice) for x in xs]
+    pos = [P.to_dev(x.pos) for x in xs]
+    dets = [api.Det.init(splines[i], pos[i], delay_rank=K) for i in range(2)]
+    wf = api.Wavefunction(dets[0], dets[1])
+    assert (wf.nw, wf.nup, wf.ndn) == (nw, nup, ndn)
+    A0 = [P.gpu_slater(splines[i], pos[i]) for i in range(2)]
+    R = torch.zeros(unif.shape, dtype=torch.float64, device=P.dev())
+    acc = torch.zeros(unif.shape, dtype=torch.uint8, device=P.dev())
+    wf.sweep(pos[0], pos[1], P.to_dev(delta), P.to_dev(unif), ratios_out=R, accept_out=acc)
+    R, acc = R.cpu().numpy(), acc.cpu().numpy()
+    assert 0.05 < acc.mean() < 0.999
+    # oracle: fp64 from its own splines, decisions imposed (end-to-end bound of R:A10), and free-running
+    spin = []
+    for i, x in enumerate(xs):
+        coefs = x.coefs_numpy()
+        B, ld, sg = oracle.init_walkers(coefs, x.lattice, x.pos)
+        spin.append(dict(coefs=coefs, lattice=x.lattice, pos=x.pos, B=B, logdet=ld, sign=sg))
+    up, dn, Ro, ao = oracle.wf_sweep(spin, delta, unif, forced=acc, want_bnorm=True, nthreads=oracle.max_threads())
+    phimax = max(float(np.max(np.abs(a))) for a in A0)
+    # (bnorm of every sweep: run the replay sweep by sweep)
+    bn_all = np.zeros_like(R)
+    st = [dict(s_) for s_ in spin]
+    for sw in range(nsw):
+        u_, d_, _, _ = oracle.wf_sweep(st, delta[sw:sw + 1], unif[sw:sw + 1], forced=acc[sw:sw + 1], want_bnorm=True)
+        bn_all[sw, :nup], bn_all[sw, nup:] = u_["bnorm"][0], d_["bnorm"][0]
+        for i, r_ in enumerate((u_, d_)):
+            st[i].update(pos=r_["pos"], B=r_["B"], logdet=r_["logdet"], sign=r_["sign"])
+    tol = P.ratio_tol(Ro, bn_all, phimax)
+    assert np.max(np.abs(R - Ro) / tol) < 1.0
+    assert np.array_equal(pos[0].cpu().numpy(), up["pos"]) and np.array_equal(pos[1].cpu().numpy(), dn["pos"])
+    lp, sg = (t.cpu().numpy() for t in wf.get_stats())
+    assert np.max(np.abs(lp - (up["logdet"] + dn["logdet"]))) < 1e-4 and np.array_equal(sg, up["sign"] * dn["sign"])
+    _, _, Rf, af = oracle.wf_sweep(spin, delta, unif, want_bnorm=False)
+    mism = (af != acc)
+    for w in range(nw):
+        m = np.nonzero(mism.reshape(-1, nw)[:, w])[0]
+        if len(m):
+            i = m[0]
+            r_, u_ = Rf.reshape(-1, nw)[i, w], unif.reshape(-1, nw)[i, w]
+            t_ = tol.reshape(-1, nw)[i, w]
+            assert abs(r_ ** 2 - u_) < P.BAND + 2 * abs(r_) * t_ + t_ ** 2
+    # each determinant against the identical-vector replay is covered by test_sweep_parity_protocol; here: the
+    # product's kinetic energy = the sum of the two determinants' (fp64 oracle with the GPU's inverses)
+    ek = wf.kinetic(pos[0], pos[1]).cpu().numpy()
+    ref = sum(oracle.det_kinetic(spin[i]["coefs"], xs[i].lattice, pos[i].cpu().numpy(),
+                                 dets[i].get_inverse().cpu().numpy())["ekin"] for i in range(2))
+    assert np.max(np.abs(ek - ref)) < 1e-5 * np.max(np.abs(ref))
+    wf.destroy()
+    for d_ in dets:
+        d_.destroy()
+    for s_ in splines:
+        s_.destroy()

@@ -758,3 +758,53 @@ def test_fp32_stored_inverse(sweep_case):
     # and b32 = K with a window that closes after every step is b32 = 1 exactly
     o_k1 = oracle.sweep(coefs, x.lattice, x.pos, B32, ld, sg, x.delta, x.unif, b32=1, forced=out["accept"])
     assert np.array_equal(o_k1["B"], out["B"])
+
+
+# ----------------------------------------------------------------------------- D_up D_dn (eq. 26)
+def test_wf_sweep_is_the_block_diagonal_determinant():
+    """Psi_T = D_up D_dn (eq. 26 with one determinant per spin): oracle.wf_sweep (two
+    independent sweeps) against numpy determinants of the BLOCK-DIAGONAL Slater matrix of all N_up + N_dn
+    electrons: every ratio is det(M') / det(M) with the moved electron's row replaced, log|Psi| telescopes
+    over the accepted moves, and an up move leaves the down block (and its inverse) untouched."""
+    from scipy.linalg import block_diag
+    cfgs = [inputs.custom_config("up", (10, 9, 11), 7, SKEW * 1.5, nw=2, nsweeps=2, sigma=0.3, index=201),
+            inputs.custom_config("dn", (10, 9, 11), 5, SKEW * 1.5, nw=2, nsweeps=2, sigma=0.3, index=202)]
+    xs = [inputs.make_inputs(c) for c in cfgs]
+    spin = []
+    for x in xs:
+        coefs = x.coefs_numpy()
+        B, ld, sg = oracle.init_walkers(coefs, x.lattice, x.pos)
+        spin.append(dict(coefs=coefs, lattice=x.lattice, pos=x.pos, B=B, logdet=ld, sign=sg))
+    nup, ndn, nw, nsw = 7, 5, 2, 2
+    delta = np.concatenate([xs[0].delta, xs[1].delta], axis=1)
+    unif = np.concatenate([xs[0].unif, xs[1].unif], axis=1)
+    up, dn, ratios, accept = oracle.wf_sweep(spin, delta, unif)
+    assert 0 < accept.sum() < accept.size
+
+    def full_matrix(w, pu, pd):
+        return block_diag(oracle.slater_matrix(spin[0]["coefs"], xs[0].lattice, pu[None])[0],
+                          oracle.slater_matrix(spin[1]["coefs"], xs[1].lattice, pd[None])[0])
+
+    for w in range(nw):
+        pu, pd = xs[0].pos[w].copy(), xs[1].pos[w].copy()
+        s0, l0 = np.linalg.slogdet(full_matrix(w, pu, pd))
+        tele = 0.0
+        for s_ in range(nsw):
+            for k in range(nup + ndn):
+                tu, td = pu.copy(), pd.copy()
+                if k < nup:
+                    tu[k] = pu[k] + delta[s_, k, w]
+                else:
+                    td[k - nup] = pd[k - nup] + delta[s_, k, w]
+                sa, la = np.linalg.slogdet(full_matrix(w, pu, pd))
+                sb, lb = np.linalg.slogdet(full_matrix(w, tu, td))
+                brute = sa * sb * np.exp(lb - la)
+                assert abs(ratios[s_, k, w] - brute) < 1e-8 * max(1.0, abs(brute)), (s_, k, w)
+                assert accept[s_, k, w] == (ratios[s_, k, w] ** 2 > unif[s_, k, w])
+                if accept[s_, k, w]:
+                    pu, pd = tu, td
+                    tele += np.log(abs(ratios[s_, k, w]))
+        s1, l1 = np.linalg.slogdet(full_matrix(w, pu, pd))
+        assert np.array_equal(pu, up["pos"][w]) and np.array_equal(pd, dn["pos"][w])
+        assert abs((up["logdet"][w] + dn["logdet"][w]) - l1) < 1e-8 and up["sign"][w] * dn["sign"][w] == int(s1)
+        assert abs(tele - (l1 - l0)) < 1e-8
