@@ -40,8 +40,8 @@ UNIT = "moves/s"
 # rank-16 window is the faster one on this kernel)
 DEFAULT_DELAY = {"tiny": [0], "small": [16, 0], "mid": [16, 0], "large": [16, 0], "xlarge": [16, 32, 0]}
 # further arms reported as variants (fewer timed steps each): (delay rank, fp32-stored inverse)
-EXTRA_ARMS = {"large": [(16, True), (0, True), (24, False), (32, False)], "mid": [(16, True)],
-              "xlarge": [(16, True), (24, False)]}
+EXTRA_ARMS = {"large": [(16, True), (0, True), (24, False), (32, False), (0, False, "drift"), (16, False, "updn")],
+              "mid": [(16, True), (16, False, "updn")], "xlarge": [(16, True), (24, False)]}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures
 # (profiles/r01_*.md), config `large`
 # keyed by (kernel, delay rank); value = (bytes per launch, the file the figure comes from)
@@ -181,6 +181,50 @@ def run_reference(args, rank, world):
     print(json.dumps(line), flush=True)
 
 
+def flush_micro(args, api, spline, cfg, pos_np, nw, nel, dev, peak, fp64_peak):
+    """Kernel-level timing of the delayed flush on real window data: per repetition, K standalone steps
+    (qmc_spo_vgl -> qmc_det_ratio -> qmc_det_accept_update with ~81 % of the walkers accepting each step),
+    then qmc_det_flush bracketed by the library's per-kernel CUDA events (kind `delayed_flush`)."""
+    ranks = [args.delay] if args.delay >= 2 else [16, 24, 32]
+    g = torch.Generator(device=dev).manual_seed(1234)
+    for K in ranks:
+        for fp32 in ([True] if args.fp32_inverse else [False, True]):
+            pos = torch.from_numpy(pos_np).to(dev)
+            det = api.Det.init(spline, pos, delay_rank=K, fp32_inverse=fp32)
+            times, paccs = [], []
+            for rep in range(args.warmup + args.steps):
+                k0 = (rep * K) % max(1, nel - K)
+                pacc = torch.zeros(nw, device=dev)
+                for l in range(K):
+                    k = k0 + l
+                    newpos = pos[:, k] + cfg.sigma * torch.randn((nw, 3), dtype=torch.float64, device=dev, generator=g)
+                    phi = api.spo_vgl(spline, newpos, want_gl=False)
+                    R = det.ratio(k, phi)
+                    acc = ((torch.rand(nw, device=dev, generator=g) < 0.81) & torch.isfinite(R) & (R.abs() > 0.05)).to(torch.uint8)
+                    det.accept_update(k, phi, R, acc)
+                    pos[:, k] = torch.where(acc.bool()[:, None], newpos, pos[:, k])
+                    pacc += acc
+                det.profile(True)
+                det.flush()
+                torch.cuda.synchronize()
+                prof = det.profile_read()
+                det.profile(False)
+                if rep >= args.warmup:
+                    times.append(prof["delayed_flush"][0])
+                    paccs.append(float(pacc.mean().item()))
+            ms = float(np.median(times))
+            pbar = float(np.mean(paccs))
+            eb = det.storage_bytes
+            byt = nw * 2 * eb * nel * det.ld + nw * pbar * (8 * det.ld + 4 * spline.row_pitch)
+            fl = 4.0 * pbar * nw * nel * nel
+            print(json.dumps({"flush_micro": True, "workload": args.config, "N": nel, "walkers": nw, "rank": K,
+                              "storage": "f32" if fp32 else "f64", "accepted_per_window": pbar, "flush_ms": ms,
+                              "GB/s": byt / ms / 1e6, "frac_of_hbm_peak": byt / ms / 1e6 / peak,
+                              "fp64_TFLOP/s": fl / ms / 1e9, "frac_of_fp64_dmma_peak": fl / ms / 1e9 / fp64_peak,
+                              "ring": os.environ.get("QMC_FLUSH_RING", "1")}), flush=True)
+            det.destroy()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -194,6 +238,10 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--fp32-inverse", action="store_true", help="store the inverse in fp32 (QMC_DET_FP32_INVERSE)")
     ap.add_argument("--no-variants", action="store_true", help="skip the extra variant arms of the default run")
+    ap.add_argument("--flush-micro", action="store_true",
+                    help="time qmc_det_flush alone: windows filled through qmc_det_ratio / qmc_det_accept_update "
+                         "(81 %% of --delay steps accepted), one JSON line per (rank, storage) with the flush kernel's "
+                         "CUDA-event time; a kernel-level A/B tool (QMC_FLUSH_RING=0 selects flush.cu), not the metric")
     ap.add_argument("--walkers", type=int, default=0, help="override walkers per GPU (debug)")
     args = ap.parse_args()
 
@@ -258,7 +306,7 @@ def main():
     def max_over_ranks(ms):
         return sharding.max_over_ranks(ms, device=dev)
 
-    def run_arm(delay, fp32=False, steps=None):
+    def run_arm(delay, fp32=False, mode=None, steps=None):
         """W warm-up sweeps + K timed sweeps with the inverse update `delay` (0 = rank-1), device
         resident; then the same K sweeps end to end from pinned host buffers.  fp32: the inverse is
         stored in single precision (QMC_DET_FP32_INVERSE)."""
@@ -272,8 +320,25 @@ def main():
         torch.cuda.synchronize()
         t_init = time.perf_counter() - t0
 
+        drift_tau = float(cfg.sigma) ** 2 if mode == "drift" else 0.0     # chi = the config's Gaussian displacements
+        wf = det2 = pos2 = None
+        if mode == "updn":        # closed shell: a second determinant of the same orbitals at other positions
+            g = torch.Generator(device=dev).manual_seed(inputs.BASE_SEED + 77 + rank)
+            lat_t = torch.tensor(x.lattice, dtype=torch.float64, device=dev)
+            pos2 = torch.rand((nw, nel, 3), dtype=torch.float64, device=dev, generator=g) @ lat_t
+            det2 = api.Det.init(spline, pos2, delay_rank=delay, fp32_inverse=fp32)
+            wf = api.Wavefunction(det, det2)
+            delta2 = torch.cat([delta, cfg.sigma * torch.randn(delta.shape, dtype=torch.float64, device=dev, generator=g)], dim=1)
+            unif2 = torch.cat([unif, torch.rand(unif.shape, dtype=torch.float64, device=dev, generator=g)], dim=1)
+            accept = torch.zeros(unif2.shape, dtype=torch.uint8, device=dev)
+            ratios = torch.zeros(unif2.shape, dtype=torch.float64, device=dev)
+
         def step(i):
-            api.sweep(det, pos, delta[i:i + 1], unif[i:i + 1], ratios_out=ratios[i:i + 1], accept_out=accept[i:i + 1])
+            if wf is not None:
+                wf.sweep(pos, pos2, delta2[i:i + 1], unif2[i:i + 1], ratios_out=ratios[i:i + 1], accept_out=accept[i:i + 1])
+            else:
+                api.sweep(det, pos, delta[i:i + 1], unif[i:i + 1], ratios_out=ratios[i:i + 1], accept_out=accept[i:i + 1],
+                          drift_tau=drift_tau)
 
         # ---- device-resident timing: inputs in HBM, CUDA events on the launching stream, no
         #      per-kernel instrumentation inside the timed region
@@ -292,14 +357,17 @@ def main():
         clocks = sampler.stop()
         launches = api.launch_count() - launches0
         ms = max_over_ranks(e0.elapsed_time(e1))
-        moves = nsteps * nel * nw * world
+        nmoved = (2 if wf is not None else 1) * nel          # electrons moved per walker and sweep
+        moves = nsteps * nmoved * nw * world
         value = moves / (ms * 1e-3)
-        acc_rate = float(accept[args.warmup:].to(torch.float64).mean().item())
+        acc_rate = float(accept[args.warmup:nsteps_total].to(torch.float64).mean().item())
 
         # ---- per-kernel split: a SECOND pass of `nprof` sweeps with every launch bracketed by CUDA
         #      events (qmc_det_profile); the walk goes on with the random numbers of the first timed sweeps
         nprof = min(nsteps, 5)
         det.profile(True)
+        if det2 is not None:
+            det2.profile(True)
         e0.record()
         for i in range(args.warmup, args.warmup + nprof):
             step(i)
@@ -307,14 +375,18 @@ def main():
         barrier()
         prof = det.profile_read()
         det.profile(False)
+        if det2 is not None:
+            p2 = det2.profile_read()
+            det2.profile(False)
+            prof = {k: (prof[k][0] + p2[k][0], prof[k][1] + p2[k][1]) for k in prof}
         ms_prof = e0.elapsed_time(e1)
         n_acc = float(accept[args.warmup:args.warmup + nprof].to(torch.float64).sum().item())
 
         # ---- roofline of the dominant kernel (rank-local, from the per-launch CUDA events)
         ld, npitch, K, eb = det.ld, spline.row_pitch, det.delay_rank, det.storage_bytes
         per_launch = {   # algorithmic bytes per launch; eb = bytes per stored element of B
-            "spo_vgl": (nprof * nel * nw / max(prof["spo_vgl"][1], 1)) * (64 + 5) * npitch * 4,
-            "ratio_rowcopy": nw * ((eb + 8) * ld + 4 * nel),
+            "spo_vgl": (nprof * nmoved * nw * (2 if drift_tau else 1) / max(prof["spo_vgl"][1], 1)) * (64 + 5) * npitch * 4,
+            "ratio_rowcopy": nw * ((eb + 8) * ld + 4 * nel) * (0.75 if drift_tau else 1.0),   # drift: averaged with the propose kernel
             "sm_update": (n_acc / max(prof["sm_update"][1], 1)) * (2 * eb * nel * ld + 12 * nel),
             "delayed_flush": nw * 2 * eb * nel * ld + (n_acc / max(prof["delayed_flush"][1], 1)) * (8 * ld + 4 * npitch),
             # window: K rows of B0 and K vectors in, R' rows out
@@ -358,34 +430,47 @@ def main():
 
         # ---- end to end through the C ABI with HOST buffers (pinned): H2D of pos/delta/unif and D2H
         #      of pos/ratios/decisions inside the timed region, every step
-        pos_h = pos.cpu().pin_memory()
-        ratios_h = torch.zeros(unif_h.shape, dtype=torch.float64).pin_memory()
-        accept_h = torch.zeros(unif_h.shape, dtype=torch.uint8).pin_memory()
+        e2e = None
+        if mode is None:
+            pos_h = pos.cpu().pin_memory()
+            ratios_h = torch.zeros(unif_h.shape, dtype=torch.float64).pin_memory()
+            accept_h = torch.zeros(unif_h.shape, dtype=torch.uint8).pin_memory()
 
-        def step_host(i):
-            api.sweep_host(det, pos_h, delta_h[i:i + 1], unif_h[i:i + 1], ratios_out=ratios_h[i:i + 1],
-                           accept_out=accept_h[i:i + 1])
+            def step_host(i):
+                api.sweep_host(det, pos_h, delta_h[i:i + 1], unif_h[i:i + 1], ratios_out=ratios_h[i:i + 1],
+                               accept_out=accept_h[i:i + 1])
 
-        step_host(0)
-        barrier()
-        e0.record()
-        for i in range(args.warmup, nsteps_total):
-            step_host(i)
-        e1.record()
-        barrier()
-        ms_e2e = max_over_ranks(e0.elapsed_time(e1))
-        h2d = pos_h.numel() * 8 + delta_h[0].numel() * 8 + unif_h[0].numel() * 8
-        d2h = pos_h.numel() * 8 + ratios_h[0].numel() * 8 + accept_h[0].numel()
-        e2e = {"value": moves / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d * world,
-               "d2h_bytes_per_step": d2h * world}
+            step_host(0)
+            barrier()
+            e0.record()
+            for i in range(args.warmup, nsteps_total):
+                step_host(i)
+            e1.record()
+            barrier()
+            ms_e2e = max_over_ranks(e0.elapsed_time(e1))
+            h2d = pos_h.numel() * 8 + delta_h[0].numel() * 8 + unif_h[0].numel() * 8
+            d2h = pos_h.numel() * 8 + ratios_h[0].numel() * 8 + accept_h[0].numel()
+            e2e = {"value": moves / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d * world,
+                   "d2h_bytes_per_step": d2h * world}
         update = "sherman-morrison rank-1" if K == 0 else f"delayed rank-{K} (same result as rank-1)"
         if fp32:
             update += ", fp32-stored inverse (fp64 arithmetic; R:A19)"
+        if mode == "drift":
+            update += f", drift moves tau = {drift_tau:.4g} (eq. 11-13)"
+        if mode == "updn":
+            update += f", D_up D_dn: 2 x {nel} electrons per walker (eq. 26)"
+            wf.destroy()
+            det2.destroy()
         det.destroy()
         return {"value": value, "ms_per_step": ms / nsteps, "steps": nsteps, "update": update, "accept_rate": acc_rate,
                 "kernel_split": f"second pass of {nprof} sweeps with per-launch CUDA events ({ms_prof / nprof:.2f} ms per sweep)",
                 "init_s": t_init, "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
-                "kernels": kernels, "spline_evals_per_s": value * nel}
+                "kernels": kernels, "spline_evals_per_s": value * nel * (2 if drift_tau else 1)}
+
+    if args.flush_micro:
+        flush_micro(args, api, spline, cfg, pos_np, nw, nel, dev, peak, fp64_peak)
+        spline.destroy()
+        return
 
     ws_table, ws_binv = cfg.table_bytes() / 1e9, nw * nel * nel * 8 / 1e9
     l2_note = (f"working set ({ws_table:.2f} GB table + {ws_binv:.2f} GB inverses) "
@@ -394,7 +479,7 @@ def main():
     delays = [args.delay] if args.delay >= 0 else DEFAULT_DELAY.get(args.config, [0])
     arms = [run_arm(dl, fp32=args.fp32_inverse) for dl in dict.fromkeys(delays)]
     if args.delay < 0 and not args.fp32_inverse and not args.no_variants:
-        arms += [run_arm(dl, fp32=f32, steps=5) for dl, f32 in EXTRA_ARMS.get(args.config, [])]
+        arms += [run_arm(a[0], fp32=a[1], mode=a[2] if len(a) > 2 else None, steps=5) for a in EXTRA_ARMS.get(args.config, [])]
     main_arm = arms[0]
     line = {
         "metric": METRIC, "value": main_arm["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
