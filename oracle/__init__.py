@@ -16,4 +16,10 @@ from .binding import (  # noqa: F401
     sweep,
     wf_sweep,
     max_threads,
+    Jastrow,
+    b3,
+    jastrow_u,
+    min_image,
+    jastrow_value,
+    jastrow_dj,
 )

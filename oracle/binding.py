@@ -11,6 +11,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "qmc_oracle.c")
+_SRC_J = os.path.join(_HERE, "qmc_jastrow_oracle.c")
 _LIB = os.path.join(_HERE, "libqmc_oracle.so")
 _lib = None
 
@@ -23,15 +24,46 @@ _bp = ctypes.POINTER(ctypes.c_ubyte)
 class SweepOpts(ctypes.Structure):
     """orc_sweep_opts of qmc_oracle.c."""
     _fields_ = [("tau", ctypes.c_double), ("rprop_in", _dp), ("rprop_out", _dp), ("fcur_out", _dp),
-                ("logt_out", _dp), ("b32", ctypes.c_int)]
+                ("logt_out", _dp), ("b32", ctypes.c_int), ("jas", ctypes.c_void_p), ("other", _dp),
+                ("nother", ctypes.c_int), ("jratio_out", _dp)]
+
+
+class JastrowC(ctypes.Structure):
+    """orc_jastrow of qmc_jastrow_oracle.c."""
+    _fields_ = [("nfunc", ctypes.c_int), ("rc", _dp), ("M", _ip), ("poff", _ip), ("p", _dp),
+                ("f_same", ctypes.c_int), ("f_opp", ctypes.c_int), ("lattice", _dp), ("nion", ctypes.c_int),
+                ("ion", _dp), ("ion_func", _ip), ("range", ctypes.c_int)]
+
+
+class Jastrow:
+    """One- and two-body B-spline Jastrow factor (eq. 30-33) for the oracle: function table
+    funcs = [(rc, p[0..M]), ...]; f_same / f_opp index the electron-electron functions (-1: none);
+    ions [nion][3] with ion_func [nion]; lattice 3x3 or None (open boundary conditions)."""
+
+    def __init__(self, funcs, f_same=-1, f_opp=-1, lattice=None, ions=None, ion_func=None, image_range=1):
+        self.rc = np.ascontiguousarray([f[0] for f in funcs], dtype=np.float64)
+        self.M = np.ascontiguousarray([len(f[1]) - 1 for f in funcs], dtype=np.int32)
+        self.poff = np.ascontiguousarray(np.concatenate([[0], np.cumsum(self.M + 1)[:-1]]), dtype=np.int32)
+        self.p = np.ascontiguousarray(np.concatenate([np.asarray(f[1], dtype=np.float64) for f in funcs]))
+        self.lattice = None if lattice is None else _c64(lattice).reshape(9).copy()
+        self.ions = np.zeros((0, 3)) if ions is None else _c64(ions).reshape(-1, 3).copy()
+        self.ion_func = (np.zeros(0, dtype=np.int32) if ion_func is None
+                         else np.ascontiguousarray(ion_func, dtype=np.int32))
+        assert len(self.ion_func) == len(self.ions)
+        self.c = JastrowC(len(funcs), _d(self.rc), self.M.ctypes.data_as(_ip), self.poff.ctypes.data_as(_ip),
+                          _d(self.p), int(f_same), int(f_opp), _d(self.lattice), len(self.ions), _d(self.ions),
+                          self.ion_func.ctypes.data_as(_ip), int(image_range))
+
+    def ref(self):
+        return ctypes.cast(ctypes.pointer(self.c), ctypes.c_void_p)
 
 
 def build(force=False):
     """Compile qmc_oracle.c with gcc -O2 (no fast-math, no intrinsics) into oracle/."""
     if (not force and os.path.exists(_LIB)
-            and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC)):
+            and os.path.getmtime(_LIB) >= max(os.path.getmtime(_SRC), os.path.getmtime(_SRC_J))):
         return _LIB
-    cmd = ["gcc", "-O2", "-std=c99", "-fopenmp", "-shared", "-fPIC", "-o", _LIB, _SRC, "-lm"]
+    cmd = ["gcc", "-O2", "-std=c99", "-fopenmp", "-shared", "-fPIC", "-o", _LIB, _SRC, _SRC_J, "-lm"]
     subprocess.run(cmd, check=True)
     return _LIB
 
@@ -67,6 +99,16 @@ def _load():
         lib.orc_det_kinetic.argtypes = ([ctypes.c_int] * 4 + [_dp, _fp, ctypes.c_int, ctypes.c_int] + [_dp] * 6)
         lib.orc_max_threads.restype = ctypes.c_int
         lib.orc_max_threads.argtypes = []
+        lib.orc_b3.restype = ctypes.c_double
+        lib.orc_b3.argtypes = [ctypes.c_double]
+        lib.orc_jastrow_u.restype = ctypes.c_double
+        lib.orc_jastrow_u.argtypes = [ctypes.c_double, ctypes.c_double, ctypes.c_int, _dp]
+        lib.orc_min_image.restype = ctypes.c_double
+        lib.orc_min_image.argtypes = [_dp, _dp, _dp, ctypes.c_int]
+        lib.orc_jastrow_value.restype = ctypes.c_double
+        lib.orc_jastrow_value.argtypes = [ctypes.c_void_p, ctypes.c_int, _dp, ctypes.c_int, _dp]
+        lib.orc_jastrow_dj.restype = ctypes.c_double
+        lib.orc_jastrow_dj.argtypes = [ctypes.c_void_p, ctypes.c_int, _dp, ctypes.c_int, _dp, ctypes.c_int, _dp]
         _lib = lib
     return _lib
 
@@ -208,7 +250,7 @@ def init_walkers(coefs, lattice, pos, nthreads=1, want_A=False):
 
 def sweep(coefs, lattice, pos, B, logdet, sign, delta, unif, A=None, iel_count=None,
           forced=None, phi_in=None, want_phi=False, mode=0, nthreads=1, want_bnorm=False,
-          fixed_node=False, want_force=False, tau=0.0, rprop_in=None, b32=0):
+          fixed_node=False, want_force=False, tau=0.0, rprop_in=None, b32=0, jastrow=None, other=None):
     """Run nsweeps particle-by-particle sweeps.  Inputs are copied; returns a dict with
     pos, B, A, logdet, sign, ratios [nsweeps][nel][nw], accept (uint8, same shape), phi, force
     (F = 2 grad log|Psi| of the moved electron at the proposed configuration, [nsweeps][nel][nw][3]).
@@ -254,7 +296,16 @@ def sweep(coefs, lattice, pos, B, logdet, sign, delta, unif, A=None, iel_count=N
         rprop_in = _c64(rprop_in, (nsweeps, nel, nw, 3))
     if b32:
         assert np.array_equal(B, B.astype(np.float32).astype(np.float64)), "b32: B must hold fp32 values"
-    opts = SweepOpts(float(tau), _d(rprop_in), _d(rprop), _d(fcur), _d(logt), int(b32))
+    jratio = None
+    nother = 0
+    if jastrow is not None:
+        jratio = np.ones((nsweeps, nel, nw))
+        if other is not None:
+            other = _c64(other)
+            assert other.shape[0] == nw and other.shape[2] == 3
+            nother = other.shape[1]
+    opts = SweepOpts(float(tau), _d(rprop_in), _d(rprop), _d(fcur), _d(logt), int(b32),
+                     None if jastrow is None else jastrow.ref(), _d(other) if nother else None, nother, _d(jratio))
     rc = lib.orc_sweep_ex(nx, ny, nz, norb, _d(lat), coefs.ctypes.data_as(_fp), nw, nel,
                           _d(pos), _d(B), _d(A), _d(logdet), sign.ctypes.data_as(_ip),
                           _d(delta), _d(unif), nsweeps, int(iel_count), _d(ratios),
@@ -262,7 +313,38 @@ def sweep(coefs, lattice, pos, B, logdet, sign, delta, unif, A=None, iel_count=N
                           int(nthreads), _d(bnorm), int(bool(fixed_node)), _d(force), ctypes.byref(opts))
     _check(rc, "sweep")
     return dict(pos=pos, B=B, A=A, logdet=logdet, sign=sign, ratios=ratios, accept=accept,
-                phi=phi_out, bnorm=bnorm, force=force, rprop=rprop, fcur=fcur, logt=logt)
+                phi=phi_out, bnorm=bnorm, force=force, rprop=rprop, fcur=fcur, logt=logt, jratio=jratio)
+
+
+def b3(x):
+    """Cardinal cubic B-spline of eq. 33 (support [-3, 1), centred at -1)."""
+    return float(_load().orc_b3(float(x)))
+
+
+def jastrow_u(r, rc, p):
+    """u(r) of eq. 33 with control points p[0..M] and cutoff rc."""
+    p = _c64(p)
+    return float(_load().orc_jastrow_u(float(r), float(rc), len(p) - 1, _d(p)))
+
+
+def min_image(lattice, a, b, image_range=1):
+    lat = None if lattice is None else _c64(lattice).reshape(9)
+    return float(_load().orc_min_image(_d(lat), _d(_c64(a, (3,))), _d(_c64(b, (3,))), int(image_range)))
+
+
+def jastrow_value(jas, pos, other=None):
+    """J (eq. 30, one- and two-body terms) of ONE walker: pos [nel][3], other [nother][3] (other spin)."""
+    pos = _c64(pos).reshape(-1, 3)
+    other = np.zeros((0, 3)) if other is None else _c64(other).reshape(-1, 3)
+    return float(_load().orc_jastrow_value(jas.ref(), len(pos), _d(pos), len(other), _d(other) if len(other) else None))
+
+
+def jastrow_dj(jas, pos, k, rnew, other=None):
+    """J(electron k at rnew) - J(electron k at pos[k]) of ONE walker; the move's ratio is exp(-dJ)."""
+    pos = _c64(pos).reshape(-1, 3)
+    other = np.zeros((0, 3)) if other is None else _c64(other).reshape(-1, 3)
+    return float(_load().orc_jastrow_dj(jas.ref(), len(pos), _d(pos), len(other), _d(other) if len(other) else None,
+                                        int(k), _d(_c64(rnew, (3,)))))
 
 
 def wf_sweep(spin, delta, unif, forced=None, phi_in=None, nthreads=1, **kw):
@@ -273,6 +355,8 @@ def wf_sweep(spin, delta, unif, forced=None, phi_in=None, nthreads=1, **kw):
 
     spin: two dicts (up, down) with coefs, lattice, pos, B, logdet, sign.  delta [nsweeps][nup+ndn][nw][3],
     unif / forced [nsweeps][nup+ndn][nw]; phi_in: None or a pair of float32 [nsweeps][n_s][nw][n_s].
+    With jastrow=...: the electrons of the other spin, at their current positions, are the fixed `other`
+    particles of each per-spin sweep (opposite-spin function).
     Returns (up result, down result, ratios [nsweeps][nup+ndn][nw], accept likewise)."""
     nup, ndn = spin[0]["pos"].shape[1], spin[1]["pos"].shape[1]
     nsweeps, n, nw, _ = delta.shape
@@ -288,7 +372,7 @@ def wf_sweep(spin, delta, unif, forced=None, phi_in=None, nthreads=1, **kw):
                       np.ascontiguousarray(delta[sw:sw + 1, lo:hi]), np.ascontiguousarray(unif[sw:sw + 1, lo:hi]),
                       forced=None if forced is None else np.ascontiguousarray(forced[sw:sw + 1, lo:hi]),
                       phi_in=None if phi_in is None else np.ascontiguousarray(phi_in[sp][sw:sw + 1]),
-                      nthreads=nthreads, **kw)
+                      nthreads=nthreads, other=state[1 - sp]["pos"] if kw.get("jastrow") is not None else None, **kw)
             state[sp] = dict(pos=r["pos"], B=r["B"], logdet=r["logdet"], sign=r["sign"])
             ratios[sw, lo:hi] = r["ratios"][0]
             accept[sw, lo:hi] = r["accept"][0]

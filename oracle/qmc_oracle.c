@@ -389,7 +389,20 @@ typedef struct orc_sweep_opts {
     const double *rprop_in;
     double *rprop_out, *fcur_out, *logt_out;
     int b32;
+    /* Jastrow factor (eq. 26, eq. 28-33; qmc_jastrow_oracle.c): Psi_T = e^{-J} D, so the move of
+     * electron k has |Psi'/Psi|^2 = R^2 exp(-2 dJ), dJ = orc_jastrow_dj at the walker's CURRENT positions;
+     * the move is accepted iff R^2 exp(-2 dJ) > u (eq. 12, symmetric T).  `other` holds the electrons of the
+     * other spin, [nw][nother][3], fixed during this sweep.  Not combined with drift moves (the drift
+     * would need grad J, which is not built): tau > 0 with a Jastrow factor is an error. */
+    const struct orc_jastrow *jas;
+    const double *other;
+    int nother;
+    double *jratio_out;    /* NULL, or [nsweeps][nel][nw]: exp(-dJ) of every move */
 } orc_sweep_opts;
+
+struct orc_jastrow;
+double orc_jastrow_dj(const struct orc_jastrow *J, int nel, const double *pos, int nother, const double *other,
+                      int k, const double rnew[3]);
 
 static void round_to_fp32(double *x, size_t n)
 {
@@ -413,6 +426,8 @@ int orc_sweep_ex(int nx, int ny, int nz, int norb, const double lattice[9], cons
     double *fcur_out = opts ? opts->fcur_out : NULL;
     double *logt_out = opts ? opts->logt_out : NULL;
     if (b32 < 0 || (opts && opts->tau < 0.0)) return -1;
+    const struct orc_jastrow *jas = opts ? opts->jas : NULL;
+    if (jas && drift) return -1;
     int rc_all = 0;
     size_t nn = (size_t)nel * nel;
 #ifdef _OPENMP
@@ -478,8 +493,16 @@ int orc_sweep_ex(int nx, int ny, int nz, int norb, const double lattice[9], cons
                     logt = (fwd - bwd) / (2.0 * tau);
                     if (logt_out) logt_out[mv] = logt;
                 }
+                double jfac2 = 1.0;    /* exp(-2 dJ): the Jastrow part of |Psi'/Psi|^2 */
+                if (jas) {
+                    double dj = orc_jastrow_dj(jas, nel, pos + (size_t)w * nel * 3, opts->nother,
+                                               opts->other ? opts->other + (size_t)w * opts->nother * 3 : NULL, k, rnew);
+                    jfac2 = exp(-2.0 * dj);
+                    if (opts->jratio_out) opts->jratio_out[mv] = exp(-dj);
+                }
                 int acc;
                 if (forced) acc = forced[mv] != 0 && isfinite(R) && R != 0.0; /* R:A18 */
+                else if (jas) acc = isfinite(R) && isfinite(jfac2) && (R * R * jfac2 > unif[mv]) && !(fixed_node && R < 0.0);
                 else if (drift) acc = isfinite(R) && isfinite(logt) && (R * R * exp(logt) > unif[mv]) && !(fixed_node && R < 0.0);
                 else acc = isfinite(R) && (R * R > unif[mv]) && !(fixed_node && R < 0.0);
                 if (ratios_out) ratios_out[mv] = R;

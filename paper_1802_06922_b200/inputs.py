@@ -160,3 +160,42 @@ def make_inputs(cfg, device="cpu", nw=None, nsweeps=None, with_table=True):
     unif = rng.uniform(0.0, 1.0, size=(nsweeps, nel, nw))
     return QmcInputs(cfg, lat, coefs, np.ascontiguousarray(pos), np.ascontiguousarray(delta),
                      np.ascontiguousarray(unif), pw)
+
+
+@dataclass
+class JastrowInputs:
+    funcs: list                  # [(r_c, control points p[0..M]), ...]: e-e same spin, e-e opposite spin, species 0, 1
+    f_same: int
+    f_opp: int
+    ions: np.ndarray             # float64 [nion][3]
+    ion_func: np.ndarray         # int32 [nion]: function of each ion's species
+    other: np.ndarray            # float64 [nw][nother][3]: electrons of the other spin (fixed during a sweep)
+
+
+def make_jastrow(cfg, lattice, nother=0, nion=None, nw=None, seed_offset=5000):
+    """Seeded parameters of a one- and two-body B-spline Jastrow factor (eq. 30-33) shaped like the
+    paper's solid-state workloads: cutoffs below the Wigner-Seitz radius of the cell (L375), 8-10 control
+    points per function, two ionic species, nion = max(2, N / 6) ions uniform in the cell (NiO-128 has
+    1536 valence electrons on 128 atoms; per spin determinant that is 6 electrons per atom).  Control
+    points: a smooth decaying profile amp (1 - m / M)^2 with 20 % seeded noise and p_M = 0 (u continuous
+    at the cutoff).  Draws only: none of the method's arithmetic lives here."""
+    if isinstance(cfg, str):
+        cfg = CONFIGS[cfg]
+    rng = np.random.Generator(np.random.Philox(BASE_SEED + seed_offset + cfg.index))
+    lat = np.asarray(lattice, dtype=np.float64).reshape(3, 3)
+    # inscribed-sphere radius of the Wigner-Seitz cell is at least half the smallest cell height
+    vol = abs(np.linalg.det(lat))
+    heights = [vol / np.linalg.norm(np.cross(lat[(d + 1) % 3], lat[(d + 2) % 3])) for d in range(3)]
+    rws = 0.5 * min(heights)
+    funcs = []
+    for amp, frac, M in ((0.25, 0.95, 10), (0.5, 0.95, 10), (-0.6, 0.8, 8), (-0.9, 0.7, 8)):
+        m = np.arange(M + 1, dtype=np.float64)
+        p = amp * (1.0 - m / M) ** 2 * (1.0 + 0.2 * rng.uniform(-1.0, 1.0, M + 1))
+        p[M] = 0.0
+        funcs.append((float(frac * rws), p))
+    nw = cfg.nw if nw is None else int(nw)
+    nion = max(2, cfg.norb // 6) if nion is None else int(nion)
+    ions = rng.uniform(0.0, 1.0, size=(nion, 3)) @ lat
+    ion_func = (2 + (np.arange(nion) % 2)).astype(np.int32)
+    other = rng.uniform(0.0, 1.0, size=(nw, nother, 3)) @ lat
+    return JastrowInputs(funcs, 0, 1, np.ascontiguousarray(ions), ion_func, np.ascontiguousarray(other))
