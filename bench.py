@@ -40,8 +40,11 @@ UNIT = "moves/s"
 # rank-16 window is the faster one on this kernel)
 DEFAULT_DELAY = {"tiny": [0], "small": [16, 0], "mid": [16, 0], "large": [16, 0], "xlarge": [16, 32, 0]}
 # further arms reported as variants (fewer timed steps each): (delay rank, fp32-stored inverse)
-EXTRA_ARMS = {"large": [(16, True), (0, True), (24, False), (32, False), (0, False, "drift"), (16, False, "updn")],
-              "mid": [(16, True), (16, False, "updn")], "xlarge": [(16, True), (24, False)]}
+EXTRA_ARMS = {"large": [(16, True), (0, True), (24, False), (32, False), (0, False, "drift"), (16, False, "updn"),
+                        (16, False, "jastrow")],
+              "mid": [(16, True), (16, False, "updn")], "xlarge": [(16, True), (24, False)],
+              # L2-resident configs: the sweep is launch-bound; the same sweep replayed from a CUDA graph
+              "tiny": [(0, False, "graph")], "small": [(16, False, "graph"), (0, False, "graph")]}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures
 # (profiles/r01_*.md), config `large`
 # keyed by (kernel, delay rank); value = (bytes per launch, the file the figure comes from)
@@ -243,6 +246,9 @@ def main():
                          "(81 %% of --delay steps accepted), one JSON line per (rank, storage) with the flush kernel's "
                          "CUDA-event time; a kernel-level A/B tool (QMC_FLUSH_RING=0 selects flush.cu), not the metric")
     ap.add_argument("--walkers", type=int, default=0, help="override walkers per GPU (debug)")
+    ap.add_argument("--probe-fp64", action="store_true",
+                    help="print the fp64-pipe microbenchmark table (qmc_probe_fp64_pipe: DMMA / DFMA / mixed by warps "
+                         "per SM and accumulator chains) and exit; not the metric")
     args = ap.parse_args()
 
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
@@ -267,6 +273,15 @@ def main():
     api.load_library()                       # no fallback: raises if the CUDA library is missing
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (use --impl reference for the CPU oracle)"
     torch.cuda.set_device(local_rank)
+    if args.probe_fp64:
+        if rank == 0:
+            for mode, name in ((0, "dmma"), (1, "dfma"), (2, "dmma+2dfma")):
+                for warps in (4, 8, 16, 32):
+                    for chains in (1, 2, 4, 8):
+                        a_, b_ = api.probe_fp64_pipe(mode, warps, chains)
+                        print(json.dumps({"probe": "fp64_pipe", "mix": name, "warps_per_sm": warps, "chains_per_warp": chains,
+                                          "dmma_TFLOP/s": round(a_, 2), "dfma_TFLOP/s": round(b_, 2)}), flush=True)
+        return
     dev = torch.device("cuda", local_rank)
     if world > 1:
         import torch.distributed as dist
@@ -321,7 +336,10 @@ def main():
         t_init = time.perf_counter() - t0
 
         drift_tau = float(cfg.sigma) ** 2 if mode == "drift" else 0.0     # chi = the config's Gaussian displacements
-        wf = det2 = pos2 = None
+        wf = det2 = pos2 = jas = graph = None
+        if mode == "jastrow":     # one- and two-body B-spline Jastrow factor (eq. 28-33), seeded parameters
+            jx = inputs.make_jastrow(cfg, x.lattice, nother=0, nw=1)
+            jas = api.Jastrow(jx.funcs, f_same=jx.f_same, f_opp=jx.f_opp, lattice=x.lattice, ions=jx.ions, ion_func=jx.ion_func)
         if mode == "updn":        # closed shell: a second determinant of the same orbitals at other positions
             g = torch.Generator(device=dev).manual_seed(inputs.BASE_SEED + 77 + rank)
             lat_t = torch.tensor(x.lattice, dtype=torch.float64, device=dev)
@@ -333,17 +351,31 @@ def main():
             accept = torch.zeros(unif2.shape, dtype=torch.uint8, device=dev)
             ratios = torch.zeros(unif2.shape, dtype=torch.float64, device=dev)
 
+        d_buf = u_buf = r_buf = a_buf = None
+
         def step(i):
             if wf is not None:
                 wf.sweep(pos, pos2, delta2[i:i + 1], unif2[i:i + 1], ratios_out=ratios[i:i + 1], accept_out=accept[i:i + 1])
+            elif graph is not None:     # fresh random numbers into the graph's static buffers, replay, keep the outputs
+                d_buf.copy_(delta[i:i + 1]); u_buf.copy_(unif[i:i + 1])
+                graph.replay()
+                ratios[i:i + 1].copy_(r_buf); accept[i:i + 1].copy_(a_buf)
             else:
                 api.sweep(det, pos, delta[i:i + 1], unif[i:i + 1], ratios_out=ratios[i:i + 1], accept_out=accept[i:i + 1],
-                          drift_tau=drift_tau)
+                          drift_tau=drift_tau, jastrow=jas)
 
         # ---- device-resident timing: inputs in HBM, CUDA events on the launching stream, no
         #      per-kernel instrumentation inside the timed region
         for i in range(args.warmup):
             step(i)
+        if mode == "graph":       # capture one sweep (after the eager warm-up sweeps), then replay it
+            d_buf, u_buf = delta[0:1].clone(), unif[0:1].clone()
+            r_buf, a_buf = torch.zeros_like(u_buf), torch.zeros(u_buf.shape, dtype=torch.uint8, device=dev)
+            torch.cuda.synchronize()
+            c0 = api.launch_count()
+            graph = api.SweepGraph(det, pos, d_buf, u_buf, ratios_out=r_buf, accept_out=a_buf)
+            graph_launches = api.launch_count() - c0      # kernels of one sweep, recorded in the graph
+            step(0)
         barrier()
         launches0 = api.launch_count()
         sampler = ClockSampler(local_rank)
@@ -356,6 +388,8 @@ def main():
         barrier()
         clocks = sampler.stop()
         launches = api.launch_count() - launches0
+        if mode == "graph":
+            launches = graph_launches * nsteps             # replayed by the graph: counted at capture
         ms = max_over_ranks(e0.elapsed_time(e1))
         nmoved = (2 if wf is not None else 1) * nel          # electrons moved per walker and sweep
         moves = nsteps * nmoved * nw * world
@@ -365,6 +399,8 @@ def main():
         # ---- per-kernel split: a SECOND pass of `nprof` sweeps with every launch bracketed by CUDA
         #      events (qmc_det_profile); the walk goes on with the random numbers of the first timed sweeps
         nprof = min(nsteps, 5)
+        if graph is not None:     # the per-kernel split needs eager launches (events are recorded by the library)
+            graph = None
         det.profile(True)
         if det2 is not None:
             det2.profile(True)
@@ -457,6 +493,11 @@ def main():
             update += ", fp32-stored inverse (fp64 arithmetic; R:A19)"
         if mode == "drift":
             update += f", drift moves tau = {drift_tau:.4g} (eq. 11-13)"
+        if mode == "jastrow":
+            update += ", one- and two-body B-spline Jastrow factor (eq. 28-33)"
+            jas.destroy()
+        if mode == "graph":
+            update += ", sweep replayed from a CUDA graph (api.SweepGraph)"
         if mode == "updn":
             update += f", D_up D_dn: 2 x {nel} electrons per walker (eq. 26)"
             wf.destroy()

@@ -37,6 +37,7 @@ extern "C" {
 
 typedef struct qmc_spline qmc_spline_t; /* opaque: padded fp32 coefficient table on device */
 typedef struct qmc_det qmc_det_t;       /* opaque: per-walker fp64 inverse + scratch       */
+typedef struct qmc_jastrow qmc_jastrow_t; /* opaque: Jastrow function table + ions on device */
 
 /* Thread-local text of the last error raised on this thread ("" if none). */
 const char *qmc_last_error(void);
@@ -238,6 +239,18 @@ typedef struct qmc_sweep_opts {
     double *rprop_out;   /* NULL, or dev double [nsweeps][nel][nw][3]: the proposed positions (drift)   */
     double *logt_out;    /* NULL, or dev double [nsweeps][nel][nw]: log T(r'->r)/T(r->r') (drift)       */
     double *fcur_out;    /* NULL, or dev double [nsweeps][nel][nw][3]: F_k(r) at the current config.    */
+    const struct qmc_jastrow *jastrow;   /* NULL, or a Jastrow factor (qmc_jastrow_create): Psi_T = e^{-J} D      */
+                         /*   (eq. 26, eq. 28-33), so |Psi'/Psi|^2 = R^2 exp(-2 dJ) and the move is     */
+                         /*   accepted iff R^2 exp(-2 dJ) > u (eq. 12, symmetric T), dJ taken at the walker's    */
+                         /*   CURRENT configuration.  ratios_out stays the determinant ratio R.  Rank-1 mode: one */
+                         /*   more small launch per step; delayed mode: one launch per window (dJ of its K        */
+                         /*   proposals against the window-start configuration) and an O(p) correction per step   */
+                         /*   inside the window kernel for the electrons the window has already moved.  Not with  */
+                         /*   drift_tau > 0 (the drift would need grad J): QMC_EINVAL.                            */
+    const double *jastrow_other;   /* NULL, or dev double [nw][jastrow_nother][3]: the electrons of the other    */
+    int jastrow_nother;            /*   spin (fixed during this sweep; opposite-spin function).  qmc_wf_sweep    */
+                                   /*   fills both in from the other determinant's positions.                    */
+    double *jratio_out;  /* NULL, or dev double [nsweeps][nel][nw]: exp(-dJ) of every move                        */
 } qmc_sweep_opts_t;
 
 int qmc_sweep_ex(qmc_det_t *det, const qmc_spline_t *spline, double *pos, const double *delta,
@@ -298,8 +311,10 @@ int qmc_det_kinetic(qmc_det_t *det, const qmc_spline_t *spline, const double *po
  *   qmc_wf_sweep    pos_up dev double [nw][nup][3], pos_dn dev double [nw][ndn][3] (in/out);
  *                   delta dev double [nsweeps][nup+ndn][nw][3], uniforms / ratios_out / accept_out /
  *                   forced_accept [nsweeps][nup+ndn][nw] (electron index: up first); opts as in
- *                   qmc_sweep_ex (fixed_node, force_out, drift_tau and its outputs, with the
- *                   [nup+ndn] electron axis; iel_begin / iel_count / phi_record must be 0 / NULL).
+ *                   qmc_sweep_ex (fixed_node, force_out, drift_tau and its outputs, jastrow and
+ *                   jratio_out, with the [nup+ndn] electron axis; iel_begin / iel_count / phi_record
+ *                   must be 0 / NULL; jastrow_other / jastrow_nother are filled in by the call: the
+ *                   other determinant's electrons at their current positions).
  *   qmc_wf_kinetic  ekin_out dev double [nw] = -1/2 sum over ALL electrons of lap_i Psi / Psi (eq. 3),
  *                   the sum of the two determinants' qmc_det_kinetic.
  *   qmc_wf_get_stats  logpsi dev double [nw] = log|D_up| + log|D_dn|, sign dev int [nw] = their
@@ -315,6 +330,39 @@ int qmc_wf_sweep(qmc_wf_t *wf, double *pos_up, double *pos_dn, const double *del
                  const unsigned char *forced_accept, const qmc_sweep_opts_t *opts, void *stream);
 int qmc_wf_kinetic(qmc_wf_t *wf, const double *pos_up, const double *pos_dn, double *ekin_out, void *stream);
 int qmc_wf_get_stats(qmc_wf_t *wf, double *logpsi, int *sign, void *stream);
+
+/* ---------------------------------------------------------------------------------------
+ * qmc_jastrow_* -- one- and two-body Jastrow factor with cubic B-spline functors, sec 7:
+ * Psi = e^{-J} Phi (eq. 28, eq. 29), J = sum_i u_1(r_i) + 1/2 sum_{i != j} u_2(r_i, r_j) (eq. 30 up to the
+ * two-body term), u_1(r_i) = sum_I u_{species(I)}(|r_i - R_I|) (eq. 31), u_2 = u_{ss'}(|r_i - r_j|) (eq. 32,
+ * first term; one function for equal spins and one for opposite spins, L365), each functor
+ *     u(r) = sum_{m=0}^{M} p_m B_3(r / (r_c / M) - m),   B_3 the cardinal cubic B-spline on [-3, 1)   (eq. 33)
+ * and u = 0 for r >= r_c (reading R:A21).  Periodic cells use the nearest image of every pair ("the cutoffs
+ * must be smaller than the simulation cell Wigner-Seitz radius", L375); lattice == NULL is open boundaries.
+ * The three-body term (eq. 32 second term, eq. 35) is not built.
+ *
+ *   qmc_jastrow_create  all arguments HOST: lattice 9 doubles (rows = cell vectors) or NULL; nfunc <= 8
+ *                       functors with cutoffs rc[f], M[f] >= 1 intervals and control points
+ *                       p[sum_{g<f}(M[g]+1) .. + M[f]] (at most 256 - 4 nfunc in all); f_same / f_opp: the
+ *                       electron-electron functors (-1 = none); nion ions at ion_pos [nion][3] with functor
+ *                       ion_func [nion] (-1 = none).  Copies everything to the current device.
+ *   qmc_jastrow_ratio   the move of electron iel of every walker to rnew (dev double [nwalkers][3]):
+ *                       dj_out[w] = J(R') - J(R) = the terms of eq. 30 that contain the electron, at rnew minus at
+ *                       pos[w][iel]; ratio_out[w] = exp(-dJ) = the Jastrow part of Psi'/Psi.  pos dev double
+ *                       [nwalkers][nel][3] (one spin); other dev double [nwalkers][nother][3] (the other spin)
+ *                       or NULL with nother = 0.  Either output may be NULL.  One launch, fp64, fixed order.
+ *   qmc_jastrow_value   j_out[w] = J of walker w (dev double [nwalkers]); O(N^2), for checks.
+ * In a sweep: qmc_sweep_opts_t.jastrow (above).
+ */
+int qmc_jastrow_create(qmc_jastrow_t **out, const double *lattice, int nfunc, const double *rc, const int *M,
+                       const double *p, int f_same, int f_opp, int nion, const double *ion_pos,
+                       const int *ion_func);
+int qmc_jastrow_destroy(qmc_jastrow_t *jastrow);
+int qmc_jastrow_ratio(const qmc_jastrow_t *jastrow, int nwalkers, int nel, const double *pos, int nother,
+                      const double *other, int iel, const double *rnew, double *ratio_out, double *dj_out,
+                      void *stream);
+int qmc_jastrow_value(const qmc_jastrow_t *jastrow, int nwalkers, int nel, const double *pos, int nother,
+                      const double *other, double *j_out, void *stream);
 
 /* ---------------------------------------------------------------------------------------
  * Per-kernel timing of qmc_sweep* (bench.py's roofline): with profiling enabled every kernel
@@ -344,6 +392,12 @@ int qmc_det_profile_read(qmc_det_t *det, double *ms_host, long long *launches_ho
  * the delayed flush (the "genuine dense fp64 contraction" of north_star) against it,
  * since MEASURED_PEAKS.json holds no fp64 figure.  Synchronises the stream. */
 int qmc_probe_fp64_dmma(double *tflops_host, void *stream);
+/* The fp64 pipe of an SM sub-partition under different mixes (what the flush kernels are laid out around;
+ * profiles/r02_fp64_pipe.md): mode 0 = DMMA.8x8x4 only, 1 = DFMA only, 2 = one DMMA + two DFMA per slot;
+ * warps_per_sm in 1..32 (one CTA per SM), chains in {1, 2, 4, 8} independent accumulators per warp.  Returns
+ * the DMMA and the DFMA throughput in TFLOP/s (host pointers; 0 for the absent instruction).  Synchronises. */
+int qmc_probe_fp64_pipe(int mode, int warps_per_sm, int chains, double *tflops_dmma_host,
+                        double *tflops_dfma_host, void *stream);
 
 /* Number of kernel launches this library has enqueued since load (bench.py's gpu_launches). */
 long long qmc_launch_count(void);

@@ -7,6 +7,7 @@ Names follow the C ABI: Spline.create -> qmc_spline_create, spo_vgl -> qmc_spo_v
 import ctypes
 import os
 
+import numpy as np
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -24,6 +25,7 @@ EXPORTS = [
     "qmc_probe_fp64_dmma", "qmc_det_kinetic", "qmc_det_ratio_points",
     "qmc_det_init_ex", "qmc_det_storage", "qmc_det_recompute", "qmc_det_residual",
     "qmc_wf_create", "qmc_wf_destroy", "qmc_wf_info", "qmc_wf_sweep", "qmc_wf_kinetic", "qmc_wf_get_stats",
+    "qmc_jastrow_create", "qmc_jastrow_destroy", "qmc_jastrow_ratio", "qmc_jastrow_value", "qmc_probe_fp64_pipe",
 ]
 QMC_DET_FP32_INVERSE = 1
 PROF_KINDS = ["spo_vgl", "sm_update", "delayed_window", "delayed_accept", "delayed_flush", "ratio_rowcopy"]
@@ -33,7 +35,8 @@ class SweepOpts(ctypes.Structure):
     _fields_ = [("iel_begin", ctypes.c_int), ("iel_count", ctypes.c_int),
                 ("phi_record", _vp), ("nrecord", ctypes.c_int), ("fixed_node", ctypes.c_int),
                 ("force_out", _vp), ("drift_tau", ctypes.c_double), ("rprop_out", _vp), ("logt_out", _vp),
-                ("fcur_out", _vp)]
+                ("fcur_out", _vp), ("jastrow", _vp), ("jastrow_other", _vp), ("jastrow_nother", ctypes.c_int),
+                ("jratio_out", _vp)]
 
 
 class QmcError(RuntimeError):
@@ -75,6 +78,7 @@ def load_library(path=None):
         "qmc_det_profile": [_vp, i],
         "qmc_det_profile_read": [_vp, ctypes.POINTER(d), ctypes.POINTER(ctypes.c_longlong)],
         "qmc_probe_fp64_dmma": [ctypes.POINTER(d), _vp],
+        "qmc_probe_fp64_pipe": [i, i, i, ctypes.POINTER(d), ctypes.POINTER(d), _vp],
         "qmc_det_kinetic": [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp],
         "qmc_det_ratio_points": [_vp, i, i, _vp, i, _vp, _vp],
         "qmc_det_init_ex": [ctypes.POINTER(_vp), _vp, i, i, _vp, i, ctypes.c_uint, _vp],
@@ -87,6 +91,11 @@ def load_library(path=None):
         "qmc_wf_sweep": [_vp, _vp, _vp, _vp, _vp, i, _vp, _vp, _vp, ctypes.POINTER(SweepOpts), _vp],
         "qmc_wf_kinetic": [_vp, _vp, _vp, _vp, _vp],
         "qmc_wf_get_stats": [_vp, _vp, _vp, _vp],
+        "qmc_jastrow_create": [ctypes.POINTER(_vp), ctypes.POINTER(d), i, ctypes.POINTER(d), ctypes.POINTER(i),
+                               ctypes.POINTER(d), i, i, i, ctypes.POINTER(d), ctypes.POINTER(i)],
+        "qmc_jastrow_destroy": [_vp],
+        "qmc_jastrow_ratio": [_vp, i, i, _vp, i, _vp, i, _vp, _vp, _vp, _vp],
+        "qmc_jastrow_value": [_vp, i, i, _vp, i, _vp, _vp, _vp],
     }
     for name, args in sigs.items():
         fn = getattr(lib, name)
@@ -134,6 +143,14 @@ def probe_fp64_dmma(stream=None):
     out = ctypes.c_double(0.0)
     _check(load_library().qmc_probe_fp64_dmma(ctypes.byref(out), _stream(stream)), "qmc_probe_fp64_dmma")
     return out.value
+
+
+def probe_fp64_pipe(mode, warps_per_sm, chains, stream=None):
+    """qmc_probe_fp64_pipe: (DMMA TFLOP/s, DFMA TFLOP/s) of the fp64 pipe under the given instruction mix."""
+    a, b = ctypes.c_double(0.0), ctypes.c_double(0.0)
+    _check(load_library().qmc_probe_fp64_pipe(int(mode), int(warps_per_sm), int(chains), ctypes.byref(a), ctypes.byref(b),
+                                              _stream(stream)), "qmc_probe_fp64_pipe")
+    return a.value, b.value
 
 
 class Spline:
@@ -328,8 +345,12 @@ class Det:
 
 def sweep(det, pos, delta, unif, ratios_out=None, accept_out=None, forced_accept=None, iel_begin=0,
           iel_count=0, phi_record=None, nrecord=0, fixed_node=False, force_out=None, drift_tau=0.0,
-          rprop_out=None, logt_out=None, fcur_out=None, stream=None):
+          rprop_out=None, logt_out=None, fcur_out=None, jastrow=None, jastrow_other=None, jratio_out=None,
+          stream=None):
     """qmc_sweep / qmc_sweep_ex on device tensors (pos updated in place).
+
+    jastrow: a Jastrow handle (accept iff R^2 exp(-2 dJ) > u); jastrow_other double [nw][nother][3] or None:
+    the electrons of the other spin; jratio_out double [nsweeps][nel][nw] or None: exp(-dJ) of every move.
 
     pos double [nw][nel][3]; delta double [nsweeps][nel][nw][3]; unif double [nsweeps][nel][nw];
     ratios_out double / accept_out uint8 / forced_accept uint8: [nsweeps][nel][nw] or None;
@@ -350,7 +371,8 @@ def sweep(det, pos, delta, unif, ratios_out=None, accept_out=None, forced_accept
     args = [det._h, det.spline._h, _dev(pos, torch.float64), _dev(delta, torch.float64),
             _dev(unif, torch.float64), nsweeps, _dev(ratios_out, torch.float64, True),
             _dev(accept_out, torch.uint8, True), _dev(forced_accept, torch.uint8, True)]
-    if iel_begin or iel_count or phi_record is not None or fixed_node or force_out is not None or drift_tau:
+    if (iel_begin or iel_count or phi_record is not None or fixed_node or force_out is not None or drift_tau
+            or jastrow is not None):
         if phi_record is not None and tuple(phi_record.shape) != (nsweeps, det.nel, nrecord, det.nel):
             raise QmcError("phi_record must be [nsweeps][nel][nrecord][nel]")
         if force_out is not None and tuple(force_out.shape) != tuple(unif.shape) + (3,):
@@ -362,11 +384,36 @@ def sweep(det, pos, delta, unif, ratios_out=None, accept_out=None, forced_accept
                          float(drift_tau),
                          None if rprop_out is None else _dev(rprop_out, torch.float64).value,
                          None if logt_out is None else _dev(logt_out, torch.float64).value,
-                         None if fcur_out is None else _dev(fcur_out, torch.float64).value)
+                         None if fcur_out is None else _dev(fcur_out, torch.float64).value,
+                         None if jastrow is None else jastrow._h,
+                         None if jastrow_other is None else _dev(jastrow_other, torch.float64).value,
+                         0 if jastrow_other is None else int(jastrow_other.shape[1]),
+                         None if jratio_out is None else _dev(jratio_out, torch.float64).value)
         rc = lib.qmc_sweep_ex(*args, ctypes.byref(opts), _stream(stream))
         _check(rc, "qmc_sweep_ex")
     else:
         _check(lib.qmc_sweep(*args, _stream(stream)), "qmc_sweep")
+
+
+class SweepGraph:
+    """One qmc_sweep call captured into a CUDA graph and replayed (the sequential loop over
+    electrons is 2-3 small launches per electron step; on the L2-resident configs -- tiny, small -- the sweep is
+    launch-bound, and a graph replays its launches without the per-launch host cost).
+
+    The tensors passed in are the graph's static buffers: refresh `delta` / `unif` in place (copy_) between
+    replays; `pos`, the handle's inverse and the outputs are updated by every replay exactly as by
+    `sweep(...)`.  Run one eager `sweep` first: the library allocates its scratch and streams on first use,
+    which a capture must not do.  Plumbing only: torch.cuda.CUDAGraph captures the launches the library
+    enqueues on torch's current stream."""
+
+    def __init__(self, det, pos, delta, unif, **kw):
+        self.graph = torch.cuda.CUDAGraph()
+        self._keep = (det, pos, delta, unif, kw)
+        with torch.cuda.graph(self.graph):
+            sweep(det, pos, delta, unif, **kw)
+
+    def replay(self):
+        self.graph.replay()
 
 
 def sweep_host(det, pos, delta, unif, ratios_out=None, accept_out=None, stream=None):
@@ -380,6 +427,63 @@ def sweep_host(det, pos, delta, unif, ratios_out=None, accept_out=None, stream=N
                             _ptr(unif, torch.float64), nsweeps, _ptr(ratios_out, torch.float64, True),
                             _ptr(accept_out, torch.uint8, True), _stream(stream))
     _check(rc, "qmc_sweep_host")
+
+
+class Jastrow:
+    """qmc_jastrow_t: one- and two-body B-spline Jastrow factor (PAPER.md eq. 28-33).  funcs = [(r_c, p[0..M]), ...];
+    f_same / f_opp: the electron-electron functors (-1 = none); lattice 3x3 or None (open boundaries);
+    ions [nion][3] with functor index ion_func [nion].  Host inputs (numpy), copied to the current device."""
+
+    def __init__(self, funcs, f_same=-1, f_opp=-1, lattice=None, ions=None, ion_func=None):
+        lib = load_library()
+        d, i = ctypes.c_double, ctypes.c_int
+        rc_a = np.ascontiguousarray([f[0] for f in funcs], dtype=np.float64)
+        m_a = np.ascontiguousarray([len(f[1]) - 1 for f in funcs], dtype=np.int32)
+        p_a = np.ascontiguousarray(np.concatenate([np.asarray(f[1], dtype=np.float64) for f in funcs]))
+        lat = None if lattice is None else np.ascontiguousarray(lattice, dtype=np.float64).reshape(9)
+        ions = np.zeros((0, 3)) if ions is None else np.ascontiguousarray(ions, dtype=np.float64).reshape(-1, 3)
+        ifn = np.zeros(0, dtype=np.int32) if ion_func is None else np.ascontiguousarray(ion_func, dtype=np.int32)
+        if len(ifn) != len(ions):
+            raise QmcError("ion_func must have one entry per ion")
+        dp = lambda a: None if a is None or a.size == 0 else a.ctypes.data_as(ctypes.POINTER(d))
+        ip = lambda a: None if a.size == 0 else a.ctypes.data_as(ctypes.POINTER(i))
+        h = _vp()
+        rc = lib.qmc_jastrow_create(ctypes.byref(h), dp(lat), len(funcs), dp(rc_a), ip(m_a), dp(p_a), int(f_same),
+                                    int(f_opp), len(ions), dp(ions), ip(ifn))
+        _check(rc, "qmc_jastrow_create")
+        self._h = h
+
+    def destroy(self):
+        if self._h:
+            _check(load_library().qmc_jastrow_destroy(self._h), "qmc_jastrow_destroy")
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def ratio(self, pos, iel, rnew, other=None, stream=None):
+        """qmc_jastrow_ratio: (exp(-dJ), dJ) double [nw] for the move of electron iel of every walker to rnew [nw][3]."""
+        nw, nel, _ = pos.shape
+        ratio = torch.empty(nw, dtype=torch.float64, device=pos.device)
+        dj = torch.empty(nw, dtype=torch.float64, device=pos.device)
+        rc = load_library().qmc_jastrow_ratio(self._h, nw, nel, _dev(pos, torch.float64),
+                                              0 if other is None else int(other.shape[1]), _dev(other, torch.float64, True),
+                                              int(iel), _dev(rnew, torch.float64), _dev(ratio, None), _dev(dj, None), _stream(stream))
+        _check(rc, "qmc_jastrow_ratio")
+        return ratio, dj
+
+    def value(self, pos, other=None, stream=None):
+        """qmc_jastrow_value: J double [nw]."""
+        nw, nel, _ = pos.shape
+        out = torch.empty(nw, dtype=torch.float64, device=pos.device)
+        rc = load_library().qmc_jastrow_value(self._h, nw, nel, _dev(pos, torch.float64),
+                                              0 if other is None else int(other.shape[1]), _dev(other, torch.float64, True),
+                                              _dev(out, None), _stream(stream))
+        _check(rc, "qmc_jastrow_value")
+        return out
 
 
 class Wavefunction:
@@ -404,16 +508,18 @@ class Wavefunction:
             pass
 
     def sweep(self, pos_up, pos_dn, delta, unif, ratios_out=None, accept_out=None, forced_accept=None,
-              fixed_node=False, force_out=None, drift_tau=0.0, stream=None):
+              fixed_node=False, force_out=None, drift_tau=0.0, jastrow=None, jratio_out=None, stream=None):
         """qmc_wf_sweep: delta [nsweeps][nup+ndn][nw][3], unif / outputs [nsweeps][nup+ndn][nw]."""
         n, nsweeps = self.nup + self.ndn, delta.shape[0]
         if tuple(delta.shape) != (nsweeps, n, self.nw, 3) or tuple(unif.shape) != (nsweeps, n, self.nw):
             raise QmcError("delta / unif shapes do not match the wavefunction")
         opts = None
-        if fixed_node or force_out is not None or drift_tau:
+        if fixed_node or force_out is not None or drift_tau or jastrow is not None:
             opts = ctypes.byref(SweepOpts(0, 0, None, 0, 1 if fixed_node else 0,
                                           None if force_out is None else _dev(force_out, torch.float64).value,
-                                          float(drift_tau), None, None, None))
+                                          float(drift_tau), None, None, None,
+                                          None if jastrow is None else jastrow._h, None, 0,
+                                          None if jratio_out is None else _dev(jratio_out, torch.float64).value))
         rc = load_library().qmc_wf_sweep(self._h, _dev(pos_up, torch.float64), _dev(pos_dn, torch.float64),
                                          _dev(delta, torch.float64), _dev(unif, torch.float64), nsweeps,
                                          _dev(ratios_out, torch.float64, True), _dev(accept_out, torch.uint8, True),

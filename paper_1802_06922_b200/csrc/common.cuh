@@ -96,6 +96,7 @@ struct qmc_det {
     // drift moves (qmc_sweep_ex drift_tau > 0): allocated on first use
     float *vgl_cur;             // [kSpoBatch][nw][5][np] SPO-VGL at the CURRENT positions of a batch of electrons
     double *rprop, *fcur, *tfac;   // [nw][3], [nw][3], [nw]: proposal, F_k(r), T(r'->r)/T(r->r') of the current step
+    double *jas_dj;             // [max(delay, 1)][nw] Jastrow dJ of the steps of a window / exp(-2 dJ) of a step (on first use)
     double *rowk;               // [nw][ld]      copy of row iel of B taken before the update
     double *ratio;              // [nw]      ratio of the current step (ratio_rowcopy_kernel -> sm_update_kernel)
     unsigned char *acc;         // [nw]

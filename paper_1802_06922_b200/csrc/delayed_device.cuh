@@ -23,8 +23,17 @@ int delayed_max_rank(int ld);                                // largest K whose 
 // SPO-VGL is in d->vgl; ratios, decisions, moves and the flush.  Pointers are offset to the first step.
 // fixed_node: reject R < 0; force_out: NULL or [nb][nw][3], F = 2 grad log Psi_T at the proposed configuration;
 // record_mid: record d->ev_main on `s` between the window kernel and the flush (sweep.cu's second stream).
+// jas: Jastrow factor of the window (table NULL = none): base[j][w] = dJ of step j against the configuration at
+// the start of the window (jastrow_move_kernel); the window kernel adds the change due to the electrons the
+// window has moved before step j and accepts iff R^2 exp(-2 dJ) > u.
+struct JasTable;
+struct WindowJastrow {
+    const JasTable *table;
+    const double *base;           // [nb][nw]
+    double *jratio_out;           // [nb][nw] or NULL: exp(-dJ)
+};
 int delayed_sweep_window(qmc_det *d, double *pos, const double *delta, const double *unif, int iel0, int nb,
                          double *ratios_out, unsigned char *accept_out, const unsigned char *forced,
-                         int fixed_node, double *force_out, int record_mid, cudaStream_t s);
+                         int fixed_node, double *force_out, int record_mid, const WindowJastrow &jas, cudaStream_t s);
 
 }  // namespace qmc

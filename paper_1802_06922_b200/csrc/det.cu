@@ -272,7 +272,7 @@ static void det_free(qmc_det *d)
     }
     if (d->vgl_buf[1]) cudaFree(d->vgl_buf[1]);
     d->vgl = d->vgl_buf[0] ? d->vgl_buf[0] : d->vgl;
-    cudaFree(d->vgl_cur); cudaFree(d->rprop); cudaFree(d->fcur); cudaFree(d->tfac);
+    cudaFree(d->vgl_cur); cudaFree(d->rprop); cudaFree(d->fcur); cudaFree(d->tfac); cudaFree(d->jas_dj);
     cudaFree(d->B); cudaFree(d->Bf); cudaFree(d->logdet); cudaFree(d->sign); cudaFree(d->naccept);
     cudaFree(d->vgl); cudaFree(d->rowk); cudaFree(d->ratio); cudaFree(d->acc);
     cudaFree(d->win_count); cudaFree(d->win_iel); cudaFree(d->win_slot); cudaFree(d->win_phi); cudaFree(d->win_rows);

@@ -6,12 +6,24 @@
 // (delayed mode, per window of K steps: K1, then delayed_window_kernel = S3 + S4 of the K steps,
 //  then flush_dmma_kernel = S5')
 #include "delayed_device.cuh"
+#include "jastrow_device.cuh"
 #include "spo_device.cuh"
 #include "update_device.cuh"
 
 namespace qmc {
 
 void spo_launch_shape(int np, int *threads, int *tiles);
+int jastrow_move_launch(const qmc_jastrow *J, int nw, int nel, const double *pos, int nother, const double *other,
+                        int iel0, int nb, const double *delta, const double *rnew, double *dj_out, double *ratio_out,
+                        double *tfac_out, cudaStream_t s);
+
+// Jastrow factor of a sweep (qmc_sweep_opts_t.jastrow): what the step loops need.
+struct SweepJastrow {
+    const qmc_jastrow *J;     // NULL: none
+    const double *other;
+    int nother;
+    double *jratio_out;       // [nsweeps][nel][nw] or NULL
+};
 
 // SPO-VGL of a BATCH of electron steps in one launch.  The proposal of electron k does not depend
 // on the outcome of the moves before it (r' = pos[w][k] + delta, and pos[w][k] only changes at step
@@ -196,7 +208,7 @@ int spo_batch_vgl(qmc_det *d, const qmc_spline *sp, const double *pos, const dou
 static int sweep_delayed(qmc_det *d, const qmc_spline *sp, double *pos, const double *delta, const double *unif,
                          int nsweeps, int k0, int kn, double *ratios_out, unsigned char *accept_out,
                          const unsigned char *forced, int fixed_node, double *force, float *rec, int nrec,
-                         cudaStream_t s)
+                         const SweepJastrow &jas, cudaStream_t s)
 {
     const int nw = d->nw, nel = d->nel, batch = d->spo_batch;
     const int wins_per_sweep = (kn + batch - 1) / batch;
@@ -230,9 +242,17 @@ static int sweep_delayed(qmc_det *d, const qmc_spline *sp, double *pos, const do
         if (overlap) QMC_CUDA(cudaStreamWaitEvent(s, d->ev_spo[i & 1], 0));
         else if ((rc = spo(i, s))) return rc;
         d->vgl = d->vgl_buf[overlap ? (i & 1) : 0];
+        WindowJastrow wj{};
+        if (jas.J) {
+            // dJ of the window's nb proposals against the configuration at the start of the window; the window
+            // kernel corrects it for the electrons the window itself has moved by then
+            if ((rc = jastrow_move_launch(jas.J, nw, nel, pos, jas.nother, jas.other, k, nb, delta + 3 * mv, nullptr,
+                                          d->jas_dj, nullptr, nullptr, s))) return rc;
+            wj.table = jas.J->table; wj.base = d->jas_dj; wj.jratio_out = jas.jratio_out ? jas.jratio_out + mv : nullptr;
+        }
         rc = delayed_sweep_window(d, pos, delta + 3 * mv, unif + mv, k, nb, ratios_out ? ratios_out + mv : nullptr,
                                   accept_out ? accept_out + mv : nullptr, forced ? forced + mv : nullptr, fixed_node,
-                                  force ? force + 3 * mv : nullptr, overlap && i + 1 < nwin ? 1 : 0, s);
+                                  force ? force + 3 * mv : nullptr, overlap && i + 1 < nwin ? 1 : 0, wj, s);
         if (rc) return rc;
         if (overlap && i + 1 < nwin) {
             // (delayed_sweep_window recorded ev_main between its window kernel and its flush)
@@ -353,14 +373,29 @@ static int sweep_impl(qmc_det *d, const qmc_spline *sp, double *pos, const doubl
         QMC_REQUIRE(k0 >= 0 && kn >= 0 && k0 + kn <= nel, "qmc_sweep_ex: electron range %d+%d outside 0..%d", k0, kn, nel);
         QMC_REQUIRE(nrec >= 0 && nrec <= nw, "qmc_sweep_ex: nrecord=%d outside 0..%d", nrec, nw);
         QMC_REQUIRE(opts->drift_tau >= 0.0 && isfinite(opts->drift_tau), "qmc_sweep_ex: drift_tau=%g", opts->drift_tau);
+        QMC_REQUIRE(!(opts->jastrow && opts->drift_tau > 0.0), "qmc_sweep_ex: a Jastrow factor with drift moves needs grad J, which is not built");
         if (opts->drift_tau > 0.0)
             return sweep_drift(d, sp, pos, delta, unif, nsweeps, k0, kn, ratios_out, accept_out, forced, fixed_node, force,
                                rec, nrec, opts->drift_tau, opts->rprop_out, opts->logt_out, opts->fcur_out, s);
     }
     const int batch = d->spo_batch;
     const size_t slot_stride = (size_t)nw * 5 * d->np;
+    SweepJastrow jas{};
+    if (opts && opts->jastrow) {
+        jas.J = opts->jastrow;
+        jas.nother = opts->jastrow_nother;
+        jas.other = jas.nother > 0 ? opts->jastrow_other : nullptr;
+        jas.jratio_out = opts->jratio_out;
+        QMC_REQUIRE(jas.nother >= 0 && (jas.nother == 0 || jas.other), "qmc_sweep_ex: jastrow_nother=%d without positions", jas.nother);
+        QMC_REQUIRE(jas.J->device == d->device, "qmc_sweep_ex: the Jastrow factor lives on another device");
+        if (!d->jas_dj) {
+            const size_t bytes = (size_t)(d->delay > 1 ? d->delay : 1) * nw * sizeof(double);
+            cudaError_t e = cudaMalloc((void **)&d->jas_dj, bytes);
+            if (e != cudaSuccess) { set_error("qmc_sweep_ex (jastrow): cudaMalloc(%zu bytes) -> %s", bytes, cudaGetErrorString(e)); (void)cudaGetLastError(); return QMC_ENOMEM; }
+        }
+    }
     if (d->delay) return sweep_delayed(d, sp, pos, delta, unif, nsweeps, k0, kn, ratios_out, accept_out, forced,
-                                       fixed_node, force, rec, nrec, s);
+                                       fixed_node, force, rec, nrec, jas, s);
     for (int sw = 0; sw < nsweeps; ++sw) {
         for (int k = k0; k < k0 + kn; ++k) {
             const size_t mv = ((size_t)sw * nel + k) * nw;
@@ -382,6 +417,12 @@ static int sweep_impl(qmc_det *d, const qmc_spline *sp, double *pos, const doubl
             u.B = d->b32 ? (void *)d->Bf : (void *)d->B; u.nel = nel; u.ld = d->ld; u.iel = k;
             u.phi = phi; u.ldphi = (size_t)5 * d->np; u.rowk = d->rowk;
             u.ratio = d->ratio;
+            if (jas.J) {              // exp(-2 dJ) at the current configuration: the Jastrow part of |Psi'/Psi|^2
+                int rc = jastrow_move_launch(jas.J, nw, nel, pos, jas.nother, jas.other, k, 1, delta + 3 * mv, nullptr, nullptr,
+                                             jas.jratio_out ? jas.jratio_out + mv : nullptr, d->jas_dj, s);
+                if (rc) return rc;
+                u.tfac = d->jas_dj;
+            }
             u.unif = unif + mv;
             u.forced = forced ? forced + mv : nullptr;
             u.fixed_node = fixed_node;

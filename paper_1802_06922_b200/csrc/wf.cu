@@ -1,5 +1,5 @@
 // qmc_wf_*: the product of two spin determinants, Psi_T = D_up D_dn (eq. 26, with one
-// determinant per spin and no Jastrow factor: e^J = 1, c_1 = 1).  A particle-by-particle sweep iterates
+// determinant per spin, c_1 = 1; a Jastrow factor is an option of the sweep, qmc_sweep_opts_t.jastrow).  A particle-by-particle sweep iterates
 // "sequentially over all electrons" (L195): the N_up electrons of the up determinant, then the N_dn of
 // the down determinant.  Moving an up electron leaves D_dn unchanged, so the ratio of the move is
 // D_up'/D_up and only the up inverse is updated (and vice versa): the sweep is the up sweep followed
@@ -98,6 +98,11 @@ extern "C" int qmc_wf_sweep(qmc_wf_t *wf, double *pos_up, double *pos_dn, const 
                 if (o.rprop_out) o.rprop_out += 3 * mv;
                 if (o.fcur_out) o.fcur_out += 3 * mv;
                 if (o.logt_out) o.logt_out += mv;
+                if (o.jastrow) {          // the other spin's electrons, where they are now, are the fixed particles
+                    o.jastrow_other = pos[1 - sp];
+                    o.jastrow_nother = wf->det[1 - sp]->nel;
+                    if (o.jratio_out) o.jratio_out += mv;
+                }
             }
             int rc = qmc_sweep_ex(wf->det[sp], wf->spline[sp], pos[sp], delta + 3 * mv, unif + mv, 1,
                                   ratios_out ? ratios_out + mv : nullptr, accept_out ? accept_out + mv : nullptr,

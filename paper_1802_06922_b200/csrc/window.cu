@@ -18,6 +18,7 @@
 // R' = S^-T Rows (Rows[l] = B0[k_l]; the flush overwrites B in place and computes B -= Q R').
 #include "delayed_device.cuh"
 #include "dmma.cuh"
+#include "jastrow_device.cuh"
 #include "update_device.cuh"
 
 namespace qmc {
@@ -44,6 +45,7 @@ struct WindowArgs {
     int *win_iel;                 // [nw][K]
     int *win_slot;                // [nw][K]
     double *win_rows;             // [nw][K][ld]   row l <- R'[l]
+    WindowJastrow jas;            // table == NULL: no Jastrow factor
 };
 
 // G[i][j] = x_i . B0[iel0 + j] for the nb vectors x_i = x0 + i * vstep (fp32) of one walker, into
@@ -110,7 +112,7 @@ __device__ __forceinline__ void window_contract(const float *x0, size_t vstep, c
 // One block per walker, 8 warps.  Phases 1-2: G (and, with FORCE, the same contraction for the three
 // gradient vectors of every proposal).  Phase 3: warp 0 walks the nb steps.  Phase 4: R' = S^-T Rows,
 // 8-column tiles over the warps.
-template <typename TB, int KMAX, bool FORCE>
+template <typename TB, int KMAX, bool FORCE, bool JAS>
 __global__ void __launch_bounds__(kWinThreads) delayed_window_kernel(WindowArgs a)
 {
     constexpr int GS = KMAX + 1;
@@ -119,6 +121,12 @@ __global__ void __launch_bounds__(kWinThreads) delayed_window_kernel(WindowArgs 
     __shared__ double sinv_s[KMAX * GS];
     __shared__ long long rowoff_s[KMAX];
     __shared__ int p_s;
+    __shared__ JasTable jas_s[JAS ? 1 : 0 + !JAS];          // used only with a Jastrow factor (JAS)
+    if (JAS) {                                     // (visible to warp 0 after window_contract's barriers)
+        const int *src = reinterpret_cast<const int *>(a.jas.table);
+        int *dst = reinterpret_cast<int *>(&jas_s[0]);
+        for (int i = threadIdx.x; i < (int)(sizeof(JasTable) / sizeof(int)); i += kWinThreads) dst[i] = src[i];
+    }
     const int w = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nb = a.nb, ld = a.ld, np = a.np, K = a.K;
     const size_t vstep = (size_t)a.nw * 5 * np;             // stride between steps in vgl
@@ -140,6 +148,16 @@ __global__ void __launch_bounds__(kWinThreads) delayed_window_kernel(WindowArgs 
         const int f_l = (step_l && a.forced) ? (a.forced[mv_l] != 0) : 0;
         double R_l = 1.0;                                             // ratio of step `lane`
         double F_l[3] = {0.0, 0.0, 0.0};                              // force of step `lane`
+        // Jastrow factor: lane l holds the old and the proposed position of the electron of step l and the
+        // dJ of that step against the window-start configuration
+        constexpr bool jas = JAS;
+        double ro_l[3] = {0.0, 0.0, 0.0}, rn_l[3] = {0.0, 0.0, 0.0}, dj_l = 0.0, jr_l = 1.0;
+        if (jas && step_l) {
+            const double *r = a.pos + ((size_t)w * a.nel + a.iel0 + lane) * 3;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) { ro_l[c] = r[c]; rn_l[c] = r[c] + a.delta[3 * mv_l + c]; }
+            dj_l = a.jas.base[mv_l];
+        }
         unsigned acc_mask = 0;                                        // accepted steps (same in every lane)
         int p = 0, mine = 0;
         for (int i = 0; i < nb; ++i) {
@@ -156,7 +174,21 @@ __global__ void __launch_bounds__(kWinThreads) delayed_window_kernel(WindowArgs 
             const double R = G_s[i * GS + i] - warp_sum(x * y);
             const double u_i = __shfl_sync(0xffffffffu, u_l, i);
             const int f_i = __shfl_sync(0xffffffffu, f_l, i);
-            const bool acc_w = (a.forced ? (f_i != 0) : (metropolis(R, u_i) && !(a.fixed_node && R < 0.0))) && usable_ratio(R);
+            double tf = 1.0;                                          // exp(-2 dJ): the Jastrow part of |Psi'/Psi|^2
+            if (jas) {
+                // the electrons of the accepted steps m < i sit at their proposed positions now: replace their
+                // window-start contribution to dJ of step i (same-spin function) by the current one
+                double ro_i[3], rn_i[3];
+#pragma unroll
+                for (int c = 0; c < 3; ++c) { ro_i[c] = __shfl_sync(0xffffffffu, ro_l[c], i); rn_i[c] = __shfl_sync(0xffffffffu, rn_l[c], i); }
+                double corr = 0.0;
+                if (lane < i && ((acc_mask >> lane) & 1u))
+                    corr = jas_pair_delta(jas_s[0], jas_s[0].f_same, rn_i, ro_i, rn_l) - jas_pair_delta(jas_s[0], jas_s[0].f_same, rn_i, ro_i, ro_l);
+                const double dj = __shfl_sync(0xffffffffu, dj_l, i) + warp_sum(corr);
+                tf = exp(-2.0 * dj);
+                if (lane == i) jr_l = exp(-dj);
+            }
+            const bool acc_w = (a.forced ? (f_i != 0) : (metropolis_t(R, tf, u_i) && !(a.fixed_node && R < 0.0))) && usable_ratio(R);
             if (lane == i) R_l = R;
             if (FORCE) {
                 // grad phi(r'_i) . B_cur[k_i] = gd - xg^T S^-1 c with the same y = S^-1 c as the ratio
@@ -190,6 +222,7 @@ __global__ void __launch_bounds__(kWinThreads) delayed_window_kernel(WindowArgs 
         if (step_l) {
             if (a.ratios_out) a.ratios_out[mv_l] = R_l;
             if (a.accept_out) a.accept_out[mv_l] = acc_l ? 1 : 0;
+            if (jas && a.jas.jratio_out) a.jas.jratio_out[mv_l] = jr_l;
             if (FORCE) {
                 a.force_out[3 * mv_l + 0] = F_l[0];
                 a.force_out[3 * mv_l + 1] = F_l[1];
@@ -228,7 +261,7 @@ __global__ void __launch_bounds__(kWinThreads) delayed_window_kernel(WindowArgs 
 
 int delayed_sweep_window(qmc_det *d, double *pos, const double *delta, const double *unif, int iel0, int nb,
                          double *ratios_out, unsigned char *accept_out, const unsigned char *forced,
-                         int fixed_node, double *force_out, int record_mid, cudaStream_t s)
+                         int fixed_node, double *force_out, int record_mid, const WindowJastrow &jas, cudaStream_t s)
 {
     if (d->host_pending) {        // rows pending from standalone qmc_det_accept_update calls
         int rc = delayed_flush_reset_host(d, s);
@@ -245,17 +278,24 @@ int delayed_sweep_window(qmc_det *d, double *pos, const double *delta, const dou
     a.logdet = d->logdet; a.sign = d->sign; a.naccept = d->naccept;
     a.win_count = d->win_count; a.win_iel = d->win_iel; a.win_slot = d->win_slot;
     a.win_rows = d->win_rows;
+    a.jas = jas;
     prof_start(d, kProfDelayedRatio, s);
-#define QMC_WIN_LAUNCH(TB, KM, F) delayed_window_kernel<TB, KM, F><<<d->nw, kWinThreads, 0, s>>>(a)
-#define QMC_WIN_RANK(TB, F)                                  \
+#define QMC_WIN_LAUNCH(TB, KM, F, J) delayed_window_kernel<TB, KM, F, J><<<d->nw, kWinThreads, 0, s>>>(a)
+#define QMC_WIN_RANK(TB, F, J)                               \
     do {                                                     \
-        if (a.K <= 8) QMC_WIN_LAUNCH(TB, 8, F);              \
-        else if (a.K <= 16) QMC_WIN_LAUNCH(TB, 16, F);       \
-        else if (a.K <= 24) QMC_WIN_LAUNCH(TB, 24, F);       \
-        else QMC_WIN_LAUNCH(TB, 32, F);                      \
+        if (a.K <= 8) QMC_WIN_LAUNCH(TB, 8, F, J);           \
+        else if (a.K <= 16) QMC_WIN_LAUNCH(TB, 16, F, J);    \
+        else if (a.K <= 24) QMC_WIN_LAUNCH(TB, 24, F, J);    \
+        else QMC_WIN_LAUNCH(TB, 32, F, J);                   \
     } while (0)
-    if (d->b32) { if (force_out) QMC_WIN_RANK(float, true); else QMC_WIN_RANK(float, false); }
-    else { if (force_out) QMC_WIN_RANK(double, true); else QMC_WIN_RANK(double, false); }
+#define QMC_WIN_JAS(TB, F)                                   \
+    do {                                                     \
+        if (jas.table) QMC_WIN_RANK(TB, F, true);            \
+        else QMC_WIN_RANK(TB, F, false);                     \
+    } while (0)
+    if (d->b32) { if (force_out) QMC_WIN_JAS(float, true); else QMC_WIN_JAS(float, false); }
+    else { if (force_out) QMC_WIN_JAS(double, true); else QMC_WIN_JAS(double, false); }
+#undef QMC_WIN_JAS
 #undef QMC_WIN_RANK
 #undef QMC_WIN_LAUNCH
     prof_stop(d, s);

@@ -597,6 +597,16 @@ def test_fp64_dmma_probe():
     tf = api.probe_fp64_dmma()
     print("fp64 DMMA peak", tf, "TFLOP/s")
     assert 15.0 < tf < 80.0
+    # qmc_probe_fp64_pipe: DMMA and DFMA share one pipe on this machine (the mixed stream adds up to about the
+    # same total, not to the sum of the two peaks), which is why every fp64 add in a flush kernel costs DMMA time
+    dm, _ = api.probe_fp64_pipe(0, 16, 8)
+    _, df = api.probe_fp64_pipe(1, 16, 8)
+    mdm, mdf = api.probe_fp64_pipe(2, 16, 8)
+    print("fp64 pipe: dmma", dm, "dfma", df, "mixed", mdm, "+", mdf)
+    assert abs(dm - tf) < 0.15 * tf and 10.0 < df < 80.0
+    assert mdm + mdf < 1.25 * max(dm, df)
+    with pytest.raises(api.QmcError):
+        api.probe_fp64_pipe(3, 16, 8)
 
 
 # --------------------------------------------- NEXT-3: fp32-stored inverse with fp64 recompute
@@ -920,3 +930,46 @@ def test_wavefunction_updn_parity(K):
         d_.destroy()
     for s_ in splines:
         s_.destroy()
+
+
+# --------------------------------------------- CUDA-graph replay of a sweep (launch-bound configs)
+@pytest.mark.parametrize("case,K", [("tiny", 0), ("ragged37_skew", 0), ("ragged37_skew", 4), ("small", 16)])
+def test_sweep_graph_replay_is_bitwise_the_eager_sweep(case, K):
+    """api.SweepGraph: the launches of one qmc_sweep captured into a CUDA graph and replayed with fresh random
+    numbers copied into the static buffers give bit for bit the state, ratios and decisions of eager sweeps."""
+    x = CASES[case]()
+    if x.delta.shape[0] < 3:
+        x = inputs.make_inputs(x.cfg, nsweeps=3)
+    if case == "small":
+        x = inputs.make_inputs(x.cfg, nw=32, nsweeps=3)
+    nsw = 3
+    spline = api.Spline.create(x.coefs.to(P.dev()), x.lattice)
+    d_all, u_all = P.to_dev(x.delta[:nsw]), P.to_dev(x.unif[:nsw])
+    out = []
+    for graphed in (False, True):
+        pos = P.to_dev(x.pos)
+        det = api.Det.init(spline, pos, delay_rank=K)
+        R = torch.zeros_like(u_all)
+        acc = torch.zeros(u_all.shape, dtype=torch.uint8, device=P.dev())
+        api.sweep(det, pos, d_all[0:1], u_all[0:1], ratios_out=R[0:1], accept_out=acc[0:1])      # eager warm-up sweep
+        if graphed:
+            d_buf, u_buf = d_all[1:2].clone(), u_all[1:2].clone()
+            r_buf, a_buf = torch.zeros_like(u_buf), torch.zeros(u_buf.shape, dtype=torch.uint8, device=P.dev())
+            torch.cuda.synchronize()
+            g = api.SweepGraph(det, pos, d_buf, u_buf, ratios_out=r_buf, accept_out=a_buf)
+            # (capture does not execute: the state is still the one after the warm-up sweep)
+            for i in (1, 2):
+                d_buf.copy_(d_all[i:i + 1]); u_buf.copy_(u_all[i:i + 1])
+                g.replay()
+                R[i:i + 1].copy_(r_buf); acc[i:i + 1].copy_(a_buf)
+        else:
+            for i in (1, 2):
+                api.sweep(det, pos, d_all[i:i + 1], u_all[i:i + 1], ratios_out=R[i:i + 1], accept_out=acc[i:i + 1])
+        torch.cuda.synchronize()
+        out.append((pos.cpu().numpy(), det.get_inverse().cpu().numpy(), R.cpu().numpy(), acc.cpu().numpy(),
+                    det.get_stats()[0].cpu().numpy()))
+        det.destroy()
+    for a_, b_ in zip(out[0], out[1]):
+        assert np.array_equal(a_, b_)
+    assert out[0][3][1:].mean() > 0.05
+    spline.destroy()
