@@ -64,7 +64,7 @@ class ClockSampler:
     """Samples SM clock and throttle reasons with NVML every 100 ms while the timed region runs."""
 
     def __init__(self, index):
-        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self.samples, self.power, self.reasons, self.max_mhz = [], [], set(), None
         self._stop = threading.Event()
         self._thr = None
         try:
@@ -94,6 +94,10 @@ class ClockSampler:
                         self.reasons.add(name)
             except Exception:
                 pass
+            try:
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)      # W
+            except Exception:
+                pass
             self._stop.wait(0.1)
 
     def start(self):
@@ -106,7 +110,8 @@ class ClockSampler:
         if self._thr is not None:
             self._thr.join()
         med = statistics.median(self.samples) if self.samples else None
-        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons)}
+        pw = statistics.median(self.power) if self.power else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "power_w": pw}
 
 
 def cpu_sample(x, coefs_np, target_s=15.0):

@@ -16,7 +16,9 @@ int delayed_flush(qmc_det *d, cudaStream_t s);
 int delayed_flush_reset_host(qmc_det *d, cudaStream_t s);   // flush + forget the host-side window bookkeeping
 bool flush_ring_serves(int ld, int K);                       // flush_ring.cu has a shape for (ld, rank)
 cudaError_t flush_ring_launch(qmc_det *d, cudaStream_t s);    // enqueue it
-bool flush_ring_hp_serves(int ld, int K);                    // flush_ring_hp.cu: the same for ranks 17..32
+bool flush_ring_hi_serves(int ld, int K);                    // flush_ring_hi.cu: the same for ranks 17..32
+cudaError_t flush_ring_hi_launch(qmc_det *d, cudaStream_t s);
+bool flush_ring_hp_serves(int ld, int K);                    // flush_ring_hp.cu: ranks 17..32, the earlier pipeline (A/B)
 cudaError_t flush_ring_hp_launch(qmc_det *d, cudaStream_t s);
 int delayed_max_rank(int ld);                                // largest K whose window fits shared memory
 // One window of qmc_sweep in delayed mode: electrons iel0 .. iel0+nb-1 (nb <= delay rank), whose

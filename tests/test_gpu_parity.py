@@ -391,7 +391,12 @@ def test_delayed_standalone_api():
 @pytest.mark.parametrize("nel,K,nw,count,env", [
     (512, 16, 6, 0, {}), (512, 32, 4, 0, {}), (1000, 16, 5, 0, {}), (1024, 16, 4, 0, {}), (1024, 32, 3, 0, {}),
     (2048, 16, 2, 200, {}), (2048, 32, 2, 200, {}), (512, 24, 4, 0, {}), (1024, 24, 3, 0, {}), (1024, 20, 3, 0, {}),
-    (2048, 24, 2, 200, {}),
+    (2048, 24, 2, 200, {}), (1000, 24, 3, 0, {}), (1000, 32, 3, 0, {}),
+    # ranks 17..32 on the earlier helper-pipelined kernel (flush_ring_hp.cu)
+    (1024, 24, 3, 0, {"QMC_FLUSH_HP": "1"}), (1024, 32, 3, 0, {"QMC_FLUSH_HP": "1"}), (2048, 32, 2, 200, {"QMC_FLUSH_HP": "1"}),
+    # ranks <= 16 on the one-block-lag kernel without a service warpgroup (flush_ring.cu) and with forced lags / ping-pong
+    (1024, 16, 3, 0, {"QMC_FLUSH_LAG": "0"}), (1024, 16, 3, 0, {"QMC_FLUSH_LAG": "2"}), (1024, 16, 3, 0, {"QMC_FLUSH_PP": "1"}),
+    (2048, 16, 2, 200, {"QMC_FLUSH_LAG": "2", "QMC_FLUSH_PP": "1"}), (512, 16, 4, 0, {"QMC_FLUSH_LAG": "0"}),
     # the flush.cu kernel on the same shapes: one CTA per row block, then its cluster shapes
     (1000, 16, 4, 0, {"QMC_FLUSH_RING": "0"}), (1024, 16, 3, 0, {"QMC_FLUSH_RING": "0", "QMC_FLUSH_SHAPE": "1"}),
     (1024, 16, 3, 0, {"QMC_FLUSH_RING": "0", "QMC_FLUSH_SHAPE": "2"}), (1024, 32, 3, 0, {"QMC_FLUSH_RING": "0"}),
