@@ -40,7 +40,7 @@ UNIT = "moves/s"
 # rank-16 window is the faster one on this kernel)
 DEFAULT_DELAY = {"tiny": [0], "small": [16, 0], "mid": [16, 0], "large": [16, 0], "xlarge": [16, 32, 0]}
 # further arms reported as variants (fewer timed steps each): (delay rank, fp32-stored inverse)
-EXTRA_ARMS = {"large": [(16, True), (0, True), (24, False), (32, False), (0, False, "drift"), (16, False, "updn"),
+EXTRA_ARMS = {"large": [(16, True), (0, True), (20, False), (24, False), (32, False), (0, False, "drift"), (16, False, "updn"),
                         (16, False, "jastrow")],
               "mid": [(16, True), (16, False, "updn")], "xlarge": [(16, True), (24, False)],
               # L2-resident configs: the sweep is launch-bound; the same sweep replayed from a CUDA graph

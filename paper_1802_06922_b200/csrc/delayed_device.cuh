@@ -25,13 +25,13 @@ int delayed_max_rank(int ld);                                // largest K whose 
 // SPO-VGL is in d->vgl; ratios, decisions, moves and the flush.  Pointers are offset to the first step.
 // fixed_node: reject R < 0; force_out: NULL or [nb][nw][3], F = 2 grad log Psi_T at the proposed configuration;
 // record_mid: record d->ev_main on `s` between the window kernel and the flush (sweep.cu's second stream).
-// jas: Jastrow factor of the window (table NULL = none): base[j][w] = dJ of step j against the configuration at
-// the start of the window (jastrow_move_kernel); the window kernel adds the change due to the electrons the
-// window has moved before step j and accepts iff R^2 exp(-2 dJ) > u.
-struct JasTable;
+// jas: Jastrow factor of the window (base NULL = none): base[j][w] = dJ of step j against the configuration at
+// the start of the window, corr[w][j][m] (m < j, row stride = the delay rank) = what an accepted step m adds to
+// it (jastrow_move_kernel); the window kernel sums the pair terms of the steps it has accepted before step j
+// and accepts iff R^2 exp(-2 dJ) > u.
 struct WindowJastrow {
-    const JasTable *table;
     const double *base;           // [nb][nw]
+    const double *corr;           // [nw][K][K]
     double *jratio_out;           // [nb][nw] or NULL: exp(-dJ)
 };
 int delayed_sweep_window(qmc_det *d, double *pos, const double *delta, const double *unif, int iel0, int nb,

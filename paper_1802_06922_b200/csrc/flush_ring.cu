@@ -292,13 +292,13 @@ cudaError_t flush_ring_launch(qmc_det *d, cudaStream_t s)
     const int v = d->ld / 64;
     const char *lag = getenv("QMC_FLUSH_LAG");             // A/B hook, see below
     if (!(lag && atoi(lag) == 0)) {
-        // QMC_FLUSH_LAG: 0 = the kernel above; 1 / 2 force the lag; QMC_FLUSH_PP: 0 / 1 force ping-pong off / on.
-        // Defaults (measured on the B200 under its power cap, profiles/r02_flush_summary.md; the variants are
-        // within 5 % of each other): fp32 rows: lag 1; fp64 rows: lag 2 with ping-pong up to N = 1024, lag 1 at
-        // N = 2048 (cluster of 4: the exchange is slower, the deeper ring pays).
+        // QMC_FLUSH_LAG: 0 = the kernel above; 1 / 2 force the lag; QMC_FLUSH_PP: 1 = ping-pong on.
+        // Default (measured on the B200 under its power cap, profiles/r02_flush_summary.md): lag 1 without
+        // ping-pong for every shape and storage type -- 1.41 ms per flush at `large` (0.94 of the measured HBM
+        // peak) against 1.55-1.59 ms for lag 2 with or without ping-pong and 1.62 ms for the round-1 kernel.
         const char *ppe = getenv("QMC_FLUSH_PP");
-        const int lg = lag ? atoi(lag) : ((d->b32 || v > 16) ? 1 : 2);
-        const bool pp = ppe ? atoi(ppe) == 1 : (lg == 2 && !d->b32);
+        const int lg = lag ? atoi(lag) : 1;
+        const bool pp = ppe && atoi(ppe) == 1;
 #define X(V, KPAD, TW, NWC, CS, ST1, ST2)                                                                           \
     if (v == V) {                                                                                                   \
         if (d->b32) {                                                                                               \

@@ -59,7 +59,9 @@ __device__ __forceinline__ void ring_stream2(const RingArgs &a, int w, int p, un
     // row blocks the TMA producer runs ahead in shared memory: LAG 1 frees a stage once every compute warp
     // has loaded it for step 1; LAG 2 keeps it until step 2 has read it again
     constexpr int PF = LAG == 1 ? STAGES - 1 : STAGES - 3;
-    constexpr int kL2Ahead = 4;                             // ... and further ahead in L2 (bulk prefetch)
+    // ... and further ahead in L2 (bulk prefetch): only where the ring itself is short (LAG 2 keeps three stages
+    // busy); with the deep LAG-1 ring the prefetches only add DRAM reads (ncu: +19 % read traffic)
+    constexpr int kL2Ahead = LAG == 2 ? 4 : 0;
     static_assert(PF >= 1, "ring too short");
     TB *ring = reinterpret_cast<TB *>(smem + L::ring_off);
     double *part = reinterpret_cast<double *>(smem + L::part_off);
@@ -98,14 +100,15 @@ __device__ __forceinline__ void ring_stream2(const RingArgs &a, int w, int p, un
         const int h = warp - NWC;
         if (h == 0) {
             for (int jb = 0; jb <= PF && jb < nblk; ++jb) issue(jb);
-            for (int jb = PF + 1; jb <= PF + kL2Ahead && jb < nblk; ++jb) prefetch(jb);
+            if (kL2Ahead)
+                for (int jb = PF + 1; jb <= PF + kL2Ahead && jb < nblk; ++jb) prefetch(jb);
         }
         constexpr int NE = 64 * NTA, EPL = (NE + 127) / 128;      // elements of a block's partial Q; per lane of the warpgroup
         if (32 * h >= NE) return;
         for (int j = 0; j < nblk; ++j) {
             // LAG 2: the stage of block j + PF was released by step 2 of block j - 3 (compute iteration j - 1)
             if (LAG == 2 && h == 0 && j >= 1) {
-                if (j + PF + kL2Ahead < nblk) prefetch(j + PF + kL2Ahead);
+                if (kL2Ahead && j + PF + kL2Ahead < nblk) prefetch(j + PF + kL2Ahead);
                 if (j + PF < nblk) issue(j + PF);
             }
             const double *pbuf = part + (size_t)(j % NPB) * NWC * 8 * PS;
@@ -114,7 +117,7 @@ __device__ __forceinline__ void ring_stream2(const RingArgs &a, int w, int p, un
             mbar_wait(&pbar[j % NPB], (uint32_t)(j / NPB) & 1u);
             // LAG 1: every compute warp has loaded block j for its step 1: the stage is free
             if (LAG == 1 && h == 0) {
-                if (j + 1 + PF + kL2Ahead < nblk) prefetch(j + 1 + PF + kL2Ahead);
+                if (kL2Ahead && j + 1 + PF + kL2Ahead < nblk) prefetch(j + 1 + PF + kL2Ahead);
                 if (j + 1 + PF < nblk) issue(j + 1 + PF);
             }
 #pragma unroll

@@ -8,8 +8,8 @@
 
 namespace qmc {
 
-// X(V, KPAD, TW, NWC, CS, ST1, ST2): ld = 64 V = CS * NWC * TW * 8; ST1 = ring stages with LAG 1 (fp64 rows),
-// ST2 = with LAG 2 (fp32 rows).
+// X(V, KPAD, TW, NWC, CS, ST1, ST2): ld = 64 V = CS * NWC * TW * 8; ring stages for fp64 rows (ST1) and for fp32
+// rows (ST2); both run with LAG 1.
 #define QMC_RING2_HI_SHAPES(X)                                                     \
     X(8, 24, 4, 8, 2, 11, 16) X(16, 24, 4, 8, 4, 10, 16) X(32, 24, 4, 8, 8, 8, 12)  \
     X(8, 32, 4, 8, 2, 10, 16) X(16, 32, 4, 8, 4, 9, 14) X(32, 32, 4, 8, 8, 7, 7)
@@ -37,7 +37,7 @@ cudaError_t flush_ring_hi_launch(qmc_det *d, cudaStream_t s)
     const int v = d->ld / 64, kpad = d->delay <= 24 ? 24 : 32;
 #define X(V, KPAD, TW, NWC, CS, ST1, ST2)                                                                    \
     if (v == V && kpad == KPAD)                                                                              \
-        return d->b32 ? launch_ring2<false, 2, float, KPAD, TW, NWC, CS, ST2>(a, d->nw, d->nsm, s)           \
+        return d->b32 ? launch_ring2<false, 1, float, KPAD, TW, NWC, CS, ST2>(a, d->nw, d->nsm, s)           \
                       : launch_ring2<false, 1, double, KPAD, TW, NWC, CS, ST1>(a, d->nw, d->nsm, s);
     QMC_RING2_HI_SHAPES(X)
 #undef X

@@ -24,6 +24,9 @@ struct JasMoveArgs {
     double *dj_out;           // [nb][nw] or NULL
     double *ratio_out;        // [nb][nw] exp(-dJ) or NULL
     double *tfac_out;         // [nb][nw] exp(-2 dJ) or NULL
+    double *corr_out;         // [nw][ncorr][ncorr] or NULL: corr[w][j][m], m < j: what the ACCEPTED move of step m
+    int ncorr;                //   (earlier in the same batch) adds to dJ of step j -- the same-spin pair term with
+                              //   electron iel0 + m at its proposed instead of its old position
 };
 
 constexpr int kJasThreads = 128;
@@ -59,6 +62,14 @@ __global__ void __launch_bounds__(kJasThreads) jastrow_move_kernel(JasMoveArgs a
         for (int i = threadIdx.x; i < a.nother; i += kJasThreads) s += jas_pair_delta(T, T.f_opp, rnew, rold, ow + 3 * i);
     }
     for (int i = threadIdx.x; i < a.nion; i += kJasThreads) s += jas_pair_delta(T, a.ion_func[i], rnew, rold, a.ion + 3 * i);
+    if (a.corr_out && (int)threadIdx.x < j) {
+        const int m = threadIdx.x;
+        const double *ro_m = pw + 3 * (a.iel0 + m);
+        const double *dm = a.delta + 3 * ((size_t)m * a.nw + w);
+        const double rn_m[3] = {ro_m[0] + dm[0], ro_m[1] + dm[1], ro_m[2] + dm[2]};
+        a.corr_out[((size_t)w * a.ncorr + j) * a.ncorr + m] =
+            jas_pair_delta(T, T.f_same, rnew, rold, rn_m) - jas_pair_delta(T, T.f_same, rnew, rold, ro_m);
+    }
     const double dj = block_sum(s, red);
     if (threadIdx.x == 0) {
         const size_t o = (size_t)j * a.nw + w;
@@ -101,13 +112,14 @@ __global__ void __launch_bounds__(256) jastrow_value_kernel(const JasTable *tabl
 // step with explicit proposals.
 int jastrow_move_launch(const qmc_jastrow *J, int nw, int nel, const double *pos, int nother, const double *other,
                         int iel0, int nb, const double *delta, const double *rnew, double *dj_out, double *ratio_out,
-                        double *tfac_out, cudaStream_t s)
+                        double *tfac_out, double *corr_out, int ncorr, cudaStream_t s)
 {
     JasMoveArgs a{};
     a.table = J->table; a.nion = J->nion; a.ion = J->ion; a.ion_func = J->ion_func;
     a.nw = nw; a.nel = nel; a.nother = other ? nother : 0;
     a.pos = pos; a.other = other; a.iel0 = iel0; a.delta = delta; a.rnew = rnew;
     a.dj_out = dj_out; a.ratio_out = ratio_out; a.tfac_out = tfac_out;
+    a.corr_out = delta ? corr_out : nullptr; a.ncorr = ncorr;
     jastrow_move_kernel<<<dim3(nw, nb), kJasThreads, 0, s>>>(a);
     QMC_LAUNCHED();
     return QMC_OK;
@@ -202,7 +214,7 @@ extern "C" int qmc_jastrow_ratio(const qmc_jastrow_t *J, int nwalkers, int nel, 
     QMC_REQUIRE(nother >= 0 && (nother == 0 || other), "qmc_jastrow_ratio: nother=%d without positions", nother);
     if (nwalkers == 0) return QMC_OK;
     return jastrow_move_launch(J, nwalkers, nel, pos, nother, nother ? other : nullptr, iel, 1, nullptr, rnew, dj_out,
-                               ratio_out, nullptr, (cudaStream_t)stream);
+                               ratio_out, nullptr, nullptr, 0, (cudaStream_t)stream);
 }
 
 extern "C" int qmc_jastrow_value(const qmc_jastrow_t *J, int nwalkers, int nel, const double *pos, int nother,

@@ -18,7 +18,6 @@
 // R' = S^-T Rows (Rows[l] = B0[k_l]; the flush overwrites B in place and computes B -= Q R').
 #include "delayed_device.cuh"
 #include "dmma.cuh"
-#include "jastrow_device.cuh"
 #include "update_device.cuh"
 
 namespace qmc {
@@ -45,7 +44,7 @@ struct WindowArgs {
     int *win_iel;                 // [nw][K]
     int *win_slot;                // [nw][K]
     double *win_rows;             // [nw][K][ld]   row l <- R'[l]
-    WindowJastrow jas;            // table == NULL: no Jastrow factor
+    WindowJastrow jas;            // base == NULL: no Jastrow factor
 };
 
 // G[i][j] = x_i . B0[iel0 + j] for the nb vectors x_i = x0 + i * vstep (fp32) of one walker, into
@@ -113,7 +112,7 @@ __device__ __forceinline__ void window_contract(const float *x0, size_t vstep, c
 // gradient vectors of every proposal).  Phase 3: warp 0 walks the nb steps.  Phase 4: R' = S^-T Rows,
 // 8-column tiles over the warps.
 template <typename TB, int KMAX, bool FORCE, bool JAS>
-__global__ void __launch_bounds__(kWinThreads) delayed_window_kernel(WindowArgs a)
+__global__ void __launch_bounds__(kWinThreads, (FORCE || KMAX > 16) ? 1 : 4) delayed_window_kernel(WindowArgs a)
 {
     constexpr int GS = KMAX + 1;
     __shared__ double G_s[KMAX * GS];
@@ -121,12 +120,6 @@ __global__ void __launch_bounds__(kWinThreads) delayed_window_kernel(WindowArgs 
     __shared__ double sinv_s[KMAX * GS];
     __shared__ long long rowoff_s[KMAX];
     __shared__ int p_s;
-    __shared__ JasTable jas_s[JAS ? 1 : 0 + !JAS];          // used only with a Jastrow factor (JAS)
-    if (JAS) {                                     // (visible to warp 0 after window_contract's barriers)
-        const int *src = reinterpret_cast<const int *>(a.jas.table);
-        int *dst = reinterpret_cast<int *>(&jas_s[0]);
-        for (int i = threadIdx.x; i < (int)(sizeof(JasTable) / sizeof(int)); i += kWinThreads) dst[i] = src[i];
-    }
     const int w = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nb = a.nb, ld = a.ld, np = a.np, K = a.K;
     const size_t vstep = (size_t)a.nw * 5 * np;             // stride between steps in vgl
@@ -148,16 +141,11 @@ __global__ void __launch_bounds__(kWinThreads) delayed_window_kernel(WindowArgs 
         const int f_l = (step_l && a.forced) ? (a.forced[mv_l] != 0) : 0;
         double R_l = 1.0;                                             // ratio of step `lane`
         double F_l[3] = {0.0, 0.0, 0.0};                              // force of step `lane`
-        // Jastrow factor: lane l holds the old and the proposed position of the electron of step l and the
-        // dJ of that step against the window-start configuration
+        // Jastrow factor: lane l holds dJ of step l against the window-start configuration
         constexpr bool jas = JAS;
-        double ro_l[3] = {0.0, 0.0, 0.0}, rn_l[3] = {0.0, 0.0, 0.0}, dj_l = 0.0, jr_l = 1.0;
-        if (jas && step_l) {
-            const double *r = a.pos + ((size_t)w * a.nel + a.iel0 + lane) * 3;
-#pragma unroll
-            for (int c = 0; c < 3; ++c) { ro_l[c] = r[c]; rn_l[c] = r[c] + a.delta[3 * mv_l + c]; }
-            dj_l = a.jas.base[mv_l];
-        }
+        double dj_l = 0.0, jr_l = 1.0;
+        if (jas && step_l) dj_l = a.jas.base[mv_l];
+        const double *corr_w = jas ? a.jas.corr + (size_t)w * K * K : nullptr;
         unsigned acc_mask = 0;                                        // accepted steps (same in every lane)
         int p = 0, mine = 0;
         for (int i = 0; i < nb; ++i) {
@@ -176,14 +164,9 @@ __global__ void __launch_bounds__(kWinThreads) delayed_window_kernel(WindowArgs 
             const int f_i = __shfl_sync(0xffffffffu, f_l, i);
             double tf = 1.0;                                          // exp(-2 dJ): the Jastrow part of |Psi'/Psi|^2
             if (jas) {
-                // the electrons of the accepted steps m < i sit at their proposed positions now: replace their
-                // window-start contribution to dJ of step i (same-spin function) by the current one
-                double ro_i[3], rn_i[3];
-#pragma unroll
-                for (int c = 0; c < 3; ++c) { ro_i[c] = __shfl_sync(0xffffffffu, ro_l[c], i); rn_i[c] = __shfl_sync(0xffffffffu, rn_l[c], i); }
-                double corr = 0.0;
-                if (lane < i && ((acc_mask >> lane) & 1u))
-                    corr = jas_pair_delta(jas_s[0], jas_s[0].f_same, rn_i, ro_i, rn_l) - jas_pair_delta(jas_s[0], jas_s[0].f_same, rn_i, ro_i, ro_l);
+                // the electrons of the accepted steps m < i sit at their proposed positions now: add their pair
+                // terms (lane m owns step m; fixed butterfly order)
+                const double corr = (lane < i && ((acc_mask >> lane) & 1u)) ? corr_w[(size_t)i * K + lane] : 0.0;
                 const double dj = __shfl_sync(0xffffffffu, dj_l, i) + warp_sum(corr);
                 tf = exp(-2.0 * dj);
                 if (lane == i) jr_l = exp(-dj);
@@ -290,7 +273,7 @@ int delayed_sweep_window(qmc_det *d, double *pos, const double *delta, const dou
     } while (0)
 #define QMC_WIN_JAS(TB, F)                                   \
     do {                                                     \
-        if (jas.table) QMC_WIN_RANK(TB, F, true);            \
+        if (jas.base) QMC_WIN_RANK(TB, F, true);            \
         else QMC_WIN_RANK(TB, F, false);                     \
     } while (0)
     if (d->b32) { if (force_out) QMC_WIN_JAS(float, true); else QMC_WIN_JAS(float, false); }
