@@ -46,10 +46,10 @@ EXTRA_ARMS = {"large": [(16, True), (0, True), (20, False), (24, False), (32, Fa
               # L2-resident configs: the sweep is launch-bound; the same sweep replayed from a CUDA graph
               "tiny": [(0, False, "graph")], "small": [(16, False, "graph"), (0, False, "graph")]}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures
-# (profiles/r01_*.md), config `large`
+# (profiles/r01_rank1_summary.md: kernel unchanged since; profiles/r02_delayed_summary.md), config `large`
 # keyed by (kernel, delay rank); value = (bytes per launch, the file the figure comes from)
 NCU_TRAFFIC = {("sm_update", 0): (6.725e9, "profiles/r01_rank1_summary.md"),
-               ("delayed_flush", 16): (8.612e9, "profiles/r01_delayed_summary.md")}
+               ("delayed_flush", 16): (8.612e9, "profiles/r02_delayed_summary.md")}
 
 
 def measured_peaks():
