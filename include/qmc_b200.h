@@ -384,7 +384,11 @@ int qmc_det_profile_read(qmc_det_t *det, double *ms_host, long long *launches_ho
 /* Environment variables read by qmc_det_flush / qmc_sweep (test and A/B-measurement hooks only; unset
  * in production): QMC_FLUSH_RING=0 routes every shape to the shared-memory-window flush kernel
  * (flush.cu) instead of the register-window / TMA-ring kernel (flush_ring.cu); QMC_FLUSH_SHAPE=n
- * forces the n-th launch shape of flush.cu for the handle's leading dimension.  Results are the same
+ * forces the n-th launch shape of flush.cu for the handle's leading dimension; QMC_FLUSH_LAG=0 selects
+ * the round-1 ring kernel (reduction by two compute warps), 1 / 2 the lag between the two contractions in
+ * the warp-specialised ring kernel (default 1), QMC_FLUSH_PP=1 its ping-pong variant; QMC_FLUSH_HP=1
+ * routes ranks 17..32 to the helper-pipelined kernel (flush_ring_hp.cu) instead of flush_ring_hi.cu;
+ * QMC_SWEEP_OVERLAP=0 keeps the next window's SPO-VGL on the sweep's own stream.  Results are the same
  * to rounding with any setting (tests/test_gpu_parity.py::test_delayed_large_n_equals_rank1). */
 
 /* Measured fp64 tensor-core peak of the current device in TFLOP/s (host pointer): an issue loop of
