@@ -19,8 +19,10 @@
 //   * the loop is software-pipelined by one block: step 1 of block j is issued before step 2 of
 //     block j-1, which hides the exchange latency behind tensor-core work.
 //
-// This kernel serves ranks <= 16 (the window fragments of 16 x 64 columns per warp fill the register
-// file).  Ranks 17..32 take flush_ring_hp.cu.  TB is the storage type of the inverse: double, or float
+// This file holds round 1's kernel (flush_ring_kernel: the reduction and exchange of the partial Q by two of
+// the compute warps; QMC_FLUSH_LAG=0) and the dispatch of the ranks <= 16 to the warp-specialised kernel of
+// flush_ring2.cuh, the default (the window fragments of 16 x 64 columns per warp fill the register file).
+// Ranks 17..32 take flush_ring_hi.cu (the same kernel with 32 columns per warp) or flush_ring_hp.cu.  TB is the storage type of the inverse: double, or float
 // for the single-precision inverse of PAPER.md L82 (R:A19) -- rows are converted when a fragment is
 // loaded and rounded once when the block is stored; all arithmetic is fp64.
 #include <stdlib.h>

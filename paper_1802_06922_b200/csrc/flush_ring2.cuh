@@ -21,22 +21,24 @@ struct RingArgs {
 };
 
 // ---------------------------------------------------------------------------------------------
-// Warp-specialised variant (the default).  ncu of the kernel above (profiles/r02_flush_summary.md): every
-// warp spends 18 % of its time spinning on rbar.  There the partial Q of block j is reduced and sent by two
+// Warp-specialised ring flush (the default).  ncu of round 1's kernel (flush_ring.cu; profiles/r02_flush_summary.md):
+// every warp spent 18 % of its time spinning on rbar.  There the partial Q of block j is reduced and sent by two
 // of the COMPUTE warps, after their own step 2 of block j-1, which leaves the exchange one step 1 (~500
 // cycles of DMMA) to complete -- not enough for reduce + st.async + arrival -- and all warps wait for the
 // same event, so nothing fills the fp64 pipe meanwhile.  Here:
 //   * a SERVICE warpgroup (4 warps, setmaxnreg hands their spare registers to the compute warps) feeds the
-//     ring (TMA bulk copies, with bulk L2 prefetches further ahead) and reduces / sends the partial Q of a
-//     block the moment the last compute warp has stored its share: no DMMA work stands in front of either;
-//   * LAG = 1 (fp64 storage, HBM-bound: the ring keeps every stage for prefetch): step 2 of block j-1 follows
-//     step 1 of block j, the row block stays in registers, the exchange has step 2 of block j-1 and step 1
-//     of block j+1 (~1000+ cycles of DMMA) to complete;
-//   * LAG = 2 (fp32 storage, fp64-pipe-bound, half-size stages): step 2 runs two blocks behind step 1 and
-//     reads its rows again from the ring (a stage goes back to the producer through an `empty` mbarrier);
+//     ring (TMA bulk copies) and reduces / sends the partial Q of a block the moment the last compute warp has
+//     stored its share: no DMMA work stands in front of either;
+//   * LAG = 1 (the default for every shape and storage type): per iteration a compute warp runs step 1 of block
+//     j, publishes its partial Q, THEN waits for the exchange of block j-1 and runs step 2 on the row block it
+//     kept in registers; the exchange has step 2 of block j-2 and step 1 of block j (~1000+ cycles of DMMA) to
+//     complete, and the ring keeps every stage for prefetch;
+//   * LAG = 2 (A/B variant, QMC_FLUSH_LAG=2): step 2 runs two blocks behind step 1 and reads its rows again
+//     from the ring (a stage goes back to the producer through an `empty` mbarrier; bulk L2 prefetches run
+//     ahead of the shortened ring -- they cost 19 % extra DRAM reads, which is why LAG 1 does without);
 //   * the number of k-steps of step 2 follows p exactly (KQA = ceil(p / 4), not 2 NTA), and the -[k_l == m]
 //     term of Q is applied once by the service warps instead of by every warp in step 2;
-//   * optionally (PP) the two compute warps of an SM sub-partition take turns on the fp64 pipe.
+//   * optionally (PP, QMC_FLUSH_PP=1) the two compute warps of an SM sub-partition take turns on the fp64 pipe.
 template <int LAG, typename TB, int KPAD, int TW, int NWC, int CS, int STAGES>
 struct Ring2Smem {
     static constexpr int LDC = NWC * TW * 8, RP = LDC + 8, PS = KPAD + 4;
