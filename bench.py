@@ -41,7 +41,7 @@ UNIT = "moves/s"
 DEFAULT_DELAY = {"tiny": [0], "small": [16, 0], "mid": [16, 0], "large": [16, 0], "xlarge": [16, 32, 0]}
 # further arms reported as variants (fewer timed steps each): (delay rank, fp32-stored inverse)
 EXTRA_ARMS = {"large": [(16, True), (0, True), (20, False), (24, False), (32, False), (0, False, "drift"), (16, False, "updn"),
-                        (16, False, "jastrow")],
+                        (16, False, "jastrow"), (16, True, "aw")],
               "mid": [(16, True), (16, False, "updn")], "xlarge": [(16, True), (24, False)],
               # L2-resident configs: the sweep is launch-bound; the same sweep replayed from a CUDA graph
               "tiny": [(0, False, "graph")], "small": [(16, False, "graph"), (0, False, "graph")]}
@@ -245,6 +245,10 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--fp32-inverse", action="store_true", help="store the inverse in fp32 (QMC_DET_FP32_INVERSE)")
+    ap.add_argument("--accept-windows", action="store_true",
+                    help="with --delay <= 16: delayed windows close on an accept count (QMC_DET_ACCEPT_WINDOWS); the "
+                         "default run (no --delay) uses it for the headline arm of mid / large / xlarge and reports the "
+                         "step-count windows as a variant")
     ap.add_argument("--no-variants", action="store_true", help="skip the extra variant arms of the default run")
     ap.add_argument("--flush-micro", action="store_true",
                     help="time qmc_det_flush alone: windows filled through qmc_det_ratio / qmc_det_accept_update "
@@ -336,7 +340,7 @@ def main():
         accept = torch.zeros(unif.shape, dtype=torch.uint8, device=dev)
         ratios = torch.zeros(unif.shape, dtype=torch.float64, device=dev)
         t0 = time.perf_counter()
-        det = api.Det.init(spline, pos, delay_rank=delay, fp32_inverse=fp32)
+        det = api.Det.init(spline, pos, delay_rank=delay, fp32_inverse=fp32, accept_windows=(mode == "aw"))
         torch.cuda.synchronize()
         t_init = time.perf_counter() - t0
 
@@ -426,10 +430,15 @@ def main():
         # ---- roofline of the dominant kernel (rank-local, from the per-launch CUDA events)
         ld, npitch, K, eb = det.ld, spline.row_pitch, det.delay_rank, det.storage_bytes
         per_launch = {   # algorithmic bytes per launch; eb = bytes per stored element of B
-            "spo_vgl": (nprof * nmoved * nw * (2 if drift_tau else 1) / max(prof["spo_vgl"][1], 1)) * (64 + 5) * npitch * 4,
+            # (accept windows: every open window evaluates K + K/2 proposals of its walker, used or not)
+            "spo_vgl": ((n_acc / max(K, 1) + 0.5 * nw * nprof) * (K + K // 2) if mode == "aw"
+                        else nprof * nmoved * nw * (2 if drift_tau else 1)) / max(prof["spo_vgl"][1], 1) * (64 + 5) * npitch * 4,
             "ratio_rowcopy": nw * ((eb + 8) * ld + 4 * nel) * (0.75 if drift_tau else 1.0),   # drift: averaged with the propose kernel
             "sm_update": (n_acc / max(prof["sm_update"][1], 1)) * (2 * eb * nel * ld + 12 * nel),
-            "delayed_flush": nw * 2 * eb * nel * ld + (n_acc / max(prof["delayed_flush"][1], 1)) * (8 * ld + 4 * npitch),
+            # (accept windows: a launch serves the walkers that still have moves to apply -- about n_acc / K
+            #  full windows plus one partial window per walker and sweep in all)
+            "delayed_flush": ((n_acc / max(K, 1) + 0.5 * nw * nprof) / max(prof["delayed_flush"][1], 1) if mode == "aw" else nw)
+                             * 2 * eb * nel * ld + (n_acc / max(prof["delayed_flush"][1], 1)) * (8 * ld + 4 * npitch),
             # window: K rows of B0 and K vectors in, R' rows out
             "delayed_window": nw * max(K, 1) * (eb * ld + 4 * npitch) + (n_acc / max(prof["delayed_window"][1], 1)) * 8 * ld,
         }
@@ -472,7 +481,7 @@ def main():
         # ---- end to end through the C ABI with HOST buffers (pinned): H2D of pos/delta/unif and D2H
         #      of pos/ratios/decisions inside the timed region, every step
         e2e = None
-        if mode is None:
+        if mode in (None, "aw"):
             pos_h = pos.cpu().pin_memory()
             ratios_h = torch.zeros(unif_h.shape, dtype=torch.float64).pin_memory()
             accept_h = torch.zeros(unif_h.shape, dtype=torch.uint8).pin_memory()
@@ -503,6 +512,8 @@ def main():
             jas.destroy()
         if mode == "graph":
             update += ", sweep replayed from a CUDA graph (api.SweepGraph)"
+        if mode == "aw":
+            update += f", windows closed on {K} accepted moves (QMC_DET_ACCEPT_WINDOWS)"
         if mode == "updn":
             update += f", D_up D_dn: 2 x {nel} electrons per walker (eq. 26)"
             wf.destroy()
@@ -523,7 +534,16 @@ def main():
                + ("exceeds the 126 MB L2; no flush needed" if ws_table + ws_binv > 0.5 else
                   "fits L2: numbers are L2-resident, not HBM rooflines"))
     delays = [args.delay] if args.delay >= 0 else DEFAULT_DELAY.get(args.config, [0])
-    arms = [run_arm(dl, fp32=args.fp32_inverse) for dl in dict.fromkeys(delays)]
+    # the headline arm of the HBM-resident configs closes its windows on 16 ACCEPTED moves (same result; every
+    # flush then applies a full window); the step-count windows of round 1 are reported beside it
+    aw_default = args.delay < 0 and not args.fp32_inverse and args.config in ("mid", "large", "xlarge")
+    def arm_mode(i, dl):
+        if 2 <= dl <= 16 and (args.accept_windows or (aw_default and i == 0)):
+            return "aw"
+        return None
+    arms = [run_arm(dl, fp32=args.fp32_inverse, mode=arm_mode(i, dl)) for i, dl in enumerate(dict.fromkeys(delays))]
+    if aw_default and not args.no_variants:
+        arms.append(run_arm(16, steps=10))
     if args.delay < 0 and not args.fp32_inverse and not args.no_variants:
         arms += [run_arm(a[0], fp32=a[1], mode=a[2] if len(a) > 2 else None, steps=5) for a in EXTRA_ARMS.get(args.config, [])]
     main_arm = arms[0]

@@ -28,6 +28,7 @@ EXPORTS = [
     "qmc_jastrow_create", "qmc_jastrow_destroy", "qmc_jastrow_ratio", "qmc_jastrow_value", "qmc_probe_fp64_pipe",
 ]
 QMC_DET_FP32_INVERSE = 1
+QMC_DET_ACCEPT_WINDOWS = 2
 PROF_KINDS = ["spo_vgl", "sm_update", "delayed_window", "delayed_accept", "delayed_flush", "ratio_rowcopy"]
 
 
@@ -230,14 +231,16 @@ class Det:
         self.storage_bytes = a.value            # 8: fp64 inverse, 4: fp32-stored inverse
 
     @classmethod
-    def init(cls, spline, pos, delay_rank=0, fp32_inverse=False, stream=None):
-        """qmc_det_init / qmc_det_init_ex: pos double [nw][nel][3] on the device."""
+    def init(cls, spline, pos, delay_rank=0, fp32_inverse=False, accept_windows=False, stream=None):
+        """qmc_det_init / qmc_det_init_ex: pos double [nw][nel][3] on the device.  accept_windows: delayed windows
+        close on delay_rank ACCEPTED moves (QMC_DET_ACCEPT_WINDOWS)."""
         lib = load_library()
         nw, nel, _ = pos.shape
         h = _vp()
-        if fp32_inverse:
+        flags = (QMC_DET_FP32_INVERSE if fp32_inverse else 0) | (QMC_DET_ACCEPT_WINDOWS if accept_windows else 0)
+        if flags:
             rc = lib.qmc_det_init_ex(ctypes.byref(h), spline._h, nw, nel, _dev(pos, torch.float64), int(delay_rank),
-                                     QMC_DET_FP32_INVERSE, _stream(stream))
+                                     flags, _stream(stream))
         else:
             rc = lib.qmc_det_init(ctypes.byref(h), spline._h, nw, nel, _dev(pos, torch.float64), int(delay_rank),
                                   _stream(stream))

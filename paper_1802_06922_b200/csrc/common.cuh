@@ -111,6 +111,9 @@ struct qmc_det {
     size_t win_vec_wstride, win_vec_sstride;   // its walker and slot strides (floats)
     double *win_sinv;           // [nw][delay][delay] inverse of S
     int *win_full;              // [1] set when any walker's window is full
+    int accept_windows;         // QMC_DET_ACCEPT_WINDOWS: windows close on delay accepted moves; spo_batch = steps per window
+    int *cur;                   // [nw] electron cursor of every walker within the current sweep (accept_windows)
+    int win_kend;               // end of the electron range of the sweep in progress (accept_windows)
     int host_pending;           // electron steps appended to the open window (host bookkeeping)
     unsigned char *win_host_iel;   // host [nel]: electrons touched in the open window
     double *kin_lap;            // [nw][nel] scratch of qmc_det_kinetic (allocated on first use)

@@ -7,7 +7,7 @@ namespace qmc {
 // SPO-VGL of electrons iel0 .. iel0+nb-1 of every walker at pos + delta (delta NULL: at pos) into `out`
 // ([nb][nw][5][np], e.g. d->vgl) (sweep.cu); nb <= d->spo_batch.
 int spo_batch_vgl(qmc_det *d, const qmc_spline *sp, const double *pos, const double *delta, int iel0, int nb,
-                  float *phi_record, int nrecord, float *out, cudaStream_t s);
+                  float *phi_record, int nrecord, float *out, cudaStream_t s, bool per_walker_cursor = false);
 
 int delayed_ratio(qmc_det *d, int iel, const float *phi, int ldo, double *ratio, cudaStream_t s);
 int delayed_accept(qmc_det *d, int iel, const float *phi, int ldo, const double *ratio,

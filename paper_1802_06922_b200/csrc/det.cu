@@ -272,7 +272,7 @@ static void det_free(qmc_det *d)
     }
     if (d->vgl_buf[1]) cudaFree(d->vgl_buf[1]);
     d->vgl = d->vgl_buf[0] ? d->vgl_buf[0] : d->vgl;
-    cudaFree(d->vgl_cur); cudaFree(d->rprop); cudaFree(d->fcur); cudaFree(d->tfac); cudaFree(d->jas_dj);
+    cudaFree(d->cur); cudaFree(d->vgl_cur); cudaFree(d->rprop); cudaFree(d->fcur); cudaFree(d->tfac); cudaFree(d->jas_dj);
     cudaFree(d->B); cudaFree(d->Bf); cudaFree(d->logdet); cudaFree(d->sign); cudaFree(d->naccept);
     cudaFree(d->vgl); cudaFree(d->rowk); cudaFree(d->ratio); cudaFree(d->acc);
     cudaFree(d->win_count); cudaFree(d->win_iel); cudaFree(d->win_slot); cudaFree(d->win_phi); cudaFree(d->win_rows);
@@ -378,7 +378,9 @@ extern "C" int qmc_det_init_ex(qmc_det_t **out, const qmc_spline_t *sp, int nw, 
 {
     QMC_REQUIRE(out && sp && pos, "qmc_det_init: NULL argument");
     *out = nullptr;
-    QMC_REQUIRE((flags & ~(unsigned)QMC_DET_FP32_INVERSE) == 0, "qmc_det_init_ex: unknown flags 0x%x", flags);
+    QMC_REQUIRE((flags & ~(unsigned)(QMC_DET_FP32_INVERSE | QMC_DET_ACCEPT_WINDOWS)) == 0, "qmc_det_init_ex: unknown flags 0x%x", flags);
+    QMC_REQUIRE(!(flags & QMC_DET_ACCEPT_WINDOWS) || (delay_rank >= 2 && delay_rank <= 16),
+                "qmc_det_init_ex: QMC_DET_ACCEPT_WINDOWS needs 2 <= delay_rank <= 16 (got %d)", delay_rank);
     QMC_REQUIRE(nw >= 1, "qmc_det_init: nwalkers=%d", nw);
     QMC_REQUIRE(nel == sp->view.norb, "qmc_det_init: nel=%d must equal the spline's norb=%d", nel, sp->view.norb);
     QMC_REQUIRE(nel <= kMaxNel, "qmc_det_init: nel=%d exceeds the supported maximum %d", nel, kMaxNel);
@@ -394,6 +396,8 @@ extern "C" int qmc_det_init_ex(qmc_det_t **out, const qmc_spline_t *sp, int nw, 
     d->nw = nw; d->nel = nel; d->ld = update_ld(nel); d->np = sp->view.np;
     d->delay = delay_rank <= 1 ? 0 : delay_rank;
     d->spo_batch = d->delay ? d->delay : kSpoBatch;
+    d->accept_windows = (flags & QMC_DET_ACCEPT_WINDOWS) ? 1 : 0;
+    if (d->accept_windows) d->spo_batch = d->delay + d->delay / 2;      // steps a window may take to collect `delay` accepts
     d->b32 = (flags & QMC_DET_FP32_INVERSE) ? 1 : 0;
     const int ld = d->ld, np = d->np, K = d->delay;
     int rc;
@@ -428,7 +432,8 @@ extern "C" int qmc_det_init_ex(qmc_det_t **out, const qmc_spline_t *sp, int nw, 
             (rc = dev_alloc(&d->win_slot, (size_t)nw * K, "win_slot")) ||
             (rc = dev_alloc(&d->win_phi, (size_t)nw * K * np, "win_phi")) ||
             (rc = dev_alloc(&d->win_rows, (size_t)nw * K * ld, "win_rows")) ||
-            (rc = dev_alloc(&d->win_sinv, (size_t)nw * K * K, "win_sinv")) || (rc = dev_alloc(&d->win_full, 1, "win_full"))) {
+            (rc = dev_alloc(&d->win_sinv, (size_t)nw * K * K, "win_sinv")) || (rc = dev_alloc(&d->win_full, 1, "win_full")) ||
+            (d->accept_windows && (rc = dev_alloc(&d->cur, nw, "cur")))) {
             det_free(d);
             return rc;
         }

@@ -17,6 +17,12 @@ int jastrow_move_launch(const qmc_jastrow *J, int nw, int nel, const double *pos
                         int iel0, int nb, const double *delta, const double *rnew, double *dj_out, double *ratio_out,
                         double *tfac_out, double *corr_out, int ncorr, cudaStream_t s);
 
+__global__ void fill_int_kernel(int *p, int n, int v)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) p[i] = v;
+}
+
 // Jastrow factor of a sweep (qmc_sweep_opts_t.jastrow): what the step loops need.
 struct SweepJastrow {
     const qmc_jastrow *J;     // NULL: none
@@ -37,6 +43,10 @@ struct SpoBatchArgs {
     float *vgl;            // [nb][nw][5][np]
     float *phi_record;     // [nb][nrecord][nel_record], offset to (sweep, first electron), or NULL
     int nrecord, nel_record;
+    // QMC_DET_ACCEPT_WINDOWS: every walker is at its own electron; step j of the batch is electron cur[w] + j
+    // (nothing to do beyond kend), delta and phi_record are then offset to (sweep, electron 0)
+    const int *cur;
+    int kend;
 };
 
 // One block per (orbital tile, walker, step of the batch).  Thread t owns orbitals 4t..4t+3 of the
@@ -45,10 +55,13 @@ __global__ void __launch_bounds__(256) spo_batch_kernel(SpoBatchArgs a)
 {
     __shared__ StencilSmem st;
     const int w = blockIdx.y, j = blockIdx.z;
-    const double *r = a.pos + ((size_t)w * a.nel + a.iel0 + j) * 3;
+    const int iel = a.cur ? a.cur[w] + j : a.iel0 + j;
+    if (a.cur && iel >= a.kend) return;                    // this walker's sweep ends before step j (block-uniform)
+    const int jd = a.cur ? iel : j;                        // index into delta / phi_record
+    const double *r = a.pos + ((size_t)w * a.nel + iel) * 3;
     double dx = 0.0, dy = 0.0, dz = 0.0;
     if (a.delta) {
-        const double *dl = a.delta + 3 * ((size_t)j * a.nw + w);
+        const double *dl = a.delta + 3 * ((size_t)jd * a.nw + w);
         dx = dl[0]; dy = dl[1]; dz = dl[2];
     }
     stage_stencil(a.sp, r[0] + dx, r[1] + dy, r[2] + dz, st);
@@ -64,7 +77,7 @@ __global__ void __launch_bounds__(256) spo_batch_kernel(SpoBatchArgs a)
     *reinterpret_cast<float4 *>(o + 3 * (size_t)np) = gz;
     *reinterpret_cast<float4 *>(o + 4 * (size_t)np) = lp;
     if (a.phi_record && w < a.nrecord) {
-        float *rec = a.phi_record + ((size_t)j * a.nrecord + w) * a.nel_record;
+        float *rec = a.phi_record + ((size_t)jd * a.nrecord + w) * a.nel_record;
         if (col + 0 < a.nel_record) rec[col + 0] = v.x;
         if (col + 1 < a.nel_record) rec[col + 1] = v.y;
         if (col + 2 < a.nel_record) rec[col + 2] = v.z;
@@ -179,7 +192,7 @@ ratio_rowcopy_kernel(const TB *__restrict__ B, int nel, int ld, int iel, const f
 }
 
 int spo_batch_vgl(qmc_det *d, const qmc_spline *sp, const double *pos, const double *delta, int iel0, int nb,
-                  float *phi_record, int nrecord, float *out, cudaStream_t s)
+                  float *phi_record, int nrecord, float *out, cudaStream_t s, bool per_walker_cursor)
 {
     int threads, tiles;
     spo_launch_shape(d->np, &threads, &tiles);
@@ -189,6 +202,7 @@ int spo_batch_vgl(qmc_det *d, const qmc_spline *sp, const double *pos, const dou
     a.nel = d->nel; a.iel0 = iel0; a.nw = d->nw;
     a.vgl = out;
     a.phi_record = phi_record; a.nrecord = nrecord; a.nel_record = d->nel;
+    if (per_walker_cursor) { a.cur = d->cur; a.kend = d->win_kend; }
     prof_start(d, kProfSpoRatio, s);
     spo_batch_kernel<<<dim3(tiles, d->nw, nb), threads, 0, s>>>(a);
     prof_stop(d, s);
@@ -211,7 +225,11 @@ static int sweep_delayed(qmc_det *d, const qmc_spline *sp, double *pos, const do
                          const SweepJastrow &jas, cudaStream_t s)
 {
     const int nw = d->nw, nel = d->nel, batch = d->spo_batch;
-    const int wins_per_sweep = (kn + batch - 1) / batch;
+    const bool aw = d->accept_windows != 0;
+    // accept windows: a window takes at least min(delay, remaining) steps of every walker, so ceil(kn / delay)
+    // windows always finish the sweep (the last ones find most walkers done: their CTAs exit at once)
+    const int wins_per_sweep = aw ? (kn + d->delay - 1) / d->delay : (kn + batch - 1) / batch;
+    if (aw) d->win_kend = k0 + kn;
     const long long nwin = (long long)nsweeps * wins_per_sweep;
     if (nwin == 0) return QMC_OK;
     bool overlap = d->overlap && !d->prof_on;     // per-kernel event timing needs the kernels one after another
@@ -222,13 +240,25 @@ static int sweep_delayed(qmc_det *d, const qmc_spline *sp, double *pos, const do
         QMC_CUDA(cudaEventCreateWithFlags(&d->ev_main, cudaEventDisableTiming));
     }
     auto spo = [&](long long i, cudaStream_t st) -> int {     // K1 of window i into buffer i & 1
-        const int sw = (int)(i / wins_per_sweep), k = k0 + (int)(i % wins_per_sweep) * batch;
+        const int sw = (int)(i / wins_per_sweep);
+        if (aw) {                                             // every walker from its own cursor; arrays offset to the sweep
+            const size_t mv0 = (size_t)sw * nel * nw;
+            return spo_batch_vgl(d, sp, pos, delta + 3 * mv0, 0, batch, rec ? rec + mv0 / nw * (size_t)nrec * nel : nullptr,
+                                 nrec, d->vgl_buf[overlap ? (i & 1) : 0], st, true);
+        }
+        const int k = k0 + (int)(i % wins_per_sweep) * batch;
         const int nb = min(batch, k0 + kn - k);
         const size_t mv = ((size_t)sw * nel + k) * nw;
         return spo_batch_vgl(d, sp, pos, delta + 3 * mv, k, nb, rec ? rec + mv / nw * (size_t)nrec * nel : nullptr,
-                             nrec, d->vgl_buf[overlap ? (i & 1) : 0], st);
+                             nrec, d->vgl_buf[overlap ? (i & 1) : 0], st, false);
+    };
+    auto reset_cursors = [&]() -> int {                       // start of a sweep: every walker at electron k0
+        fill_int_kernel<<<(nw + 127) / 128, 128, 0, s>>>(d->cur, nw, k0);
+        QMC_LAUNCHED();
+        return QMC_OK;
     };
     int rc;
+    if (aw && (rc = reset_cursors())) return rc;
     if (overlap) {
         QMC_CUDA(cudaEventRecord(d->ev_main, s));
         QMC_CUDA(cudaStreamWaitEvent(d->aux, d->ev_main, 0));
@@ -236,8 +266,10 @@ static int sweep_delayed(qmc_det *d, const qmc_spline *sp, double *pos, const do
         QMC_CUDA(cudaEventRecord(d->ev_spo[0], d->aux));
     }
     for (long long i = 0; i < nwin; ++i) {
-        const int sw = (int)(i / wins_per_sweep), k = k0 + (int)(i % wins_per_sweep) * batch;
-        const int nb = min(batch, k0 + kn - k);
+        const int sw = (int)(i / wins_per_sweep);
+        // accept windows: the per-move arrays are offset to the sweep and indexed with the walker's own electron
+        const int k = aw ? 0 : k0 + (int)(i % wins_per_sweep) * batch;
+        const int nb = aw ? batch : min(batch, k0 + kn - k);
         const size_t mv = ((size_t)sw * nel + k) * nw;
         if (overlap) QMC_CUDA(cudaStreamWaitEvent(s, d->ev_spo[i & 1], 0));
         else if ((rc = spo(i, s))) return rc;
@@ -256,6 +288,11 @@ static int sweep_delayed(qmc_det *d, const qmc_spline *sp, double *pos, const do
                                   accept_out ? accept_out + mv : nullptr, forced ? forced + mv : nullptr, fixed_node,
                                   force ? force + 3 * mv : nullptr, overlap && i + 1 < nwin ? 1 : 0, wj, s);
         if (rc) return rc;
+        if (aw && i + 1 < nwin && (i + 1) % wins_per_sweep == 0) {
+            // next window starts a new sweep: cursors back to k0 (after this window's kernel, before the next SPO)
+            if ((rc = reset_cursors())) return rc;
+            if (overlap) QMC_CUDA(cudaEventRecord(d->ev_main, s));
+        }
         if (overlap && i + 1 < nwin) {
             // (delayed_sweep_window recorded ev_main between its window kernel and its flush)
             QMC_CUDA(cudaStreamWaitEvent(d->aux, d->ev_main, 0));
@@ -309,7 +346,7 @@ static int sweep_drift(qmc_det *d, const qmc_spline *sp, double *pos, const doub
             const int slot = (k - k0) % kSpoBatch;
             if (slot == 0) {          // gradients at the current positions of the next 16 electrons
                 const int nb = min(kSpoBatch, k0 + kn - k);
-                int rc = spo_batch_vgl(d, sp, pos, nullptr, k, nb, nullptr, 0, d->vgl_cur, s);
+                int rc = spo_batch_vgl(d, sp, pos, nullptr, k, nb, nullptr, 0, d->vgl_cur, s, false);
                 if (rc) return rc;
             }
             double *rprop = rprop_out ? rprop_out + 3 * mv : d->rprop;
@@ -390,6 +427,7 @@ static int sweep_impl(qmc_det *d, const qmc_spline *sp, double *pos, const doubl
         jas.jratio_out = opts->jratio_out;
         QMC_REQUIRE(jas.nother >= 0 && (jas.nother == 0 || jas.other), "qmc_sweep_ex: jastrow_nother=%d without positions", jas.nother);
         QMC_REQUIRE(jas.J->device == d->device, "qmc_sweep_ex: the Jastrow factor lives on another device");
+        QMC_REQUIRE(!d->accept_windows, "qmc_sweep_ex: a Jastrow factor is not supported with QMC_DET_ACCEPT_WINDOWS");
         if (!d->jas_dj) {
             const size_t kk = d->delay > 1 ? d->delay : 1;       // dJ [K][nw] + pair terms [nw][K][K]
             const size_t bytes = (kk * nw + (size_t)nw * kk * kk) * sizeof(double);
@@ -406,7 +444,7 @@ static int sweep_impl(qmc_det *d, const qmc_spline *sp, double *pos, const doubl
             if (slot == 0) {          // K1: SPO-VGL of the next `nb` electron steps, all walkers
                 const int nb = min(batch, k0 + kn - k);
                 int rc = spo_batch_vgl(d, sp, pos, delta + 3 * mv, k, nb,
-                                       rec ? rec + mv / nw * (size_t)nrec * nel : nullptr, nrec, d->vgl, s);
+                                       rec ? rec + mv / nw * (size_t)nrec * nel : nullptr, nrec, d->vgl, s, false);
                 if (rc) return rc;
             }
             const float *phi = d->vgl + slot * slot_stride;

@@ -45,6 +45,10 @@ struct WindowArgs {
     int *win_slot;                // [nw][K]
     double *win_rows;             // [nw][K][ld]   row l <- R'[l]
     WindowJastrow jas;            // base == NULL: no Jastrow factor
+    // QMC_DET_ACCEPT_WINDOWS: the walker's window starts at electron cur[w], ends before kend, and closes when
+    // pmax moves have been accepted; the per-move arrays are then offset to (sweep, electron 0)
+    int *cur;
+    int kend, pmax;
 };
 
 // G[i][j] = x_i . B0[iel0 + j] for the nb vectors x_i = x0 + i * vstep (fp32) of one walker, into
@@ -121,10 +125,17 @@ __global__ void __launch_bounds__(kWinThreads, (FORCE || KMAX > 16) ? 1 : 4) del
     __shared__ long long rowoff_s[KMAX];
     __shared__ int p_s;
     const int w = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int nb = a.nb, ld = a.ld, np = a.np, K = a.K;
+    const int iel0 = a.cur ? a.cur[w] : a.iel0;            // first electron of this walker's window
+    const int ebase = a.cur ? iel0 : 0;                    // index of step 0 in the per-move arrays
+    const int nb = a.cur ? min(a.nb, a.kend - iel0) : a.nb;
+    const int ld = a.ld, np = a.np, K = a.K;
+    if (nb <= 0) {                                         // this walker has finished its sweep (block-uniform)
+        if (tid == 0) a.win_count[w] = 0;
+        return;
+    }
     const size_t vstep = (size_t)a.nw * 5 * np;             // stride between steps in vgl
     const float *v0 = a.vgl + (size_t)w * 5 * np;
-    const TB *b0 = reinterpret_cast<const TB *>(a.B) + ((size_t)w * a.nel + a.iel0) * ld;
+    const TB *b0 = reinterpret_cast<const TB *>(a.B) + ((size_t)w * a.nel + iel0) * ld;
 
     window_contract<KMAX, TB>(v0, vstep, b0, nb, ld, np, G_s);
     if (FORCE)
@@ -135,7 +146,7 @@ __global__ void __launch_bounds__(kWinThreads, (FORCE || KMAX > 16) ? 1 : 4) del
     // uniform / forced decision of step i before it and writes ratio, decision and the moved
     // position of step i after it, so a step costs shuffles, shared memory and fp64 arithmetic only.
     if (warp == 0) {
-        const size_t mv_l = (size_t)lane * a.nw + w;                  // move of step `lane`
+        const size_t mv_l = (size_t)(ebase + lane) * a.nw + w;        // move of step `lane`
         const bool step_l = lane < nb;
         const double u_l = (step_l && !a.forced) ? a.unif[mv_l] : 0.0;
         const int f_l = (step_l && a.forced) ? (a.forced[mv_l] != 0) : 0;
@@ -148,7 +159,9 @@ __global__ void __launch_bounds__(kWinThreads, (FORCE || KMAX > 16) ? 1 : 4) del
         const double *corr_w = jas ? a.jas.corr + (size_t)w * K * K : nullptr;
         unsigned acc_mask = 0;                                        // accepted steps (same in every lane)
         int p = 0, mine = 0;
+        int nproc = nb;                                               // steps this window really takes
         for (int i = 0; i < nb; ++i) {
+            if (p == a.pmax) { nproc = i; break; }                    // the window is full (accept windows; warp-uniform)
             const double c = lane < p ? G_s[mine * GS + i] : 0.0;     // c_m = v_{l_m} . B0[k_i]
             const double x = lane < p ? G_s[i * GS + mine] : 0.0;     // x_m = v_i . B0[k_{l_m}]
             double y = 0.0, z = 0.0;                                  // y = S^-1 c, z = S^-T x
@@ -200,9 +213,10 @@ __global__ void __launch_bounds__(kWinThreads, (FORCE || KMAX > 16) ? 1 : 4) del
             ++p;
             __syncwarp();
         }
-        // results of step `lane`
-        const bool acc_l = step_l && ((acc_mask >> lane) & 1u);
-        if (step_l) {
+        // results of step `lane` (only the steps the window took)
+        const bool done_l = lane < nproc;
+        const bool acc_l = done_l && ((acc_mask >> lane) & 1u);
+        if (done_l) {
             if (a.ratios_out) a.ratios_out[mv_l] = R_l;
             if (a.accept_out) a.accept_out[mv_l] = acc_l ? 1 : 0;
             if (jas && a.jas.jratio_out) a.jas.jratio_out[mv_l] = jr_l;
@@ -213,7 +227,7 @@ __global__ void __launch_bounds__(kWinThreads, (FORCE || KMAX > 16) ? 1 : 4) del
             }
         }
         if (acc_l) {
-            double *r = a.pos + ((size_t)w * a.nel + a.iel0 + lane) * 3;
+            double *r = a.pos + ((size_t)w * a.nel + iel0 + lane) * 3;
             r[0] += a.delta[3 * mv_l + 0];
             r[1] += a.delta[3 * mv_l + 1];
             r[2] += a.delta[3 * mv_l + 2];
@@ -221,6 +235,7 @@ __global__ void __launch_bounds__(kWinThreads, (FORCE || KMAX > 16) ? 1 : 4) del
         const double logdet_add = warp_sum(acc_l ? log(fabs(R_l)) : 0.0);     // fixed (butterfly) order
         const unsigned neg = __ballot_sync(0xffffffffu, acc_l && R_l < 0.0);
         if (lane == 0) {
+            if (a.cur) a.cur[w] = iel0 + nproc;
             a.win_count[w] = p;
             p_s = p;
             if (p) {
@@ -230,7 +245,7 @@ __global__ void __launch_bounds__(kWinThreads, (FORCE || KMAX > 16) ? 1 : 4) del
             }
         }
         if (lane < p) {
-            a.win_iel[(size_t)w * K + lane] = a.iel0 + mine;
+            a.win_iel[(size_t)w * K + lane] = iel0 + mine;
             a.win_slot[(size_t)w * K + lane] = mine;
             rowoff_s[lane] = (long long)mine * ld;
         }
@@ -262,13 +277,16 @@ int delayed_sweep_window(qmc_det *d, double *pos, const double *delta, const dou
     a.win_count = d->win_count; a.win_iel = d->win_iel; a.win_slot = d->win_slot;
     a.win_rows = d->win_rows;
     a.jas = jas;
+    a.pmax = d->delay;
+    if (d->accept_windows) { a.cur = d->cur; a.kend = d->win_kend; }
+    const int kwin = d->accept_windows ? d->spo_batch : a.K;     // steps per window: what the G matrix must hold
     prof_start(d, kProfDelayedRatio, s);
 #define QMC_WIN_LAUNCH(TB, KM, F, J) delayed_window_kernel<TB, KM, F, J><<<d->nw, kWinThreads, 0, s>>>(a)
 #define QMC_WIN_RANK(TB, F, J)                               \
     do {                                                     \
-        if (a.K <= 8) QMC_WIN_LAUNCH(TB, 8, F, J);           \
-        else if (a.K <= 16) QMC_WIN_LAUNCH(TB, 16, F, J);    \
-        else if (a.K <= 24) QMC_WIN_LAUNCH(TB, 24, F, J);    \
+        if (kwin <= 8) QMC_WIN_LAUNCH(TB, 8, F, J);          \
+        else if (kwin <= 16) QMC_WIN_LAUNCH(TB, 16, F, J);   \
+        else if (kwin <= 24) QMC_WIN_LAUNCH(TB, 24, F, J);   \
         else QMC_WIN_LAUNCH(TB, 32, F, J);                   \
     } while (0)
 #define QMC_WIN_JAS(TB, F)                                   \

@@ -94,7 +94,7 @@ def compare_decisions(acc_g, R_g, acc_o, R_o, unif, tol=None):
     return ndiverged
 
 
-def run_protocol(x, delay_rank=0, walkers=None, free_oracle=True, coefs_np=None):
+def run_protocol(x, delay_rank=0, walkers=None, free_oracle=True, coefs_np=None, accept_windows=False):
     """Parity protocol on inputs x (tests/conftest shapes).  Returns a dict of measured errors.
 
     walkers: None = all walkers are replayed by the oracle; else the first `walkers` of them
@@ -111,7 +111,7 @@ def run_protocol(x, delay_rank=0, walkers=None, free_oracle=True, coefs_np=None)
 
     # GPU free run, recording ratios, decisions and the fp32 orbital vectors of the checked walkers
     A0_g = gpu_slater(spline, pos0)[:nchk]
-    det = api.Det.init(spline, pos0, delay_rank=delay_rank)
+    det = api.Det.init(spline, pos0, delay_rank=delay_rank, accept_windows=accept_windows)
     B0_g = det.get_inverse().cpu().numpy()[:nchk]
     ld0_g, sg0_g, _ = (t.cpu().numpy() for t in det.get_stats())
     pos_g = pos0.clone()

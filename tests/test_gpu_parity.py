@@ -978,3 +978,58 @@ def test_sweep_graph_replay_is_bitwise_the_eager_sweep(case, K):
         assert np.array_equal(a_, b_)
     assert out[0][3][1:].mean() > 0.05
     spline.destroy()
+
+
+# --------------------------------------------- windows that close on an accept count (QMC_DET_ACCEPT_WINDOWS)
+@pytest.mark.parametrize("case,K", [("tiny", 4), ("ragged37_skew", 4), ("ragged37_skew", 16), ("n130_two_tiles", 7),
+                                    ("small", 16)])
+def test_accept_windows_parity_protocol(case, K):
+    """QMC_DET_ACCEPT_WINDOWS: every walker closes its window after K accepted moves (per-walker electron
+    cursors, no lockstep over the electrons).  Which moves share a window does not change the result: the
+    full parity protocol against the oracle (identical vectors, end to end) applies unchanged."""
+    x = CASES[case]()
+    out = P.run_protocol(x, delay_rank=K, coefs_np=x.coefs_numpy(), accept_windows=True)
+    print(case, K, "accept windows", out)
+    assert 0.0 < out["accept_rate"] < 1.0
+
+
+@pytest.mark.parametrize("nel,K,nw,count,fp32", [(512, 16, 5, 0, False), (1000, 16, 4, 0, False), (1024, 16, 4, 0, False),
+                                                 (2048, 16, 2, 300, False), (1024, 12, 3, 0, False), (1024, 16, 3, 0, True)])
+def test_accept_windows_equal_rank1_large_n(nel, K, nw, count, fp32):
+    """The same at N >= 512 (ring flush shapes) against the rank-1 path on the GPU: decisions and positions
+    bitwise, ratios and inverse to rounding; multiple sweeps (cursor reset), a partial electron range, forced
+    decisions and the fixed-node rule."""
+    cfg = inputs.custom_config(f"aw{nel}", (24, 24, 24), nel, (9.0, 8.5, 9.5), nw=nw, nsweeps=2, sigma=0.3)
+    x = inputs.make_inputs(cfg, device=P.dev())
+    spline = api.Spline.create(x.coefs, x.lattice)
+    pos0, delta, unif = P.to_dev(x.pos), P.to_dev(x.delta), P.to_dev(x.unif)
+    res = {}
+    for mode in ("rank1", "aw"):
+        det = api.Det.init(spline, pos0, delay_rank=0 if mode == "rank1" else K, fp32_inverse=fp32,
+                           accept_windows=(mode == "aw"))
+        pos = pos0.clone()
+        R = torch.zeros_like(unif)
+        acc = torch.zeros(unif.shape, dtype=torch.uint8, device=P.dev())
+        api.sweep(det, pos, delta, unif, ratios_out=R, accept_out=acc, iel_begin=5 if count else 0, iel_count=count,
+                  fixed_node=True)
+        res[mode] = (pos, R, acc, det.get_inverse(), det.get_stats())
+        if mode == "aw" and not fp32:
+            # forced replay of the same decisions reproduces the state bit for bit
+            det2 = api.Det.init(spline, pos0, delay_rank=K, accept_windows=True)
+            pos2 = pos0.clone()
+            api.sweep(det2, pos2, delta, unif, forced_accept=acc, iel_begin=5 if count else 0, iel_count=count)
+            assert torch.equal(pos2, pos) and torch.equal(det2.get_inverse(), res[mode][3])
+            det2.destroy()
+        det.destroy()
+    a, b = res["rank1"], res["aw"]
+    if fp32:      # the two round at different points (per move / per window): compare loosely
+        assert float((a[2] != b[2]).float().mean()) < 0.02
+    else:
+        assert torch.equal(a[2], b[2]) and torch.equal(a[0], b[0])
+        assert float((a[1] - b[1]).abs().max() / a[1].abs().max()) < 1e-10
+        assert float((a[3] - b[3]).abs().max()) < 1e-9 * float(a[3].abs().max())
+        assert float((a[4][0] - b[4][0]).abs().max()) < 1e-8
+        assert torch.equal(a[4][1], b[4][1]) and torch.equal(a[4][2], b[4][2])
+    with pytest.raises(api.QmcError):
+        api.Det.init(spline, pos0, delay_rank=24, accept_windows=True)
+    spline.destroy()
