@@ -112,7 +112,10 @@ struct qmc_det {
     double *win_sinv;           // [nw][delay][delay] inverse of S
     int *win_full;              // [1] set when any walker's window is full
     int accept_windows;         // QMC_DET_ACCEPT_WINDOWS: windows close on delay accepted moves; spo_batch = steps per window
-    int *cur;                   // [nw] electron cursor of every walker within the current sweep (accept_windows)
+    int *cur;                   // [2][nw] accept_windows: electron cursor of every walker within the current sweep, and
+                                //   (second half, `ev`) the electron up to which its proposals' SPO-VGL has been evaluated
+    int vgl_ring;               // accept_windows: the SPO-VGL scratch is a ring of this many slots (2 x spo_batch),
+                                //   slot = electron % ring: proposals a window did not reach are reused by the next
     int win_kend;               // end of the electron range of the sweep in progress (accept_windows)
     int host_pending;           // electron steps appended to the open window (host bookkeeping)
     unsigned char *win_host_iel;   // host [nel]: electrons touched in the open window

@@ -397,14 +397,18 @@ extern "C" int qmc_det_init_ex(qmc_det_t **out, const qmc_spline_t *sp, int nw, 
     d->delay = delay_rank <= 1 ? 0 : delay_rank;
     d->spo_batch = d->delay ? d->delay : kSpoBatch;
     d->accept_windows = (flags & QMC_DET_ACCEPT_WINDOWS) ? 1 : 0;
-    if (d->accept_windows) d->spo_batch = d->delay + d->delay / 2;      // steps a window may take to collect `delay` accepts
+    if (d->accept_windows) {
+        d->spo_batch = d->delay + d->delay / 2;      // steps a window may take to collect `delay` accepts
+        d->vgl_ring = 2 * d->spo_batch;
+    }
     d->b32 = (flags & QMC_DET_FP32_INVERSE) ? 1 : 0;
     const int ld = d->ld, np = d->np, K = d->delay;
     int rc;
     if ((rc = d->b32 ? dev_alloc(&d->Bf, (size_t)nw * nel * ld, "B (fp32)") : dev_alloc(&d->B, (size_t)nw * nel * ld, "B")) ||
         (rc = dev_alloc(&d->logdet, nw, "logdet")) ||
         (rc = dev_alloc(&d->sign, nw, "sign")) || (rc = dev_alloc(&d->naccept, nw, "naccept")) ||
-        (rc = dev_alloc(&d->vgl, (size_t)d->spo_batch * nw * 5 * np, "vgl")) || (rc = dev_alloc(&d->rowk, (size_t)nw * ld, "rowk")) ||
+        (rc = dev_alloc(&d->vgl, (size_t)(d->accept_windows ? d->vgl_ring : d->spo_batch) * nw * 5 * np, "vgl")) ||
+        (rc = dev_alloc(&d->rowk, (size_t)nw * ld, "rowk")) ||
         (rc = dev_alloc(&d->ratio, nw, "ratio")) ||
         (rc = dev_alloc(&d->acc, nw, "acc"))) {
         det_free(d);
@@ -414,7 +418,7 @@ extern "C" int qmc_det_init_ex(qmc_det_t **out, const qmc_spline_t *sp, int nw, 
     if (K) {
         const char *env = getenv("QMC_SWEEP_OVERLAP");      // A/B measurements: 0 keeps everything on one stream
         d->overlap = !(env && atoi(env) == 0);
-        if (d->overlap && (rc = dev_alloc(&d->vgl_buf[1], (size_t)d->spo_batch * nw * 5 * np, "vgl (second buffer)"))) {
+        if (d->overlap && !d->accept_windows && (rc = dev_alloc(&d->vgl_buf[1], (size_t)d->spo_batch * nw * 5 * np, "vgl (second buffer)"))) {
             det_free(d);
             return rc;
         }
@@ -433,7 +437,7 @@ extern "C" int qmc_det_init_ex(qmc_det_t **out, const qmc_spline_t *sp, int nw, 
             (rc = dev_alloc(&d->win_phi, (size_t)nw * K * np, "win_phi")) ||
             (rc = dev_alloc(&d->win_rows, (size_t)nw * K * ld, "win_rows")) ||
             (rc = dev_alloc(&d->win_sinv, (size_t)nw * K * K, "win_sinv")) || (rc = dev_alloc(&d->win_full, 1, "win_full")) ||
-            (d->accept_windows && (rc = dev_alloc(&d->cur, nw, "cur")))) {
+            (d->accept_windows && (rc = dev_alloc(&d->cur, (size_t)2 * nw, "cur")))) {
             det_free(d);
             return rc;
         }
@@ -442,7 +446,7 @@ extern "C" int qmc_det_init_ex(qmc_det_t **out, const qmc_spline_t *sp, int nw, 
         d->win_vec_sstride = (size_t)np;
     }
     cudaError_t e = cudaMemsetAsync(d->rowk, 0, (size_t)nw * ld * sizeof(double), s);
-    if (e == cudaSuccess) e = cudaMemsetAsync(d->vgl, 0, (size_t)d->spo_batch * nw * 5 * np * sizeof(float), s);
+    if (e == cudaSuccess) e = cudaMemsetAsync(d->vgl, 0, (size_t)(d->accept_windows ? d->vgl_ring : d->spo_batch) * nw * 5 * np * sizeof(float), s);
     if (e == cudaSuccess && d->vgl_buf[1]) e = cudaMemsetAsync(d->vgl_buf[1], 0, (size_t)d->spo_batch * nw * 5 * np * sizeof(float), s);
     if (e == cudaSuccess && K) e = cudaMemsetAsync(d->win_count, 0, (size_t)nw * sizeof(int), s);
     if (e == cudaSuccess && K) e = cudaMemsetAsync(d->win_full, 0, sizeof(int), s);

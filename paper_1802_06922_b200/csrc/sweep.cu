@@ -45,8 +45,10 @@ struct SpoBatchArgs {
     int nrecord, nel_record;
     // QMC_DET_ACCEPT_WINDOWS: every walker is at its own electron; step j of the batch is electron cur[w] + j
     // (nothing to do beyond kend), delta and phi_record are then offset to (sweep, electron 0)
-    const int *cur;
-    int kend;
+    // The SPO-VGL scratch is then a ring of `ring` slots (slot = electron % ring): only the proposals beyond
+    // ev[w] (those the previous windows did not evaluate yet) are evaluated, up to cur[w] + nb.
+    const int *cur, *ev;
+    int kend, ring, nb;
 };
 
 // One block per (orbital tile, walker, step of the batch).  Thread t owns orbitals 4t..4t+3 of the
@@ -55,9 +57,10 @@ __global__ void __launch_bounds__(256) spo_batch_kernel(SpoBatchArgs a)
 {
     __shared__ StencilSmem st;
     const int w = blockIdx.y, j = blockIdx.z;
-    const int iel = a.cur ? a.cur[w] + j : a.iel0 + j;
-    if (a.cur && iel >= a.kend) return;                    // this walker's sweep ends before step j (block-uniform)
+    const int iel = a.cur ? a.ev[w] + j : a.iel0 + j;
+    if (a.cur && iel >= min(a.cur[w] + a.nb, a.kend)) return;     // beyond this walker's next window (block-uniform)
     const int jd = a.cur ? iel : j;                        // index into delta / phi_record
+    const int slot = a.cur ? iel % a.ring : j;             // where the result goes in the scratch
     const double *r = a.pos + ((size_t)w * a.nel + iel) * 3;
     double dx = 0.0, dy = 0.0, dz = 0.0;
     if (a.delta) {
@@ -70,7 +73,7 @@ __global__ void __launch_bounds__(256) spo_batch_kernel(SpoBatchArgs a)
     if (col >= np) return;
     float4 v, gx, gy, gz, lp;
     gather4<true>(a.sp, st, col, v, gx, gy, gz, lp);
-    float *o = a.vgl + ((size_t)j * a.nw + w) * 5 * np + col;
+    float *o = a.vgl + ((size_t)slot * a.nw + w) * 5 * np + col;
     *reinterpret_cast<float4 *>(o) = v;
     *reinterpret_cast<float4 *>(o + np) = gx;
     *reinterpret_cast<float4 *>(o + 2 * (size_t)np) = gy;
@@ -202,7 +205,7 @@ int spo_batch_vgl(qmc_det *d, const qmc_spline *sp, const double *pos, const dou
     a.nel = d->nel; a.iel0 = iel0; a.nw = d->nw;
     a.vgl = out;
     a.phi_record = phi_record; a.nrecord = nrecord; a.nel_record = d->nel;
-    if (per_walker_cursor) { a.cur = d->cur; a.kend = d->win_kend; }
+    if (per_walker_cursor) { a.cur = d->cur; a.ev = d->cur + d->nw; a.kend = d->win_kend; a.ring = d->vgl_ring; a.nb = nb; }
     prof_start(d, kProfSpoRatio, s);
     spo_batch_kernel<<<dim3(tiles, d->nw, nb), threads, 0, s>>>(a);
     prof_stop(d, s);
@@ -233,6 +236,7 @@ static int sweep_delayed(qmc_det *d, const qmc_spline *sp, double *pos, const do
     const long long nwin = (long long)nsweeps * wins_per_sweep;
     if (nwin == 0) return QMC_OK;
     bool overlap = d->overlap && !d->prof_on;     // per-kernel event timing needs the kernels one after another
+    auto vbuf = [&](long long i) { return d->vgl_buf[(overlap && !aw) ? (i & 1) : 0]; };   // accept windows: one ring
     if (overlap && !d->aux) {
         QMC_CUDA(cudaStreamCreateWithFlags(&d->aux, cudaStreamNonBlocking));
         QMC_CUDA(cudaEventCreateWithFlags(&d->ev_spo[0], cudaEventDisableTiming));
@@ -244,16 +248,16 @@ static int sweep_delayed(qmc_det *d, const qmc_spline *sp, double *pos, const do
         if (aw) {                                             // every walker from its own cursor; arrays offset to the sweep
             const size_t mv0 = (size_t)sw * nel * nw;
             return spo_batch_vgl(d, sp, pos, delta + 3 * mv0, 0, batch, rec ? rec + mv0 / nw * (size_t)nrec * nel : nullptr,
-                                 nrec, d->vgl_buf[overlap ? (i & 1) : 0], st, true);
+                                 nrec, vbuf(i), st, true);
         }
         const int k = k0 + (int)(i % wins_per_sweep) * batch;
         const int nb = min(batch, k0 + kn - k);
         const size_t mv = ((size_t)sw * nel + k) * nw;
         return spo_batch_vgl(d, sp, pos, delta + 3 * mv, k, nb, rec ? rec + mv / nw * (size_t)nrec * nel : nullptr,
-                             nrec, d->vgl_buf[overlap ? (i & 1) : 0], st, false);
+                             nrec, vbuf(i), st, false);
     };
     auto reset_cursors = [&]() -> int {                       // start of a sweep: every walker at electron k0
-        fill_int_kernel<<<(nw + 127) / 128, 128, 0, s>>>(d->cur, nw, k0);
+        fill_int_kernel<<<(2 * nw + 127) / 128, 128, 0, s>>>(d->cur, 2 * nw, k0);      // cursors and evaluated-up-to marks
         QMC_LAUNCHED();
         return QMC_OK;
     };
@@ -273,7 +277,7 @@ static int sweep_delayed(qmc_det *d, const qmc_spline *sp, double *pos, const do
         const size_t mv = ((size_t)sw * nel + k) * nw;
         if (overlap) QMC_CUDA(cudaStreamWaitEvent(s, d->ev_spo[i & 1], 0));
         else if ((rc = spo(i, s))) return rc;
-        d->vgl = d->vgl_buf[overlap ? (i & 1) : 0];
+        d->vgl = vbuf(i);
         WindowJastrow wj{};
         if (jas.J) {
             // dJ of the window's nb proposals against the configuration at the start of the window, and for every

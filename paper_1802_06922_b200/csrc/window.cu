@@ -47,8 +47,8 @@ struct WindowArgs {
     WindowJastrow jas;            // base == NULL: no Jastrow factor
     // QMC_DET_ACCEPT_WINDOWS: the walker's window starts at electron cur[w], ends before kend, and closes when
     // pmax moves have been accepted; the per-move arrays are then offset to (sweep, electron 0)
-    int *cur;
-    int kend, pmax;
+    int *cur, *ev;                // ev[w]: electron up to which the walker's proposals have been evaluated
+    int kend, pmax, ring;         // ring: slots of the SPO-VGL scratch (slot = electron % ring); 0: slot = step
 };
 
 // G[i][j] = x_i . B0[iel0 + j] for the nb vectors x_i = x0 + i * vstep (fp32) of one walker, into
@@ -57,7 +57,7 @@ struct WindowArgs {
 // the 8 partial G are summed in a fixed order.  Ends with a __syncthreads().
 template <int KMAX, typename TB>
 __device__ __forceinline__ void window_contract(const float *x0, size_t vstep, const TB *b0, int nb, int ld,
-                                                int np, double *G_dst)
+                                                int np, double *G_dst, int slot0, int ring)
 {
     constexpr int MB = KMAX / 8;
     constexpr int GS = KMAX + 1;
@@ -69,6 +69,12 @@ __device__ __forceinline__ void window_contract(const float *x0, size_t vstep, c
 #pragma unroll
         for (int j = 0; j < MB; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
+    const float *xrow[MB];                                 // vector of step 8 ib + g (ring: slot = electron % ring)
+#pragma unroll
+    for (int ib = 0; ib < MB; ++ib) {
+        const int i = 8 * ib + g;
+        xrow[ib] = x0 + (size_t)(ring ? (slot0 + i) % ring : i) * vstep;
+    }
     for (int c0 = 16 * warp; c0 < np; c0 += 16 * (kWinThreads / 32)) {
         const int col = c0 + 4 * t;
         double av[MB][4], bv[MB][4];
@@ -86,7 +92,7 @@ __device__ __forceinline__ void window_contract(const float *x0, size_t vstep, c
         for (int ib = 0; ib < MB; ++ib) {
             const int i = 8 * ib + g;
             float4 f = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (i < nb) f = *reinterpret_cast<const float4 *>(x0 + (size_t)i * vstep + col);
+            if (i < nb) f = *reinterpret_cast<const float4 *>(xrow[ib] + col);
             av[ib][0] = f.x; av[ib][1] = f.y; av[ib][2] = f.z; av[ib][3] = f.w;
         }
 #pragma unroll
@@ -116,7 +122,7 @@ __device__ __forceinline__ void window_contract(const float *x0, size_t vstep, c
 // gradient vectors of every proposal).  Phase 3: warp 0 walks the nb steps.  Phase 4: R' = S^-T Rows,
 // 8-column tiles over the warps.
 template <typename TB, int KMAX, bool FORCE, bool JAS>
-__global__ void __launch_bounds__(kWinThreads, (FORCE || KMAX > 16) ? 1 : 4) delayed_window_kernel(WindowArgs a)
+__global__ void __launch_bounds__(kWinThreads, (FORCE || KMAX > 24) ? 1 : (KMAX > 16 ? 2 : 4)) delayed_window_kernel(WindowArgs a)
 {
     constexpr int GS = KMAX + 1;
     __shared__ double G_s[KMAX * GS];
@@ -137,9 +143,10 @@ __global__ void __launch_bounds__(kWinThreads, (FORCE || KMAX > 16) ? 1 : 4) del
     const float *v0 = a.vgl + (size_t)w * 5 * np;
     const TB *b0 = reinterpret_cast<const TB *>(a.B) + ((size_t)w * a.nel + iel0) * ld;
 
-    window_contract<KMAX, TB>(v0, vstep, b0, nb, ld, np, G_s);
+    const int ring = a.cur ? a.ring : 0;
+    window_contract<KMAX, TB>(v0, vstep, b0, nb, ld, np, G_s, iel0, ring);
     if (FORCE)
-        for (int d = 0; d < 3; ++d) window_contract<KMAX, TB>(v0 + (size_t)(1 + d) * np, vstep, b0, nb, ld, np, Gd_s + d * KMAX * GS);
+        for (int d = 0; d < 3; ++d) window_contract<KMAX, TB>(v0 + (size_t)(1 + d) * np, vstep, b0, nb, ld, np, Gd_s + d * KMAX * GS, iel0, ring);
 
     // ---- phase 3: the nb steps in sequence; lane m owns accepted move m (its step index `mine`).
     // Everything that lives in global memory stays outside the sequential loop: lane i fetches the
@@ -235,7 +242,7 @@ __global__ void __launch_bounds__(kWinThreads, (FORCE || KMAX > 16) ? 1 : 4) del
         const double logdet_add = warp_sum(acc_l ? log(fabs(R_l)) : 0.0);     // fixed (butterfly) order
         const unsigned neg = __ballot_sync(0xffffffffu, acc_l && R_l < 0.0);
         if (lane == 0) {
-            if (a.cur) a.cur[w] = iel0 + nproc;
+            if (a.cur) { a.cur[w] = iel0 + nproc; a.ev[w] = iel0 + nb; }
             a.win_count[w] = p;
             p_s = p;
             if (p) {
@@ -246,7 +253,7 @@ __global__ void __launch_bounds__(kWinThreads, (FORCE || KMAX > 16) ? 1 : 4) del
         }
         if (lane < p) {
             a.win_iel[(size_t)w * K + lane] = iel0 + mine;
-            a.win_slot[(size_t)w * K + lane] = mine;
+            a.win_slot[(size_t)w * K + lane] = ring ? (iel0 + mine) % ring : mine;
             rowoff_s[lane] = (long long)mine * ld;
         }
     }
@@ -278,7 +285,7 @@ int delayed_sweep_window(qmc_det *d, double *pos, const double *delta, const dou
     a.win_rows = d->win_rows;
     a.jas = jas;
     a.pmax = d->delay;
-    if (d->accept_windows) { a.cur = d->cur; a.kend = d->win_kend; }
+    if (d->accept_windows) { a.cur = d->cur; a.ev = d->cur + d->nw; a.kend = d->win_kend; a.ring = d->vgl_ring; }
     const int kwin = d->accept_windows ? d->spo_batch : a.K;     // steps per window: what the G matrix must hold
     prof_start(d, kProfDelayedRatio, s);
 #define QMC_WIN_LAUNCH(TB, KM, F, J) delayed_window_kernel<TB, KM, F, J><<<d->nw, kWinThreads, 0, s>>>(a)
