@@ -430,9 +430,8 @@ def main():
         # ---- roofline of the dominant kernel (rank-local, from the per-launch CUDA events)
         ld, npitch, K, eb = det.ld, spline.row_pitch, det.delay_rank, det.storage_bytes
         per_launch = {   # algorithmic bytes per launch; eb = bytes per stored element of B
-            # (accept windows: every open window evaluates K + K/2 proposals of its walker, used or not)
-            "spo_vgl": ((n_acc / max(K, 1) + 0.5 * nw * nprof) * (K + K // 2) if mode == "aw"
-                        else nprof * nmoved * nw * (2 if drift_tau else 1)) / max(prof["spo_vgl"][1], 1) * (64 + 5) * npitch * 4,
+            # (accept windows too: the scratch is a ring indexed by electron, every proposal is evaluated once)
+            "spo_vgl": (nprof * nmoved * nw * (2 if drift_tau else 1) / max(prof["spo_vgl"][1], 1)) * (64 + 5) * npitch * 4,
             "ratio_rowcopy": nw * ((eb + 8) * ld + 4 * nel) * (0.75 if drift_tau else 1.0),   # drift: averaged with the propose kernel
             "sm_update": (n_acc / max(prof["sm_update"][1], 1)) * (2 * eb * nel * ld + 12 * nel),
             # (accept windows: a launch serves the walkers that still have moves to apply -- about n_acc / K
