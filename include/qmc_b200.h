@@ -124,7 +124,7 @@ int qmc_det_destroy(qmc_det_t *det);
  * inverse is amortised over delay_rank accepted moves, not over 0.8 delay_rank.  The walkers of a handle then
  * advance through the electrons at their own pace (a per-walker cursor on the device; the SPO-VGL scratch is a
  * ring indexed by electron, so every proposal is still evaluated once); decisions, ratios and the inverse are
- * the same as with any other window choice.  qmc_sweep* only; not with a Jastrow factor. */
+ * the same as with any other window choice.  qmc_sweep* only. */
 #define QMC_DET_ACCEPT_WINDOWS 2u
 int qmc_det_init_ex(qmc_det_t **out, const qmc_spline_t *spline, int nwalkers, int nel,
                     const double *pos, int delay_rank, unsigned flags, void *stream);

@@ -31,7 +31,8 @@ int delayed_max_rank(int ld);                                // largest K whose 
 // and accepts iff R^2 exp(-2 dJ) > u.
 struct WindowJastrow {
     const double *base;           // [nb][nw]
-    const double *corr;           // [nw][K][K]
+    const double *corr;           // [nw][ncorr][ncorr], ncorr = steps per window
+    int ncorr;
     double *jratio_out;           // [nb][nw] or NULL: exp(-dJ)
 };
 int delayed_sweep_window(qmc_det *d, double *pos, const double *delta, const double *unif, int iel0, int nb,

@@ -27,6 +27,8 @@ struct JasMoveArgs {
     double *corr_out;         // [nw][ncorr][ncorr] or NULL: corr[w][j][m], m < j: what the ACCEPTED move of step m
     int ncorr;                //   (earlier in the same batch) adds to dJ of step j -- the same-spin pair term with
                               //   electron iel0 + m at its proposed instead of its old position
+    const int *cur;           // accept windows: step j moves electron cur[w] + j (nothing beyond kend) and delta is
+    int kend;                 //   offset to (sweep, electron 0) and indexed with the electron
 };
 
 constexpr int kJasThreads = 128;
@@ -38,18 +40,21 @@ __global__ void __launch_bounds__(kJasThreads) jastrow_move_kernel(JasMoveArgs a
 {
     __shared__ JasTable T;
     __shared__ double red[33];
+    const int w = blockIdx.x, j = blockIdx.y;
+    const int first = a.cur ? a.cur[w] : a.iel0, k = first + j;
+    if (a.cur && k >= a.kend) return;                      // beyond this walker's sweep (block-uniform, before any barrier)
     {
         const int *src = reinterpret_cast<const int *>(a.table);
         int *dst = reinterpret_cast<int *>(&T);
         for (int i = threadIdx.x; i < (int)(sizeof(JasTable) / sizeof(int)); i += kJasThreads) dst[i] = src[i];
     }
     __syncthreads();
-    const int w = blockIdx.x, j = blockIdx.y, k = a.iel0 + j;
+    const int jd0 = a.cur ? first : 0;                     // delta index of step 0
     const double *pw = a.pos + (size_t)w * a.nel * 3;
     const double rold[3] = {pw[3 * k], pw[3 * k + 1], pw[3 * k + 2]};
     double rnew[3];
     if (a.delta) {
-        const double *dl = a.delta + 3 * ((size_t)j * a.nw + w);
+        const double *dl = a.delta + 3 * ((size_t)(jd0 + j) * a.nw + w);
         rnew[0] = rold[0] + dl[0]; rnew[1] = rold[1] + dl[1]; rnew[2] = rold[2] + dl[2];
     } else {
         rnew[0] = a.rnew[3 * (size_t)w]; rnew[1] = a.rnew[3 * (size_t)w + 1]; rnew[2] = a.rnew[3 * (size_t)w + 2];
@@ -64,8 +69,8 @@ __global__ void __launch_bounds__(kJasThreads) jastrow_move_kernel(JasMoveArgs a
     for (int i = threadIdx.x; i < a.nion; i += kJasThreads) s += jas_pair_delta(T, a.ion_func[i], rnew, rold, a.ion + 3 * i);
     if (a.corr_out && (int)threadIdx.x < j) {
         const int m = threadIdx.x;
-        const double *ro_m = pw + 3 * (a.iel0 + m);
-        const double *dm = a.delta + 3 * ((size_t)m * a.nw + w);
+        const double *ro_m = pw + 3 * (first + m);
+        const double *dm = a.delta + 3 * ((size_t)(jd0 + m) * a.nw + w);
         const double rn_m[3] = {ro_m[0] + dm[0], ro_m[1] + dm[1], ro_m[2] + dm[2]};
         a.corr_out[((size_t)w * a.ncorr + j) * a.ncorr + m] =
             jas_pair_delta(T, T.f_same, rnew, rold, rn_m) - jas_pair_delta(T, T.f_same, rnew, rold, ro_m);
@@ -112,7 +117,7 @@ __global__ void __launch_bounds__(256) jastrow_value_kernel(const JasTable *tabl
 // step with explicit proposals.
 int jastrow_move_launch(const qmc_jastrow *J, int nw, int nel, const double *pos, int nother, const double *other,
                         int iel0, int nb, const double *delta, const double *rnew, double *dj_out, double *ratio_out,
-                        double *tfac_out, double *corr_out, int ncorr, cudaStream_t s)
+                        double *tfac_out, double *corr_out, int ncorr, cudaStream_t s, const int *cur, int kend)
 {
     JasMoveArgs a{};
     a.table = J->table; a.nion = J->nion; a.ion = J->ion; a.ion_func = J->ion_func;
@@ -120,6 +125,7 @@ int jastrow_move_launch(const qmc_jastrow *J, int nw, int nel, const double *pos
     a.pos = pos; a.other = other; a.iel0 = iel0; a.delta = delta; a.rnew = rnew;
     a.dj_out = dj_out; a.ratio_out = ratio_out; a.tfac_out = tfac_out;
     a.corr_out = delta ? corr_out : nullptr; a.ncorr = ncorr;
+    a.cur = cur; a.kend = kend;
     jastrow_move_kernel<<<dim3(nw, nb), kJasThreads, 0, s>>>(a);
     QMC_LAUNCHED();
     return QMC_OK;
@@ -214,7 +220,7 @@ extern "C" int qmc_jastrow_ratio(const qmc_jastrow_t *J, int nwalkers, int nel, 
     QMC_REQUIRE(nother >= 0 && (nother == 0 || other), "qmc_jastrow_ratio: nother=%d without positions", nother);
     if (nwalkers == 0) return QMC_OK;
     return jastrow_move_launch(J, nwalkers, nel, pos, nother, nother ? other : nullptr, iel, 1, nullptr, rnew, dj_out,
-                               ratio_out, nullptr, nullptr, 0, (cudaStream_t)stream);
+                               ratio_out, nullptr, nullptr, 0, (cudaStream_t)stream, nullptr, 0);
 }
 
 extern "C" int qmc_jastrow_value(const qmc_jastrow_t *J, int nwalkers, int nel, const double *pos, int nother,

@@ -15,7 +15,7 @@ namespace qmc {
 void spo_launch_shape(int np, int *threads, int *tiles);
 int jastrow_move_launch(const qmc_jastrow *J, int nw, int nel, const double *pos, int nother, const double *other,
                         int iel0, int nb, const double *delta, const double *rnew, double *dj_out, double *ratio_out,
-                        double *tfac_out, double *corr_out, int ncorr, cudaStream_t s);
+                        double *tfac_out, double *corr_out, int ncorr, cudaStream_t s, const int *cur = nullptr, int kend = 0);
 
 __global__ void fill_int_kernel(int *p, int n, int v)
 {
@@ -283,10 +283,10 @@ static int sweep_delayed(qmc_det *d, const qmc_spline *sp, double *pos, const do
             // dJ of the window's nb proposals against the configuration at the start of the window, and for every
             // pair of steps m < j what an accepted move m changes in dJ of step j; the window kernel adds the
             // pair terms of the steps it has accepted by then
-            double *corr = d->jas_dj + (size_t)d->delay * nw;
+            double *corr = d->jas_dj + (size_t)batch * nw;
             if ((rc = jastrow_move_launch(jas.J, nw, nel, pos, jas.nother, jas.other, k, nb, delta + 3 * mv, nullptr,
-                                          d->jas_dj, nullptr, nullptr, corr, d->delay, s))) return rc;
-            wj.base = d->jas_dj; wj.corr = corr; wj.jratio_out = jas.jratio_out ? jas.jratio_out + mv : nullptr;
+                                          d->jas_dj, nullptr, nullptr, corr, batch, s, aw ? d->cur : nullptr, d->win_kend))) return rc;
+            wj.base = d->jas_dj; wj.corr = corr; wj.ncorr = batch; wj.jratio_out = jas.jratio_out ? jas.jratio_out + mv : nullptr;
         }
         rc = delayed_sweep_window(d, pos, delta + 3 * mv, unif + mv, k, nb, ratios_out ? ratios_out + mv : nullptr,
                                   accept_out ? accept_out + mv : nullptr, forced ? forced + mv : nullptr, fixed_node,
@@ -431,9 +431,8 @@ static int sweep_impl(qmc_det *d, const qmc_spline *sp, double *pos, const doubl
         jas.jratio_out = opts->jratio_out;
         QMC_REQUIRE(jas.nother >= 0 && (jas.nother == 0 || jas.other), "qmc_sweep_ex: jastrow_nother=%d without positions", jas.nother);
         QMC_REQUIRE(jas.J->device == d->device, "qmc_sweep_ex: the Jastrow factor lives on another device");
-        QMC_REQUIRE(!d->accept_windows, "qmc_sweep_ex: a Jastrow factor is not supported with QMC_DET_ACCEPT_WINDOWS");
         if (!d->jas_dj) {
-            const size_t kk = d->delay > 1 ? d->delay : 1;       // dJ [K][nw] + pair terms [nw][K][K]
+            const size_t kk = d->delay > 1 ? d->spo_batch : 1;   // dJ [K][nw] + pair terms [nw][K][K], K = steps per window
             const size_t bytes = (kk * nw + (size_t)nw * kk * kk) * sizeof(double);
             cudaError_t e = cudaMalloc((void **)&d->jas_dj, bytes);
             if (e != cudaSuccess) { set_error("qmc_sweep_ex (jastrow): cudaMalloc(%zu bytes) -> %s", bytes, cudaGetErrorString(e)); (void)cudaGetLastError(); return QMC_ENOMEM; }

@@ -162,8 +162,8 @@ __global__ void __launch_bounds__(kWinThreads, (FORCE || KMAX > 24) ? 1 : (KMAX 
         // Jastrow factor: lane l holds dJ of step l against the window-start configuration
         constexpr bool jas = JAS;
         double dj_l = 0.0, jr_l = 1.0;
-        if (jas && step_l) dj_l = a.jas.base[mv_l];
-        const double *corr_w = jas ? a.jas.corr + (size_t)w * K * K : nullptr;
+        if (jas && step_l) dj_l = a.jas.base[(size_t)lane * a.nw + w];
+        const double *corr_w = jas ? a.jas.corr + (size_t)w * a.jas.ncorr * a.jas.ncorr : nullptr;
         unsigned acc_mask = 0;                                        // accepted steps (same in every lane)
         int p = 0, mine = 0;
         int nproc = nb;                                               // steps this window really takes
@@ -186,7 +186,7 @@ __global__ void __launch_bounds__(kWinThreads, (FORCE || KMAX > 24) ? 1 : (KMAX 
             if (jas) {
                 // the electrons of the accepted steps m < i sit at their proposed positions now: add their pair
                 // terms (lane m owns step m; fixed butterfly order)
-                const double corr = (lane < i && ((acc_mask >> lane) & 1u)) ? corr_w[(size_t)i * K + lane] : 0.0;
+                const double corr = (lane < i && ((acc_mask >> lane) & 1u)) ? corr_w[(size_t)i * a.jas.ncorr + lane] : 0.0;
                 const double dj = __shfl_sync(0xffffffffu, dj_l, i) + warp_sum(corr);
                 tf = exp(-2.0 * dj);
                 if (lane == i) jr_l = exp(-dj);

@@ -87,9 +87,10 @@ def _case(name):
     return inputs.make_inputs("small", nw=16, nsweeps=1)
 
 
-@pytest.mark.parametrize("case,K", [("ragged37_skew", 0), ("ragged37_skew", 4), ("ragged37_skew", 16), ("n130", 0),
-                                    ("n130", 7), ("small", 0), ("small", 16), ("small", 24)])
-def test_sweep_with_jastrow(case, K):
+@pytest.mark.parametrize("case,K,aw", [("ragged37_skew", 0, False), ("ragged37_skew", 4, False), ("ragged37_skew", 16, False),
+                                       ("n130", 0, False), ("n130", 7, False), ("small", 0, False), ("small", 16, False),
+                                       ("small", 24, False), ("ragged37_skew", 4, True), ("n130", 7, True), ("small", 16, True)])
+def test_sweep_with_jastrow(case, K, aw):
     """qmc_sweep_ex with a Jastrow factor, rank-1 and delayed handles: the oracle replays the GPU's fp32 orbital
     vectors (a) with the GPU's decisions imposed -- every determinant ratio, every exp(-dJ), positions bitwise --
     and (b) deciding for itself: decisions agree except where |R^2 exp(-2 dJ) - u| < 1e-6.  The Jastrow factor
@@ -101,7 +102,7 @@ def test_sweep_with_jastrow(case, K):
     jg, jo = both_sides(jx, x.lattice)
     spline = api.Spline.create(x.coefs.to(P.dev()), x.lattice)
     pos0 = P.to_dev(x.pos)
-    det = api.Det.init(spline, pos0, delay_rank=K)
+    det = api.Det.init(spline, pos0, delay_rank=K, accept_windows=aw)      # aw: windows closed on K accepted moves
     B0 = det.get_inverse().cpu().numpy()
     ld0, sg0, _ = (t.cpu().numpy() for t in det.get_stats())
     pos = pos0.clone()
@@ -137,7 +138,7 @@ def test_sweep_with_jastrow(case, K):
             assert abs(val - x.unif.reshape(-1, nw)[i, w]) < P.BAND, (w, i, val)
     plain = oracle.sweep(dummy, x.lattice, x.pos, B0, ld0, sg0, x.delta, x.unif, phi_in=rec, nthreads=nth)
     assert not np.array_equal(plain["accept"], acc)
-    print(case, K, "jastrow sweep: exp(-dJ) rel err", ej, "accept", acc.mean(), "plain accept", plain["accept"].mean(),
+    print(case, K, aw, "jastrow sweep: exp(-dJ) rel err", ej, "accept", acc.mean(), "plain accept", plain["accept"].mean(),
           "diverged", ndiv)
     # drift moves with a Jastrow factor are refused on both sides
     with pytest.raises(api.QmcError):
