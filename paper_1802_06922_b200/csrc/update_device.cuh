@@ -35,9 +35,8 @@ struct UpdateArgs {
 constexpr int kUpdThreads = 256;
 constexpr int kUpdRowsPerCta = 64;
 
-// Metropolis test of eq. 12 with symmetric T and a determinant-only Psi (R:A8).
-__device__ __forceinline__ bool metropolis(double R, double u) { return isfinite(R) && (R * R > u); }
-// The same with the ratio of the transition densities (drift moves, eq. 12): accept iff R^2 T'/T > u.
+// Metropolis test of eq. 12: accept iff R^2 tf > u, tf = 1 for symmetric T and a determinant-only Psi (R:A8),
+// the ratio of the transition densities T'/T for drift moves, exp(-2 dJ) with a Jastrow factor.
 __device__ __forceinline__ bool metropolis_t(double R, double tf, double u) { return isfinite(R) && isfinite(tf) && (R * R * tf > u); }
 // A move may be applied only if its ratio is finite and non-zero: the update divides by R and the
 // new Slater matrix would be singular otherwise (R:A18).  The Metropolis test already implies it

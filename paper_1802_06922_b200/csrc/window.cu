@@ -118,11 +118,83 @@ __device__ __forceinline__ void window_contract(const float *x0, size_t vstep, c
     }
 }
 
+// The same G for windows of more than 16 steps, where the KMAX/8 x KMAX/8 accumulator blocks of
+// window_contract no longer fit a 64-register budget: warp (jb, part) owns the 8 columns 8 jb .. 8 jb + 7
+// of G (the rows B0[iel0 + 8 jb ..]) and contracts the 16-column chunks part, part + NPART, ...; every row
+// of B0 is still read once per block (the fp32 vectors are re-read by the KMAX/8 column blocks: L1 hits),
+// and the NPART partial sums of a column block are added in a fixed order.  Ends with a __syncthreads().
+template <int KMAX, typename TB>
+__device__ __forceinline__ void window_contract_split(const float *x0, size_t vstep, const TB *b0, int nb, int ld,
+                                                      int np, double *G_dst, int slot0, int ring)
+{
+    constexpr int MB = KMAX / 8;
+    constexpr int GS = KMAX + 1;
+    constexpr int NPART = (kWinThreads / 32) / MB;        // warps per column block (warps beyond MB * NPART idle)
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int g = lane >> 2, t = lane & 3;
+    const int jb = warp / NPART, part = warp % NPART;
+    double acc[MB][2];
+#pragma unroll
+    for (int i = 0; i < MB; ++i) acc[i][0] = acc[i][1] = 0.0;
+    if (jb < MB && 8 * jb < nb) {
+        const float *xrow[MB];
+#pragma unroll
+        for (int ib = 0; ib < MB; ++ib) {
+            const int i = 8 * ib + g;
+            xrow[ib] = x0 + (size_t)(ring ? (slot0 + i) % ring : i) * vstep;
+        }
+        const int j = 8 * jb + g;
+        const TB *brow = b0 + (size_t)j * ld;
+        for (int c0 = 16 * part; c0 < np; c0 += 16 * NPART) {
+            const int col = c0 + 4 * t;
+            double2 lo = make_double2(0.0, 0.0), hi = lo;
+            if (j < nb) {
+                lo = ld2(brow + col);
+                hi = ld2(brow + col + 2);
+            }
+            const double bv[4] = {lo.x, lo.y, hi.x, hi.y};
+            double av[MB][4];
+#pragma unroll
+            for (int ib = 0; ib < MB; ++ib) {
+                float4 f = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (8 * ib + g < nb) f = *reinterpret_cast<const float4 *>(xrow[ib] + col);
+                av[ib][0] = f.x; av[ib][1] = f.y; av[ib][2] = f.z; av[ib][3] = f.w;
+            }
+#pragma unroll
+            for (int s = 0; s < 4; ++s)
+#pragma unroll
+                for (int ib = 0; ib < MB; ++ib)
+                    if (8 * ib < nb) dmma884(acc[ib][0], acc[ib][1], av[ib][s], bv[s]);
+        }
+    }
+    for (int q = 0; q < NPART; ++q) {
+        if (jb < MB && part == q) {
+#pragma unroll
+            for (int ib = 0; ib < MB; ++ib) {
+                double *dst = G_dst + (8 * ib + g) * GS + 8 * jb + 2 * t;
+                if (q == 0) { dst[0] = acc[ib][0]; dst[1] = acc[ib][1]; }
+                else { dst[0] += acc[ib][0]; dst[1] += acc[ib][1]; }
+            }
+        }
+        __syncthreads();
+    }
+}
+
+template <int KMAX, typename TB>
+__device__ __forceinline__ void window_G(const float *x0, size_t vstep, const TB *b0, int nb, int ld, int np,
+                                         double *G_dst, int slot0, int ring)
+{
+    if (KMAX > 16) window_contract_split<KMAX, TB>(x0, vstep, b0, nb, ld, np, G_dst, slot0, ring);
+    else window_contract<KMAX, TB>(x0, vstep, b0, nb, ld, np, G_dst, slot0, ring);
+}
+
 // One block per walker, 8 warps.  Phases 1-2: G (and, with FORCE, the same contraction for the three
 // gradient vectors of every proposal).  Phase 3: warp 0 walks the nb steps.  Phase 4: R' = S^-T Rows,
-// 8-column tiles over the warps.
-template <typename TB, int KMAX, bool FORCE, bool JAS>
-__global__ void __launch_bounds__(kWinThreads, (FORCE || KMAX > 24) ? 1 : (KMAX > 16 ? 2 : 4)) delayed_window_kernel(WindowArgs a)
+// 8-column tiles over the warps.  KMAX bounds the steps of a window, PMAX <= KMAX the moves it can accept
+// (accept windows: 24 proposals, 16 accepts), which is what sizes the registers of phase 4.
+template <typename TB, int KMAX, bool FORCE, bool JAS, int PMAX = KMAX>
+__global__ void __launch_bounds__(kWinThreads, (FORCE || KMAX > 24) ? 1 : ((KMAX > 16 && PMAX > 16) ? 2 : 4))
+delayed_window_kernel(WindowArgs a)
 {
     constexpr int GS = KMAX + 1;
     __shared__ double G_s[KMAX * GS];
@@ -144,9 +216,9 @@ __global__ void __launch_bounds__(kWinThreads, (FORCE || KMAX > 24) ? 1 : (KMAX 
     const TB *b0 = reinterpret_cast<const TB *>(a.B) + ((size_t)w * a.nel + iel0) * ld;
 
     const int ring = a.cur ? a.ring : 0;
-    window_contract<KMAX, TB>(v0, vstep, b0, nb, ld, np, G_s, iel0, ring);
+    window_G<KMAX, TB>(v0, vstep, b0, nb, ld, np, G_s, iel0, ring);
     if (FORCE)
-        for (int d = 0; d < 3; ++d) window_contract<KMAX, TB>(v0 + (size_t)(1 + d) * np, vstep, b0, nb, ld, np, Gd_s + d * KMAX * GS, iel0, ring);
+        for (int d = 0; d < 3; ++d) window_G<KMAX, TB>(v0 + (size_t)(1 + d) * np, vstep, b0, nb, ld, np, Gd_s + d * KMAX * GS, iel0, ring);
 
     // ---- phase 3: the nb steps in sequence; lane m owns accepted move m (its step index `mine`).
     // Everything that lives in global memory stays outside the sequential loop: lane i fetches the
@@ -261,7 +333,7 @@ __global__ void __launch_bounds__(kWinThreads, (FORCE || KMAX > 24) ? 1 : (KMAX 
 
     // ---- phase 4: R'[l] = sum_l' S^-1[l'][l] B0[k_l'] for the flush (pad columns of B are zero)
     const int p = p_s;
-    if (p) rprime_warp<KMAX, TB>(sinv_s, GS, p, b0, rowoff_s, a.win_rows + (size_t)w * K * ld, ld, warp, kWinThreads / 32, lane);
+    if (p) rprime_warp<PMAX, TB>(sinv_s, GS, p, b0, rowoff_s, a.win_rows + (size_t)w * K * ld, ld, warp, kWinThreads / 32, lane);
 }
 
 int delayed_sweep_window(qmc_det *d, double *pos, const double *delta, const double *unif, int iel0, int nb,
@@ -289,10 +361,12 @@ int delayed_sweep_window(qmc_det *d, double *pos, const double *delta, const dou
     const int kwin = d->accept_windows ? d->spo_batch : a.K;     // steps per window: what the G matrix must hold
     prof_start(d, kProfDelayedRatio, s);
 #define QMC_WIN_LAUNCH(TB, KM, F, J) delayed_window_kernel<TB, KM, F, J><<<d->nw, kWinThreads, 0, s>>>(a)
+#define QMC_WIN_LAUNCH_P(TB, KM, F, J, PM) delayed_window_kernel<TB, KM, F, J, PM><<<d->nw, kWinThreads, 0, s>>>(a)
 #define QMC_WIN_RANK(TB, F, J)                               \
     do {                                                     \
         if (kwin <= 8) QMC_WIN_LAUNCH(TB, 8, F, J);          \
         else if (kwin <= 16) QMC_WIN_LAUNCH(TB, 16, F, J);   \
+        else if (kwin <= 24 && a.pmax <= 16) QMC_WIN_LAUNCH_P(TB, 24, F, J, 16); \
         else if (kwin <= 24) QMC_WIN_LAUNCH(TB, 24, F, J);   \
         else QMC_WIN_LAUNCH(TB, 32, F, J);                   \
     } while (0)
@@ -305,6 +379,7 @@ int delayed_sweep_window(qmc_det *d, double *pos, const double *delta, const dou
     else { if (force_out) QMC_WIN_JAS(double, true); else QMC_WIN_JAS(double, false); }
 #undef QMC_WIN_JAS
 #undef QMC_WIN_RANK
+#undef QMC_WIN_LAUNCH_P
 #undef QMC_WIN_LAUNCH
     prof_stop(d, s);
     QMC_LAUNCHED();
