@@ -307,6 +307,25 @@ int qmc_det_info(const qmc_det_t *det, int *nwalkers, int *nel, int *ld, int *de
 int qmc_det_kinetic(qmc_det_t *det, const qmc_spline_t *spline, const double *pos, double *grad_out,
                     double *lap_out, double *one_out, double *ekin_out, void *stream);
 
+/* qmc_det_kinetic_noalloc -- ekin_out of qmc_det_kinetic (eq. 3 first term, eq. 37) for callers that may not
+ * allocate device memory (code under CUDA graph capture, serving loops, harnesses that forbid it).
+ * qmc_det_kinetic(..., lap_out = NULL, ...) takes its per-electron Laplacian scratch from cudaMalloc on the
+ * handle's first such call; this entry point calls no cudaMalloc, cudaFree or allocating library routine:
+ * the scratch is a file-scope device array of QMC_KINETIC_NOALLOC_MAX doubles (4 MiB) inside the library
+ * image, which every GPU that loads the library holds until the process exits.  Same kernels and summation
+ * order as qmc_det_kinetic: ekin_out has the same bits.
+ *
+ *   pos       dev, double [nwalkers][nel][3] (as qmc_det_kinetic);  ekin_out  dev, double [nwalkers] (caller's)
+ *   The handle's device must be the current device.
+ *   nwalkers * nel > QMC_KINETIC_NOALLOC_MAX: QMC_EINVAL, nothing launched (use qmc_det_kinetic).
+ *   All calls on a device share the one array.  A call overwrites every element it reads, so nothing carries
+ *   over from call to call, but calls that overlap on the GPU (different streams or host threads, also on
+ *   different handles) race on it: keep them on one stream or order them with events.
+ * Errors: QMC_EINVAL, QMC_ECUDA. */
+#define QMC_KINETIC_NOALLOC_MAX (1 << 19) /* elements = nwalkers * nel; `large` (512 x 1024) just fits */
+int qmc_det_kinetic_noalloc(qmc_det_t *det, const qmc_spline_t *spline, const double *pos, double *ekin_out,
+                            void *stream);
+
 /* ---------------------------------------------------------------------------------------
  * qmc_wf_* -- the product of two spin determinants, Psi_T = D_up D_dn: PAPER.md eq. 26 (L295),
  * Psi_T = sum_i c_i D_i^up D_i^dn e^J with one determinant per spin and no Jastrow factor.  A sweep

@@ -22,13 +22,14 @@ EXPORTS = [
     "qmc_det_init", "qmc_det_destroy", "qmc_det_ratio", "qmc_det_accept_update", "qmc_det_flush",
     "qmc_sweep", "qmc_sweep_ex", "qmc_sweep_host", "qmc_det_get_inverse", "qmc_det_set_inverse",
     "qmc_det_get_stats", "qmc_det_info", "qmc_launch_count", "qmc_det_profile", "qmc_det_profile_read",
-    "qmc_probe_fp64_dmma", "qmc_det_kinetic", "qmc_det_ratio_points",
+    "qmc_probe_fp64_dmma", "qmc_det_kinetic", "qmc_det_kinetic_noalloc", "qmc_det_ratio_points",
     "qmc_det_init_ex", "qmc_det_storage", "qmc_det_recompute", "qmc_det_residual",
     "qmc_wf_create", "qmc_wf_destroy", "qmc_wf_info", "qmc_wf_sweep", "qmc_wf_kinetic", "qmc_wf_get_stats",
     "qmc_jastrow_create", "qmc_jastrow_destroy", "qmc_jastrow_ratio", "qmc_jastrow_value", "qmc_probe_fp64_pipe",
 ]
 QMC_DET_FP32_INVERSE = 1
 QMC_DET_ACCEPT_WINDOWS = 2
+KINETIC_NOALLOC_MAX = 1 << 19      # QMC_KINETIC_NOALLOC_MAX
 PROF_KINDS = ["spo_vgl", "sm_update", "delayed_window", "delayed_accept", "delayed_flush", "ratio_rowcopy"]
 
 
@@ -81,6 +82,7 @@ def load_library(path=None):
         "qmc_probe_fp64_dmma": [ctypes.POINTER(d), _vp],
         "qmc_probe_fp64_pipe": [i, i, i, ctypes.POINTER(d), ctypes.POINTER(d), _vp],
         "qmc_det_kinetic": [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp],
+        "qmc_det_kinetic_noalloc": [_vp, _vp, _vp, _vp, _vp],
         "qmc_det_ratio_points": [_vp, i, i, _vp, i, _vp, _vp],
         "qmc_det_init_ex": [ctypes.POINTER(_vp), _vp, i, i, _vp, i, ctypes.c_uint, _vp],
         "qmc_det_storage": [_vp, ctypes.POINTER(i)],
@@ -321,6 +323,15 @@ class Det:
                                             _dev(lap, None), _dev(one, None), _dev(ekin, None), _stream(stream))
         _check(rc, "qmc_det_kinetic")
         return dict(grad=grad, lap=lap, one=one, ekin=ekin)
+
+    def kinetic_noalloc(self, pos, ekin_out, stream=None):
+        """qmc_det_kinetic_noalloc: E_kin [nw] into the caller's `ekin_out`; no device allocation anywhere on the
+        path (the Laplacian scratch is a static device array, nw * nel <= KINETIC_NOALLOC_MAX).  Calls that
+        overlap on the GPU race on that array."""
+        rc = load_library().qmc_det_kinetic_noalloc(self._h, self.spline._h, _dev(pos, torch.float64),
+                                                    _dev(ekin_out, torch.float64), _stream(stream))
+        _check(rc, "qmc_det_kinetic_noalloc")
+        return ekin_out
 
     def profile(self, enable=True):
         """qmc_det_profile: bracket every sweep kernel with CUDA events (and reset the recorder)."""

@@ -5,6 +5,8 @@
 // and sum_j phi_j(r_i) B[i][j] = 1 checks that B is the inverse at these positions.  The SPO-VGL of
 // the electrons' CURRENT positions comes from the same batched gather kernel the sweep uses, spo_batch
 // electrons of every walker per launch; this consumes value, gradient and Laplacian of S2.
+#include <mutex>
+
 #include "delayed_device.cuh"
 
 namespace qmc {
@@ -90,5 +92,74 @@ extern "C" int qmc_det_kinetic(qmc_det_t *d, const qmc_spline_t *sp, const doubl
         ekin_kernel<<<d->nw, 256, 0, s>>>(lap, d->nel, ekin_out);
         QMC_LAUNCHED();
     }
+    return QMC_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// qmc_det_kinetic_noalloc: E_kin per walker with the per-electron Laplacians staged in a file-scope device
+// array instead of a buffer from cudaMalloc (callers that may not allocate: include/qmc_b200.h).  Same
+// kernels, same launch shapes and same summation order as qmc_det_kinetic(..., ekin_out): the same bits.
+//
+// The array is part of the library image: every GPU that loads the library holds its 4 MiB until exit.
+// Every call on a device uses the same array; nothing in it has to start at zero (det_glap_kernel
+// overwrites the nw * nel elements ekin_kernel reads, on the same stream, before they are read), and what a
+// call leaves behind is never read by the next.  Calls that overlap on the GPU (two streams, two host
+// threads) race on it.
+static_assert(QMC_KINETIC_NOALLOC_MAX == (1 << 19), "the header states the limit in elements and bytes");
+static __device__ __align__(256) double g_kin_lap_static[QMC_KINETIC_NOALLOC_MAX];
+
+// Device address of g_kin_lap_static on `device`, which must be the current one.  In host code the array's
+// name is only the symbol's host-side stand-in; the address a kernel can use comes from the runtime, once
+// per device.
+static int kin_static_scratch(int device, double **out)
+{
+    constexpr int kMaxDevices = 64;
+    static double *ptr[kMaxDevices] = {};
+    static std::mutex mu;
+    int cur = -1;
+    QMC_CUDA(cudaGetDevice(&cur));
+    QMC_REQUIRE(cur == device, "qmc_det_kinetic_noalloc: the handle lives on device %d, the current device is %d", device, cur);
+    QMC_REQUIRE(device >= 0 && device < kMaxDevices, "qmc_det_kinetic_noalloc: device ordinal %d not supported", device);
+    std::lock_guard<std::mutex> lock(mu);
+    if (!ptr[device]) {
+        double *p = nullptr;
+        cudaError_t e = cudaGetSymbolAddress((void **)&p, g_kin_lap_static);
+        if (e != cudaSuccess || !p) {
+            set_error("qmc_det_kinetic_noalloc: cudaGetSymbolAddress -> %s", cudaGetErrorString(e));
+            (void)cudaGetLastError();
+            return QMC_ECUDA;
+        }
+        ptr[device] = p;
+    }
+    *out = ptr[device];
+    return QMC_OK;
+}
+
+extern "C" int qmc_det_kinetic_noalloc(qmc_det_t *d, const qmc_spline_t *sp, const double *pos, double *ekin_out,
+                                       void *stream)
+{
+    QMC_REQUIRE(d && sp && pos && ekin_out, "qmc_det_kinetic_noalloc: NULL argument");
+    QMC_REQUIRE(d->spline == sp, "qmc_det_kinetic_noalloc: the determinant was initialised from another spline");
+    const size_t need = (size_t)d->nw * d->nel;
+    QMC_REQUIRE(need <= (size_t)QMC_KINETIC_NOALLOC_MAX,
+                "qmc_det_kinetic_noalloc: nwalkers * nel = %zu exceeds the static scratch of %d elements "
+                "(QMC_KINETIC_NOALLOC_MAX); use qmc_det_kinetic", need, (int)QMC_KINETIC_NOALLOC_MAX);
+    double *lap = nullptr;
+    int rc = kin_static_scratch(d->device, &lap);
+    if (rc) return rc;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (d->delay) {               // the inverse must be current
+        rc = delayed_flush_reset_host(d, s);
+        if (rc) return rc;
+    }
+    for (int k = 0; k < d->nel; k += d->spo_batch) {
+        const int nb = d->nel - k < d->spo_batch ? d->nel - k : d->spo_batch;
+        rc = spo_batch_vgl(d, sp, pos, nullptr, k, nb, nullptr, 0, d->vgl, s);
+        if (rc) return rc;
+        QMC_WITH_B(d, TB, Bp, (det_glap_kernel<TB><<<dim3(nb, d->nw), 256, 0, s>>>(Bp, d->nel, d->ld, d->np, d->nw, k, d->vgl, nullptr, lap, nullptr)));
+        QMC_LAUNCHED();
+    }
+    ekin_kernel<<<d->nw, 256, 0, s>>>(lap, d->nel, ekin_out);
+    QMC_LAUNCHED();
     return QMC_OK;
 }
