@@ -6,6 +6,7 @@ may import this package.  It imports nothing from paper_1802_06922_b200.
 from .binding import (  # noqa: F401
     build,
     spline_vgl,
+    spline_vgl_twist,
     lu_inverse,
     binv_from_A,
     det_ratio,

@@ -75,6 +75,9 @@ def _load():
         lib = ctypes.CDLL(_LIB)
         lib.orc_spline_vgl.restype = ctypes.c_int
         lib.orc_spline_vgl.argtypes = [ctypes.c_int] * 4 + [_dp, _fp, ctypes.c_int, _dp, _dp, _dp, _dp]
+        lib.orc_spline_vgl_twist.restype = ctypes.c_int
+        lib.orc_spline_vgl_twist.argtypes = ([ctypes.c_int] * 4 + [_dp, _fp, ctypes.c_int, _dp, _ip,
+                                             _dp, _dp, _dp])
         lib.orc_lu_inverse.restype = ctypes.c_int
         lib.orc_lu_inverse.argtypes = [ctypes.c_int, _dp, _dp, _dp, _ip]
         lib.orc_binv_from_A.restype = ctypes.c_int
@@ -153,6 +156,25 @@ def spline_vgl(coefs, lattice, pos, want_gl=True):
                             _d(pos), _d(v), _d(g), _d(l))
     _check(rc, "spline_vgl")
     return (v, g, l) if want_gl else v
+
+
+def spline_vgl_twist(coefs, lattice, pos, half_twist):
+    """spline_vgl for real orbitals at a half twist: half_twist = 3 flags, 1 = twist angle pi
+    along that cell vector (eq. 43)."""
+    lib = _load()
+    coefs = _coefs(coefs)
+    nx, ny, nz, norb = coefs.shape
+    lat = _c64(lattice).reshape(9)
+    pos = _c64(pos).reshape(-1, 3)
+    npos = pos.shape[0]
+    tw = np.ascontiguousarray(np.asarray(half_twist, dtype=np.int32).reshape(3))
+    v = np.empty((npos, norb))
+    g = np.empty((npos, 3, norb))
+    l = np.empty((npos, norb))
+    rc = lib.orc_spline_vgl_twist(nx, ny, nz, norb, _d(lat), coefs.ctypes.data_as(_fp), npos,
+                                  _d(pos), tw.ctypes.data_as(_ip), _d(v), _d(g), _d(l))
+    _check(rc, "spline_vgl_twist")
+    return v, g, l
 
 
 def lu_inverse(A):

@@ -113,9 +113,9 @@ static void cell_of(double u, int n, int *i, double *t)
  * positions.  v [npos][norb], g [npos][3][norb], l [npos][norb], all double;
  * g and l may be NULL.  Returns 0, or -1 on bad arguments.
  */
-int orc_spline_vgl(int nx, int ny, int nz, int norb, const double lattice[9],
-                   const float *coefs, int npos, const double *pos,
-                   double *v, double *g, double *l)
+static int spline_vgl_tw(int nx, int ny, int nz, int norb, const double lattice[9],
+                         const float *coefs, int npos, const double *pos, const int *half_twist,
+                         double *v, double *g, double *l)
 {
     double Li[9];
     if (nx < 1 || ny < 1 || nz < 1 || norb < 1 || npos < 0) return -1;
@@ -138,6 +138,22 @@ int orc_spline_vgl(int nx, int ny, int nz, int norb, const double lattice[9],
             double u = r[0] * Li[0 + d] + r[1] * Li[3 + d] + r[2] * Li[6 + d];
             cell_of(u, nd[d], &i[d], &t[d]);
             bspline_weights(t[d], b[d], db[d], d2b[d]);
+            if (half_twist && half_twist[d] && isfinite(u)) {
+                /* Twist angle pi along cell vector d (eq. 43 with Theta_d = pi; R:A23):
+                 * the table holds one cell of an ANTIPERIODIC function, c[i + m n] = (-1)^m c[i].
+                 * The point lies in image floor(u) (one more when u - floor(u) rounded up to 1.0
+                 * and cell_of moved it to u = 0, R:A7); control point i + a lies (i + a) / n
+                 * images further on. */
+                double fu = floor(u);
+                long long img = (long long)fmod(fu, 2.0);
+                if ((u - fu) * (double)nd[d] >= (double)nd[d]) img += 1;
+                for (int a = 0; a < 4; ++a)
+                    if ((img + (i[d] + a) / nd[d]) & 1) {
+                        b[d][a] = -b[d][a];
+                        db[d][a] = -db[d][a];
+                        d2b[d][a] = -d2b[d][a];
+                    }
+            }
         }
         memset(acc, 0, (size_t)norb * 10 * sizeof(double));
         for (int a = 0; a < 4; ++a)
@@ -197,6 +213,26 @@ int orc_spline_vgl(int nx, int ny, int nz, int norb, const double lattice[9],
     }
     free(acc);
     return 0;
+}
+
+int orc_spline_vgl(int nx, int ny, int nz, int norb, const double lattice[9],
+                   const float *coefs, int npos, const double *pos,
+                   double *v, double *g, double *l)
+{
+    return spline_vgl_tw(nx, ny, nz, norb, lattice, coefs, npos, pos, NULL, v, g, l);
+}
+
+/*
+ * The same evaluation for real orbitals at a half twist (sec 9.2, eq. 43 with
+ * twist angle Theta_d = pi along every cell vector d with half_twist[d] != 0, 0 along the others):
+ * phi(r + L_d) = -phi(r).  half_twist = {0,0,0} is orc_spline_vgl.  Reading R:A23 in DESIGN.md.
+ */
+int orc_spline_vgl_twist(int nx, int ny, int nz, int norb, const double lattice[9],
+                         const float *coefs, int npos, const double *pos, const int half_twist[3],
+                         double *v, double *g, double *l)
+{
+    if (!half_twist) return -1;
+    return spline_vgl_tw(nx, ny, nz, norb, lattice, coefs, npos, pos, half_twist, v, g, l);
 }
 
 /* ------------------------------------------------------------------------- */
