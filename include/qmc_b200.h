@@ -63,6 +63,18 @@ int qmc_spline_create(qmc_spline_t **out, int nx, int ny, int nz, int norb,
                       const double *lattice, const float *coefs, int coefs_on_device,
                       void *stream);
 int qmc_spline_destroy(qmc_spline_t *spline);
+/* qmc_spline_set_half_twist -- PAPER.md L449-455 (sec 9.2, eq. 43): real orbitals at a half twist,
+ * twist angle Theta_d = K . a_d = pi along every cell vector d with half_twist[d] == 1 and 0 along
+ * the others, so phi(r + a_d) = -phi(r) there (reading R:A23 in DESIGN.md).  The table then holds one
+ * cell of an antiperiodic function: control points reached across the face of cell vector d, and
+ * positions in odd images of the cell, take the factor -1 in every later evaluation through this
+ * handle (qmc_spo_vgl, qmc_det_*, qmc_sweep*): ratios, inverses and sweeps follow unchanged.
+ *   half_twist   host, 3 ints, each 0 or 1; {0,0,0} (the state after qmc_spline_create) is periodic.
+ * Host-side flag only: no device work, no allocation; set it before the first launch that uses the
+ * handle, not while one is in flight.  General twists need complex orbitals: DESIGN.md section 9.
+ * Errors: QMC_EINVAL (NULL, a value other than 0 / 1).
+ */
+int qmc_spline_set_half_twist(qmc_spline_t *spline, const int *half_twist);
 /* Row pitch Np (floats) and bytes of the padded device table; either pointer may be NULL. */
 int qmc_spline_info(const qmc_spline_t *spline, int *row_pitch, size_t *table_bytes);
 

@@ -35,6 +35,10 @@
  *                     "single, double and mixed precision" (R:A19: B rounded to fp32 when stored,
  *                     all arithmetic in fp64), with orc_init_walkers as the recompute-from-scratch.
  *
+ *   orc_spline_vgl_twist   L449-455 (sec 9.2, eq. 43): the same evaluation for real orbitals at a
+ *                     half twist, twist angle pi along chosen cell vectors (R:A23): the table is
+ *                     one cell of an antiperiodic function.  Pins: tests/test_twist_pins.py.
+ *
  * Pins (tests/test_oracle_pins.py, run with -m "not gpu"): partition of unity,
  * polynomial reproduction, plane-wave node closed form, periodicity, C2
  * continuity, scipy.interpolate.BSpline tensor product, central finite

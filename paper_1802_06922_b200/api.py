@@ -26,6 +26,7 @@ EXPORTS = [
     "qmc_det_init_ex", "qmc_det_storage", "qmc_det_recompute", "qmc_det_residual",
     "qmc_wf_create", "qmc_wf_destroy", "qmc_wf_info", "qmc_wf_sweep", "qmc_wf_kinetic", "qmc_wf_get_stats",
     "qmc_jastrow_create", "qmc_jastrow_destroy", "qmc_jastrow_ratio", "qmc_jastrow_value", "qmc_probe_fp64_pipe",
+    "qmc_spline_set_half_twist",
 ]
 QMC_DET_FP32_INVERSE = 1
 QMC_DET_ACCEPT_WINDOWS = 2
@@ -63,6 +64,7 @@ def load_library(path=None):
     sigs = {
         "qmc_spline_create": [ctypes.POINTER(_vp), i, i, i, i, ctypes.POINTER(d), _vp, i, _vp],
         "qmc_spline_destroy": [_vp],
+        "qmc_spline_set_half_twist": [_vp, ctypes.POINTER(i)],
         "qmc_spline_info": [_vp, ctypes.POINTER(i), ctypes.POINTER(ctypes.c_size_t)],
         "qmc_spo_vgl": [_vp, i, _vp, _vp, _vp, _vp, i, _vp],
         "qmc_det_init": [ctypes.POINTER(_vp), _vp, i, i, _vp, i, _vp],
@@ -182,6 +184,11 @@ class Spline:
         if not coefs.is_cuda:
             torch.cuda.synchronize()
         return cls(h, (nx, ny, nz), norb)
+
+    def set_half_twist(self, half_twist):
+        """qmc_spline_set_half_twist: 3 flags, 1 = twist angle pi along that cell vector (eq. 43)."""
+        tw = (ctypes.c_int * 3)(*[int(t) for t in half_twist])
+        _check(load_library().qmc_spline_set_half_twist(self._h, tw), "qmc_spline_set_half_twist")
 
     def destroy(self):
         if self._h:

@@ -63,6 +63,7 @@ struct SplineView {
     double linv[9];       // lattice^-1, row-major: u_d = sum_j r_j linv[3j+d]
     double jac[9];        // jac[3j+d] = linv[3j+d] * N_d = d s_d / d r_j
     double metric[6];     // G_de = sum_j jac[j][d] jac[j][e]: xx,yy,zz,xy,xz,yz
+    int half_twist[3];    // 1: twist angle pi along cell vector d (eq. 43, R:A23); 0: periodic
 };
 
 }  // namespace qmc

@@ -154,6 +154,16 @@ extern "C" int qmc_spline_destroy(qmc_spline_t *h)
     return QMC_OK;
 }
 
+extern "C" int qmc_spline_set_half_twist(qmc_spline_t *h, const int *half_twist)
+{
+    QMC_REQUIRE(h && half_twist, "qmc_spline_set_half_twist: NULL argument");
+    for (int d = 0; d < 3; ++d)
+        QMC_REQUIRE(half_twist[d] == 0 || half_twist[d] == 1,
+                    "qmc_spline_set_half_twist: half_twist[%d]=%d is neither 0 nor 1", d, half_twist[d]);
+    for (int d = 0; d < 3; ++d) h->view.half_twist[d] = half_twist[d];
+    return QMC_OK;
+}
+
 extern "C" int qmc_spline_info(const qmc_spline_t *h, int *row_pitch, size_t *table_bytes)
 {
     QMC_REQUIRE(h, "qmc_spline_info: NULL handle");

@@ -44,14 +44,31 @@ __device__ __forceinline__ void stage_stencil(const SplineView &sp, double rx, d
         const int d = tid;
         const int n = d == 0 ? sp.nx : (d == 1 ? sp.ny : sp.nz);
         double u = rx * sp.linv[0 + d] + ry * sp.linv[3 + d] + rz * sp.linv[6 + d];
+        const double u0 = u;
         u -= floor(u);
         const double s = u * (double)n;
         const double fl = floor(s);
         int i = (int)fl;
         const double t = s - fl;
-        if (i >= n) i = 0;
+        bool up = false;
+        if (i >= n) { i = 0; up = true; }
         st.cell[d] = i;
         bspline1d(t, st.b1d[d][0], st.b1d[d][1], st.b1d[d][2]);
+        if (sp.half_twist[d]) {
+            // Half twist along cell vector d (eq. 43, twist angle pi; R:A23): the table is one
+            // cell of an antiperiodic function.  Control point i + a lives in image m + (i + a) / n of
+            // the cell, m the image of the point itself (one further when u rounded up to 1.0); an odd
+            // image flips the sign of that control point's 1-D weights, so the 64 products carry it.
+            const double m = floor(u0) + (up ? 1.0 : 0.0);
+            const int odd = (int)(m - 2.0 * floor(0.5 * m));
+#pragma unroll
+            for (int a = 0; a < 4; ++a)
+                if ((odd + (i + a) / n) & 1) {
+                    st.b1d[d][0][a] = -st.b1d[d][0][a];
+                    st.b1d[d][1][a] = -st.b1d[d][1][a];
+                    st.b1d[d][2][a] = -st.b1d[d][2][a];
+                }
+        }
     }
     __syncthreads();
     for (int e = tid; e < 64; e += blockDim.x) {

@@ -94,7 +94,8 @@ def compare_decisions(acc_g, R_g, acc_o, R_o, unif, tol=None):
     return ndiverged
 
 
-def run_protocol(x, delay_rank=0, walkers=None, free_oracle=True, coefs_np=None, accept_windows=False):
+def run_protocol(x, delay_rank=0, walkers=None, free_oracle=True, coefs_np=None, accept_windows=False,
+                 half_twist=None):
     """Parity protocol on inputs x (tests/conftest shapes).  Returns a dict of measured errors.
 
     walkers: None = all walkers are replayed by the oracle; else the first `walkers` of them
@@ -105,6 +106,11 @@ def run_protocol(x, delay_rank=0, walkers=None, free_oracle=True, coefs_np=None,
     nchk = nw if walkers is None else min(nw, walkers)
     coefs_t = x.coefs.to(dev())
     spline = api.Spline.create(coefs_t, x.lattice)
+    if half_twist is not None:
+        # real orbitals at a half twist (R:A23): the oracle's own sweep evaluates the periodic table, so
+        # only the identical-vector legs (4)-(6) apply; the twisted vectors are checked in test_gpu_twist.py
+        assert not free_oracle
+        spline.set_half_twist(half_twist)
     pos0 = to_dev(x.pos)
     delta_t, unif_t = to_dev(x.delta), to_dev(x.unif)
     out = {}
